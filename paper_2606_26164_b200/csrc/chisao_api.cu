@@ -1,0 +1,628 @@
+// chisao_api.cu -- host side of the C ABI declared in include/chisao.h: validation, workspace carving,
+// parameter packing, the per-cycle launch sequence (Algorithm 1) and state exchange.
+// Every step of the path runs in the kernels; the host only enqueues.  There is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "chisao_eval_kernels.cuh"
+
+using namespace chisao;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+struct Segment { size_t off, bytes; };
+
+struct Layout {
+  size_t total = 0;
+  size_t take(size_t bytes) {
+    const size_t off = total;
+    total += (bytes + 255) & ~size_t(255);
+    return off;
+  }
+};
+
+struct TimedRec { int cls; cudaEvent_t a, b; };
+
+}  // namespace
+
+struct chisao_ctx {
+  chisao_config cfg;
+  Hyper hp;
+  DevObj obj;
+  State st;
+  cudaStream_t stream;
+  int cycle = 0;
+  std::vector<float> lo, hi, recs_host;
+  std::string err;
+  uint64_t launches = 0;
+  bool timing = false;
+  std::vector<TimedRec> recs;
+  std::vector<cudaEvent_t> pool;
+  size_t ws_bytes = 0;
+};
+
+namespace {
+
+int fail(chisao_ctx *c, int code, const std::string &msg) {
+  g_last_error = msg;
+  if (c) c->err = msg;
+  return code;
+}
+int cuda_fail(chisao_ctx *c, cudaError_t e, const char *what) {
+  return fail(c, CHISAO_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                   \
+  do {                                                             \
+    cudaError_t e_ = (call);                                       \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);       \
+  } while (0)
+
+int validate(const chisao_config *cfg, const chisao_objective *obj, std::string &why) {
+  if (!cfg || !obj) { why = "null config/objective"; return CHISAO_E_INVALID; }
+  if (cfg->d < 1 || cfg->d > CHISAO_MAX_D) { why = "d must be in 1..64"; return CHISAO_E_INVALID; }
+  if (obj->d != cfg->d) { why = "objective.d != config.d"; return CHISAO_E_INVALID; }
+  if (cfg->N < 0) { why = "N < 0"; return CHISAO_E_INVALID; }
+  if (cfg->lbfgs_m < 1 || cfg->lbfgs_m > CHISAO_MAX_M) { why = "lbfgs_m must be in 1..16"; return CHISAO_E_INVALID; }
+  if (cfg->hlc_M < 1 || cfg->hlc_M > PTILE) { why = "hlc_M must be in 1..256"; return CHISAO_E_INVALID; }
+  if (cfg->ls_max < 0 || cfg->ls_max > 30) { why = "ls_max must be in 0..30"; return CHISAO_E_INVALID; }
+  if (cfg->reseed_cands < 1 || cfg->reseed_cands > 16) { why = "reseed_cands must be in 1..16"; return CHISAO_E_INVALID; }
+  if (cfg->n_osc < 1 || cfg->n_conv < 0 || cfg->n_anti < 0 || cfg->n_cloud < 0) { why = "negative iteration count"; return CHISAO_E_INVALID; }
+  if (!(cfg->fd_h > 0.0f)) { why = "fd_h must be > 0"; return CHISAO_E_INVALID; }
+  if (!(cfg->sigma_s > 0.0f)) { why = "sigma_s must be > 0"; return CHISAO_E_INVALID; }
+  if (!cfg->lo || !cfg->hi) { why = "null bounds"; return CHISAO_E_INVALID; }
+  for (int j = 0; j < cfg->d; ++j)
+    if (!(cfg->lo[j] <= cfg->hi[j])) { why = "lo > hi"; return CHISAO_E_INVALID; }
+  if (obj->id < 0 || obj->id > 4) { why = "unknown objective id"; return CHISAO_E_INVALID; }
+  if (obj->K < 1) { why = "K < 1"; return CHISAO_E_INVALID; }
+  if (obj->id == CHISAO_OBJ_QUAD && obj->K != 1) { why = "QUAD needs K = 1"; return CHISAO_E_INVALID; }
+  if (!obj->mats) { why = "objective.mats is null"; return CHISAO_E_INVALID; }
+  if (obj->id != CHISAO_OBJ_RFF && !obj->means) { why = "objective.means is null"; return CHISAO_E_INVALID; }
+  if (obj->id != CHISAO_OBJ_QUAD && !obj->vec_a) { why = "objective.vec_a is null"; return CHISAO_E_INVALID; }
+  if (obj->id == CHISAO_OBJ_RFF && !obj->vec_b) { why = "objective.vec_b is null"; return CHISAO_E_INVALID; }
+  if (!(obj->sigma_noise >= 0.0f)) { why = "sigma_noise < 0"; return CHISAO_E_INVALID; }
+  return CHISAO_OK;
+}
+
+// workspace carve; fills st pointers relative to `base` (may be null when only sizing)
+size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *base, State *st, const float **recs_dev) {
+  Layout L;
+  const size_t N = (size_t)c.N, d = (size_t)c.d, m = (size_t)c.lbfgs_m, M = (size_t)c.hlc_M;
+  const int DP = padded_dim(c.d);
+  const size_t rec = (size_t)record_floats(o.id, DP);
+  const size_t nb = (N + 1023) / 1024;
+  auto F = [&](size_t n) { return L.take(n * 4); };
+  const size_t o_ctrl = L.take(sizeof(Ctrl));
+  const size_t o_recs = F((size_t)o.K * rec);
+  const size_t o_lo = F(d), o_hi = F(d);
+  const size_t o_f = F(N), o_ft = F(N), o_dec = F(N), o_tcur = F(N), o_ginf = F(N);
+  const size_t o_g = F(N * d), o_v = F(N * d), o_xt = F(N * d), o_gn = F(N * d), o_p = F(N * d), o_gh = F(N * d);
+  const size_t o_S = F(m * N * d), o_Y = F(m * N * d);
+  const size_t o_hl = F(N), o_hh = F(N), o_lsb = F(N), o_rss = F(N), o_rsc = F(N);
+  const size_t o_st = L.take(N), o_rm = L.take(N), o_sl = L.take(N);
+  size_t o_lists[9];
+  for (auto &x : o_lists) x = F(N);
+  const size_t o_blk = F(3 * nb + 3);
+  const size_t o_hf = F(N * M);
+  const size_t o_q = F(d * d);
+  if (base && st) {
+    auto P = [&](size_t off) { return reinterpret_cast<float *>(base + off); };
+    auto I = [&](size_t off) { return reinterpret_cast<int32_t *>(base + off); };
+    st->ctrl = reinterpret_cast<Ctrl *>(base + o_ctrl);
+    *recs_dev = P(o_recs);
+    st->lo = P(o_lo); st->hi = P(o_hi);
+    st->f = P(o_f); st->ft = P(o_ft); st->dec = P(o_dec); st->tcur = P(o_tcur); st->ginf = P(o_ginf);
+    st->g = P(o_g); st->v = P(o_v); st->xt = P(o_xt); st->gn = P(o_gn); st->p = P(o_p); st->ghat = P(o_gh);
+    st->S = P(o_S); st->Y = P(o_Y);
+    st->hist_len = I(o_hl); st->hist_head = I(o_hh); st->ls_b = I(o_lsb); st->rs_src = I(o_rss); st->rs_cand = I(o_rsc);
+    st->stuck = base + o_st; st->removed = base + o_rm; st->stalled = base + o_sl;
+    st->listA = I(o_lists[0]); st->listP = I(o_lists[1]); st->listR = I(o_lists[2]); st->listE = I(o_lists[3]);
+    st->listP0 = I(o_lists[4]); st->ls_list[0] = I(o_lists[5]); st->ls_list[1] = I(o_lists[6]);
+    st->ls_list[2] = I(o_lists[7]); st->fd_list = I(o_lists[8]);
+    st->blk_cnt = I(o_blk);
+    st->hlc_f = P(o_hf);
+    st->grQ = P(o_q);
+  }
+  return L.total;
+}
+
+// pack the objective into fixed-size records (pure data movement; layouts in chisao_common.cuh)
+void pack_records(const chisao_objective &o, int DP, std::vector<float> &out, float &s0) {
+  const int d = o.d, K = o.K, rec = record_floats(o.id, DP);
+  out.assign((size_t)K * rec, 0.0f);
+  s0 = 0.0f;
+  for (int k = 0; k < K; ++k) {
+    float *r = out.data() + (size_t)k * rec;
+    switch (o.id) {
+      case CHISAO_OBJ_GMM_ISO:
+        for (int j = 0; j < d; ++j) r[j] = o.means[(size_t)k * d + j];
+        r[DP] = o.vec_a[k];
+        break;
+      case CHISAO_OBJ_GMM_DIAG:
+        for (int j = 0; j < d; ++j) { r[j] = o.means[(size_t)k * d + j]; r[DP + j] = o.mats[(size_t)k * d + j]; }
+        r[2 * DP] = o.vec_a[k];
+        break;
+      case CHISAO_OBJ_GMM_FULL:
+      case CHISAO_OBJ_QUAD:
+        for (int a = 0; a < d; ++a)
+          for (int b = 0; b < d; ++b) r[a * DP + b] = o.mats[((size_t)k * d + a) * d + b];
+        for (int j = 0; j < d; ++j) r[DP * DP + j] = o.means[(size_t)k * d + j];
+        r[DP * DP + DP] = (o.id == CHISAO_OBJ_GMM_FULL) ? o.vec_a[k] : 0.0f;
+        break;
+      case CHISAO_OBJ_RFF:
+        for (int j = 0; j < d; ++j) r[j] = o.mats[(size_t)k * d + j];
+        r[DP] = o.vec_a[k]; r[DP + 1] = o.vec_b[k];
+        break;
+    }
+  }
+  if (o.id == CHISAO_OBJ_GMM_ISO) s0 = (float)(1.0 / (2.0 * (double)o.mats[0] * (double)o.mats[0]));
+  if (o.id == CHISAO_OBJ_RFF) s0 = o.scalar0;
+}
+
+struct Scope {   // optional CUDA-event bracket around a launch group
+  chisao_ctx *c; int cls; cudaEvent_t a = nullptr, b = nullptr;
+  Scope(chisao_ctx *ctx, int k) : c(ctx), cls(k) {
+    if (!c->timing) return;
+    auto get = [&]() { cudaEvent_t e; if (!c->pool.empty()) { e = c->pool.back(); c->pool.pop_back(); } else cudaEventCreate(&e); return e; };
+    a = get(); b = get();
+    cudaEventRecord(a, c->stream);
+  }
+  ~Scope() {
+    if (!a) return;
+    cudaEventRecord(b, c->stream);
+    c->recs.push_back({cls, a, b});
+  }
+};
+
+cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const int32_t *count, int mode, float *g_out,
+                    int phase, int iter, int counter) {
+  const State &s = c->st;
+  if (s.N == 0) return cudaSuccess;
+  FdArgs a{};
+  a.X = X; a.list = list; a.count = count; a.max_count = s.N; a.mode = mode; a.d = s.d; a.cycle = c->cycle;
+  a.phase = phase; a.iter = iter; a.counter = counter; a.g_out = g_out; a.x = s.x; a.v = s.v; a.lo = s.lo; a.hi = s.hi;
+  a.h = c->hp.fd_h; a.mu = c->hp.mu; a.alpha = c->hp.alpha_anti; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
+  const int spt = NT / s.d;
+  const int grid = (s.N + spt - 1) / spt;
+  Scope sc(c, 0);
+  c->launches += 1;
+  switch (c->obj.id) {
+    case 0: return launch_fd_obj_0(c->obj, a, grid, c->stream);
+    case 1: return launch_fd_obj_1(c->obj, a, grid, c->stream);
+    case 2: return launch_fd_obj_2(c->obj, a, grid, c->stream);
+    case 3: return launch_fd_obj_3(c->obj, a, grid, c->stream);
+    default: return launch_fd_obj_4(c->obj, a, grid, c->stream);
+  }
+}
+
+cudaError_t eval_points(chisao_ctx *c, int mode, int b, int iter) {
+  const State &s = c->st;
+  if (s.N == 0) return cudaSuccess;
+  PtArgs a{};
+  a.mode = mode; a.b = b; a.d = s.d; a.cycle = c->cycle; a.iter = iter; a.ls_max = c->hp.ls_max; a.max_count = s.N;
+  a.f = s.f; a.ft = s.ft; a.dec = s.dec; a.tcur = s.tcur; a.xt = s.xt; a.x = s.x; a.p = s.p; a.g = s.g; a.lo = s.lo; a.hi = s.hi;
+  a.ls_b = s.ls_b; a.fd_list = s.fd_list; a.fd_cnt = &s.ctrl->fd_cnt;
+  a.c1 = c->hp.ls_c1; a.shrink = c->hp.ls_shrink; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
+  if (mode == PT_CENTRE) {
+    a.X = s.x; a.list = nullptr; a.count = nullptr;
+  } else {
+    a.X = s.xt; a.list = s.ls_list[b % 3]; a.count = &s.ctrl->ls_cnt[b % 3];
+    a.next_list = s.ls_list[(b + 1) % 3]; a.next_cnt = &s.ctrl->ls_cnt[(b + 1) % 3];
+    a.zero_cnt = &s.ctrl->ls_cnt[(b + 2) % 3];
+  }
+  const int grid = (s.N + PTILE - 1) / PTILE;
+  Scope sc(c, 1);
+  c->launches += 1;
+  switch (c->obj.id) {
+    case 0: return launch_pt_obj_0(c->obj, a, grid, c->stream);
+    case 1: return launch_pt_obj_1(c->obj, a, grid, c->stream);
+    case 2: return launch_pt_obj_2(c->obj, a, grid, c->stream);
+    case 3: return launch_pt_obj_3(c->obj, a, grid, c->stream);
+    default: return launch_pt_obj_4(c->obj, a, grid, c->stream);
+  }
+}
+
+cudaError_t hlc_step(chisao_ctx *c, int iter) {
+  const State &s = c->st;
+  if (s.N == 0) return cudaSuccess;
+  HlcArgs a{};
+  a.list = s.listE; a.count = &s.ctrl->nE; a.max_count = s.N; a.d = s.d; a.M = s.M; a.cycle = c->cycle; a.iter = iter;
+  a.baseline = c->hp.hlc_baseline; a.x = s.x; a.ghat = s.ghat; a.hlc_f = s.hlc_f; a.lo = s.lo; a.hi = s.hi;
+  a.sigma = c->hp.sigma_s; a.eta = c->hp.eta_hlc; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
+  const int spt = std::min(PTILE / s.M, HLC_MAX_SPT);
+  const int grid = (s.N + spt - 1) / spt;
+  Scope sc(c, 2);
+  c->launches += 1;
+  switch (c->obj.id) {
+    case 0: return launch_hlc_obj_0(c->obj, a, grid, c->stream);
+    case 1: return launch_hlc_obj_1(c->obj, a, grid, c->stream);
+    case 2: return launch_hlc_obj_2(c->obj, a, grid, c->stream);
+    case 3: return launch_hlc_obj_3(c->obj, a, grid, c->stream);
+    default: return launch_hlc_obj_4(c->obj, a, grid, c->stream);
+  }
+}
+
+// ---- units of Algorithm 1 --------------------------------------------------------------------------------
+int run_release_eval(chisao_ctx *ctx) {   // Phase 1 start: release all + f, g at x
+  { Scope sc(ctx, 4); CK(launch_release(ctx->st, ctx->stream)); ctx->launches += 1; }
+  CK(eval_points(ctx, PT_CENTRE, 0, 0));
+  CK(eval_fd(ctx, ctx->st.x, nullptr, nullptr, FD_GRAD, ctx->st.g, 1, 0, EV_INIT));
+  return CHISAO_OK;
+}
+int run_lbfgs_iter(chisao_ctx *ctx, int it) {   // one L-BFGS iteration (R-4)
+  const State &s = ctx->st;
+  CK(cudaMemsetAsync(s.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
+  { Scope sc(ctx, 3); CK(launch_lbfgs_direction(s, ctx->hp, ctx->stream)); ctx->launches += 1; }
+  for (int b = 0; b <= ctx->hp.ls_max; ++b) CK(eval_points(ctx, PT_LS, b, it));
+  CK(eval_fd(ctx, s.xt, s.fd_list, &s.ctrl->fd_cnt, FD_GRAD, s.gn, 1, it, EV_LBFGS_FD));
+  { Scope sc(ctx, 4); CK(launch_lbfgs_update(s, ctx->hp, ctx->stream)); ctx->launches += 1; }
+  return CHISAO_OK;
+}
+int run_stick(chisao_ctx *ctx) {
+  Scope sc(ctx, 5);
+  CK(launch_stick(ctx->st, ctx->hp, ctx->stream));
+  ctx->launches += 5;
+  return CHISAO_OK;
+}
+int run_dedup(chisao_ctx *ctx) {
+  Scope sc(ctx, 5);
+  CK(launch_dedup(ctx->st, ctx->hp, ctx->stream));
+  ctx->launches += 8;
+  return CHISAO_OK;
+}
+int run_reseed(chisao_ctx *ctx) {
+  Scope sc(ctx, 6);
+  CK(launch_reseed(ctx->st, ctx->hp, ctx->cycle, ctx->stream));
+  ctx->launches += 3;
+  return CHISAO_OK;
+}
+int run_explore_list(chisao_ctx *ctx) {
+  Scope sc(ctx, 5);
+  CK(launch_explore_list(ctx->st, ctx->stream));
+  ctx->launches += 3;
+  return CHISAO_OK;
+}
+int run_hlc(chisao_ctx *ctx, int t) {
+  if (!(ctx->hp.phase_mask & (1u << 5))) return CHISAO_OK;
+  CK(hlc_step(ctx, t));
+  return CHISAO_OK;
+}
+int run_anti(chisao_ctx *ctx, int t) {
+  if (!(ctx->hp.phase_mask & (1u << 6))) return CHISAO_OK;
+  const State &s = ctx->st;
+  CK(eval_fd(ctx, s.x, s.listE, &s.ctrl->nE, FD_ANTI, nullptr, 6, t, EV_ANTI));
+  return CHISAO_OK;
+}
+
+int read_stats(chisao_ctx *ctx, chisao_stats *out) {
+  Ctrl h;
+  CK(cudaMemcpyAsync(&h, ctx->st.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  out->cycle = ctx->cycle; out->n_stuck = h.n_stuck; out->k_lost = h.k_lost; out->n_active = h.n_active;
+  out->reseed_strategy = h.strategy; out->gr_enabled = h.gr_enabled;
+  for (int k = 0; k < 8; ++k) out->evals[k] = h.evals[k];
+  out->f_max = dec_ordered(h.fmax_enc);
+  return CHISAO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int chisao_workspace_bytes(const chisao_config *cfg, const chisao_objective *obj, size_t *bytes) {
+  std::string why;
+  const int rc = validate(cfg, obj, why);
+  if (rc) return fail(nullptr, rc, why);
+  if (!bytes) return fail(nullptr, CHISAO_E_INVALID, "bytes is null");
+  *bytes = carve(*cfg, *obj, nullptr, nullptr, nullptr);
+  return CHISAO_OK;
+}
+
+int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objective *obj, float *x_dev,
+                void *workspace_dev, size_t workspace_bytes, void *stream) {
+  std::string why;
+  int rc = validate(cfg, obj, why);
+  if (rc) return fail(nullptr, rc, why);
+  if (!out) return fail(nullptr, CHISAO_E_INVALID, "out is null");
+  if (cfg->N > 0 && !x_dev) return fail(nullptr, CHISAO_E_INVALID, "x_dev is null");
+  const size_t need = carve(*cfg, *obj, nullptr, nullptr, nullptr);
+  if (!workspace_dev || workspace_bytes < need) return fail(nullptr, CHISAO_E_WORKSPACE, "workspace too small");
+  if (reinterpret_cast<uintptr_t>(workspace_dev) & 255) return fail(nullptr, CHISAO_E_WORKSPACE, "workspace not 256-byte aligned");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) return cuda_fail(nullptr, e == cudaSuccess ? cudaErrorNoDevice : e, "no CUDA device");
+
+  chisao_ctx *ctx = new chisao_ctx();
+  ctx->cfg = *cfg;
+  ctx->stream = reinterpret_cast<cudaStream_t>(stream);
+  ctx->ws_bytes = need;
+  ctx->lo.assign(cfg->lo, cfg->lo + cfg->d);
+  ctx->hi.assign(cfg->hi, cfg->hi + cfg->d);
+  ctx->cfg.lo = ctx->lo.data(); ctx->cfg.hi = ctx->hi.data();
+  Hyper &h = ctx->hp;
+  h.n_osc = cfg->n_osc; h.n_conv = cfg->n_conv; h.n_anti = cfg->n_anti; h.n_cloud = cfg->n_cloud; h.hlc_M = cfg->hlc_M;
+  h.lbfgs_m = cfg->lbfgs_m; h.ls_max = cfg->ls_max; h.reseed_cands = cfg->reseed_cands; h.hlc_baseline = cfg->hlc_baseline;
+  h.phase_mask = cfg->phase_mask; h.fd_h = cfg->fd_h; h.eps_grad = cfg->eps_grad; h.eps_dup = cfg->eps_dup;
+  h.log_delta = cfg->log_delta; h.mu = cfg->mu; h.alpha_anti = cfg->alpha_anti; h.eta_hlc = cfg->eta_hlc;
+  h.sigma_s = cfg->sigma_s; h.ls_c1 = cfg->ls_c1; h.ls_shrink = cfg->ls_shrink; h.seed = cfg->seed;
+
+  State &s = ctx->st;
+  std::memset(&s, 0, sizeof(s));
+  s.N = cfg->N; s.d = cfg->d; s.m = cfg->lbfgs_m; s.M = cfg->hlc_M; s.x = x_dev;
+  const float *recs_dev = nullptr;
+  carve(*cfg, *obj, static_cast<unsigned char *>(workspace_dev), &s, &recs_dev);
+
+  DevObj &o = ctx->obj;
+  o.id = obj->id; o.d = obj->d; o.K = obj->K; o.DP = padded_dim(obj->d);
+  o.rec = record_floats(o.id, o.DP);
+  o.kc = std::max(1, std::min(o.K, CHUNK_BYTES / (o.rec * 4)));
+  o.sigma_noise = obj->sigma_noise;
+  o.recs = recs_dev;
+  pack_records(*obj, o.DP, ctx->recs_host, o.s0);
+  if (eval_smem_bytes(o, hlc_extra_bytes(o.DP)) > 200 * 1024) {
+    delete ctx;
+    return fail(nullptr, CHISAO_E_INVALID, "objective record too large for shared memory");
+  }
+
+#define CKI(call)                                                                   \
+  do {                                                                              \
+    cudaError_t e_ = (call);                                                        \
+    if (e_ != cudaSuccess) { int r_ = cuda_fail(nullptr, e_, #call); delete ctx; return r_; } \
+  } while (0)
+  switch (o.id) {
+    case 0: CKI(configure_obj_0()); break;
+    case 1: CKI(configure_obj_1()); break;
+    case 2: CKI(configure_obj_2()); break;
+    case 3: CKI(configure_obj_3()); break;
+    default: CKI(configure_obj_4()); break;
+  }
+  // zero everything except the parameter records, then upload parameters and bounds
+  CKI(cudaMemsetAsync(workspace_dev, 0, need, ctx->stream));
+  CKI(cudaMemcpyAsync(const_cast<float *>(recs_dev), ctx->recs_host.data(), ctx->recs_host.size() * 4,
+                      cudaMemcpyHostToDevice, ctx->stream));
+  CKI(cudaMemcpyAsync(s.lo, ctx->lo.data(), 4 * (size_t)cfg->d, cudaMemcpyHostToDevice, ctx->stream));
+  CKI(cudaMemcpyAsync(s.hi, ctx->hi.data(), 4 * (size_t)cfg->d, cudaMemcpyHostToDevice, ctx->stream));
+  const int32_t one = 1;
+  CKI(cudaMemcpyAsync(&s.ctrl->gr_enabled, &one, 4, cudaMemcpyHostToDevice, ctx->stream));
+#undef CKI
+  *out = ctx;
+  return CHISAO_OK;
+}
+
+int chisao_seed_population(chisao_ctx *ctx) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  CK(launch_seed_population(ctx->st, ctx->hp, ctx->stream));
+  ctx->launches += 1;
+  return CHISAO_OK;
+}
+
+int chisao_step(chisao_ctx *ctx, chisao_stats *stats) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  if (ctx->cycle >= ctx->hp.n_osc) return fail(ctx, CHISAO_E_STATE, "all n_osc cycles already done");
+  ctx->cycle += 1;                                    // "for k = 1..n_osc"
+  int rc;
+  if ((rc = run_release_eval(ctx))) return rc;        // Phase 1: release all, then converge
+  for (int it = 1; it <= ctx->hp.n_conv; ++it)
+    if ((rc = run_lbfgs_iter(ctx, it))) return rc;
+  if ((rc = run_stick(ctx))) return rc;               // Phase 2
+  if ((rc = run_dedup(ctx))) return rc;               // Phase 3
+  CK(cudaMemsetAsync(&ctx->st.ctrl->strategy, 0, 4, ctx->stream));
+  if (ctx->cycle < ctx->hp.n_osc) {                   // "if k < n_osc"
+    if ((rc = run_reseed(ctx))) return rc;            // Phase 4
+    if ((rc = run_explore_list(ctx))) return rc;
+    for (int t = 1; t <= ctx->hp.n_cloud; ++t)        // Phase 5
+      if ((rc = run_hlc(ctx, t))) return rc;
+    for (int t = 1; t <= ctx->hp.n_anti; ++t)         // Phase 6
+      if ((rc = run_anti(ctx, t))) return rc;
+  }
+  if (stats) return read_stats(ctx, stats);
+  return CHISAO_OK;
+}
+
+int chisao_step_host(chisao_ctx *ctx, const float *x_in, float *x_out, float *f_out, uint8_t *stuck_out,
+                     chisao_stats *stats) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  const size_t N = ctx->st.N, d = ctx->st.d;
+  if (x_in) CK(cudaMemcpyAsync(ctx->st.x, x_in, N * d * 4, cudaMemcpyHostToDevice, ctx->stream));
+  const int rc = chisao_step(ctx, nullptr);
+  if (rc) return rc;
+  if (x_out) CK(cudaMemcpyAsync(x_out, ctx->st.x, N * d * 4, cudaMemcpyDeviceToHost, ctx->stream));
+  if (f_out) CK(cudaMemcpyAsync(f_out, ctx->st.f, N * 4, cudaMemcpyDeviceToHost, ctx->stream));
+  if (stuck_out) CK(cudaMemcpyAsync(stuck_out, ctx->st.stuck, N, cudaMemcpyDeviceToHost, ctx->stream));
+  if (stats) return read_stats(ctx, stats);
+  CK(cudaStreamSynchronize(ctx->stream));
+  return CHISAO_OK;
+}
+
+int chisao_phase(chisao_ctx *ctx, int32_t phase_id, int32_t iter) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  switch (phase_id) {
+    case CHISAO_PH_RELEASE_EVAL: return run_release_eval(ctx);
+    case CHISAO_PH_LBFGS_ITER: return run_lbfgs_iter(ctx, iter);
+    case CHISAO_PH_STICK: return run_stick(ctx);
+    case CHISAO_PH_DEDUP: return run_dedup(ctx);
+    case CHISAO_PH_RESEED: return run_reseed(ctx);
+    case CHISAO_PH_HLC_STEP: { const int rc = run_explore_list(ctx); return rc ? rc : run_hlc(ctx, iter); }
+    case CHISAO_PH_ANTI_STEP: { const int rc = run_explore_list(ctx); return rc ? rc : run_anti(ctx, iter); }
+  }
+  return fail(ctx, CHISAO_E_INVALID, "unknown phase id");
+}
+
+int chisao_get_stats(chisao_ctx *ctx, chisao_stats *stats) {
+  if (!ctx || !stats) return fail(ctx, CHISAO_E_INVALID, "null argument");
+  return read_stats(ctx, stats);
+}
+
+int chisao_modes(chisao_ctx *ctx, float *modes_out, float *f_out, int32_t *idx_out, int32_t cap, int32_t *n_modes) {
+  if (!ctx || !n_modes || cap < 0) return fail(ctx, CHISAO_E_INVALID, "bad argument");
+  const State &s = ctx->st;
+  const size_t N = s.N, d = s.d;
+  std::vector<uint8_t> stuck(N);
+  std::vector<float> f(N);
+  if (N) {
+    CK(cudaMemcpyAsync(stuck.data(), s.stuck, N, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(f.data(), s.f, N * 4, cudaMemcpyDeviceToHost, ctx->stream));
+  }
+  CK(cudaStreamSynchronize(ctx->stream));
+  std::vector<int32_t> idx;
+  for (size_t i = 0; i < N; ++i) if (stuck[i]) idx.push_back((int32_t)i);
+  std::stable_sort(idx.begin(), idx.end(), [&](int32_t a, int32_t b) { return f[a] > f[b]; });  // (f desc, index asc)
+  *n_modes = (int32_t)idx.size();
+  const int n = std::min<int>(cap, (int)idx.size());
+  if (n > 0) {
+    if (modes_out) {   // gather on the device (gn and fd_list are free between cycles)
+      CK(cudaMemcpyAsync(s.fd_list, idx.data(), (size_t)n * 4, cudaMemcpyHostToDevice, ctx->stream));
+      CK(launch_gather_rows(s.x, s.fd_list, n, (int)d, s.gn, ctx->stream));
+      ctx->launches += 1;
+      CK(cudaMemcpyAsync(modes_out, s.gn, (size_t)n * d * 4, cudaMemcpyDeviceToHost, ctx->stream));
+      CK(cudaStreamSynchronize(ctx->stream));
+    }
+    for (int q = 0; q < n; ++q) {
+      if (f_out) f_out[q] = f[idx[q]];
+      if (idx_out) idx_out[q] = idx[q];
+    }
+  }
+  if ((int)idx.size() > cap) return fail(ctx, CHISAO_E_CAPACITY, "cap < n_modes");
+  return CHISAO_OK;
+}
+
+static int field_info(chisao_ctx *ctx, int32_t field, void **dev, size_t *bytes) {
+  const State &s = ctx->st;
+  const size_t N = s.N, d = s.d, M = s.M;
+  switch (field) {
+    case CHISAO_X: *dev = s.x; *bytes = N * d * 4; return 0;
+    case CHISAO_F: *dev = s.f; *bytes = N * 4; return 0;
+    case CHISAO_G: *dev = s.g; *bytes = N * d * 4; return 0;
+    case CHISAO_V: *dev = s.v; *bytes = N * d * 4; return 0;
+    case CHISAO_STUCK: *dev = s.stuck; *bytes = N; return 0;
+    case CHISAO_REMOVED: *dev = s.removed; *bytes = N; return 0;
+    case CHISAO_STALLED: *dev = s.stalled; *bytes = N; return 0;
+    case CHISAO_HIST_LEN: *dev = s.hist_len; *bytes = N * 4; return 0;
+    case CHISAO_P: *dev = s.p; *bytes = N * d * 4; return 0;
+    case CHISAO_LS_B: *dev = s.ls_b; *bytes = N * 4; return 0;
+    case CHISAO_GHAT: *dev = s.ghat; *bytes = N * d * 4; return 0;
+    case CHISAO_HLC_F: *dev = s.hlc_f; *bytes = N * M * 4; return 0;
+    case CHISAO_RS_SRC: *dev = s.rs_src; *bytes = N * 4; return 0;
+    case CHISAO_RS_CAND: *dev = s.rs_cand; *bytes = N * 4; return 0;
+    case CHISAO_XT: *dev = s.xt; *bytes = N * d * 4; return 0;
+    case CHISAO_GR_Q: *dev = s.grQ; *bytes = d * d * 4; return 0;
+  }
+  return -1;
+}
+
+int chisao_get_state(chisao_ctx *ctx, int32_t field, void *dst, size_t bytes) {
+  if (!ctx || (!dst && bytes)) return fail(ctx, CHISAO_E_INVALID, "null argument");
+  const State &s = ctx->st;
+  const size_t N = s.N, d = s.d, m = s.m;
+  if (field == CHISAO_CTRL) {
+    if (bytes != 32) return fail(ctx, CHISAO_E_INVALID, "CTRL is 8 x i32");
+    Ctrl h;
+    CK(cudaMemcpyAsync(&h, s.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    int32_t c[8] = {ctx->cycle, h.gr_enabled, h.gr_unproductive, h.gr_prev_modes, h.gr_used_last, h.k_lost, h.n_stuck, h.n_active};
+    std::memcpy(dst, c, 32);
+    return CHISAO_OK;
+  }
+  if (field == CHISAO_HIST_S || field == CHISAO_HIST_Y) {
+    if (bytes != m * N * d * 4) return fail(ctx, CHISAO_E_INVALID, "wrong size for history field");
+    std::vector<float> phys(m * N * d);
+    std::vector<int32_t> head(N), len(N);
+    if (N) {
+      CK(cudaMemcpyAsync(phys.data(), field == CHISAO_HIST_S ? s.S : s.Y, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+      CK(cudaMemcpyAsync(head.data(), s.hist_head, N * 4, cudaMemcpyDeviceToHost, ctx->stream));
+      CK(cudaMemcpyAsync(len.data(), s.hist_len, N * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    CK(cudaStreamSynchronize(ctx->stream));
+    float *o = static_cast<float *>(dst);
+    std::memset(o, 0, bytes);
+    for (size_t i = 0; i < N; ++i)
+      for (int l = 0; l < len[i]; ++l) {
+        const size_t ph = (size_t)(head[i] + l) % m;
+        std::memcpy(o + ((size_t)l * N + i) * d, phys.data() + (ph * N + i) * d, d * 4);
+      }
+    return CHISAO_OK;
+  }
+  void *dev = nullptr; size_t fb = 0;
+  if (field_info(ctx, field, &dev, &fb)) return fail(ctx, CHISAO_E_INVALID, "unknown state field");
+  if (fb != bytes) return fail(ctx, CHISAO_E_INVALID, "wrong size for state field");
+  if (bytes) CK(cudaMemcpyAsync(dst, dev, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  return CHISAO_OK;
+}
+
+int chisao_set_state(chisao_ctx *ctx, int32_t field, const void *src, size_t bytes) {
+  if (!ctx || (!src && bytes)) return fail(ctx, CHISAO_E_INVALID, "null argument");
+  const State &s = ctx->st;
+  const size_t N = s.N, d = s.d, m = s.m;
+  if (field == CHISAO_CTRL) {
+    if (bytes != 32) return fail(ctx, CHISAO_E_INVALID, "CTRL is 8 x i32");
+    int32_t c[8];
+    std::memcpy(c, src, 32);
+    ctx->cycle = c[0];
+    CK(cudaMemcpyAsync(&s.ctrl->cycle, c, 32, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return CHISAO_OK;
+  }
+  if (field == CHISAO_HIST_S || field == CHISAO_HIST_Y) {
+    // logical order in, physical = logical: ring heads are reset (set HIST_S, HIST_Y and HIST_LEN together)
+    if (bytes != m * N * d * 4) return fail(ctx, CHISAO_E_INVALID, "wrong size for history field");
+    if (bytes) {
+      CK(cudaMemcpyAsync(field == CHISAO_HIST_S ? s.S : s.Y, src, bytes, cudaMemcpyHostToDevice, ctx->stream));
+      CK(cudaMemsetAsync(s.hist_head, 0, N * 4, ctx->stream));
+    }
+    CK(cudaStreamSynchronize(ctx->stream));
+    return CHISAO_OK;
+  }
+  if (field >= CHISAO_P) return fail(ctx, CHISAO_E_INVALID, "diagnostic fields are read-only");
+  void *dev = nullptr; size_t fb = 0;
+  if (field_info(ctx, field, &dev, &fb)) return fail(ctx, CHISAO_E_INVALID, "unknown state field");
+  if (fb != bytes) return fail(ctx, CHISAO_E_INVALID, "wrong size for state field");
+  if (bytes) CK(cudaMemcpyAsync(dev, src, bytes, cudaMemcpyHostToDevice, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  return CHISAO_OK;
+}
+
+uint64_t chisao_launch_count(const chisao_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int chisao_timing_enable(chisao_ctx *ctx, int32_t on) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  ctx->timing = on != 0;
+  return CHISAO_OK;
+}
+int chisao_timing_reset(chisao_ctx *ctx) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  CK(cudaStreamSynchronize(ctx->stream));
+  for (auto &r : ctx->recs) { ctx->pool.push_back(r.a); ctx->pool.push_back(r.b); }
+  ctx->recs.clear();
+  return CHISAO_OK;
+}
+int chisao_timing_get(chisao_ctx *ctx, int32_t which, double *ms, uint64_t *launches) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  CK(cudaStreamSynchronize(ctx->stream));
+  double tot = 0.0; uint64_t n = 0;
+  for (auto &r : ctx->recs) {
+    if (r.cls != which) continue;
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, r.a, r.b));
+    tot += t; n += 1;
+  }
+  if (ms) *ms = tot;
+  if (launches) *launches = n;
+  return CHISAO_OK;
+}
+
+const char *chisao_last_error(const chisao_ctx *ctx) { return ctx ? ctx->err.c_str() : g_last_error.c_str(); }
+
+void chisao_destroy(chisao_ctx *ctx) {
+  if (!ctx) return;
+  for (auto &r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (auto &e : ctx->pool) cudaEventDestroy(e);
+  delete ctx;
+}
+
+}  // extern "C"
