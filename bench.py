@@ -1,0 +1,275 @@
+#!/usr/bin/env python
+"""bench.py -- samples*cycles/sec of the CHISAO oscillation cycle (BASELINE.json metric) on one node.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one full convergence / anti-convergence cycle (chisao_step: phases 1-6 of Algorithm 1,
+PAPER.md:141-176) over the whole population of the workload (default: BASELINE.json configs[4] = C5, the
+configuration the north_star targets are quoted on: d = 64, N = 65536, full-covariance mixture).
+N > 1 GPUs run independent replicas (replicas only, no data-path collective).
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC, UNIT = "samples_cycles_per_sec", "samples*cycles/s"
+
+WORKLOAD_TEXT = {
+    1: "C1: d=2 N=256 iso-GMM K=4 (BASELINE.json configs[0])",
+    2: "C2: d=8 N=4096 diag-GMM K=16 noisy (configs[1])",
+    3: "C3: d=32 N=16384 random-Fourier K=256 (configs[2])",
+    4: "C4: d=64 N=16384 ill-conditioned quadratic (configs[3])",
+    5: "C5: d=64 N=65536 full-covariance GMM K=64 noisy, RM/GR reseeding (configs[4])",
+}
+
+
+def flop_per_eval(obj) -> float:
+    """Plain-definition flop count of one objective evaluation."""
+    d, K = obj.d, obj.K
+    return {0: K * (3.0 * d + 4), 1: K * (4.0 * d + 4), 2: K * (2.0 * d * d + 3 * d + 4), 3: K * (2.0 * d + 8) + 2 * d,
+            4: 2.0 * d * d + 3 * d}[obj.id]
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([s.strip() for s in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm, reasons, mx = [], set(), None
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def oracle_throughput(c: int, steps: int, warmup: int, rank_seed: int = 0):
+    """Time the oracle as it stands on a bounded sample of workload `c` (host cores of this box)."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle as O
+    from paper_2606_26164_b200 import inputs
+    cores = len(os.sched_getaffinity(0))
+    full = inputs.config(c)
+    # ~1.7 GFLOP per sample-cycle at C5: a few samples per core keep one step in the 5-15 s range
+    per_core = {1: 256, 2: 64, 3: 6, 4: 8, 5: 1}[c]
+    Ns = min(full.hp.N, max(8, per_core * cores))
+    wl = inputs.config(c, N=Ns, n_osc=max(full.hp.n_osc, steps + warmup + 1))
+    o = O.Oracle(wl, threads=cores)
+    for _ in range(warmup):
+        o.step()
+    ev0 = sum(o.stats().evals)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step()
+    dt = time.perf_counter() - t0
+    ev = sum(o.stats().evals) - ev0
+    o.close()
+    return {"value": Ns * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{Ns} of {full.hp.N} samples x {steps} full cycle(s) after {warmup} warm-up cycle(s), fp64, "
+                      f"OpenMP over samples; per-sample cost is N-independent except deduplication",
+            "f_evals_per_sec": ev / dt, "seconds": dt}, wl
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    # the oracle is slow by design: one warm-up cycle is enough to page everything in
+    res, wl = oracle_throughput(args.config, max(1, args.steps), min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * res["seconds"] / max(1, args.steps),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_TEXT[args.config], "sampled": res["sample"]},
+            "cpu_baseline": {k: res[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": res["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "f_evals_per_sec": res["f_evals_per_sec"], "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, local_rank, world):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_26164_b200 import binding as B, inputs, replicas
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    K, W, c = args.steps, args.warmup, args.config
+    full = inputs.config(c)
+    N = args.N or full.hp.N
+    n_osc = max(full.hp.n_osc, K + W + 1)                   # timed cycles are all full cycles (phases 1-6)
+    wl = replicas.replica_workload(c, rank, N=N, n_osc=n_osc)
+    hp = wl.hp
+
+    # ---- device-resident timing: W warm-up cycles, then exactly K cycles between CUDA events -------------
+    g = B.Chisao(wl, device=dev)
+    for _ in range(W):
+        g.step(stats=False)
+    st0 = g.stats()
+    g.timing_enable(True); g.timing_reset()
+    l0 = g.launch_count()
+    sampler = ClockSampler(local_rank); sampler.start()
+    time.sleep(0.25)
+    ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev_a.record()
+    for _ in range(K):
+        g.step(stats=False)
+    ev_b.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = ev_a.elapsed_time(ev_b)
+    clocks = sampler.stop()
+    launches = g.launch_count() - l0
+    st1 = g.stats()
+    phase_ms = g.timing()
+    g.timing_enable(False)
+    evals = np.array(st1.evals[:], np.int64) - np.array(st0.evals[:], np.int64)
+    ms_max = replicas.max_over_ranks(ms, dist if world > 1 else None, dev)
+    total_evals = replicas.sum_over_ranks(float(evals.sum()), dist if world > 1 else None, dev)
+
+    # ---- end to end through the host-buffer C-ABI call (H2D + cycle + D2H inside the timed region) -------
+    g2 = B.Chisao(wl, device=dev)
+    x_host = torch.from_numpy(np.ascontiguousarray(wl.x0, np.float32)).pin_memory()
+    x_out = torch.empty_like(x_host).pin_memory()
+    f_out = torch.empty(hp.N, dtype=torch.float32).pin_memory()
+    s_out = torch.empty(hp.N, dtype=torch.uint8).pin_memory()
+    for _ in range(W):
+        g2.step_host(x_host, x_out, f_out, s_out)
+        x_host.copy_(x_out)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        g2.step_host(x_host, x_out, f_out, s_out)           # synchronises before returning
+        x_host.copy_(x_out)
+    e2e_s = time.perf_counter() - t0
+    e2e_s = replicas.max_over_ranks(e2e_s, dist if world > 1 else None, dev)
+    g2.close()
+
+    # ---- roofline of the dominant kernel (k_eval_fd: objective evaluation + FD stencil) -------------------
+    peaks, peaks_src = measured_peaks()
+    fpe = flop_per_eval(wl.obj)
+    fd_evals = float(evals[0] - K * hp.N + evals[2] + evals[6])     # counter 0 also holds the N centre values
+    fd_ms, fd_n = phase_ms["eval_fd"]
+    alu_peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12   # TFLOP/s, FP32 FMA lanes x clock
+    achieved = fd_evals * fpe / (fd_ms * 1e-3) / 1e12 if fd_ms > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "k_eval_fd", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": achieved / alu_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(c),
+                "peak_source": f"148 SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json clocks)",
+                "launches": fd_n, "ms_per_launch": fd_ms / max(fd_n, 1), "flop_per_eval": fpe,
+                "share_of_step": fd_ms / ms if ms > 0 else None}
+    # HBM-bound history kernel (two-loop recursion over the spilled (s, y) pairs)
+    dir_ms, dir_n = phase_ms["lbfgs_direction"]
+    hist_bytes = K * hp.n_conv * hp.N * (2 * hp.lbfgs_m * hp.d + 5 * hp.d) * 4.0   # upper bound: full history
+    hbm = {"kernel": "k_lbfgs_direction", "achieved_gbs_upper": hist_bytes / (dir_ms * 1e-3) / 1e9 if dir_ms > 0 else 0.0,
+           "peak_gbs": peaks["hbm_gbs"], "ms_per_launch": dir_ms / max(dir_n, 1)}
+
+    if rank == 0:
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            cpu, _ = oracle_throughput(c, 1, 0)
+            cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "f_evals_per_sec")}
+        value = world * hp.N * K / (ms_max * 1e-3)
+        bi = hp.N * hp.d * 4
+        bo = hp.N * hp.d * 4 + hp.N * 4 + hp.N
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOAD_TEXT[c], "N_per_gpu": hp.N, "d": hp.d, "n_conv": hp.n_conv, "lbfgs_m": hp.lbfgs_m,
+                       "hlc_M": hp.hlc_M, "n_cloud": hp.n_cloud, "n_anti": hp.n_anti, "fd_h": hp.fd_h,
+                       "parallelism": "replicas" if world > 1 else "single",
+                       "l2": f"state per cycle {g.workspace_bytes / 2**20:.0f} MiB vs 126 MB L2: "
+                             + ("inputs larger than L2" if g.workspace_bytes > 126e6 else "fits L2 (latency-bound config)")},
+            "f_evals_per_sec": total_evals / (ms_max * 1e-3),
+            "evals_per_step": float(evals.sum()) / K,
+            "clocks": clocks,
+            "e2e": {"value": world * hp.N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo},
+            "gpu_launches": int(launches),
+            "roofline": roofline, "hbm_kernel": hbm,
+            "phase_ms_per_step": {k: round(v[0] / K, 4) for k, v in phase_ms.items()},
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per k_eval_fd launch from the committed `ncu --set full`
+# capture (profiles/); None until a capture of that workload exists.
+TRAFFIC_BYTES_PER_LAUNCH = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--N", type=int, default=0, help="override the population size (parity/debug runs only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3
+        run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

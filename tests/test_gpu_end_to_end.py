@@ -1,0 +1,243 @@
+"""End-to-end and edge-case tests of the CUDA path through the C ABI (free-running cycles, mode sets,
+invariants at any size, degenerate inputs, error behaviour)."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+from paper_2606_26164_b200 import inputs
+
+import parity as PT
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_26164_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _run_both(orc, B, wl, cycles=None):
+    o, g = orc.Oracle(wl, threads=8), B.Chisao(wl)
+    hist = []
+    for _ in range(cycles or wl.hp.n_osc):
+        so, sg = o.step(), g.step()
+        hist.append((so, sg))
+    return o, g, hist
+
+
+def test_c1_full_run_recovers_the_oracles_mode_set(orc, B):
+    """C1 (BASELINE.json configs[0]) complete: same mode set, matched modes within 1e-3 L2 (north_star)."""
+    wl = inputs.config(1)
+    o, g, hist = _run_both(orc, B, wl)
+    xo, fo, _ = o.modes()
+    xg, fg, ig, n = g.modes()
+    assert n == len(fo) and n >= 1
+    assert PT.match_modes(xg, xo, 1e-3) == n
+    assert np.all(np.abs(np.sort(fg.astype(np.float64)) - np.sort(fo)) <= 1e-4)
+    assert np.all(np.diff(fg) <= 0)                                     # sorted by f descending
+    for so, sg in hist:
+        assert sg.n_stuck == so.n_stuck and sg.reseed_strategy == so.reseed_strategy
+    with pytest.raises(B.ChisaoError) as ei:                            # step past n_osc
+        g.step()
+    assert ei.value.code == B.E_STATE
+
+
+@pytest.mark.parametrize("c,N,cycles,tol", [(2, 1024, 6, 1e-3), (5, 256, 4, 1e-3)])
+def test_noise_free_mixtures_recover_the_same_modes(orc, B, c, N, cycles, tol):
+    """C2 / C5 with sigma_noise = 0 at reduced N (R-14): every mode of one side has a partner on the
+    other within 1e-3 L2 after the final cycle; noise-free thresholds follow the fp32 FD floor."""
+    over = dict(eps_grad=5e-2, eps_dup=1e-2, log_delta=float(np.log(1e-3))) if c == 2 else \
+        dict(eps_grad=5e-2, eps_dup=1e-2, log_delta=-30.0, n_conv=40)
+    wl = inputs.config(c, N=N, n_osc=cycles, noise=0.0, **over)
+    o, g, hist = _run_both(orc, B, wl)
+    xo, fo, _ = o.modes()
+    xg, fg, _, n = g.modes()
+    assert n >= 1 and len(fo) >= 1
+    both = PT.match_modes(xg, xo, tol)
+    assert both >= 0.9 * max(n, len(fo)), (both, n, len(fo))
+
+
+def test_c4_side_run_unimodal_collapses_to_the_maximiser(orc, B):
+    """Remark 1 on the ill-conditioned quadratic: with enough iterations every sample sticks at c
+    and deduplication leaves one mode (C4 side run of DESIGN.md: d = 64 bowl, N = 256, n_conv = 300)."""
+    wl = inputs.config(4, N=256, n_osc=1, n_conv=300, eps_grad=0.5, eps_dup=0.05)
+    g = B.Chisao(wl)
+    st = g.step()
+    xg, fg, _, n = g.modes()
+    assert st.n_stuck == 1 and st.k_lost == 255 and n == 1
+    assert np.linalg.norm(xg[0] - wl.obj.truth["c"]) < 5e-2
+    assert abs(fg[0]) < 1e-2
+
+
+@pytest.mark.parametrize("c,N", [(2, 4096), (3, 1000), (5, 515)])
+def test_invariants_over_free_running_cycles(B, c, N):
+    """GPU alone, every cycle: N conserved and inside Theta, frozen rows bit-identical across phases 5-6,
+    survivors pairwise >= eps_dup apart, counters follow the Eq. 8 structure, no NaN."""
+    wl = inputs.config(c, N=N, n_osc=4)
+    hp = wl.hp
+    g = B.Chisao(wl)
+    prev_ev = np.zeros(8, np.int64)
+    for k in range(1, 5):
+        g.set(B.CTRL, [k, 1, 0, 0, 0, 0, 0, 0])
+        g.phase(B.PH_RELEASE_EVAL)
+        for it in range(1, hp.n_conv + 1):
+            g.phase(B.PH_LBFGS_ITER, it)
+        g.phase(B.PH_STICK); g.phase(B.PH_DEDUP)
+        st = g.stats()
+        stuck = g.get(B.STUCK).astype(bool); removed = g.get(B.REMOVED).astype(bool)
+        assert st.n_stuck == stuck.sum() and st.k_lost == removed.sum() and not (stuck & removed).any()
+        assert st.n_stuck + st.k_lost + st.n_active == N
+        x = g.get(B.X)
+        surv = x[stuck].astype(np.float64)
+        if 1 < len(surv) <= 3000:
+            D = np.max(np.abs(surv[:, None, :] - surv[None, :, :]), axis=2) + 1e9 * np.eye(len(surv))
+            assert D.min() >= hp.eps_dup * (1 - 1e-6)
+        ev = np.array(st.evals[:], np.int64)
+        assert ev[0] - prev_ev[0] == N * (2 * hp.d + 1)
+        assert (ev[2] - prev_ev[2]) % (2 * hp.d) == 0 and ev[2] - prev_ev[2] <= N * hp.n_conv * 2 * hp.d
+        assert ev[1] - prev_ev[1] >= (ev[2] - prev_ev[2]) // (2 * hp.d)     # >= one trial per accepted step
+        g.phase(B.PH_RESEED)
+        st2 = g.stats()
+        assert not g.get(B.REMOVED).any() and st2.n_active == N - st2.n_stuck
+        frozen = g.get(B.STUCK).astype(bool)
+        xf = g.get(B.X)[frozen].copy()
+        for t in range(1, hp.n_cloud + 1):
+            g.phase(B.PH_HLC_STEP, t)
+        for t in range(1, hp.n_anti + 1):
+            g.phase(B.PH_ANTI_STEP, t)
+        x = g.get(B.X)
+        assert np.array_equal(x[frozen], xf)                                # frozen samples never move
+        assert np.isfinite(x).all() and np.all(x >= hp.lo[None, :]) and np.all(x <= hp.hi[None, :])
+        st3 = g.stats()
+        ev3 = np.array(st3.evals[:], np.int64)
+        assert ev3[5] - prev_ev[5] == hp.n_cloud * hp.hlc_M * (N - st2.n_stuck)
+        assert ev3[6] - prev_ev[6] == hp.n_anti * 2 * hp.d * (N - st2.n_stuck)
+        prev_ev = ev3
+
+
+@pytest.mark.parametrize("d,N,M,m", [(1, 5, 1, 1), (3, 257, 7, 3), (5, 1, 10, 16), (7, 300, 256, 2), (33, 129, 9, 5), (64, 3, 33, 10)])
+def test_ragged_and_degenerate_shapes_match_the_oracle(orc, B, d, N, M, m):
+    """odd d (scalar row loads), d not a multiple of 4, single sample, M = 1 and M = 256, m = 1 and m = 16."""
+    obj = inputs.gmm_diag(d, 3, 2.0, 40 + d) if d != 33 else inputs.rff(d, 37, 41)
+    wl = inputs.custom(obj, 3.0, N, seed=90 + d, hlc_M=M, lbfgs_m=m, n_conv=4, fd_h=1e-2, eps_grad=1e-3, n_osc=2,
+                       hlc_baseline=1)
+    o, g = orc.Oracle(wl), B.Chisao(wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL)
+    for it in range(1, 5):
+        PT.sync_oracle_to_gpu(o, g, orc, B)
+        o.phase(orc.PH_LBFGS_ITER, it); g.phase(B.PH_LBFGS_ITER, it)
+        safe = (o.get(orc.LS_MARGIN) > PT.LS_MARGIN_MIN) & (o.get(orc.ASC_MARGIN) > PT.REL_MARGIN_MIN)
+        assert np.array_equal(g.get(B.LS_B)[safe], o.get(orc.LS_B)[safe])
+        xo = o.get(orc.X)
+        assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1)[safe] <= PT.x_tol(xo, wl.hp.lo, wl.hp.hi)[safe])
+    PT.sync_oracle_to_gpu(o, g, orc, B)
+    o.phase(orc.PH_HLC_STEP, 1); g.phase(B.PH_HLC_STEP, 1)
+    fo = o.get(orc.HLC_F)
+    assert np.all(np.abs(g.get(B.HLC_F) - fo) <= PT.F_REL * np.maximum(np.abs(fo), 1.0))
+    PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+    o.phase(orc.PH_ANTI_STEP, 1); g.phase(B.PH_ANTI_STEP, 1)
+    xo = o.get(orc.X)
+    assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1) <= 10 * PT.x_tol(xo, wl.hp.lo, wl.hp.hi))
+
+
+def test_empty_population(B):
+    wl = inputs.custom(inputs.gmm_iso(2, 2, 0.3, 1.0, 3), 2.0, 0, n_osc=2)
+    g = B.Chisao(wl)
+    st = g.step()
+    assert (st.n_stuck, st.k_lost, st.n_active) == (0, 0, 0) and st.f_max == -np.inf
+    xg, fg, ig, n = g.modes()
+    assert n == 0
+    g.step()
+
+
+def test_nonfinite_values_cannot_stick_and_are_rejected(B):
+    """R-12: a non-finite f or g never sticks; trials with non-finite values are rejected."""
+    wl = inputs.custom(inputs.gmm_iso(2, 2, 0.3, 1.0, 3), 2.0, 64, eps_grad=1.0)
+    g = B.Chisao(wl)
+    f = np.zeros(64, np.float32); f[3] = np.nan; f[5] = np.inf; f[7] = -np.inf
+    gr = np.zeros((64, 2), np.float32); gr[9, 1] = np.nan
+    g.set(B.F, f); g.set(B.G, gr)
+    g.phase(B.PH_STICK)
+    stuck = g.get(B.STUCK)
+    assert not stuck[[3, 5, 7, 9]].any() and stuck.sum() == 60
+    assert g.stats().f_max == 0.0
+
+
+def test_seed_population_is_the_philox_uniform_stream(orc, B):
+    """chisao_seed_population: x_ij = lo + U (hi - lo) with U the j-th uniform of stream (sample i, cycle 0,
+    tag INIT); both sides implement the same counter-based generator (R-15)."""
+    wl = inputs.custom(inputs.gmm_iso(5, 2, 0.3, 1.0, 3), 2.0, 300, seed=1234)
+    g = B.Chisao(wl, seed_population=True)
+    x = g.get(B.X).astype(np.float64)
+    assert np.all(x >= -2.0) and np.all(x <= 2.0)
+    tag = orc.tag(0, 0, 0)
+    for i in (0, 1, 17, 299):
+        for j in range(5):
+            u = orc.uniform(1234, i, 0, tag, j)
+            assert abs(x[i, j] - (-2.0 + 4.0 * u)) <= 4 * PT.EPS32 * 2.0
+    assert abs(x.mean()) < 0.1 and abs(x.std() - 4.0 / np.sqrt(12.0)) < 0.05
+    g2 = B.Chisao(wl, seed_population=True)
+    assert np.array_equal(g2.get(B.X), g.get(B.X))                         # deterministic
+
+
+def test_state_round_trip_and_history_order(B):
+    wl = inputs.config(2, N=100)
+    g = B.Chisao(wl)
+    rng = np.random.default_rng(0)
+    m, N, d = wl.hp.lbfgs_m, 100, wl.hp.d
+    for fld, shape, dt in ((B.X, (N, d), np.float32), (B.G, (N, d), np.float32), (B.V, (N, d), np.float32),
+                           (B.F, (N,), np.float32), (B.HIST_LEN, (N,), np.int32), (B.STUCK, (N,), np.uint8)):
+        a = (rng.integers(0, m + 1, size=shape) if dt != np.float32 else rng.standard_normal(shape)).astype(dt)
+        if fld == B.STUCK:
+            a = (a > 0).astype(np.uint8)
+        g.set(fld, a)
+        assert np.array_equal(g.get(fld), a)
+    S = rng.standard_normal((m, N, d)).astype(np.float32)
+    g.set(B.HIST_S, S); g.set(B.HIST_Y, 2 * S)
+    ln = g.get(B.HIST_LEN)
+    Sg, Yg = g.get(B.HIST_S), g.get(B.HIST_Y)
+    for i in (0, 5, 99):
+        assert np.array_equal(Sg[:ln[i], i], S[:ln[i], i]) and np.array_equal(Yg[:ln[i], i], 2 * S[:ln[i], i])
+        assert not Sg[ln[i]:, i].any()
+    with pytest.raises(B.ChisaoError) as ei:
+        g._ck(g._L.chisao_get_state(g._h, B.X, S.ctypes.data, 12))
+    assert ei.value.code == B.E_INVALID
+
+
+def test_argument_errors(B):
+    L = B.load_library()
+    wl = inputs.config(1)
+    for field, bad in (("d", 65), ("lbfgs_m", 17), ("hlc_M", 257), ("N", -1), ("fd_h", 0.0)):
+        cfg, obj, keep = B.marshal(wl)
+        setattr(cfg, field, bad)
+        if field == "d":
+            obj.d = bad
+        n = C.c_size_t(0)
+        assert L.chisao_workspace_bytes(C.byref(cfg), C.byref(obj), C.byref(n)) == B.E_INVALID
+        assert L.chisao_last_error(None)
+    cfg, obj, keep = B.marshal(wl)
+    h = C.c_void_p(None)
+    assert L.chisao_init(C.byref(h), C.byref(cfg), C.byref(obj), None, None, 0, None) in (B.E_INVALID, B.E_WORKSPACE)
+    g = B.Chisao(wl)
+    st = g.step()
+    x, f, idx, n = g.modes(cap=1)
+    assert len(f) <= 1 and n == st.n_stuck
+    with pytest.raises(B.ChisaoError):
+        g.phase(99)
+
+
+def test_step_host_matches_device_resident_step(B):
+    """chisao_step_host (host buffers in, host buffers out) runs the same cycle as chisao_step."""
+    wl = inputs.config(2, N=512, n_osc=3)
+    a, b = B.Chisao(wl), B.Chisao(wl)
+    x_in = np.ascontiguousarray(wl.x0, np.float32)
+    x_out = np.empty_like(x_in); f_out = np.empty(512, np.float32); s_out = np.empty(512, np.uint8)
+    sa = a.step()
+    sb = b.step_host(x_in, x_out, f_out, s_out, stats=True)
+    assert np.array_equal(x_out, a.get(B.X)) and np.array_equal(f_out, a.get(B.F)) and np.array_equal(s_out, a.get(B.STUCK))
+    assert (sa.n_stuck, sa.k_lost, sa.n_active) == (sb.n_stuck, sb.k_lost, sb.n_active)
+    assert list(sa.evals) == list(sb.evals)

@@ -1,0 +1,279 @@
+"""GPU <-> oracle parity, teacher-forced per phase; all calls go through
+the C ABI (paper_2606_26164_b200.binding -> libchisao.so).  Sizes span several 256-point tiles and a ragged
+tail; C1..C5 are BASELINE.json's configs at reduced N (the full-size checks are in test_gpu_fullsize.py)."""
+import numpy as np
+import pytest
+
+from paper_2606_26164_b200 import inputs
+
+import parity as PT
+
+pytestmark = pytest.mark.gpu
+
+CASES = [(1, 256), (2, 777), (3, 300), (4, 261), (5, 200)]
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_26164_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _pair(orc, B, wl):
+    return orc.Oracle(wl, threads=8), B.Chisao(wl)
+
+
+@pytest.mark.parametrize("c,N", CASES)
+def test_a1_eval_and_fd_gradient(orc, B, c, N):
+    """a1: f within 1e-5 relative, FD gradient within 1e-3 relative + fp32 floor (north_star)."""
+    wl = inputs.config(c, N=N)
+    o, g = _pair(orc, B, wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0]); g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL); g.phase(B.PH_RELEASE_EVAL)
+    fo, fg = o.get(orc.F), g.get(B.F).astype(np.float64)
+    assert np.all(np.abs(fg - fo) <= PT.f_tol(fo)), float(np.max(np.abs(fg - fo) / np.maximum(np.abs(fo), 1)))
+    ok, err, tol = PT.grad_ok(g.get(B.G).astype(np.float64), o.get(orc.G), fo, wl.hp.fd_h, wl.obj.sigma_noise)
+    assert np.all(ok), (float(np.max(err / tol)), int(np.sum(~ok)))
+    # release: flags and history cleared; evaluation counter = N (2d + 1)   (Eq. 8 structure)
+    assert not g.get(B.STUCK).any() and not g.get(B.HIST_LEN).any()
+    assert g.stats().evals[0] == N * (2 * wl.hp.d + 1) == o.stats().evals[0]
+
+
+@pytest.mark.parametrize("c,N", CASES)
+def test_a2_lbfgs_iterations_teacher_forced(orc, B, c, N):
+    """a2: direction, accepted trial, updated position, curvature pair, history bookkeeping, per iteration."""
+    wl = inputs.config(c, N=N)
+    hp = wl.hp
+    o, g = _pair(orc, B, wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL)
+    n_dec = n_excl = 0
+    for it in range(1, min(hp.n_conv, 8) + 1):
+        PT.sync_oracle_to_gpu(o, g, orc, B)
+        x0 = o.get(orc.X).copy(); len0 = o.get(orc.HIST_LEN).copy(); f0 = o.get(orc.F).copy()
+        o.phase(orc.PH_LBFGS_ITER, it); g.phase(B.PH_LBFGS_ITER, it)
+        bo, bg = o.get(orc.LS_B), g.get(B.LS_B)
+        po, pg = o.get(orc.P), g.get(B.P).astype(np.float64)
+        active = bo != -2
+        assert np.array_equal(bg == -2, ~active)           # skip decisions (Eq. 3 gradient test on equal inputs)
+        # direction: ||dp||_2 <= 1e-4 ||p||_2 wherever the ascent test is not marginal
+        safe_dir = active & (o.get(orc.ASC_MARGIN) > PT.REL_MARGIN_MIN)
+        dn = np.linalg.norm(pg - po, axis=1); pn = np.linalg.norm(po, axis=1)
+        assert np.all(dn[safe_dir] <= 1e-4 * pn[safe_dir] + 1e-30), float(np.max(dn[safe_dir] / (pn[safe_dir] + 1e-30)))
+        # accepted trial index: exact away from the Armijo threshold
+        safe = safe_dir & (o.get(orc.LS_MARGIN) > PT.LS_MARGIN_MIN)
+        n_dec += int(active.sum()); n_excl += int((active & ~safe).sum())
+        assert np.array_equal(bg[safe], bo[safe]), int(np.sum(bg[safe] != bo[safe]))
+        # updated position (rule 4) and value
+        xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
+        tol = PT.x_tol(xo, hp.lo, hp.hi)
+        ex = np.max(np.abs(xg - xo), axis=1)
+        assert np.all(ex[safe] <= tol[safe]), float(np.max(ex[safe] / tol[safe]))
+        assert np.array_equal(xg[~active], x0[~active])
+        fo, fg = o.get(orc.F), g.get(B.F).astype(np.float64)
+        acc = safe & (bo >= 0)
+        assert np.all(np.abs(fg - fo)[acc] <= 2 * PT.f_tol(fo)[acc])
+        assert np.array_equal(fg[safe & (bo < 0)], f0[safe & (bo < 0)])
+        # new gradient at the accepted point
+        ok, err, gtol = PT.grad_ok(g.get(B.G).astype(np.float64), o.get(orc.G), fo, hp.fd_h, wl.obj.sigma_noise)
+        assert np.all(ok[acc]), float(np.max(err[acc] / gtol[acc]))
+        # history: length exact away from the curvature threshold; newest pair values
+        safe_h = acc & (o.get(orc.CURV_MARGIN) > PT.REL_MARGIN_MIN)
+        lo_, lg_ = o.get(orc.HIST_LEN), g.get(B.HIST_LEN)
+        assert np.array_equal(lg_[safe_h], lo_[safe_h])
+        assert np.array_equal(lg_[safe & (bo < 0)], lo_[safe & (bo < 0)])
+        So, Sg = o.get(orc.HIST_S), g.get(B.HIST_S).astype(np.float64)
+        Yo, Yg = o.get(orc.HIST_Y), g.get(B.HIST_Y).astype(np.float64)
+        rows = np.nonzero(safe_h & (lo_ > 0))[0]
+        if len(rows):
+            newest = lo_[rows] - 1
+            so, sg = So[newest, rows], Sg[newest, rows]
+            yo, yg = Yo[newest, rows], Yg[newest, rows]
+            assert np.all(np.max(np.abs(sg - so), axis=1) <= 2 * tol[rows])
+            ytol = PT.G_REL * np.max(np.abs(yo), axis=1) + 2 * gtol[rows] + 2e-3 * np.max(np.abs(o.get(orc.G)[rows]), axis=1)
+            assert np.all(np.max(np.abs(yg - yo), axis=1) <= ytol)
+        assert np.array_equal(g.get(B.STALLED)[safe], o.get(orc.STALLED)[safe])
+        assert np.all(len0[~active] == lg_[~active])
+    assert n_excl <= max(2, PT.MAX_EXCLUDED_FRACTION * 4 * n_dec), (n_excl, n_dec)
+
+
+def _converged_pair(orc, B, wl, n_conv=None):
+    o, g = _pair(orc, B, wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL)
+    for it in range(1, (n_conv or wl.hp.n_conv) + 1):
+        o.phase(orc.PH_LBFGS_ITER, it)
+    return o, g
+
+
+@pytest.mark.parametrize("c,N,n_conv", [(1, 256, 20), (2, 777, 10), (5, 200, 18), (4, 130, 5)])
+def test_a3_stick_and_a4_dedup(orc, B, c, N, n_conv):
+    """a3: f_max, Eq. 3 flags exact away from the thresholds; a4: Eq. 4 removed mask, K_lost, counts."""
+    wl = inputs.config(c, N=N)
+    hp = wl.hp
+    o, g = _converged_pair(orc, B, wl, n_conv)
+    PT.sync_oracle_to_gpu(o, g, orc, B)
+    o.phase(orc.PH_STICK); g.phase(B.PH_STICK)
+    so, sg = o.stats(), g.stats()
+    assert abs(sg.f_max - so.f_max) <= 1e-5 * max(abs(so.f_max), 1.0)
+    fo, go = o.get(orc.F), o.get(orc.G)
+    ginf = np.max(np.abs(go), axis=1)
+    thr = so.f_max + hp.log_delta
+    near = (np.abs(ginf - hp.eps_grad) <= 1e-6 * ginf) | (np.abs(fo - thr) <= 2e-5 * np.maximum(np.abs(fo), 1.0))
+    assert near.sum() <= max(2, 0.005 * N)
+    assert np.array_equal(g.get(B.STUCK)[~near], o.get(orc.STUCK)[~near])
+    if not near.any():
+        assert (sg.n_stuck, sg.k_lost, sg.n_active) == (so.n_stuck, so.k_lost, so.n_active)
+    # dedup from identical flags
+    g.set(B.STUCK, o.get(orc.STUCK))
+    o.phase(orc.PH_DEDUP); g.phase(B.PH_DEDUP)
+    so, sg = o.stats(), g.stats()
+    x = o.get(orc.X); st0 = (o.get(orc.STUCK) | o.get(orc.REMOVED)).astype(bool)
+    # pairs whose L-inf distance is within fp32 rounding of eps_dup are not required to agree
+    idx = np.nonzero(st0)[0]
+    amb = np.zeros(N, bool)
+    if len(idx):
+        D = np.max(np.abs(x[idx][:, None, :] - x[idx][None, :, :]), axis=2)
+        amb[idx] = np.any(np.abs(D - hp.eps_dup) <= 1e-6 * max(1.0, float(np.abs(x).max())), axis=1)
+    assert np.array_equal(g.get(B.REMOVED)[~amb], o.get(orc.REMOVED)[~amb])
+    assert np.array_equal(g.get(B.STUCK)[~amb], o.get(orc.STUCK)[~amb])
+    if not amb.any():
+        assert (sg.n_stuck, sg.k_lost, sg.n_active) == (so.n_stuck, so.k_lost, so.n_active)
+        assert sg.n_stuck + sg.k_lost == int(st0.sum())
+
+
+def test_a4_dedup_many_duplicates_and_ties(orc, B):
+    """dense duplicate clusters, exact f ties (lower index survives), phase mask off removes nothing (R-7)."""
+    obj = inputs.gmm_iso(3, 2, 0.5, 2.0, 5)
+    wl = inputs.custom(obj, 3.0, 1500, eps_dup=0.05, eps_grad=1.0)
+    o, g = _pair(orc, B, wl)
+    rng = np.random.default_rng(3)
+    centres = rng.uniform(-2.5, 2.5, size=(12, 3))
+    x = PT.f32(centres[rng.integers(0, 12, 1500)] + rng.uniform(-0.02, 0.02, size=(1500, 3)))
+    f = PT.f32(np.round(rng.standard_normal(1500), 1))          # many exact ties
+    stuck = (rng.uniform(size=1500) < 0.8).astype(np.uint8)
+    for fld_o, fld_g, val in ((orc.X, B.X, x), (orc.F, B.F, f), (orc.STUCK, B.STUCK, stuck)):
+        o.set(fld_o, val); g.set(fld_g, val)
+    o.phase(orc.PH_DEDUP); g.phase(B.PH_DEDUP)
+    assert np.array_equal(g.get(B.REMOVED), o.get(orc.REMOVED))
+    assert np.array_equal(g.get(B.STUCK), o.get(orc.STUCK))
+    so, sg = o.stats(), g.stats()
+    assert (sg.n_stuck, sg.k_lost, sg.n_active) == (so.n_stuck, so.k_lost, so.n_active)
+    assert sg.k_lost > 500
+    # survivors are pairwise >= eps_dup apart (invariant) and a second application removes nothing
+    surv = x[g.get(B.STUCK).astype(bool)]
+    D = np.max(np.abs(surv[:, None, :] - surv[None, :, :]), axis=2) + np.eye(len(surv))
+    assert D.min() >= 0.05
+    g.phase(B.PH_DEDUP)
+    assert g.stats().k_lost == 0
+
+
+@pytest.mark.parametrize("strategy", [1, 2, 3])
+def test_a5_reseed_via_dedup(orc, B, strategy):
+    """a5 through the real pipeline: a crafted stuck set with duplicates -> DEDUP -> RESEED on both sides."""
+    obj = inputs.gmm_diag(8, 16, 5.0, 1002)
+    wl = inputs.custom(obj, 5.0, 640, eps_dup=0.05, eps_grad=1.0, reseed_cands=4, seed=77)
+    hp = wl.hp
+    o, g = _pair(orc, B, wl)
+    N, d = 640, 8
+    rng = np.random.default_rng(20 + strategy)
+    centres = rng.uniform(-4.5, 4.5, size=(25, d))
+    x = PT.f32(rng.uniform(-5, 5, size=(N, d)))
+    stuck = np.zeros(N, np.uint8)
+    n_dup = 200 if strategy == 1 else N - 3
+    dup = rng.choice(N, n_dup, replace=False)
+    x[dup] = PT.f32(centres[rng.integers(0, 25, n_dup)] + rng.uniform(-0.01, 0.01, size=(n_dup, d)))
+    stuck[dup] = 1
+    f = PT.f32(rng.standard_normal(N))
+    ctrl = [2, 1 if strategy != 3 else 0, 0, 0, 0, 0, int(stuck.sum()), N - int(stuck.sum())]
+    for fo, fg, val in ((orc.X, B.X, x), (orc.F, B.F, f), (orc.STUCK, B.STUCK, stuck), (orc.CTRL, B.CTRL, ctrl)):
+        o.set(fo, val); g.set(fg, val)
+    g.set(B.V, np.ones((N, d), np.float32)); o.set(orc.V, np.ones((N, d)))
+    g.set(B.HIST_LEN, np.full(N, 2, np.int32)); o.set(orc.HIST_LEN, np.full(N, 2, np.int32))
+    o.phase(orc.PH_DEDUP); g.phase(B.PH_DEDUP)
+    removed = o.get(orc.REMOVED).astype(bool)
+    assert np.array_equal(g.get(B.REMOVED).astype(bool), removed)
+    o.phase(orc.PH_RESEED); g.phase(B.PH_RESEED)
+    so, sg = o.stats(), g.stats()
+    assert sg.reseed_strategy == so.reseed_strategy == strategy
+    assert (sg.n_stuck, sg.k_lost, sg.n_active) == (so.n_stuck, so.k_lost, so.n_active)
+    src_o, src_g = o.get(orc.RS_SRC), g.get(B.RS_SRC)
+    assert np.array_equal(src_g, src_o)
+    if strategy == 1:
+        safe = removed & (o.get(orc.RS_MARGIN) > 1e-5)
+        assert safe.sum() >= 0.99 * removed.sum()
+    else:
+        safe = removed
+    assert np.array_equal(g.get(B.RS_CAND)[safe], o.get(orc.RS_CAND)[safe])
+    xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
+    tol = PT.x_tol(xo, hp.lo, hp.hi)
+    assert np.all(np.max(np.abs(xg - xo), axis=1)[safe] <= tol[safe])
+    assert np.array_equal(xg[~removed], x[~removed])                       # nobody else moves
+    assert np.all(xg >= hp.lo[None, :]) and np.all(xg <= hp.hi[None, :])   # inside Theta
+    assert not g.get(B.REMOVED).any() and not g.get(B.STUCK)[removed].any()  # "marked as unstuck" PAPER.md:111
+    assert not g.get(B.HIST_LEN)[removed].any() and not g.get(B.V)[removed].any()
+    assert np.all(g.get(B.HIST_LEN)[~removed] == 2)
+    if strategy == 2:
+        Q = g.get(B.GR_Q).astype(np.float64)
+        assert np.allclose(Q.T @ Q, np.eye(d), atol=5e-6)
+        assert np.allclose(Q, o.gr_basis(2), atol=2e-5)
+
+
+@pytest.mark.parametrize("c,N,baseline", [(1, 256, 1), (2, 500, 1), (3, 300, 1), (4, 140, 1), (5, 150, 1), (2, 300, 0)])
+def test_a6_hlc_step(orc, B, c, N, baseline):
+    """a6: every f_k within 1e-5 relative, ghat within 1e-3 relative + floor, x by rule 4; stuck rows frozen."""
+    wl = inputs.config(c, N=N, hlc_baseline=baseline)
+    hp = wl.hp
+    o, g = _converged_pair(orc, B, wl, 3)
+    o.phase(orc.PH_STICK)
+    stuck = o.get(orc.STUCK).copy(); stuck[::7] = 1            # make sure some rows are frozen
+    o.set(orc.STUCK, stuck)
+    for t in (1, 2):
+        PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+        x0 = o.get(orc.X).copy()
+        o.phase(orc.PH_HLC_STEP, t); g.phase(B.PH_HLC_STEP, t)
+        act = stuck == 0
+        fo, fg = o.get(orc.HLC_F), g.get(B.HLC_F).astype(np.float64)
+        assert np.all(np.abs(fg - fo)[act] <= PT.F_REL * np.maximum(np.abs(fo[act]), 1.0))
+        gho, ghg = o.get(orc.GHAT), g.get(B.GHAT).astype(np.float64)
+        u_inf = 5.5
+        floor = 8 * PT.EPS32 * np.max(np.abs(fo), axis=1) * u_inf / hp.sigma_s
+        err = np.max(np.abs(ghg - gho), axis=1)
+        tol = PT.G_REL * np.max(np.abs(gho), axis=1) + floor
+        assert np.all(err[act] <= tol[act]), float(np.max(err[act] / tol[act]))
+        xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
+        step = np.max(np.abs(xo - x0), axis=1)
+        xt = PT.x_tol(xo, hp.lo, hp.hi, step, grad_inside=True) + hp.eta_hlc * floor
+        assert np.all(np.max(np.abs(xg - xo), axis=1)[act] <= xt[act])
+        assert np.array_equal(xg[~act], x0[~act])              # frozen rows bit-identical
+    assert g.stats().evals[5] == 2 * int((stuck == 0).sum()) * hp.hlc_M
+
+
+@pytest.mark.parametrize("c,N", [(1, 256), (2, 500), (3, 300), (4, 140), (5, 150)])
+def test_a7_anti_convergence_step(orc, B, c, N):
+    """a7: Eq. 6 with the FD gradient computed inside the unit; v and x; stuck rows frozen."""
+    wl = inputs.config(c, N=N)
+    hp = wl.hp
+    o, g = _converged_pair(orc, B, wl, 3)
+    o.phase(orc.PH_STICK)
+    stuck = o.get(orc.STUCK).copy(); stuck[::5] = 1
+    o.set(orc.STUCK, stuck)
+    act = stuck == 0
+    for t in (1, 2, 3):
+        PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+        x0 = o.get(orc.X).copy(); v0 = o.get(orc.V).copy()
+        o.phase(orc.PH_ANTI_STEP, t); g.phase(B.PH_ANTI_STEP, t)
+        vo, vg = o.get(orc.V), g.get(B.V).astype(np.float64)
+        xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
+        # the gradient inside the step: recover it from the oracle's update for the tolerance
+        vprev = np.zeros_like(v0) if t == 1 else v0
+        g_used = (hp.mu * vprev - vo) / hp.alpha_anti
+        f_here = np.abs(o.get(orc.F))
+        floor = PT.fd_floor(f_here, hp.fd_h, wl.obj.sigma_noise) * 4
+        vtol = hp.alpha_anti * (PT.G_REL * np.max(np.abs(g_used), axis=1) + floor) + 4 * PT.EPS32 * np.max(np.abs(vo), axis=1)
+        assert np.all(np.max(np.abs(vg - vo), axis=1)[act] <= vtol[act]), float(np.max((np.max(np.abs(vg - vo), axis=1) / vtol)[act]))
+        xt = PT.x_tol(xo, hp.lo, hp.hi) + vtol
+        assert np.all(np.max(np.abs(xg - xo), axis=1)[act] <= xt[act])
+        assert np.array_equal(xg[~act], x0[~act])              # "Stuck samples are excluded" PAPER.md:129
+    assert g.stats().evals[6] == 3 * int(act.sum()) * 2 * hp.d
