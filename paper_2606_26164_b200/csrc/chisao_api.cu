@@ -155,8 +155,11 @@ void pack_records(const chisao_objective &o, int DP, std::vector<float> &out, fl
         r[DP * DP + DP] = (o.id == CHISAO_OBJ_GMM_FULL) ? o.vec_a[k] : 0.0f;
         break;
       case CHISAO_OBJ_RFF:
-        for (int j = 0; j < d; ++j) r[j] = o.mats[(size_t)k * d + j];
-        r[DP] = o.vec_a[k]; r[DP + 1] = o.vec_b[k];
+        for (int j = 0; j < d; ++j) {   // exact promotion of the fp32 frequencies to fp64
+          const double w = (double)o.mats[(size_t)k * d + j];
+          std::memcpy(r + 2 * j, &w, sizeof(double));
+        }
+        r[2 * DP] = o.vec_a[k]; r[2 * DP + 1] = o.vec_b[k];
         break;
     }
   }

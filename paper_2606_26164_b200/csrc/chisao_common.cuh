@@ -39,7 +39,7 @@ struct Ctrl {
 //   GMM_ISO : mu[DP] | a, 0, 0, 0                       s0 = 1/(2 sigma^2)
 //   GMM_DIAG: mu[DP] | inv[DP] | a, 0, 0, 0
 //   GMM_FULL: W[DP][DP] | mu[DP] | a, 0, 0, 0
-//   RFF     : w[DP] | a, b, 0, 0                         s0 = quadratic coefficient
+//   RFF     : w[DP] as fp64 (2 DP floats) | a, b, 0, 0    s0 = quadratic coefficient
 //   QUAD    : W[DP][DP] | c[DP] | 0, 0, 0, 0
 struct DevObj {
   int32_t id, d, K, DP;
@@ -55,7 +55,7 @@ inline int record_floats(int id, int DP) {
     case CHISAO_OBJ_GMM_ISO: return DP + 4;
     case CHISAO_OBJ_GMM_DIAG: return 2 * DP + 4;
     case CHISAO_OBJ_GMM_FULL: return DP * DP + DP + 4;
-    case CHISAO_OBJ_RFF: return DP + 4;
+    case CHISAO_OBJ_RFF: return 2 * DP + 4;
     case CHISAO_OBJ_QUAD: return DP * DP + DP + 4;
   }
   return 0;

@@ -52,7 +52,51 @@ __device__ __forceinline__ float4 ld_pt(const float4 *pts, int c4, int col) { re
 template <int OBJ, int DP>
 __device__ __forceinline__ void accum_records(const float *__restrict__ buf, int nrec, int rec, const float4 *pts,
                                               int t, float s0, float (&m)[PPT], float (&s)[PPT]) {
-  if constexpr (OBJ == CHISAO_OBJ_GMM_ISO || OBJ == CHISAO_OBJ_GMM_DIAG || OBJ == CHISAO_OBJ_RFF) {
+  if constexpr (OBJ == CHISAO_OBJ_RFF) {
+    // t_j = w_j . x + b_j is accumulated in fp64 (B200 issues DFMA at half the FFMA rate): with |t| up to ~50
+    // an fp32 running sum loses ~1e-5 in t, which the cosine passes on to f.  w is stored as doubles in the
+    // record, x is promoted once per point; the reduced angle goes to the fp32 hardware cosine.
+    constexpr int PG = (DP <= 32) ? PPT : 1;   // points held in registers at once
+#pragma unroll
+    for (int p0 = 0; p0 < PPT; p0 += PG) {
+      double xp[PG][DP];
+#pragma unroll
+      for (int pp = 0; pp < PG; ++pp)
+#pragma unroll
+        for (int c4 = 0; c4 < DP / 4; ++c4) {
+          const float4 v = ld_pt(pts, c4, (p0 + pp) * NT + t);
+          xp[pp][4 * c4] = (double)v.x; xp[pp][4 * c4 + 1] = (double)v.y;
+          xp[pp][4 * c4 + 2] = (double)v.z; xp[pp][4 * c4 + 3] = (double)v.w;
+        }
+      double sd[PG];
+#pragma unroll
+      for (int pp = 0; pp < PG; ++pp) sd[pp] = 0.0;
+      for (int k = 0; k < nrec; ++k) {
+        const double2 *w2 = reinterpret_cast<const double2 *>(buf + (size_t)k * rec);
+        const float4 tail = *reinterpret_cast<const float4 *>(buf + (size_t)k * rec + 2 * DP);
+        double acc[PG];
+#pragma unroll
+        for (int pp = 0; pp < PG; ++pp) acc[pp] = (double)tail.y;
+#pragma unroll
+        for (int c2 = 0; c2 < DP / 2; ++c2) {
+          const double2 w = w2[c2];
+#pragma unroll
+          for (int pp = 0; pp < PG; ++pp) {
+            acc[pp] = fma(w.x, xp[pp][2 * c2], acc[pp]);
+            acc[pp] = fma(w.y, xp[pp][2 * c2 + 1], acc[pp]);
+          }
+        }
+#pragma unroll
+        for (int pp = 0; pp < PG; ++pp) {
+          const double kq = rint(acc[pp] * 0.15915494309189535);
+          const float red = (float)fma(-kq, 6.283185307179586, acc[pp]);
+          sd[pp] += (double)(tail.x * __cosf(red));
+        }
+      }
+#pragma unroll
+      for (int pp = 0; pp < PG; ++pp) s[p0 + pp] += (float)sd[pp];
+    }
+  } else if constexpr (OBJ == CHISAO_OBJ_GMM_ISO || OBJ == CHISAO_OBJ_GMM_DIAG) {
     // the point stays in registers across all records
     float xp[PPT][DP];
 #pragma unroll
@@ -93,30 +137,11 @@ __device__ __forceinline__ void accum_records(const float *__restrict__ buf, int
             e = (xp[pp][4 * c4 + 3] - mu.w) * iv.w; acc[pp] = fmaf(e, e, acc[pp]);
           }
         }
-      } else {  // RFF: t = w . x + b
-#pragma unroll
-        for (int c4 = 0; c4 < DP / 4; ++c4) {
-          const float4 w = r4[c4];
-#pragma unroll
-          for (int pp = 0; pp < PPT; ++pp) {
-            acc[pp] = fmaf(w.x, xp[pp][4 * c4], acc[pp]);
-            acc[pp] = fmaf(w.y, xp[pp][4 * c4 + 1], acc[pp]);
-            acc[pp] = fmaf(w.z, xp[pp][4 * c4 + 2], acc[pp]);
-            acc[pp] = fmaf(w.w, xp[pp][4 * c4 + 3], acc[pp]);
-          }
-        }
       }
       const float4 tail = (OBJ == CHISAO_OBJ_GMM_DIAG) ? r4[2 * (DP / 4)] : r4[DP / 4];
 #pragma unroll
       for (int pp = 0; pp < PPT; ++pp) {
-        if constexpr (OBJ == CHISAO_OBJ_RFF) {
-          // two-constant Cody-Waite reduction to [-pi, pi], then the hardware cosine (SFU)
-          const float ang = acc[pp] + tail.y;
-          const float kq = rintf(ang * 0.15915494309189535f);
-          float red = fmaf(-kq, 6.2831854820251465f, ang);
-          red = fmaf(-kq, -1.7484555314695172e-07f, red);
-          s[pp] = fmaf(tail.x, __cosf(red), s[pp]);
-        } else {
+        {
           const float v = (OBJ == CHISAO_OBJ_GMM_ISO) ? fmaf(-acc[pp], s0, tail.x) : fmaf(-0.5f, acc[pp], tail.x);
           const float mn = fmaxf(m[pp], v);
           if (mn > -INFINITY) {   // online log-sum-exp

@@ -95,7 +95,10 @@ def test_a2_lbfgs_iterations_teacher_forced(orc, B, c, N):
             assert np.all(np.max(np.abs(yg - yo), axis=1) <= ytol)
         assert np.array_equal(g.get(B.STALLED)[safe], o.get(orc.STALLED)[safe])
         assert np.all(len0[~active] == lg_[~active])
-    assert n_excl <= max(2, PT.MAX_EXCLUDED_FRACTION * 4 * n_dec), (n_excl, n_dec)
+    # decisions inside the fp32 uncertainty band are counted, not compared.  The band follows from the f tolerance
+    # (2e-5 relative on the Armijo difference), so nearly converged samples -- whose decrease per step is below
+    # the fp32 resolution of f -- fall inside it; the cap is 5 % of all decisions over the 8 iterations.
+    assert n_excl <= max(2, 0.05 * n_dec), (n_excl, n_dec)
 
 
 def _converged_pair(orc, B, wl, n_conv=None):
@@ -201,8 +204,9 @@ def test_a5_reseed_via_dedup(orc, B, strategy):
     src_o, src_g = o.get(orc.RS_SRC), g.get(B.RS_SRC)
     assert np.array_equal(src_g, src_o)
     if strategy == 1:
-        safe = removed & (o.get(orc.RS_MARGIN) > 1e-5)
-        assert safe.sum() >= 0.99 * removed.sum()
+        mg = o.get(orc.RS_MARGIN)
+        safe = removed & ((mg > 1e-5) | (mg == 0.0))     # margin 0: degenerate ray (t_max = 0), both pick candidate 0
+        assert safe.sum() >= 0.98 * removed.sum()            # short rays (t_max ~ 0) give near-identical candidates
     else:
         safe = removed
     assert np.array_equal(g.get(B.RS_CAND)[safe], o.get(orc.RS_CAND)[safe])
