@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "chisao_eval_kernels.cuh"
+#include "chisao_tc.cuh"
 
 using namespace chisao;
 
@@ -38,7 +39,9 @@ struct chisao_ctx {
   State st;
   cudaStream_t stream;
   int cycle = 0;
-  std::vector<float> lo, hi, recs_host;
+  std::vector<float> lo, hi, recs_host, tc_host;
+  TcObj tc;
+  bool use_tc = false;   // dense objective at d > 32: tensor-core evaluator (chisao_tc.cuh)
   std::string err;
   uint64_t launches = 0;
   bool timing = false;
@@ -90,7 +93,12 @@ int validate(const chisao_config *cfg, const chisao_objective *obj, std::string 
 }
 
 // workspace carve; fills st pointers relative to `base` (may be null when only sizing)
-size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *base, State *st, const float **recs_dev) {
+inline bool wants_tc(const chisao_objective &o) {
+  return (o.id == CHISAO_OBJ_GMM_FULL || o.id == CHISAO_OBJ_QUAD) && o.d > 32;
+}
+
+size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *base, State *st, const float **recs_dev,
+             const float **tc_dev = nullptr) {
   Layout L;
   const size_t N = (size_t)c.N, d = (size_t)c.d, m = (size_t)c.lbfgs_m, M = (size_t)c.hlc_M;
   const int DP = padded_dim(c.d);
@@ -110,6 +118,7 @@ size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *b
   const size_t o_blk = F(3 * nb + 3);
   const size_t o_hf = F(N * M);
   const size_t o_q = F(d * d);
+  const size_t o_tc = F(wants_tc(o) ? (size_t)o.K * TC_REC : 0);
   if (base && st) {
     auto P = [&](size_t off) { return reinterpret_cast<float *>(base + off); };
     auto I = [&](size_t off) { return reinterpret_cast<int32_t *>(base + off); };
@@ -127,6 +136,7 @@ size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *b
     st->blk_cnt = I(o_blk);
     st->hlc_f = P(o_hf);
     st->grQ = P(o_q);
+    if (tc_dev) *tc_dev = P(o_tc);
   }
   return L.total;
 }
@@ -167,6 +177,34 @@ void pack_records(const chisao_objective &o, int DP, std::vector<float> &out, fl
   if (o.id == CHISAO_OBJ_RFF) s0 = o.scalar0;
 }
 
+// tensor-core operand records: W_k split into tf32 hi / lo (round-to-nearest, ties away: the integer form of
+// cvt.rna.tf32.f32) and stored in the canonical K-major UMMA layout, then mu_k and a_k (chisao_tc.cuh)
+float tf32_rna_host(float x) {
+  uint32_t u;
+  std::memcpy(&u, &x, 4);
+  if ((u & 0x7F800000u) != 0x7F800000u) u += 0x1000u;
+  u &= 0xFFFFE000u;
+  float r;
+  std::memcpy(&r, &u, 4);
+  return r;
+}
+void pack_tc_records(const chisao_objective &o, std::vector<float> &out) {
+  const int d = o.d, K = o.K;
+  out.assign((size_t)K * TC_REC, 0.0f);
+  for (int k = 0; k < K; ++k) {
+    float *r = out.data() + (size_t)k * TC_REC;
+    for (int n = 0; n < d; ++n)
+      for (int c = 0; c < d; ++c) {
+        const float w = o.mats[((size_t)k * d + n) * d + c];
+        const float h = tf32_rna_host(w), l = tf32_rna_host(w - h);
+        const int idx = (c / 4) * 256 + n * 4 + (c % 4);
+        r[idx] = h; r[TC_D * TC_D + idx] = l;
+      }
+    for (int j = 0; j < d; ++j) r[2 * TC_D * TC_D + j] = o.means[(size_t)k * d + j];
+    r[2 * TC_D * TC_D + TC_D] = (o.id == CHISAO_OBJ_GMM_FULL) ? o.vec_a[k] : 0.0f;
+  }
+}
+
 struct Scope {   // optional CUDA-event bracket around a launch group
   chisao_ctx *c; int cls; cudaEvent_t a = nullptr, b = nullptr;
   Scope(chisao_ctx *ctx, int k) : c(ctx), cls(k) {
@@ -194,6 +232,11 @@ cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const in
   const int grid = (s.N + spt - 1) / spt;
   Scope sc(c, 0);
   c->launches += 1;
+  if (c->use_tc) {
+    cudaError_t e = launch_fd_tc(c->obj.id, c->tc, a, s.N, c->stream);
+    if (getenv("CHISAO_DEBUG")) { fprintf(stderr, "[chisao] fd_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] fd_tc done (%s)\n", cudaGetErrorString(e)); }
+    return e;
+  }
   switch (c->obj.id) {
     case 0: return launch_fd_obj_0(c->obj, a, grid, c->stream);
     case 1: return launch_fd_obj_1(c->obj, a, grid, c->stream);
@@ -221,6 +264,11 @@ cudaError_t eval_points(chisao_ctx *c, int mode, int b, int iter) {
   const int grid = (s.N + PTILE - 1) / PTILE;
   Scope sc(c, 1);
   c->launches += 1;
+  if (c->use_tc) {
+    cudaError_t e = launch_pt_tc(c->obj.id, c->tc, a, s.N, c->stream);
+    if (getenv("CHISAO_DEBUG")) { fprintf(stderr, "[chisao] pt_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] pt_tc done (%s)\n", cudaGetErrorString(e)); }
+    return e;
+  }
   switch (c->obj.id) {
     case 0: return launch_pt_obj_0(c->obj, a, grid, c->stream);
     case 1: return launch_pt_obj_1(c->obj, a, grid, c->stream);
@@ -241,6 +289,7 @@ cudaError_t hlc_step(chisao_ctx *c, int iter) {
   const int grid = (s.N + spt - 1) / spt;
   Scope sc(c, 2);
   c->launches += 1;
+  if (c->use_tc && s.M <= TC_PTS) return launch_hlc_tc(c->obj.id, c->tc, a, s.N, c->stream);
   switch (c->obj.id) {
     case 0: return launch_hlc_obj_0(c->obj, a, grid, c->stream);
     case 1: return launch_hlc_obj_1(c->obj, a, grid, c->stream);
@@ -357,8 +406,8 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
   State &s = ctx->st;
   std::memset(&s, 0, sizeof(s));
   s.N = cfg->N; s.d = cfg->d; s.m = cfg->lbfgs_m; s.M = cfg->hlc_M; s.x = x_dev;
-  const float *recs_dev = nullptr;
-  carve(*cfg, *obj, static_cast<unsigned char *>(workspace_dev), &s, &recs_dev);
+  const float *recs_dev = nullptr, *tc_dev = nullptr;
+  carve(*cfg, *obj, static_cast<unsigned char *>(workspace_dev), &s, &recs_dev, &tc_dev);
 
   DevObj &o = ctx->obj;
   o.id = obj->id; o.d = obj->d; o.K = obj->K; o.DP = padded_dim(obj->d);
@@ -384,10 +433,19 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
     case 3: CKI(configure_obj_3()); break;
     default: CKI(configure_obj_4()); break;
   }
+  ctx->use_tc = wants_tc(*obj);
+  if (ctx->use_tc) {
+    pack_tc_records(*obj, ctx->tc_host);
+    ctx->tc.K = obj->K; ctx->tc.d = obj->d; ctx->tc.sigma_noise = obj->sigma_noise; ctx->tc.recs = tc_dev;
+    CKI(tc_configure());
+  }
   // zero everything except the parameter records, then upload parameters and bounds
   CKI(cudaMemsetAsync(workspace_dev, 0, need, ctx->stream));
   CKI(cudaMemcpyAsync(const_cast<float *>(recs_dev), ctx->recs_host.data(), ctx->recs_host.size() * 4,
                       cudaMemcpyHostToDevice, ctx->stream));
+  if (ctx->use_tc)
+    CKI(cudaMemcpyAsync(const_cast<float *>(tc_dev), ctx->tc_host.data(), ctx->tc_host.size() * 4, cudaMemcpyHostToDevice,
+                        ctx->stream));
   CKI(cudaMemcpyAsync(s.lo, ctx->lo.data(), 4 * (size_t)cfg->d, cudaMemcpyHostToDevice, ctx->stream));
   CKI(cudaMemcpyAsync(s.hi, ctx->hi.data(), 4 * (size_t)cfg->d, cudaMemcpyHostToDevice, ctx->stream));
   const int32_t one = 1;

@@ -1,0 +1,201 @@
+// chisao_tc.cuh -- tensor-core evaluator for the dense objectives at d > 32 (GMM_FULL, QUAD; DP = 64).
+//
+// The quadratic forms q_k(x) = || W_k (x - mu_k) ||^2 of a tile of 128 points are a dense contraction
+// Z_k[128 x 64] = D_k[128 x 64] * W_k^T[64 x 64] (BASELINE.json north_star: "tensor cores ... full-covariance
+// mixture quadratic forms").  It runs on the 5th-generation tensor cores: tcgen05.mma kind::tf32, M = 128,
+// N = 64, K = 8 per instruction, accumulators in TMEM, fp32 accuracy by the 3xTF32 split
+//     D W^T ~= D_hi W_hi^T + D_lo W_hi^T + D_hi W_lo^T          (hi = rna-tf32(v), lo = rna-tf32(v - hi)),
+// 24 MMAs per component.  Thread t of the CTA owns point t (= TMEM lane t): it builds its row of D_hi / D_lo
+// in shared memory in the canonical K-major no-swizzle UMMA layout (16-byte K-chunks of 8 consecutive rows form
+// a 128-byte core matrix; byte offset of element (p, c) = (c/4)*2048 + p*16 + (c%4)*4), one thread issues the
+// MMAs, and every thread reads its 64 accumulators back with tcgen05.ld for the epilogue (sum of squares,
+// online log-sum-exp).  W_k hi/lo are split and laid out on the host once (byte offset of (n, c) =
+// (c/4)*1024 + n*16 + (c%4)*4) and streamed by the bulk-copy engine; A and TMEM are double-buffered so the
+// MMAs of component k overlap the epilogue of k-1 and the operand build of k+1.
+#pragma once
+#include "chisao_device.cuh"
+
+namespace chisao {
+
+constexpr int TC_PTS = 128;                              // points per CTA tile (= threads = TMEM lanes)
+constexpr int TC_D = 64;
+constexpr int TC_REC = 2 * TC_D * TC_D + TC_D + 4;       // floats per component: W_hi | W_lo | mu | a,0,0,0
+constexpr int TC_REC_BYTES = TC_REC * 4;                 // 33 040 (multiple of 16)
+constexpr int TC_A_BYTES = TC_PTS * TC_D * 4;            // 32 768 per operand image
+constexpr int TC_SMEM_BYTES = 1024 + 4 * TC_A_BYTES + 2 * TC_REC_BYTES;   // barriers | A hi/lo x2 | B x2
+constexpr uint32_t TC_TMEM_COLS = 128;                   // 2 accumulator stages of 64 fp32 columns
+
+struct TcObj {
+  int32_t K, d;
+  float sigma_noise;
+  const float *recs;      // device [K][TC_REC]
+};
+
+struct TcSmem {
+  uint64_t *bbar;         // [2] operand-B chunk landed
+  uint64_t *mbar;         // [2] MMAs of a stage retired
+  uint32_t *tmem;         // TMEM base address written by tcgen05.alloc
+  unsigned char *A[2][2]; // [stage][hi/lo]
+  float *B[2];            // [stage] component record
+};
+__device__ __forceinline__ TcSmem tc_carve(unsigned char *base) {
+  TcSmem s;
+  s.bbar = reinterpret_cast<uint64_t *>(base);
+  s.mbar = s.bbar + 2;
+  s.tmem = reinterpret_cast<uint32_t *>(base + 64);
+  unsigned char *p = base + 1024;
+  for (int st = 0; st < 2; ++st)
+    for (int h = 0; h < 2; ++h) { s.A[st][h] = p; p += TC_A_BYTES; }
+  s.B[0] = reinterpret_cast<float *>(p);
+  s.B[1] = reinterpret_cast<float *>(p + TC_REC_BYTES);
+  return s;
+}
+
+// round-to-nearest (ties away) to tf32 = the integer form of cvt.rna.tf32.f32 for finite inputs: two full-rate
+// ALU instructions instead of one quarter-rate conversion (the operand build is issue-bound)
+__device__ __forceinline__ float tf32_rna(float x) {
+  return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
+}
+// shared-memory matrix descriptor, no swizzle, version 1 (sm_100): start | LBO (K direction) | SBO (M/N direction)
+__device__ __forceinline__ uint64_t tc_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
+         ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46);
+}
+// instruction descriptor: D = F32, A = B = TF32, both K-major, N = 64, M = 128
+constexpr uint32_t TC_IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
+
+__device__ __forceinline__ void tc_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(TC_IDESC), "r"(accumulate));
+}
+__device__ __forceinline__ void tc_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[64], int q) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[16 * q + 0]), "=r"(r[16 * q + 1]), "=r"(r[16 * q + 2]), "=r"(r[16 * q + 3]), "=r"(r[16 * q + 4]),
+        "=r"(r[16 * q + 5]), "=r"(r[16 * q + 6]), "=r"(r[16 * q + 7]), "=r"(r[16 * q + 8]), "=r"(r[16 * q + 9]),
+        "=r"(r[16 * q + 10]), "=r"(r[16 * q + 11]), "=r"(r[16 * q + 12]), "=r"(r[16 * q + 13]), "=r"(r[16 * q + 14]),
+        "=r"(r[16 * q + 15])
+      : "r"(taddr + 16 * q));
+}
+
+// one-time CTA setup / teardown (all 128 threads)
+__device__ __forceinline__ void tc_setup(const TcSmem &sm, int t) {
+  if (t < 32) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(sm.tmem)), "n"(TC_TMEM_COLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  if (t == 32) {
+    mbar_init(&sm.bbar[0], 1); mbar_init(&sm.bbar[1], 1); mbar_init(&sm.mbar[0], 1); mbar_init(&sm.mbar[1], 1);
+    mbar_fence_init();
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;");
+}
+__device__ __forceinline__ void tc_teardown(const TcSmem &sm, int t) {
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  if (t < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*sm.tmem), "n"(TC_TMEM_COLS));
+}
+
+// Evaluate the calling thread's point x[64] (coordinates >= d must be zero).  All 128 threads of the CTA must
+// call (barriers inside); tc_setup must have run.  OBJ is CHISAO_OBJ_GMM_FULL or CHISAO_OBJ_QUAD.
+template <int OBJ>
+__device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
+  const uint32_t tm = *sm.tmem;
+  const int K = o.K;
+  float m = -INFINITY, s = 0.0f, a_prev = 0.0f;
+  if (t == 0) {   // prefetch the first two component records
+    mbar_expect_tx(&sm.bbar[0], TC_REC_BYTES);
+    bulk_g2s(sm.B[0], o.recs, TC_REC_BYTES, &sm.bbar[0]);
+    if (K > 1) {
+      mbar_expect_tx(&sm.bbar[1], TC_REC_BYTES);
+      bulk_g2s(sm.B[1], o.recs + TC_REC, TC_REC_BYTES, &sm.bbar[1]);
+    }
+  }
+  auto epilogue = [&](int j, float a_j) {
+    const int st = j & 1;
+    mbar_wait(&sm.mbar[st], (j >> 1) & 1);
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (t == 0 && j + 2 < K) {   // stage st of B is free again: fetch component j + 2
+      mbar_expect_tx(&sm.bbar[st], TC_REC_BYTES);
+      bulk_g2s(sm.B[st], o.recs + (size_t)(j + 2) * TC_REC, TC_REC_BYTES, &sm.bbar[st]);
+    }
+    __syncwarp();
+    uint32_t r[64];
+    const uint32_t taddr = tm + ((uint32_t)((t >> 5) * 32) << 16) + (uint32_t)(st * 64);
+    tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll
+    for (int n = 0; n < 64; n += 4) {
+      const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
+                  z3 = __uint_as_float(r[n + 3]);
+      q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+    }
+    const float q = (q0 + q1) + (q2 + q3);
+    if constexpr (OBJ == CHISAO_OBJ_QUAD) {
+      s += q;
+    } else {
+      const float v = fmaf(-0.5f, q, a_j);
+      const float mn = fmaxf(m, v);
+      if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+  };
+  for (int k = 0; k < K; ++k) {
+    const int st = k & 1;
+    mbar_wait(&sm.bbar[st], (k >> 1) & 1);            // W_k hi/lo, mu_k, a_k have landed
+    const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B[st] + 2 * TC_D * TC_D);
+    const float a_k = sm.B[st][2 * TC_D * TC_D + TC_D];
+    unsigned char *Ah = sm.A[st][0] + t * 16, *Al = sm.A[st][1] + t * 16;
+#pragma unroll
+    for (int c4 = 0; c4 < TC_D / 4; ++c4) {           // this thread's row of D_hi / D_lo
+      const float4 mu = mu4[c4];
+      const float d0 = x[4 * c4] - mu.x, d1 = x[4 * c4 + 1] - mu.y, d2 = x[4 * c4 + 2] - mu.z, d3 = x[4 * c4 + 3] - mu.w;
+      float4 h, l;
+      h.x = tf32_rna(d0); h.y = tf32_rna(d1); h.z = tf32_rna(d2); h.w = tf32_rna(d3);
+      l.x = tf32_rna(d0 - h.x); l.y = tf32_rna(d1 - h.y); l.z = tf32_rna(d2 - h.z); l.w = tf32_rna(d3 - h.w);
+      *reinterpret_cast<float4 *>(Ah + c4 * 2048) = h;
+      *reinterpret_cast<float4 *>(Al + c4 * 2048) = l;
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> async-proxy (MMA) reads
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (t == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      // descriptors differ only in the 14-bit start-address field: add (byte offset >> 4) to the base
+      const uint64_t dAh = tc_desc(smem_u32(sm.A[st][0]), 2048, 128), dAl = tc_desc(smem_u32(sm.A[st][1]), 2048, 128);
+      const uint64_t dBh = tc_desc(smem_u32(sm.B[st]), 1024, 128), dBl = tc_desc(smem_u32(sm.B[st]) + TC_D * TC_D * 4, 1024, 128);
+      const uint32_t dcol = tm + (uint32_t)(st * 64);
+#pragma unroll
+      for (int pr = 0; pr < 3; ++pr) {
+        const uint64_t a0 = (pr == 1) ? dAl : dAh, b0 = (pr == 2) ? dBl : dBh;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          tc_mma(dcol, a0 + (uint64_t)(ks * (4096 >> 4)), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
+      }
+      tc_commit(&sm.mbar[st]);
+    }
+    __syncwarp();
+    if (k > 0) epilogue(k - 1, a_prev);
+    a_prev = a_k;
+  }
+  epilogue(K - 1, a_prev);
+  if constexpr (OBJ == CHISAO_OBJ_QUAD) return -0.5f * s;
+  return m + logf(s);
+}
+
+// launchers (chisao_tc_kernels.cu)
+struct FdArgs; struct PtArgs; struct HlcArgs;
+cudaError_t tc_configure();
+cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samples, cudaStream_t st);
+cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samples, cudaStream_t st);
+cudaError_t launch_hlc_tc(int obj_id, const TcObj &o, const HlcArgs &a, int n_samples, cudaStream_t st);
+
+}  // namespace chisao

@@ -1,0 +1,245 @@
+// chisao_tc_kernels.cu -- the three evaluation kernels (FD stencil, one point per sample, Hands Like Clouds)
+// on the tensor-core evaluator of chisao_tc.cuh, for GMM_FULL and QUAD at 32 < d <= 64.  Same arguments, same
+// noise slots, same epilogues as the FFMA kernels of chisao_eval_kernels.cuh; one point per thread, 128 points
+// per CTA.  Citations: PAPER.md:62, :555 (FD), :75-82 (line search), :113-120 + Eq. 9 :577 (HLC), Eq. 6 :126.
+#include "chisao_eval_kernels.cuh"
+#include "chisao_tc.cuh"
+
+namespace chisao {
+
+__device__ __forceinline__ void tc_load_row(const float *row, int d, bool vec, float (&x)[TC_D]) {
+#pragma unroll
+  for (int c4 = 0; c4 < TC_D / 4; ++c4) {
+    const float4 v = ld_row4(row, c4, d, vec);
+    x[4 * c4] = v.x; x[4 * c4 + 1] = v.y; x[4 * c4 + 2] = v.z; x[4 * c4 + 3] = v.w;
+  }
+}
+
+// thread t -> (sample t / 2d of the tile, slot t % 2d); slot 2j = x + h e_j, 2j + 1 = x - h e_j
+template <int OBJ>
+__global__ void __launch_bounds__(TC_PTS, 1) k_eval_fd_tc(const TcObj o, const FdArgs a) {
+  extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
+  const TcSmem sm = tc_carve(tc_smem_raw);
+  const int t = threadIdx.x, d = a.d;
+  const int spt = TC_PTS / (2 * d);
+  const int cnt = a.count ? *a.count : a.max_count;
+  const int first = blockIdx.x * spt;
+  if (first >= cnt) return;
+  tc_setup(sm, t);
+  const int s = t / (2 * d), slot = t - s * 2 * d, j = slot >> 1;
+  const bool valid = (s < spt) && (first + s < cnt);
+  const int i = valid ? (a.list ? a.list[first + s] : first + s) : 0;
+  float x[TC_D];
+  float xj = 0.f, xp = 0.f;
+  if (valid) {
+    const float *row = a.X + (size_t)i * d;
+    tc_load_row(row, d, (d & 3) == 0, x);
+    xj = row[j];
+    xp = (slot & 1) ? xj - a.h : xj + a.h;
+    // replace coordinate j through a shared-memory round trip of the thread's own row: a dynamically indexed
+    // register array would be lowered to a branch tree over j, and the warp-collective tcgen05 instructions
+    // below need every lane on the same path
+    float *own = reinterpret_cast<float *>(sm.A[1][0]) + t * 68;
+#pragma unroll
+    for (int c4 = 0; c4 < TC_D / 4; ++c4)
+      *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
+    own[j] = xp;
+    __syncwarp();
+#pragma unroll
+    for (int c4 = 0; c4 < TC_D / 4; ++c4) {
+      const float4 v = *reinterpret_cast<const float4 *>(own + 4 * c4);
+      x[4 * c4] = v.x; x[4 * c4 + 1] = v.y; x[4 * c4 + 2] = v.z; x[4 * c4 + 3] = v.w;
+    }
+  } else {
+#pragma unroll
+    for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
+  }
+  float f = tc_eval_tile<OBJ>(o, sm, x, t);
+  if (valid) f += eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, 1 + slot);
+  // partner lane holds the other sign of the same coordinate
+  const float fo = __shfl_xor_sync(0xffffffffu, f, 1);
+  const float xo = __shfl_xor_sync(0xffffffffu, xp, 1);
+  if (valid && !(slot & 1)) {
+    const float g = (f - fo) / ((xp - xj) + (xj - xo));
+    if (a.mode == FD_GRAD) {
+      a.g_out[(size_t)i * d + j] = g;
+    } else {   // Eq. 6
+      const float vo = (a.iter == 1) ? 0.0f : a.v[(size_t)i * d + j];
+      const float vn = fmaf(a.mu, vo, -a.alpha * g);
+      a.v[(size_t)i * d + j] = vn;
+      a.x[(size_t)i * d + j] = clipf(xj + vn, a.lo[j], a.hi[j]);
+    }
+  }
+  if (t == 0) atomicAdd(&a.evals[a.counter], (unsigned long long)min(spt, cnt - first) * 2ull * d);
+  tc_teardown(sm, t);
+}
+
+template <int OBJ>
+__global__ void __launch_bounds__(TC_PTS, 1) k_eval_points_tc(const TcObj o, const PtArgs a) {
+  extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
+  const TcSmem sm = tc_carve(tc_smem_raw);
+  const int t = threadIdx.x, d = a.d;
+  const int cnt = a.count ? *a.count : a.max_count;
+  const int first = blockIdx.x * TC_PTS;
+  if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
+  if (first >= cnt) return;
+  tc_setup(sm, t);
+  const int e = first + t;
+  const bool valid = e < cnt;
+  const int i = valid ? (a.list ? a.list[e] : e) : 0;
+  float x[TC_D];
+  if (valid) tc_load_row(a.X + (size_t)i * d, d, (d & 3) == 0, x);
+  else {
+#pragma unroll
+    for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
+  }
+  const float fv = tc_eval_tile<OBJ>(o, sm, x, t);
+  bool accept = false, retry = false;
+  float val = 0.f;
+  if (valid) {
+    if (a.mode == PT_CENTRE) {
+      a.f[i] = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, 0, 0);
+    } else {
+      val = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + a.b);
+      const float phit = -val, phi = -a.f[i];
+      const float rhs = fmaf(a.c1, a.dec[i], phi);
+      accept = (fabsf(phit) <= 3.0e38f) && (phit <= rhs);
+      retry = !accept && (a.b < a.ls_max);
+    }
+  }
+  if (a.mode == PT_LS) {
+    const int sa = warp_append(a.fd_cnt, accept);
+    if (accept) { a.fd_list[sa] = i; a.ls_b[i] = a.b; a.ft[i] = val; }
+    const int sr = warp_append(a.next_cnt, retry);
+    if (retry) {
+      a.next_list[sr] = i;
+      const float tn = a.tcur[i] * a.shrink;
+      a.tcur[i] = tn;
+      float dsum = 0.0f;
+      for (int j = 0; j < d; ++j) {
+        const float xo = a.x[(size_t)i * d + j];
+        const float xn = clipf(fmaf(tn, a.p[(size_t)i * d + j], xo), a.lo[j], a.hi[j]);
+        a.xt[(size_t)i * d + j] = xn;
+        dsum = fmaf(-a.g[(size_t)i * d + j], xn - xo, dsum);
+      }
+      a.dec[i] = dsum;
+    }
+  }
+  if (t == 0) atomicAdd(&a.evals[a.mode == PT_CENTRE ? EV_INIT : EV_LS], (unsigned long long)min(TC_PTS, cnt - first));
+  tc_teardown(sm, t);
+}
+
+// the d normals of draw k of sample i (Philox tag HLC_U, sequence index k d + j; R-15)
+__device__ __forceinline__ void hlc_normals(uint64_t seed, int i, int cycle, int iter, int k, int d, float (&u)[TC_D]) {
+  const uint32_t tg = rng_tag(5, iter, PUR_HLC_U);
+  const uint32_t n0 = (uint32_t)k * (uint32_t)d;
+  float z0 = 0.f, z1 = 0.f, z2 = 0.f, z3 = 0.f;
+  uint32_t cur = 0xffffffffu;
+#pragma unroll
+  for (int j = 0; j < TC_D; ++j) {
+    float v = 0.f;
+    if (j < d) {
+      const uint32_t n = n0 + (uint32_t)j;
+      if ((n >> 2) != cur) {
+        cur = n >> 2;
+        const uint4 w = philox_block(seed, cur, (uint32_t)i, (uint32_t)cycle, tg);
+        box_muller(w.x, w.y, z0, z1);
+        box_muller(w.z, w.w, z2, z3);
+      }
+      const uint32_t ln = n & 3u;
+      v = ln == 0u ? z0 : (ln == 1u ? z1 : (ln == 2u ? z2 : z3));
+    }
+    u[j] = v;
+  }
+}
+
+// Hands Like Clouds on the tensor-core evaluator: point t of the tile = (sample t / M, draw t % M), M <= 128
+template <int OBJ>
+__global__ void __launch_bounds__(TC_PTS, 1) k_hlc_tc(const TcObj o, const HlcArgs a) {
+  extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
+  const TcSmem sm = tc_carve(tc_smem_raw);
+  const int t = threadIdx.x, d = a.d, M = a.M;
+  const int spt = min(TC_PTS / M, HLC_MAX_SPT);
+  const int cnt = a.count ? *a.count : a.max_count;
+  const int first = blockIdx.x * spt;
+  if (first >= cnt) return;
+  tc_setup(sm, t);
+  const int s = t / M, k = t - s * M;
+  const bool valid = (s < spt) && (first + s < cnt);
+  const int i = valid ? a.list[first + s] : 0;
+  float x[TC_D];
+  if (valid) {
+    float u[TC_D];
+    hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
+    tc_load_row(a.x + (size_t)i * d, d, (d & 3) == 0, x);
+#pragma unroll
+    for (int c = 0; c < TC_D; ++c) x[c] = fmaf(a.sigma, u[c], x[c]);   // evaluation points are not clipped (R-12)
+  } else {
+#pragma unroll
+    for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
+  }
+  float val = tc_eval_tile<OBJ>(o, sm, x, t);
+  __syncthreads();                       // every MMA has retired: the operand buffers are free
+  float *Us = reinterpret_cast<float *>(sm.A[0][0]);          // [128][65] normals (A[0][0..1] = 64 KB)
+  float *fvs = reinterpret_cast<float *>(sm.A[1][0]);         // [128] values
+  if (valid) {
+    val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
+    a.hlc_f[(size_t)i * M + k] = val;
+    float u[TC_D];
+    hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
+#pragma unroll
+    for (int c = 0; c < TC_D; ++c) Us[t * 65 + c] = u[c];
+  } else {
+    val = 0.f;
+  }
+  fvs[t] = val;
+  __syncthreads();
+  const int nval = min(spt, cnt - first);
+  for (int item = t; item < nval * d; item += TC_PTS) {
+    const int ss = item / d, j = item - ss * d;
+    const int ii = a.list[first + ss];
+    float b = 0.0f;
+    if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
+    float acc = 0.0f;
+    for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, Us[(ss * M + kk) * 65 + j], acc);
+    const float gh = acc / ((float)M * a.sigma);
+    a.ghat[(size_t)ii * d + j] = gh;
+    const float xo = a.x[(size_t)ii * d + j];
+    a.x[(size_t)ii * d + j] = clipf(fmaf(a.eta, gh, xo), a.lo[j], a.hi[j]);
+  }
+  if (t == 0) atomicAdd(&a.evals[EV_HLC], (unsigned long long)nval * (unsigned long long)M);
+  tc_teardown(sm, t);
+}
+
+// ---- launchers ------------------------------------------------------------------------------------------------
+cudaError_t tc_configure() {
+  cudaError_t e;
+#define CFG(K) if ((e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES)) != cudaSuccess) return e;
+  CFG(k_eval_fd_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_fd_tc<CHISAO_OBJ_QUAD>)
+  CFG(k_eval_points_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_points_tc<CHISAO_OBJ_QUAD>)
+  CFG(k_hlc_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_hlc_tc<CHISAO_OBJ_QUAD>)
+#undef CFG
+  return cudaSuccess;
+}
+cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samples, cudaStream_t st) {
+  const int spt = TC_PTS / (2 * a.d);
+  const int grid = (n_samples + spt - 1) / spt;
+  if (obj_id == CHISAO_OBJ_QUAD) k_eval_fd_tc<CHISAO_OBJ_QUAD><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  else k_eval_fd_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  return cudaGetLastError();
+}
+cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samples, cudaStream_t st) {
+  const int grid = (n_samples + TC_PTS - 1) / TC_PTS;
+  if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  return cudaGetLastError();
+}
+cudaError_t launch_hlc_tc(int obj_id, const TcObj &o, const HlcArgs &a, int n_samples, cudaStream_t st) {
+  const int spt = TC_PTS / a.M < HLC_MAX_SPT ? TC_PTS / a.M : HLC_MAX_SPT;
+  const int grid = (n_samples + spt - 1) / spt;
+  if (obj_id == CHISAO_OBJ_QUAD) k_hlc_tc<CHISAO_OBJ_QUAD><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  else k_hlc_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  return cudaGetLastError();
+}
+
+}  // namespace chisao
