@@ -31,25 +31,19 @@ struct TcObj {
   const float *recs;      // device [K][TC_REC]
 };
 
+// shared-memory carve (all offsets are arithmetic so that nothing is indexed dynamically through a pointer table):
+//   [0,16) bbar[2] | [16,32) mbar[2] | [64,68) TMEM base | [1024, +4*32K) A[stage][hi/lo] | then B[stage] records
 struct TcSmem {
-  uint64_t *bbar;         // [2] operand-B chunk landed
-  uint64_t *mbar;         // [2] MMAs of a stage retired
-  uint32_t *tmem;         // TMEM base address written by tcgen05.alloc
-  unsigned char *A[2][2]; // [stage][hi/lo]
-  float *B[2];            // [stage] component record
+  unsigned char *base;
+  __device__ __forceinline__ uint64_t *bbar(int st) const { return reinterpret_cast<uint64_t *>(base) + st; }
+  __device__ __forceinline__ uint64_t *mbar(int st) const { return reinterpret_cast<uint64_t *>(base) + 2 + st; }
+  __device__ __forceinline__ uint32_t *tmem() const { return reinterpret_cast<uint32_t *>(base + 64); }
+  __device__ __forceinline__ unsigned char *A(int st, int lo) const { return base + 1024 + (st * 2 + lo) * TC_A_BYTES; }
+  __device__ __forceinline__ float *B(int st) const {
+    return reinterpret_cast<float *>(base + 1024 + 4 * TC_A_BYTES + st * TC_REC_BYTES);
+  }
 };
-__device__ __forceinline__ TcSmem tc_carve(unsigned char *base) {
-  TcSmem s;
-  s.bbar = reinterpret_cast<uint64_t *>(base);
-  s.mbar = s.bbar + 2;
-  s.tmem = reinterpret_cast<uint32_t *>(base + 64);
-  unsigned char *p = base + 1024;
-  for (int st = 0; st < 2; ++st)
-    for (int h = 0; h < 2; ++h) { s.A[st][h] = p; p += TC_A_BYTES; }
-  s.B[0] = reinterpret_cast<float *>(p);
-  s.B[1] = reinterpret_cast<float *>(p + TC_REC_BYTES);
-  return s;
-}
+__device__ __forceinline__ TcSmem tc_carve(unsigned char *base) { TcSmem s; s.base = base; return s; }
 
 // round-to-nearest (ties away) to tf32 = the integer form of cvt.rna.tf32.f32 for finite inputs: two full-rate
 // ALU instructions instead of one quarter-rate conversion (the operand build is issue-bound)
@@ -86,11 +80,11 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[64], int q
 // one-time CTA setup / teardown (all 128 threads)
 __device__ __forceinline__ void tc_setup(const TcSmem &sm, int t) {
   if (t < 32) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(sm.tmem)), "n"(TC_TMEM_COLS));
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(sm.tmem())), "n"(TC_TMEM_COLS));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (t == 32) {
-    mbar_init(&sm.bbar[0], 1); mbar_init(&sm.bbar[1], 1); mbar_init(&sm.mbar[0], 1); mbar_init(&sm.mbar[1], 1);
+    mbar_init(sm.bbar(0), 1); mbar_init(sm.bbar(1), 1); mbar_init(sm.mbar(0), 1); mbar_init(sm.mbar(1), 1);
     mbar_fence_init();
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
@@ -100,31 +94,31 @@ __device__ __forceinline__ void tc_setup(const TcSmem &sm, int t) {
 __device__ __forceinline__ void tc_teardown(const TcSmem &sm, int t) {
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
-  if (t < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*sm.tmem), "n"(TC_TMEM_COLS));
+  if (t < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*sm.tmem()), "n"(TC_TMEM_COLS));
 }
 
 // Evaluate the calling thread's point x[64] (coordinates >= d must be zero).  All 128 threads of the CTA must
 // call (barriers inside); tc_setup must have run.  OBJ is CHISAO_OBJ_GMM_FULL or CHISAO_OBJ_QUAD.
 template <int OBJ>
 __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
-  const uint32_t tm = *sm.tmem;
+  const uint32_t tm = *sm.tmem();
   const int K = o.K;
   float m = -INFINITY, s = 0.0f, a_prev = 0.0f;
   if (t == 0) {   // prefetch the first two component records
-    mbar_expect_tx(&sm.bbar[0], TC_REC_BYTES);
-    bulk_g2s(sm.B[0], o.recs, TC_REC_BYTES, &sm.bbar[0]);
+    mbar_expect_tx(sm.bbar(0), TC_REC_BYTES);
+    bulk_g2s(sm.B(0), o.recs, TC_REC_BYTES, sm.bbar(0));
     if (K > 1) {
-      mbar_expect_tx(&sm.bbar[1], TC_REC_BYTES);
-      bulk_g2s(sm.B[1], o.recs + TC_REC, TC_REC_BYTES, &sm.bbar[1]);
+      mbar_expect_tx(sm.bbar(1), TC_REC_BYTES);
+      bulk_g2s(sm.B(1), o.recs + TC_REC, TC_REC_BYTES, sm.bbar(1));
     }
   }
   auto epilogue = [&](int j, float a_j) {
     const int st = j & 1;
-    mbar_wait(&sm.mbar[st], (j >> 1) & 1);
+    mbar_wait(sm.mbar(st), (j >> 1) & 1);
     asm volatile("tcgen05.fence::after_thread_sync;");
     if (t == 0 && j + 2 < K) {   // stage st of B is free again: fetch component j + 2
-      mbar_expect_tx(&sm.bbar[st], TC_REC_BYTES);
-      bulk_g2s(sm.B[st], o.recs + (size_t)(j + 2) * TC_REC, TC_REC_BYTES, &sm.bbar[st]);
+      mbar_expect_tx(sm.bbar(st), TC_REC_BYTES);
+      bulk_g2s(sm.B(st), o.recs + (size_t)(j + 2) * TC_REC, TC_REC_BYTES, sm.bbar(st));
     }
     __syncwarp();
     uint32_t r[64];
@@ -150,10 +144,10 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
   };
   for (int k = 0; k < K; ++k) {
     const int st = k & 1;
-    mbar_wait(&sm.bbar[st], (k >> 1) & 1);            // W_k hi/lo, mu_k, a_k have landed
-    const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B[st] + 2 * TC_D * TC_D);
-    const float a_k = sm.B[st][2 * TC_D * TC_D + TC_D];
-    unsigned char *Ah = sm.A[st][0] + t * 16, *Al = sm.A[st][1] + t * 16;
+    mbar_wait(sm.bbar(st), (k >> 1) & 1);            // W_k hi/lo, mu_k, a_k have landed
+    const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(st) + 2 * TC_D * TC_D);
+    const float a_k = sm.B(st)[2 * TC_D * TC_D + TC_D];
+    unsigned char *Ah = sm.A(st, 0) + t * 16, *Al = sm.A(st, 1) + t * 16;
 #pragma unroll
     for (int c4 = 0; c4 < TC_D / 4; ++c4) {           // this thread's row of D_hi / D_lo
       const float4 mu = mu4[c4];
@@ -170,8 +164,8 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
     if (t == 0) {
       asm volatile("tcgen05.fence::after_thread_sync;");
       // descriptors differ only in the 14-bit start-address field: add (byte offset >> 4) to the base
-      const uint64_t dAh = tc_desc(smem_u32(sm.A[st][0]), 2048, 128), dAl = tc_desc(smem_u32(sm.A[st][1]), 2048, 128);
-      const uint64_t dBh = tc_desc(smem_u32(sm.B[st]), 1024, 128), dBl = tc_desc(smem_u32(sm.B[st]) + TC_D * TC_D * 4, 1024, 128);
+      const uint64_t dAh = tc_desc(smem_u32(sm.A(st, 0)), 2048, 128), dAl = tc_desc(smem_u32(sm.A(st, 1)), 2048, 128);
+      const uint64_t dBh = tc_desc(smem_u32(sm.B(st)), 1024, 128), dBl = tc_desc(smem_u32(sm.B(st)) + TC_D * TC_D * 4, 1024, 128);
       const uint32_t dcol = tm + (uint32_t)(st * 64);
 #pragma unroll
       for (int pr = 0; pr < 3; ++pr) {
@@ -180,7 +174,7 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
         for (int ks = 0; ks < 8; ++ks)
           tc_mma(dcol, a0 + (uint64_t)(ks * (4096 >> 4)), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
       }
-      tc_commit(&sm.mbar[st]);
+      tc_commit(sm.mbar(st));
     }
     __syncwarp();
     if (k > 0) epilogue(k - 1, a_prev);

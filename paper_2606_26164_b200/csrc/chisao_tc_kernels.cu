@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_eval_fd_tc(const TcObj o, const F
     // replace coordinate j through a shared-memory round trip of the thread's own row: a dynamically indexed
     // register array would be lowered to a branch tree over j, and the warp-collective tcgen05 instructions
     // below need every lane on the same path
-    float *own = reinterpret_cast<float *>(sm.A[1][0]) + t * 68;
+    float *own = reinterpret_cast<float *>(sm.A(1, 0)) + t * 68;
 #pragma unroll
     for (int c4 = 0; c4 < TC_D / 4; ++c4)
       *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
@@ -180,8 +180,8 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_hlc_tc(const TcObj o, const HlcAr
   }
   float val = tc_eval_tile<OBJ>(o, sm, x, t);
   __syncthreads();                       // every MMA has retired: the operand buffers are free
-  float *Us = reinterpret_cast<float *>(sm.A[0][0]);          // [128][65] normals (A[0][0..1] = 64 KB)
-  float *fvs = reinterpret_cast<float *>(sm.A[1][0]);         // [128] values
+  float *Us = reinterpret_cast<float *>(sm.A(0, 0));          // [128][65] normals (A[0][0..1] = 64 KB)
+  float *fvs = reinterpret_cast<float *>(sm.A(1, 0));         // [128] values
   if (valid) {
     val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
     a.hlc_f[(size_t)i * M + k] = val;
