@@ -1,29 +1,32 @@
 // chisao_tc.cuh -- tensor-core evaluator for the dense objectives at d > 32 (GMM_FULL, QUAD; DP = 64).
 //
-// The quadratic forms q_k(x) = || W_k (x - mu_k) ||^2 of a tile of 128 points are a dense contraction
+// The quadratic forms q_k(x) = || W_k (x - mu_k) ||^2 of a group of 128 points are a dense contraction
 // Z_k[128 x 64] = D_k[128 x 64] * W_k^T[64 x 64] (BASELINE.json north_star: "tensor cores ... full-covariance
 // mixture quadratic forms").  It runs on the 5th-generation tensor cores: tcgen05.mma kind::tf32, M = 128,
 // N = 64, K = 8 per instruction, accumulators in TMEM, fp32 accuracy by the 3xTF32 split
 //     D W^T ~= D_hi W_hi^T + D_lo W_hi^T + D_hi W_lo^T          (hi = rna-tf32(v), lo = rna-tf32(v - hi)),
-// 24 MMAs per component.  Thread t of the CTA owns point t (= TMEM lane t): it builds its row of D_hi / D_lo
+// 24 MMAs per component.  Thread t of a group owns point t (= TMEM lane t): it builds its row of D_hi / D_lo
 // in shared memory in the canonical K-major no-swizzle UMMA layout (16-byte K-chunks of 8 consecutive rows form
 // a 128-byte core matrix; byte offset of element (p, c) = (c/4)*2048 + p*16 + (c%4)*4), one thread issues the
 // MMAs, and every thread reads its 64 accumulators back with tcgen05.ld for the epilogue (sum of squares,
 // online log-sum-exp).  W_k hi/lo are split and laid out on the host once (byte offset of (n, c) =
-// (c/4)*1024 + n*16 + (c%4)*4) and streamed by the bulk-copy engine; A and TMEM are double-buffered so the
-// MMAs of component k overlap the epilogue of k-1 and the operand build of k+1.
+// (c/4)*1024 + n*16 + (c%4)*4) and streamed by a dedicated warp through two stages with the bulk-copy engine.
+// A CTA evaluates 256 points as two groups of 128 threads; each group has its own operand buffers, accumulator
+// columns and MMA mbarrier, so one group's MMAs run while the other builds operands / drains its accumulators.
 #pragma once
 #include "chisao_device.cuh"
 
 namespace chisao {
 
-constexpr int TC_PTS = 128;                              // points per CTA tile (= threads = TMEM lanes)
+constexpr int TC_GROUP = 128;                            // threads per group = points per MMA tile = TMEM lanes
+constexpr int TC_PTS = 256;                              // points per CTA tile: two groups ping-pong on the tensor pipe
+constexpr int TC_THREADS = TC_PTS + 32;                  // + one warp that streams the component records
 constexpr int TC_D = 64;
 constexpr int TC_REC = 2 * TC_D * TC_D + TC_D + 4;       // floats per component: W_hi | W_lo | mu | a,0,0,0
 constexpr int TC_REC_BYTES = TC_REC * 4;                 // 33 040 (multiple of 16)
-constexpr int TC_A_BYTES = TC_PTS * TC_D * 4;            // 32 768 per operand image
-constexpr int TC_SMEM_BYTES = 1024 + 4 * TC_A_BYTES + 2 * TC_REC_BYTES;   // barriers | A hi/lo x2 | B x2
-constexpr uint32_t TC_TMEM_COLS = 128;                   // 2 accumulator stages of 64 fp32 columns
+constexpr int TC_A_BYTES = TC_GROUP * TC_D * 4;          // 32 768 per operand image
+constexpr int TC_SMEM_BYTES = 1024 + 4 * TC_A_BYTES + 2 * TC_REC_BYTES;   // barriers | A[group][hi/lo] | B x2
+constexpr uint32_t TC_TMEM_COLS = 128;                   // one 64-column fp32 accumulator per group
 
 struct TcObj {
   int32_t K, d;
@@ -32,13 +35,15 @@ struct TcObj {
 };
 
 // shared-memory carve (all offsets are arithmetic so that nothing is indexed dynamically through a pointer table):
-//   [0,16) bbar[2] | [16,32) mbar[2] | [64,68) TMEM base | [1024, +4*32K) A[stage][hi/lo] | then B[stage] records
+//   [0,16) bbar[2] B landed | [16,32) mbar[2] MMAs of a group retired | [32,48) fbar[2] B stage free (count 2)
+//   [64,68) TMEM base | [1024, +4*32K) A[group][hi/lo] | then B[stage] records
 struct TcSmem {
   unsigned char *base;
   __device__ __forceinline__ uint64_t *bbar(int st) const { return reinterpret_cast<uint64_t *>(base) + st; }
-  __device__ __forceinline__ uint64_t *mbar(int st) const { return reinterpret_cast<uint64_t *>(base) + 2 + st; }
+  __device__ __forceinline__ uint64_t *mbar(int g) const { return reinterpret_cast<uint64_t *>(base) + 2 + g; }
+  __device__ __forceinline__ uint64_t *fbar(int st) const { return reinterpret_cast<uint64_t *>(base) + 4 + st; }
   __device__ __forceinline__ uint32_t *tmem() const { return reinterpret_cast<uint32_t *>(base + 64); }
-  __device__ __forceinline__ unsigned char *A(int st, int lo) const { return base + 1024 + (st * 2 + lo) * TC_A_BYTES; }
+  __device__ __forceinline__ unsigned char *A(int g, int lo) const { return base + 1024 + (g * 2 + lo) * TC_A_BYTES; }
   __device__ __forceinline__ float *B(int st) const {
     return reinterpret_cast<float *>(base + 1024 + 4 * TC_A_BYTES + st * TC_REC_BYTES);
   }
@@ -77,7 +82,14 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[64], int q
       : "r"(taddr + 16 * q));
 }
 
-// one-time CTA setup / teardown (all 128 threads)
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void group_sync(int g) {   // named barrier of the 128 threads of group g (ids 1, 2)
+  asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(TC_GROUP) : "memory");
+}
+
+// one-time CTA setup / teardown (all TC_THREADS threads)
 __device__ __forceinline__ void tc_setup(const TcSmem &sm, int t) {
   if (t < 32) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(sm.tmem())), "n"(TC_TMEM_COLS));
@@ -85,6 +97,7 @@ __device__ __forceinline__ void tc_setup(const TcSmem &sm, int t) {
   }
   if (t == 32) {
     mbar_init(sm.bbar(0), 1); mbar_init(sm.bbar(1), 1); mbar_init(sm.mbar(0), 1); mbar_init(sm.mbar(1), 1);
+    mbar_init(sm.fbar(0), 2); mbar_init(sm.fbar(1), 2);
     mbar_fence_init();
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
@@ -97,32 +110,67 @@ __device__ __forceinline__ void tc_teardown(const TcSmem &sm, int t) {
   if (t < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*sm.tmem()), "n"(TC_TMEM_COLS));
 }
 
-// Evaluate the calling thread's point x[64] (coordinates >= d must be zero).  All 128 threads of the CTA must
-// call (barriers inside); tc_setup must have run.  OBJ is CHISAO_OBJ_GMM_FULL or CHISAO_OBJ_QUAD.
+// Streams the K component records through the two B stages (called by the loader warp, t >= TC_PTS).
+__device__ __forceinline__ void tc_loader(const TcObj &o, const TcSmem &sm, int t) {
+  if (t != TC_PTS) return;
+  for (int k = 0; k < o.K; ++k) {
+    const int st = k & 1;
+    if (k >= 2) mbar_wait(sm.fbar(st), ((k >> 1) - 1) & 1);   // both groups are done with component k - 2
+    mbar_expect_tx(sm.bbar(st), TC_REC_BYTES);
+    bulk_g2s(sm.B(st), o.recs + (size_t)k * TC_REC, TC_REC_BYTES, sm.bbar(st));
+  }
+}
+
+// Evaluate the calling thread's point x[64] (coordinates >= d must be zero).  Called by the 256 compute threads
+// (t < TC_PTS) while the loader warp runs tc_loader; tc_setup must have run.  Group g = t / 128 owns operand
+// buffers A(g, .), accumulator columns [64 g, 64 g + 64) and mbarrier mbar(g); the two groups share the B stages
+// and alternate on the tensor pipe: while one group's 24 MMAs run, the other builds its next operand / reads its
+// accumulators.  OBJ is CHISAO_OBJ_GMM_FULL or CHISAO_OBJ_QUAD.
 template <int OBJ>
 __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
   const uint32_t tm = *sm.tmem();
-  const int K = o.K;
-  float m = -INFINITY, s = 0.0f, a_prev = 0.0f;
-  if (t == 0) {   // prefetch the first two component records
-    mbar_expect_tx(sm.bbar(0), TC_REC_BYTES);
-    bulk_g2s(sm.B(0), o.recs, TC_REC_BYTES, sm.bbar(0));
-    if (K > 1) {
-      mbar_expect_tx(sm.bbar(1), TC_REC_BYTES);
-      bulk_g2s(sm.B(1), o.recs + TC_REC, TC_REC_BYTES, sm.bbar(1));
+  const int K = o.K, g = t >> 7, tl = t & (TC_GROUP - 1);
+  float m = -INFINITY, s = 0.0f;
+  unsigned char *Ah = sm.A(g, 0) + tl * 16, *Al = sm.A(g, 1) + tl * 16;
+  const uint64_t dAh = tc_desc(smem_u32(sm.A(g, 0)), 2048, 128), dAl = tc_desc(smem_u32(sm.A(g, 1)), 2048, 128);
+  const uint32_t dcol = tm + (uint32_t)(g * 64);
+  const uint32_t taddr = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 64);
+  for (int k = 0; k < K; ++k) {
+    const int st = k & 1;
+    mbar_wait(sm.bbar(st), (k >> 1) & 1);             // W_k hi/lo, mu_k, a_k have landed
+    const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(st) + 2 * TC_D * TC_D);
+    const float a_k = sm.B(st)[2 * TC_D * TC_D + TC_D];
+#pragma unroll
+    for (int c4 = 0; c4 < TC_D / 4; ++c4) {           // this thread's row of D_hi / D_lo
+      const float4 mu = mu4[c4];
+      const float d0 = x[4 * c4] - mu.x, d1 = x[4 * c4 + 1] - mu.y, d2 = x[4 * c4 + 2] - mu.z, d3 = x[4 * c4 + 3] - mu.w;
+      float4 h, l;
+      h.x = tf32_rna(d0); h.y = tf32_rna(d1); h.z = tf32_rna(d2); h.w = tf32_rna(d3);
+      l.x = tf32_rna(d0 - h.x); l.y = tf32_rna(d1 - h.y); l.z = tf32_rna(d2 - h.z); l.w = tf32_rna(d3 - h.w);
+      *reinterpret_cast<float4 *>(Ah + c4 * 2048) = h;
+      *reinterpret_cast<float4 *>(Al + c4 * 2048) = l;
     }
-  }
-  auto epilogue = [&](int j, float a_j) {
-    const int st = j & 1;
-    mbar_wait(sm.mbar(st), (j >> 1) & 1);
-    asm volatile("tcgen05.fence::after_thread_sync;");
-    if (t == 0 && j + 2 < K) {   // stage st of B is free again: fetch component j + 2
-      mbar_expect_tx(sm.bbar(st), TC_REC_BYTES);
-      bulk_g2s(sm.B(st), o.recs + (size_t)(j + 2) * TC_REC, TC_REC_BYTES, sm.bbar(st));
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> async-proxy (MMA) reads
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    group_sync(g);
+    if (tl == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      const uint64_t dBh = tc_desc(smem_u32(sm.B(st)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
+#pragma unroll
+      for (int pr = 0; pr < 3; ++pr) {
+        const uint64_t a0 = (pr == 1) ? dAl : dAh, b0 = (pr == 2) ? dBl : dBh;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          tc_mma(dcol, a0 + (uint64_t)(ks * (4096 >> 4)), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
+      }
+      tc_commit(sm.mbar(g));
     }
     __syncwarp();
+    mbar_wait(sm.mbar(g), k & 1);                     // this group's MMAs of component k have retired
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (tl == 0) mbar_arrive(sm.fbar(st));            // B stage st is no longer needed by this group
+    __syncwarp();
     uint32_t r[64];
-    const uint32_t taddr = tm + ((uint32_t)((t >> 5) * 32) << 16) + (uint32_t)(st * 64);
     tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
     float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
@@ -136,51 +184,12 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
     if constexpr (OBJ == CHISAO_OBJ_QUAD) {
       s += q;
     } else {
-      const float v = fmaf(-0.5f, q, a_j);
+      const float v = fmaf(-0.5f, q, a_k);
       const float mn = fmaxf(m, v);
       if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
     }
-    asm volatile("tcgen05.fence::before_thread_sync;");
-  };
-  for (int k = 0; k < K; ++k) {
-    const int st = k & 1;
-    mbar_wait(sm.bbar(st), (k >> 1) & 1);            // W_k hi/lo, mu_k, a_k have landed
-    const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(st) + 2 * TC_D * TC_D);
-    const float a_k = sm.B(st)[2 * TC_D * TC_D + TC_D];
-    unsigned char *Ah = sm.A(st, 0) + t * 16, *Al = sm.A(st, 1) + t * 16;
-#pragma unroll
-    for (int c4 = 0; c4 < TC_D / 4; ++c4) {           // this thread's row of D_hi / D_lo
-      const float4 mu = mu4[c4];
-      const float d0 = x[4 * c4] - mu.x, d1 = x[4 * c4 + 1] - mu.y, d2 = x[4 * c4 + 2] - mu.z, d3 = x[4 * c4 + 3] - mu.w;
-      float4 h, l;
-      h.x = tf32_rna(d0); h.y = tf32_rna(d1); h.z = tf32_rna(d2); h.w = tf32_rna(d3);
-      l.x = tf32_rna(d0 - h.x); l.y = tf32_rna(d1 - h.y); l.z = tf32_rna(d2 - h.z); l.w = tf32_rna(d3 - h.w);
-      *reinterpret_cast<float4 *>(Ah + c4 * 2048) = h;
-      *reinterpret_cast<float4 *>(Al + c4 * 2048) = l;
-    }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> async-proxy (MMA) reads
-    asm volatile("tcgen05.fence::before_thread_sync;");
-    __syncthreads();
-    if (t == 0) {
-      asm volatile("tcgen05.fence::after_thread_sync;");
-      // descriptors differ only in the 14-bit start-address field: add (byte offset >> 4) to the base
-      const uint64_t dAh = tc_desc(smem_u32(sm.A(st, 0)), 2048, 128), dAl = tc_desc(smem_u32(sm.A(st, 1)), 2048, 128);
-      const uint64_t dBh = tc_desc(smem_u32(sm.B(st)), 1024, 128), dBl = tc_desc(smem_u32(sm.B(st)) + TC_D * TC_D * 4, 1024, 128);
-      const uint32_t dcol = tm + (uint32_t)(st * 64);
-#pragma unroll
-      for (int pr = 0; pr < 3; ++pr) {
-        const uint64_t a0 = (pr == 1) ? dAl : dAh, b0 = (pr == 2) ? dBl : dBh;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks)
-          tc_mma(dcol, a0 + (uint64_t)(ks * (4096 >> 4)), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
-      }
-      tc_commit(sm.mbar(st));
-    }
-    __syncwarp();
-    if (k > 0) epilogue(k - 1, a_prev);
-    a_prev = a_k;
+    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
   }
-  epilogue(K - 1, a_prev);
   if constexpr (OBJ == CHISAO_OBJ_QUAD) return -0.5f * s;
   return m + logf(s);
 }

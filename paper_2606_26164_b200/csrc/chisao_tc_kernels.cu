@@ -1,11 +1,13 @@
 // chisao_tc_kernels.cu -- the three evaluation kernels (FD stencil, one point per sample, Hands Like Clouds)
 // on the tensor-core evaluator of chisao_tc.cuh, for GMM_FULL and QUAD at 32 < d <= 64.  Same arguments, same
-// noise slots, same epilogues as the FFMA kernels of chisao_eval_kernels.cuh; one point per thread, 128 points
-// per CTA.  Citations: PAPER.md:62, :555 (FD), :75-82 (line search), :113-120 + Eq. 9 :577 (HLC), Eq. 6 :126.
+// noise slots, same epilogues as the FFMA kernels of chisao_eval_kernels.cuh; one point per compute thread, 256
+// points per CTA (two groups of 128 ping-pong on the tensor pipe) plus one warp that streams the parameters.  Citations: PAPER.md:62, :555 (FD), :75-82 (line search), :113-120 + Eq. 9 :577 (HLC), Eq. 6 :126.
 #include "chisao_eval_kernels.cuh"
 #include "chisao_tc.cuh"
 
 namespace chisao {
+
+__device__ __forceinline__ void compute_sync() { asm volatile("bar.sync 3, %0;" ::"n"(TC_PTS) : "memory"); }
 
 __device__ __forceinline__ void tc_load_row(const float *row, int d, bool vec, float (&x)[TC_D]) {
 #pragma unroll
@@ -17,7 +19,7 @@ __device__ __forceinline__ void tc_load_row(const float *row, int d, bool vec, f
 
 // thread t -> (sample t / 2d of the tile, slot t % 2d); slot 2j = x + h e_j, 2j + 1 = x - h e_j
 template <int OBJ>
-__global__ void __launch_bounds__(TC_PTS, 1) k_eval_fd_tc(const TcObj o, const FdArgs a) {
+__global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, const FdArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
   const TcSmem sm = tc_carve(tc_smem_raw);
   const int t = threadIdx.x, d = a.d;
@@ -26,6 +28,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_eval_fd_tc(const TcObj o, const F
   const int first = blockIdx.x * spt;
   if (first >= cnt) return;
   tc_setup(sm, t);
+  if (t >= TC_PTS) { tc_loader(o, sm, t); tc_teardown(sm, t); return; }
   const int s = t / (2 * d), slot = t - s * 2 * d, j = slot >> 1;
   const bool valid = (s < spt) && (first + s < cnt);
   const int i = valid ? (a.list ? a.list[first + s] : first + s) : 0;
@@ -39,7 +42,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_eval_fd_tc(const TcObj o, const F
     // replace coordinate j through a shared-memory round trip of the thread's own row: a dynamically indexed
     // register array would be lowered to a branch tree over j, and the warp-collective tcgen05 instructions
     // below need every lane on the same path
-    float *own = reinterpret_cast<float *>(sm.A(1, 0)) + t * 68;
+    float *own = reinterpret_cast<float *>(sm.A(0, 0)) + t * 68;
 #pragma unroll
     for (int c4 = 0; c4 < TC_D / 4; ++c4)
       *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
@@ -54,6 +57,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_eval_fd_tc(const TcObj o, const F
 #pragma unroll
     for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
   }
+  compute_sync();                        // the scratch rows overlap the operand buffers: everyone has read back
   float f = tc_eval_tile<OBJ>(o, sm, x, t);
   if (valid) f += eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, 1 + slot);
   // partner lane holds the other sign of the same coordinate
@@ -75,7 +79,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_eval_fd_tc(const TcObj o, const F
 }
 
 template <int OBJ>
-__global__ void __launch_bounds__(TC_PTS, 1) k_eval_points_tc(const TcObj o, const PtArgs a) {
+__global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o, const PtArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
   const TcSmem sm = tc_carve(tc_smem_raw);
   const int t = threadIdx.x, d = a.d;
@@ -84,6 +88,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_eval_points_tc(const TcObj o, con
   if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
   if (first >= cnt) return;
   tc_setup(sm, t);
+  if (t >= TC_PTS) { tc_loader(o, sm, t); tc_teardown(sm, t); return; }
   const int e = first + t;
   const bool valid = e < cnt;
   const int i = valid ? (a.list ? a.list[e] : e) : 0;
@@ -155,7 +160,7 @@ __device__ __forceinline__ void hlc_normals(uint64_t seed, int i, int cycle, int
 
 // Hands Like Clouds on the tensor-core evaluator: point t of the tile = (sample t / M, draw t % M), M <= 128
 template <int OBJ>
-__global__ void __launch_bounds__(TC_PTS, 1) k_hlc_tc(const TcObj o, const HlcArgs a) {
+__global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const HlcArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
   const TcSmem sm = tc_carve(tc_smem_raw);
   const int t = threadIdx.x, d = a.d, M = a.M;
@@ -164,6 +169,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_hlc_tc(const TcObj o, const HlcAr
   const int first = blockIdx.x * spt;
   if (first >= cnt) return;
   tc_setup(sm, t);
+  if (t >= TC_PTS) { tc_loader(o, sm, t); tc_teardown(sm, t); return; }
   const int s = t / M, k = t - s * M;
   const bool valid = (s < spt) && (first + s < cnt);
   const int i = valid ? a.list[first + s] : 0;
@@ -179,9 +185,9 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_hlc_tc(const TcObj o, const HlcAr
     for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
   }
   float val = tc_eval_tile<OBJ>(o, sm, x, t);
-  __syncthreads();                       // every MMA has retired: the operand buffers are free
-  float *Us = reinterpret_cast<float *>(sm.A(0, 0));          // [128][65] normals (A[0][0..1] = 64 KB)
-  float *fvs = reinterpret_cast<float *>(sm.A(1, 0));         // [128] values
+  compute_sync();                        // every MMA has retired: the operand buffers are free
+  float *Us = reinterpret_cast<float *>(sm.A(0, 0));          // [256][65] normals (the A region is 128 KB)
+  float *fvs = Us + TC_PTS * 65;                              // [256] values
   if (valid) {
     val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
     a.hlc_f[(size_t)i * M + k] = val;
@@ -193,7 +199,7 @@ __global__ void __launch_bounds__(TC_PTS, 1) k_hlc_tc(const TcObj o, const HlcAr
     val = 0.f;
   }
   fvs[t] = val;
-  __syncthreads();
+  compute_sync();
   const int nval = min(spt, cnt - first);
   for (int item = t; item < nval * d; item += TC_PTS) {
     const int ss = item / d, j = item - ss * d;
@@ -224,21 +230,21 @@ cudaError_t tc_configure() {
 cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samples, cudaStream_t st) {
   const int spt = TC_PTS / (2 * a.d);
   const int grid = (n_samples + spt - 1) / spt;
-  if (obj_id == CHISAO_OBJ_QUAD) k_eval_fd_tc<CHISAO_OBJ_QUAD><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
-  else k_eval_fd_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  if (obj_id == CHISAO_OBJ_QUAD) k_eval_fd_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
+  else k_eval_fd_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
 cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samples, cudaStream_t st) {
   const int grid = (n_samples + TC_PTS - 1) / TC_PTS;
-  if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
-  else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
+  else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
 cudaError_t launch_hlc_tc(int obj_id, const TcObj &o, const HlcArgs &a, int n_samples, cudaStream_t st) {
   const int spt = TC_PTS / a.M < HLC_MAX_SPT ? TC_PTS / a.M : HLC_MAX_SPT;
   const int grid = (n_samples + spt - 1) / spt;
-  if (obj_id == CHISAO_OBJ_QUAD) k_hlc_tc<CHISAO_OBJ_QUAD><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
-  else k_hlc_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_PTS, TC_SMEM_BYTES, st>>>(o, a);
+  if (obj_id == CHISAO_OBJ_QUAD) k_hlc_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
+  else k_hlc_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
 
