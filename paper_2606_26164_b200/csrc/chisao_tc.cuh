@@ -4,13 +4,14 @@
 // Z_k[128 x 64] = D_k[128 x 64] * W_k^T[64 x 64] (BASELINE.json north_star: "tensor cores ... full-covariance
 // mixture quadratic forms").  It runs on the 5th-generation tensor cores: tcgen05.mma kind::tf32, M = 128,
 // N = 64, K = 8 per instruction, accumulators in TMEM, fp32 accuracy by the 3xTF32 split
-//     D W^T ~= D_hi W_hi^T + D_lo W_hi^T + D_hi W_lo^T          (hi = rna-tf32(v), lo = rna-tf32(v - hi)),
-// 24 MMAs per component.  Thread t of a group owns point t (= TMEM lane t): it builds its row of D_hi / D_lo
-// in shared memory in the canonical K-major no-swizzle UMMA layout (16-byte K-chunks of 8 consecutive rows form
-// a 128-byte core matrix; byte offset of element (p, c) = (c/4)*2048 + p*16 + (c%4)*4), one thread issues the
-// MMAs, and every thread reads its 64 accumulators back with tcgen05.ld for the epilogue (sum of squares,
-// online log-sum-exp).  W_k hi/lo are split and laid out on the host once (byte offset of (n, c) =
-// (c/4)*1024 + n*16 + (c%4)*4) and streamed by a dedicated warp through two stages with the bulk-copy engine.
+//     D W^T ~= D_hi W_hi^T + D_lo W_hi^T + D_hi W_lo^T          (hi = rna-tf32(v), lo = v - hi),
+// 24 MMAs per component.  Thread t of a group owns point t (= TMEM lane t): it writes its row of D_hi / D_lo
+// straight into its TMEM lane with tcgen05.st (the A operand is read from TMEM, element c in column c, so the
+// MMA fetches only W from shared memory), one thread issues the MMAs, and every thread reads its 64
+// accumulators back with tcgen05.ld for the epilogue (sum of squares, online log-sum-exp).  W_k hi/lo are split
+// and laid out on the host once in the canonical K-major no-swizzle UMMA layout (16-byte K-chunks of 8 rows form
+// a 128-byte core matrix; byte offset of (n, c) = (c/4)*1024 + n*16 + (c%4)*4) and streamed by a dedicated warp
+// through two stages with the bulk-copy engine.
 // A CTA evaluates 256 points as two groups of 128 threads; each group has its own operand buffers, accumulator
 // columns and MMA mbarrier, so one group's MMAs run while the other builds operands / drains its accumulators.
 #pragma once
@@ -25,8 +26,9 @@ constexpr int TC_D = 64;
 constexpr int TC_REC = 2 * TC_D * TC_D + TC_D + 4;       // floats per component: W_hi | W_lo | mu | a,0,0,0
 constexpr int TC_REC_BYTES = TC_REC * 4;                 // 33 040 (multiple of 16)
 constexpr int TC_A_BYTES = TC_GROUP * TC_D * 4;          // 32 768 per operand image
-constexpr int TC_SMEM_BYTES = 1024 + 4 * TC_A_BYTES + 2 * TC_REC_BYTES;   // barriers | A[group][hi/lo] | B x2
-constexpr uint32_t TC_TMEM_COLS = 128;                   // one 64-column fp32 accumulator per group
+constexpr int TC_SCRATCH_BYTES = 72 * 1024;               // kernel scratch (FD row patch, HLC normals)
+constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TC_REC_BYTES;   // barriers | scratch | B x2
+constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D 64 | D_hi 64 | D_lo 64
 
 struct TcObj {
   int32_t K, d;
@@ -36,16 +38,16 @@ struct TcObj {
 
 // shared-memory carve (all offsets are arithmetic so that nothing is indexed dynamically through a pointer table):
 //   [0,16) bbar[2] B landed | [16,32) mbar[2] MMAs of a group retired | [32,48) fbar[2] B stage free (count 2)
-//   [64,68) TMEM base | [1024, +4*32K) A[group][hi/lo] | then B[stage] records
+//   [64,68) TMEM base | [1024, +72K) kernel scratch | then B[stage] records
 struct TcSmem {
   unsigned char *base;
   __device__ __forceinline__ uint64_t *bbar(int st) const { return reinterpret_cast<uint64_t *>(base) + st; }
   __device__ __forceinline__ uint64_t *mbar(int g) const { return reinterpret_cast<uint64_t *>(base) + 2 + g; }
   __device__ __forceinline__ uint64_t *fbar(int st) const { return reinterpret_cast<uint64_t *>(base) + 4 + st; }
   __device__ __forceinline__ uint32_t *tmem() const { return reinterpret_cast<uint32_t *>(base + 64); }
-  __device__ __forceinline__ unsigned char *A(int g, int lo) const { return base + 1024 + (g * 2 + lo) * TC_A_BYTES; }
+  __device__ __forceinline__ unsigned char *scratch() const { return base + 1024; }
   __device__ __forceinline__ float *B(int st) const {
-    return reinterpret_cast<float *>(base + 1024 + 4 * TC_A_BYTES + st * TC_REC_BYTES);
+    return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * TC_REC_BYTES);
   }
 };
 __device__ __forceinline__ TcSmem tc_carve(unsigned char *base) { TcSmem s; s.base = base; return s; }
@@ -68,6 +70,19 @@ __device__ __forceinline__ void tc_mma(uint32_t tmem_d, uint64_t da, uint64_t db
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
       "l"(da), "l"(db), "r"(TC_IDESC), "r"(accumulate));
+}
+__device__ __forceinline__ void tc_mma_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "r"(tmem_a), "l"(db), "r"(TC_IDESC), "r"(accumulate));
+}
+__device__ __forceinline__ void tc_st16(uint32_t taddr, const float (&v)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+      "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]), "f"(v[8]), "f"(v[9]),
+      "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
+      : "memory");
 }
 __device__ __forceinline__ void tc_commit(uint64_t *bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -123,7 +138,7 @@ __device__ __forceinline__ void tc_loader(const TcObj &o, const TcSmem &sm, int 
 
 // Evaluate the calling thread's point x[64] (coordinates >= d must be zero).  Called by the 256 compute threads
 // (t < TC_PTS) while the loader warp runs tc_loader; tc_setup must have run.  Group g = t / 128 owns operand
-// buffers A(g, .), accumulator columns [64 g, 64 g + 64) and mbarrier mbar(g); the two groups share the B stages
+// TMEM columns [256 g, 256 g + 192) (accumulator | D_hi | D_lo) and mbarrier mbar(g); the two groups share the B stages
 // and alternate on the tensor pipe: while one group's 24 MMAs run, the other builds its next operand / reads its
 // accumulators.  OBJ is CHISAO_OBJ_GMM_FULL or CHISAO_OBJ_QUAD.
 template <int OBJ>
@@ -131,26 +146,32 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
   const uint32_t tm = *sm.tmem();
   const int K = o.K, g = t >> 7, tl = t & (TC_GROUP - 1);
   float m = -INFINITY, s = 0.0f;
-  unsigned char *Ah = sm.A(g, 0) + tl * 16, *Al = sm.A(g, 1) + tl * 16;
-  const uint64_t dAh = tc_desc(smem_u32(sm.A(g, 0)), 2048, 128), dAl = tc_desc(smem_u32(sm.A(g, 1)), 2048, 128);
-  const uint32_t dcol = tm + (uint32_t)(g * 64);
-  const uint32_t taddr = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 64);
+  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
+  const uint32_t dcol = tm + (uint32_t)(g * 256), acol_hi = dcol + 64, acol_lo = dcol + 128;
+  const uint32_t taddr = lane_base;
   for (int k = 0; k < K; ++k) {
     const int st = k & 1;
     mbar_wait(sm.bbar(st), (k >> 1) & 1);             // W_k hi/lo, mu_k, a_k have landed
     const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(st) + 2 * TC_D * TC_D);
     const float a_k = sm.B(st)[2 * TC_D * TC_D + TC_D];
+    // this thread's row of D_hi / D_lo goes straight into its TMEM lane (A operand read from TMEM: the MMA then
+    // fetches only W from shared memory)
 #pragma unroll
-    for (int c4 = 0; c4 < TC_D / 4; ++c4) {           // this thread's row of D_hi / D_lo
-      const float4 mu = mu4[c4];
-      const float d0 = x[4 * c4] - mu.x, d1 = x[4 * c4 + 1] - mu.y, d2 = x[4 * c4 + 2] - mu.z, d3 = x[4 * c4 + 3] - mu.w;
-      float4 h, l;
-      h.x = tf32_rna(d0); h.y = tf32_rna(d1); h.z = tf32_rna(d2); h.w = tf32_rna(d3);
-      l.x = tf32_rna(d0 - h.x); l.y = tf32_rna(d1 - h.y); l.z = tf32_rna(d2 - h.z); l.w = tf32_rna(d3 - h.w);
-      *reinterpret_cast<float4 *>(Ah + c4 * 2048) = h;
-      *reinterpret_cast<float4 *>(Al + c4 * 2048) = l;
+    for (int q = 0; q < 4; ++q) {
+      float h[16], l[16];
+#pragma unroll
+      for (int c4 = 0; c4 < 4; ++c4) {
+        const float4 mu = mu4[4 * q + c4];
+        const int c = 16 * q + 4 * c4;
+        const float d0 = x[c] - mu.x, d1 = x[c + 1] - mu.y, d2 = x[c + 2] - mu.z, d3 = x[c + 3] - mu.w;
+        h[4 * c4] = tf32_rna(d0); h[4 * c4 + 1] = tf32_rna(d1); h[4 * c4 + 2] = tf32_rna(d2); h[4 * c4 + 3] = tf32_rna(d3);
+        // d - hi is exact in fp32 with at most 13 significant bits; the MMA reads its top 11 (residual 2^-22 |d|)
+        l[4 * c4] = d0 - h[4 * c4]; l[4 * c4 + 1] = d1 - h[4 * c4 + 1]; l[4 * c4 + 2] = d2 - h[4 * c4 + 2]; l[4 * c4 + 3] = d3 - h[4 * c4 + 3];
+      }
+      tc_st16(lane_base + 64 + 16 * q, h);
+      tc_st16(lane_base + 128 + 16 * q, l);
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> async-proxy (MMA) reads
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;");
     group_sync(g);
     if (tl == 0) {
@@ -158,10 +179,11 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
       const uint64_t dBh = tc_desc(smem_u32(sm.B(st)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
 #pragma unroll
       for (int pr = 0; pr < 3; ++pr) {
-        const uint64_t a0 = (pr == 1) ? dAl : dAh, b0 = (pr == 2) ? dBl : dBh;
+        const uint32_t a0 = (pr == 1) ? acol_lo : acol_hi;
+        const uint64_t b0 = (pr == 2) ? dBl : dBh;
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks)
-          tc_mma(dcol, a0 + (uint64_t)(ks * (4096 >> 4)), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
+          tc_mma_ts(dcol, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
       }
       tc_commit(sm.mbar(g));
     }

@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
     // replace coordinate j through a shared-memory round trip of the thread's own row: a dynamically indexed
     // register array would be lowered to a branch tree over j, and the warp-collective tcgen05 instructions
     // below need every lane on the same path
-    float *own = reinterpret_cast<float *>(sm.A(0, 0)) + t * 68;
+    float *own = reinterpret_cast<float *>(sm.scratch()) + t * 68;
 #pragma unroll
     for (int c4 = 0; c4 < TC_D / 4; ++c4)
       *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   }
   float val = tc_eval_tile<OBJ>(o, sm, x, t);
   compute_sync();                        // every MMA has retired: the operand buffers are free
-  float *Us = reinterpret_cast<float *>(sm.A(0, 0));          // [256][65] normals (the A region is 128 KB)
+  float *Us = reinterpret_cast<float *>(sm.scratch());        // [256][65] normals (scratch is 72 KB)
   float *fvs = Us + TC_PTS * 65;                              // [256] values
   if (valid) {
     val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
