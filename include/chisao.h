@@ -87,7 +87,9 @@ typedef struct {
   int32_t reseed_strategy;  /* 0 none, 1 Repulse Monkey, 2 Golden Rooster, 3 uniform refill */
   int32_t gr_enabled;
   uint64_t evals[8];        /* objective evaluations: [0] cycle-start centre+FD, [1] line search,
-                               [2] L-BFGS FD gradients, [5] HLC, [6] anti-convergence (cumulative) */
+                               [2] L-BFGS FD gradients, [5] HLC, [6] anti-convergence (cumulative);
+                               [7] is not a count of evaluations: algorithmic HBM bytes moved by the L-BFGS
+                               two-loop kernel (history pairs, g, x read; p, x_t written), for the roofline */
   float f_max;
 } chisao_stats;
 
@@ -124,7 +126,9 @@ enum {
   CHISAO_PH_RESEED = 4,        /* Repulse Monkey / Golden Rooster / uniform refill  */
   CHISAO_PH_HLC_STEP = 5,      /* one Hands-Like-Clouds step `iter` (1-based)  */
   CHISAO_PH_ANTI_STEP = 6,     /* one momentum anti-convergence step `iter`  */
-  CHISAO_PH_LBFGS_ITER = 11    /* one L-BFGS iteration `iter` (1-based)    */
+  CHISAO_PH_LBFGS_ITER = 11,   /* one L-BFGS iteration `iter` (1-based)    */
+  CHISAO_PH_LBFGS_DIRECTION = 12 /* only the two-loop recursion + first trial point of an iteration (the HBM-bound
+                                  history kernel; used by bench.py to time it with a full history)          */
 };
 
 /* Bytes of device workspace chisao_init needs for (cfg, obj).  Host only; no CUDA call. */

@@ -19,6 +19,7 @@ OK, E_INVALID, E_WORKSPACE, E_CAPACITY, E_CUDA, E_STATE = 0, -1, -2, -3, -4, -5
 X, F, G, V, STUCK, REMOVED, HIST_S, HIST_Y, HIST_LEN, STALLED, CTRL = range(11)
 P, LS_B, GHAT, HLC_F, RS_SRC, RS_CAND, XT, GR_Q = 20, 21, 25, 26, 27, 28, 31, 32
 PH_RELEASE_EVAL, PH_STICK, PH_DEDUP, PH_RESEED, PH_HLC_STEP, PH_ANTI_STEP, PH_LBFGS_ITER = 1, 2, 3, 4, 5, 6, 11
+PH_LBFGS_DIRECTION = 12
 TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_update", "select", "reseed")
 
 EXPORTS = ("chisao_workspace_bytes", "chisao_init", "chisao_seed_population", "chisao_step", "chisao_step_host",
@@ -50,7 +51,7 @@ class Stats(C.Structure):
                 ("f_max", C.c_float)]
 
     def total_evals(self) -> int:
-        return int(sum(self.evals))
+        return int(sum(self.evals[k] for k in (0, 1, 2, 5, 6)))
 
 
 class ChisaoError(RuntimeError):

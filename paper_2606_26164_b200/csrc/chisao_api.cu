@@ -505,6 +505,13 @@ int chisao_phase(chisao_ctx *ctx, int32_t phase_id, int32_t iter) {
   switch (phase_id) {
     case CHISAO_PH_RELEASE_EVAL: return run_release_eval(ctx);
     case CHISAO_PH_LBFGS_ITER: return run_lbfgs_iter(ctx, iter);
+    case CHISAO_PH_LBFGS_DIRECTION: {
+      CK(cudaMemsetAsync(ctx->st.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
+      Scope sc(ctx, 3);
+      CK(launch_lbfgs_direction(ctx->st, ctx->hp, ctx->stream));
+      ctx->launches += 1;
+      return CHISAO_OK;
+    }
     case CHISAO_PH_STICK: return run_stick(ctx);
     case CHISAO_PH_DEDUP: return run_dedup(ctx);
     case CHISAO_PH_RESEED: return run_reseed(ctx);

@@ -44,102 +44,153 @@ __global__ void k_release(State s) {
   s.stuck[i] = 0; s.removed[i] = 0; s.stalled[i] = 0; s.hist_len[i] = 0; s.hist_head[i] = 0;
 }
 
+// ---- half-warp helpers: 16 lanes own one sample, lane hl holds coordinates 4 hl .. 4 hl + 3 ------------------
+struct Row4 { float a, b, c, e; };
+__device__ __forceinline__ Row4 ld_row4h(const float *row, int hl, int d, bool vec) {
+  Row4 r;
+  const int j = 4 * hl;
+  if (vec) {
+    if (j < d) { const float4 v = *reinterpret_cast<const float4 *>(row + j); r.a = v.x; r.b = v.y; r.c = v.z; r.e = v.w; }
+    else { r.a = r.b = r.c = r.e = 0.f; }
+  } else {
+    r.a = (j < d) ? row[j] : 0.f; r.b = (j + 1 < d) ? row[j + 1] : 0.f;
+    r.c = (j + 2 < d) ? row[j + 2] : 0.f; r.e = (j + 3 < d) ? row[j + 3] : 0.f;
+  }
+  return r;
+}
+__device__ __forceinline__ void st_row4h(float *row, int hl, int d, bool vec, Row4 r) {
+  const int j = 4 * hl;
+  if (vec) {
+    if (j < d) *reinterpret_cast<float4 *>(row + j) = make_float4(r.a, r.b, r.c, r.e);
+  } else {
+    if (j < d) row[j] = r.a;
+    if (j + 1 < d) row[j + 1] = r.b;
+    if (j + 2 < d) row[j + 2] = r.c;
+    if (j + 3 < d) row[j + 3] = r.e;
+  }
+}
+__device__ __forceinline__ float half_sum(float v) {   // sum over the 16 lanes of a half-warp (all 32 lanes call)
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float half_max(float v) {
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float dot4(Row4 u, Row4 v) {
+  return half_sum(fmaf(u.a, v.a, fmaf(u.b, v.b, fmaf(u.c, v.c, u.e * v.e))));
+}
+__device__ __forceinline__ void axpy4(Row4 &r, float c, Row4 v) {
+  r.a = fmaf(c, v.a, r.a); r.b = fmaf(c, v.b, r.b); r.c = fmaf(c, v.c, r.c); r.e = fmaf(c, v.e, r.e);
+}
+
 // One L-BFGS iteration, part 1: skip test, direction by the two-loop recursion (Nocedal & Wright Alg. 7.4;
 // refs [19,20] of PAPER.md:77) with H0 = (s.y / y.y) I of the newest pair, steepest restart when the
 // direction is not an ascent direction for f, first trial step and trial point (R-4).
-__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_lbfgs_direction(State s, Hyper h) {
+// A half-warp owns one sample (two samples per warp, float4 per lane: one 512-byte contiguous request per warp
+// and history plane); MM = compile-time bound on the history length, so the pair loops unroll over registers.
+// Every shuffle is executed by all 32 lanes: inactive samples run with len = 0 and predicated stores.
+constexpr int DIR_WARPS = 8;   // measured: 8 warps x 1 CTA per SM (2759 GB/s at C5, full history) beats 4 warps x 3 CTAs (2258 GB/s)
+template <int MM>
+__global__ void __launch_bounds__(DIR_WARPS * 32) k_lbfgs_direction(State s, Hyper h) {
   __shared__ int sh_cnt, sh_base;
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  const int i = blockIdx.x * WARPS_PER_BLOCK + wib;
+  __shared__ unsigned int sh_bytes;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, hl = lane & 15, half = lane >> 4;
+  const int i = (blockIdx.x * DIR_WARPS + wib) * 2 + half;
   const int d = s.d, m = s.m, N = s.N;
-  const bool even = (d & 1) == 0;
-  if (threadIdx.x == 0) sh_cnt = 0;
+  const bool vec = (d & 3) == 0;
+  if (threadIdx.x == 0) { sh_cnt = 0; sh_bytes = 0u; }
   if (blockIdx.x == 0 && threadIdx.x == 0) { s.ctrl->ls_cnt[1] = 0; s.ctrl->ls_cnt[2] = 0; s.ctrl->fd_cnt = 0; }
   __syncthreads();
-  bool search = false;
-  int my_slot = 0;
-  if (i < N) {
-    const size_t ro = (size_t)i * d;
-    const Row2 g = ld_row2(s.g + ro, lane, d, even);
-    const float ginf = warp_max(fmaxf(fabsf(g.a), fabsf(g.b)));
-    // (i) stationary (Eq. 3's gradient test) or stalled: no work, no evaluations (R-6)
-    const bool skip = s.stalled[i] || !(ginf >= h.eps_grad);
-    Row2 p; p.a = 0.f; p.b = 0.f;
-    if (skip) {
-      if (lane == 0) s.ls_b[i] = -2;
+  const bool in = i < N;
+  const size_t ro = (size_t)(in ? i : 0) * d;
+  Row4 g = ld_row4h(s.g + ro, hl, d, vec);
+  if (!in) { g.a = g.b = g.c = g.e = 0.f; }
+  const float ginf = half_max(fmaxf(fmaxf(fabsf(g.a), fabsf(g.b)), fmaxf(fabsf(g.c), fabsf(g.e))));
+  // (i) stationary (Eq. 3's gradient test) or stalled: no work, no evaluations (R-6)
+  const bool act = in && !(s.stalled[in ? i : 0] || !(ginf >= h.eps_grad));
+  int len = act ? s.hist_len[i] : 0;
+  const int len_read = len;
+  const int head = act ? s.hist_head[i] : 0;
+  const int lmax = max(len, __shfl_xor_sync(0xffffffffu, len, 16));     // warp-uniform loop bound
+  Row4 Sr[MM], Yr[MM];
+#pragma unroll
+  for (int l = 0; l < MM; ++l) {
+    if (l < len) {
+      int ph = head + l; if (ph >= m) ph -= m;
+      const size_t off = ((size_t)ph * N + i) * d;
+      Sr[l] = ld_row4h(s.S + off, hl, d, vec);
+      Yr[l] = ld_row4h(s.Y + off, hl, d, vec);
     } else {
-      int len = s.hist_len[i];
-      const int head = s.hist_head[i];
-      const Row2 x = ld_row2(s.x + ro, lane, d, even);
-      Row2 gam; gam.a = -g.a; gam.b = -g.b;
-      const float gn2 = dot2(g, g);
-      if (len > 0) {
-        Row2 Sr[CHISAO_MAX_M], Yr[CHISAO_MAX_M];
-#pragma unroll
-        for (int l = 0; l < CHISAO_MAX_M; ++l) {
-          if (l < len) {
-            int ph = head + l; if (ph >= m) ph -= m;
-            const size_t off = ((size_t)ph * N + i) * d;
-            Sr[l] = ld_row2(s.S + off, lane, d, even);
-            Yr[l] = ld_row2(s.Y + off, lane, d, even);
-          }
-        }
-        float rho[CHISAO_MAX_M], al[CHISAO_MAX_M];
-#pragma unroll
-        for (int l = 0; l < CHISAO_MAX_M; ++l)
-          if (l < len) rho[l] = 1.0f / dot2(Sr[l], Yr[l]);
-        Row2 r = gam;
-#pragma unroll
-        for (int l = CHISAO_MAX_M - 1; l >= 0; --l) {
-          if (l < len) {
-            al[l] = rho[l] * dot2(Sr[l], r);
-            r.a = fmaf(-al[l], Yr[l].a, r.a); r.b = fmaf(-al[l], Yr[l].b, r.b);
-          }
-        }
-        float sy = 0.f, yy = 1.f;
-#pragma unroll
-        for (int l = 0; l < CHISAO_MAX_M; ++l)
-          if (l == len - 1) { sy = dot2(Sr[l], Yr[l]); yy = dot2(Yr[l], Yr[l]); }
-        const float h0 = sy / yy;
-        r.a *= h0; r.b *= h0;
-#pragma unroll
-        for (int l = 0; l < CHISAO_MAX_M; ++l) {
-          if (l < len) {
-            const float beta = rho[l] * dot2(Yr[l], r);
-            const float c = al[l] - beta;
-            r.a = fmaf(Sr[l].a, c, r.a); r.b = fmaf(Sr[l].b, c, r.b);
-          }
-        }
-        p.a = -r.a; p.b = -r.b;
-        const float gp = dot2(gam, p);
-        if (!(gp < 0.0f)) {  // not a descent direction for phi = -f: steepest restart, clear history
-          p.a = -gam.a; p.b = -gam.b;
-          len = 0;
-          if (lane == 0) { s.hist_len[i] = 0; s.hist_head[i] = 0; }
-        }
-      } else {
-        p.a = -gam.a; p.b = -gam.b;
-      }
-      // (iii) first trial step; (iv) trial point projected on Theta, Armijo linear term gamma.(x_t - x)
-      const float t0 = (len > 0) ? 1.0f : fminf(1.0f, 1.0f / sqrtf(gn2));
-      const Row2 lo = ld_row2(s.lo, lane, d, even), hi = ld_row2(s.hi, lane, d, even);
-      Row2 xt;
-      xt.a = clipf(fmaf(t0, p.a, x.a), lo.a, hi.a);
-      xt.b = clipf(fmaf(t0, p.b, x.b), lo.b, hi.b);
-      Row2 dx; dx.a = xt.a - x.a; dx.b = xt.b - x.b;
-      const float dec = dot2(gam, dx);
-      st_row2(s.xt + ro, lane, d, even, xt);
-      if (lane == 0) { s.dec[i] = dec; s.tcur[i] = t0; s.ls_b[i] = -1; }
-      search = true;
+      Sr[l].a = Sr[l].b = Sr[l].c = Sr[l].e = 0.f; Yr[l] = Sr[l];
     }
-    st_row2(s.p + ro, lane, d, even, p);
+  }
+  const Row4 x = ld_row4h(s.x + ro, hl, d, vec);
+  Row4 gam; gam.a = -g.a; gam.b = -g.b; gam.c = -g.c; gam.e = -g.e;
+  const float gn2 = dot4(g, g);
+  float rho[MM], al[MM];
+#pragma unroll
+  for (int l = 0; l < MM; ++l) {
+    rho[l] = 0.0f; al[l] = 0.0f;
+    if (l < lmax) { const float sy = dot4(Sr[l], Yr[l]); rho[l] = (l < len) ? 1.0f / sy : 0.0f; }
+  }
+  Row4 r = gam;
+#pragma unroll
+  for (int l = MM - 1; l >= 0; --l)
+    if (l < lmax) { al[l] = rho[l] * dot4(Sr[l], r); axpy4(r, -al[l], Yr[l]); }   // zero rows / rho for l >= len
+  float sy_n = 0.f, yy_n = 1.f;
+#pragma unroll
+  for (int l = 0; l < MM; ++l) {
+    if (l < lmax) {
+      const float yy = dot4(Yr[l], Yr[l]);
+      if (l == len - 1) { yy_n = yy; sy_n = 1.0f / rho[l]; }
+    }
+  }
+  if (len > 0) { const float h0 = sy_n / yy_n; r.a *= h0; r.b *= h0; r.c *= h0; r.e *= h0; }
+#pragma unroll
+  for (int l = 0; l < MM; ++l)
+    if (l < lmax) { const float beta = rho[l] * dot4(Yr[l], r); axpy4(r, al[l] - beta, Sr[l]); }
+  Row4 p; p.a = -r.a; p.b = -r.b; p.c = -r.c; p.e = -r.e;
+  const float gp = dot4(gam, p);
+  bool restart = false;
+  if (len > 0 && !(gp < 0.0f)) { restart = true; len = 0; }   // not a descent direction for phi = -f: steepest restart
+  if (len_read == 0 || restart) { p.a = -gam.a; p.b = -gam.b; p.c = -gam.c; p.e = -gam.e; }
+  // (iii) first trial step; (iv) trial point projected on Theta, Armijo linear term gamma.(x_t - x)
+  const float t0 = (len > 0) ? 1.0f : fminf(1.0f, 1.0f / sqrtf(gn2));
+  const Row4 lo = ld_row4h(s.lo, hl, d, vec), hi = ld_row4h(s.hi, hl, d, vec);
+  Row4 xt;
+  xt.a = clipf(fmaf(t0, p.a, x.a), lo.a, hi.a); xt.b = clipf(fmaf(t0, p.b, x.b), lo.b, hi.b);
+  xt.c = clipf(fmaf(t0, p.c, x.c), lo.c, hi.c); xt.e = clipf(fmaf(t0, p.e, x.e), lo.e, hi.e);
+  Row4 dx; dx.a = xt.a - x.a; dx.b = xt.b - x.b; dx.c = xt.c - x.c; dx.e = xt.e - x.e;
+  const float dec = dot4(gam, dx);
+  unsigned int my_bytes = 0u;   // algorithmic HBM bytes of this sample (rows read and written)
+  if (in) {
+    my_bytes = 2u * d * 4u;                               // g read, p written
+    if (act) {
+      st_row4h(s.xt + ro, hl, d, vec, xt);
+      st_row4h(s.p + ro, hl, d, vec, p);
+      if (hl == 0) {
+        s.dec[i] = dec; s.tcur[i] = t0; s.ls_b[i] = -1;
+        if (restart) { s.hist_len[i] = 0; s.hist_head[i] = 0; }
+      }
+      my_bytes += (2u * (unsigned)len_read * d + 2u * d) * 4u;   // history pairs + x read, x_t written
+    } else {
+      Row4 z; z.a = z.b = z.c = z.e = 0.f;
+      st_row4h(s.p + ro, hl, d, vec, z);
+      if (hl == 0) s.ls_b[i] = -2;
+    }
   }
   // block-aggregated append of the searching samples to line-search worklist 0
-  if (search && lane == 0) my_slot = atomicAdd(&sh_cnt, 1);
+  int my_slot = 0;
+  if (act && hl == 0) my_slot = atomicAdd(&sh_cnt, 1);
+  if (hl == 0 && my_bytes) atomicAdd(&sh_bytes, my_bytes);
   __syncthreads();
   if (threadIdx.x == 0 && sh_cnt > 0) sh_base = atomicAdd(&s.ctrl->ls_cnt[0], sh_cnt);
+  if (threadIdx.x == 0 && sh_bytes) atomicAdd(&s.ctrl->evals[7], (unsigned long long)sh_bytes);
   __syncthreads();
-  if (search && lane == 0) s.ls_list[0][sh_base + my_slot] = i;
+  if (act && hl == 0) s.ls_list[0][sh_base + my_slot] = i;
 }
 
 // One L-BFGS iteration, part 3 (after the FD gradient gn at the accepted trial point): curvature pair
@@ -191,7 +242,11 @@ cudaError_t launch_release(const State &s, cudaStream_t st) {
 }
 cudaError_t launch_lbfgs_direction(const State &s, const Hyper &h, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
-  k_lbfgs_direction<<<(s.N + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK, WARPS_PER_BLOCK * 32, 0, st>>>(s, h);
+  const int per_block = DIR_WARPS * 2, grid = (s.N + per_block - 1) / per_block;
+  if (s.m <= 4) k_lbfgs_direction<4><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+  else if (s.m <= 8) k_lbfgs_direction<8><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+  else if (s.m <= 10) k_lbfgs_direction<10><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+  else k_lbfgs_direction<16><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
   return cudaGetLastError();
 }
 cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, cudaStream_t st) {

@@ -46,8 +46,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
 #pragma unroll
     for (int c4 = 0; c4 < TC_D / 4; ++c4)
       *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
-    own[j] = xp;
-    __syncwarp();
+    own[j] = xp;                         // same thread writes and reads its row: program order suffices
 #pragma unroll
     for (int c4 = 0; c4 < TC_D / 4; ++c4) {
       const float4 v = *reinterpret_cast<const float4 *>(own + 4 * c4);

@@ -243,3 +243,34 @@ def test_step_host_matches_device_resident_step(B):
     assert np.array_equal(x_out, a.get(B.X)) and np.array_equal(f_out, a.get(B.F)) and np.array_equal(s_out, a.get(B.STUCK))
     assert (sa.n_stuck, sa.k_lost, sa.n_active) == (sb.n_stuck, sb.k_lost, sb.n_active)
     assert list(sa.evals) == list(sb.evals)
+
+
+@pytest.mark.parametrize("obj_id,d,K,N", [(2, 40, 3, 300), (2, 64, 1, 130), (2, 33, 2, 257), (4, 50, 1, 260), (2, 64, 5, 513)])
+def test_tensor_core_evaluator_shapes(orc, B, obj_id, d, K, N):
+    """dense objectives at 32 < d <= 64 run on the tcgen05 evaluator (256-point tiles, two groups): d not a
+    multiple of 4 or 8 (zero-padded to 64), one / odd numbers of components, ragged last tile; f, g, one L-BFGS
+    iteration, one HLC and one anti-convergence step against the oracle."""
+    obj = inputs.gmm_full(d, K, 3.0, 70 + d + K) if obj_id == 2 else inputs.quad(d, 71 + d, lam_max=50.0)
+    wl = inputs.custom(obj, 4.0, N, seed=123 + d, hlc_M=12, n_conv=3, fd_h=5e-2, eps_grad=1e-3, n_osc=2, hlc_baseline=1,
+                       sigma_s=0.5, eta_hlc=1e-3, alpha_anti=1e-3)
+    o, g = orc.Oracle(wl, threads=8), B.Chisao(wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0]); g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL); g.phase(B.PH_RELEASE_EVAL)
+    fo, fg = o.get(orc.F), g.get(B.F).astype(np.float64)
+    assert np.all(np.abs(fg - fo) <= PT.f_tol(fo)), float(np.max(np.abs(fg - fo) / np.maximum(np.abs(fo), 1)))
+    ok, err, tol = PT.grad_ok(g.get(B.G).astype(np.float64), o.get(orc.G), fo, wl.hp.fd_h)
+    assert np.all(ok), float(np.max(err / tol))
+    PT.sync_oracle_to_gpu(o, g, orc, B)
+    o.phase(orc.PH_LBFGS_ITER, 1); g.phase(B.PH_LBFGS_ITER, 1)
+    safe = (o.get(orc.LS_MARGIN) > PT.LS_MARGIN_MIN)
+    assert np.array_equal(g.get(B.LS_B)[safe], o.get(orc.LS_B)[safe])
+    xo = o.get(orc.X)
+    assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1)[safe] <= PT.x_tol(xo, wl.hp.lo, wl.hp.hi)[safe])
+    PT.sync_oracle_to_gpu(o, g, orc, B)
+    o.phase(orc.PH_HLC_STEP, 1); g.phase(B.PH_HLC_STEP, 1)
+    ho = o.get(orc.HLC_F)
+    assert np.all(np.abs(g.get(B.HLC_F) - ho) <= PT.F_REL * np.maximum(np.abs(ho), 1.0))
+    PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+    o.phase(orc.PH_ANTI_STEP, 1); g.phase(B.PH_ANTI_STEP, 1)
+    xo = o.get(orc.X)
+    assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1) <= 10 * PT.x_tol(xo, wl.hp.lo, wl.hp.hi))
