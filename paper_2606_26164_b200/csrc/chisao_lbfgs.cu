@@ -93,14 +93,14 @@ __device__ __forceinline__ void axpy4(Row4 &r, float c, Row4 v) {
 // and history plane); MM = compile-time bound on the history length, so the pair loops unroll over registers.
 // Every shuffle is executed by all 32 lanes: inactive samples run with len = 0 and predicated stores.
 constexpr int DIR_WARPS = 8;   // measured: 8 warps x 1 CTA per SM (2759 GB/s at C5, full history) beats 4 warps x 3 CTAs (2258 GB/s)
-template <int MM>
-__global__ void __launch_bounds__(DIR_WARPS * 32) k_lbfgs_direction(State s, Hyper h) {
+template <int MM, bool VEC>
+__global__ void __launch_bounds__(DIR_WARPS * 32, 2) k_lbfgs_direction(State s, Hyper h) {
   __shared__ int sh_cnt, sh_base;
   __shared__ unsigned int sh_bytes;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, hl = lane & 15, half = lane >> 4;
   const int i = (blockIdx.x * DIR_WARPS + wib) * 2 + half;
   const int d = s.d, m = s.m, N = s.N;
-  const bool vec = (d & 3) == 0;
+  constexpr bool vec = VEC;
   if (threadIdx.x == 0) { sh_cnt = 0; sh_bytes = 0u; }
   if (blockIdx.x == 0 && threadIdx.x == 0) { s.ctrl->ls_cnt[1] = 0; s.ctrl->ls_cnt[2] = 0; s.ctrl->fd_cnt = 0; }
   __syncthreads();
@@ -114,7 +114,6 @@ __global__ void __launch_bounds__(DIR_WARPS * 32) k_lbfgs_direction(State s, Hyp
   int len = act ? s.hist_len[i] : 0;
   const int len_read = len;
   const int head = act ? s.hist_head[i] : 0;
-  const int lmax = max(len, __shfl_xor_sync(0xffffffffu, len, 16));     // warp-uniform loop bound
   Row4 Sr[MM], Yr[MM];
 #pragma unroll
   for (int l = 0; l < MM; ++l) {
@@ -130,28 +129,28 @@ __global__ void __launch_bounds__(DIR_WARPS * 32) k_lbfgs_direction(State s, Hyp
   const Row4 x = ld_row4h(s.x + ro, hl, d, vec);
   Row4 gam; gam.a = -g.a; gam.b = -g.b; gam.c = -g.c; gam.e = -g.e;
   const float gn2 = dot4(g, g);
+  // straight-line code over all MM slots: rows beyond len are zero and rho = 0 there, so they contribute nothing,
+  // and no shuffle sits under a branch (the compiler would otherwise wrap each one in a convergence region)
   float rho[MM], al[MM];
 #pragma unroll
-  for (int l = 0; l < MM; ++l) {
-    rho[l] = 0.0f; al[l] = 0.0f;
-    if (l < lmax) { const float sy = dot4(Sr[l], Yr[l]); rho[l] = (l < len) ? 1.0f / sy : 0.0f; }
-  }
+  for (int l = 0; l < MM; ++l) { const float sy = dot4(Sr[l], Yr[l]); rho[l] = (l < len) ? 1.0f / sy : 0.0f; }
   Row4 r = gam;
 #pragma unroll
-  for (int l = MM - 1; l >= 0; --l)
-    if (l < lmax) { al[l] = rho[l] * dot4(Sr[l], r); axpy4(r, -al[l], Yr[l]); }   // zero rows / rho for l >= len
-  float sy_n = 0.f, yy_n = 1.f;
-#pragma unroll
-  for (int l = 0; l < MM; ++l) {
-    if (l < lmax) {
-      const float yy = dot4(Yr[l], Yr[l]);
-      if (l == len - 1) { yy_n = yy; sy_n = 1.0f / rho[l]; }
-    }
+  for (int l = MM - 1; l >= 0; --l) { al[l] = rho[l] * dot4(Sr[l], r); axpy4(r, -al[l], Yr[l]); }
+  // newest pair (logical len - 1): its y row is re-read (an L1/L2 hit) rather than selected out of the register
+  // array, which would turn the array into local memory; s.y of that pair = 1 / rho
+  Row4 Yn; Yn.a = Yn.b = Yn.c = Yn.e = 0.f;
+  float rho_n = 1.0f;
+  if (len > 0) {
+    int ph = head + len - 1; if (ph >= m) ph -= m;
+    Yn = ld_row4h(s.Y + ((size_t)ph * N + i) * d, hl, d, vec);
   }
-  if (len > 0) { const float h0 = sy_n / yy_n; r.a *= h0; r.b *= h0; r.c *= h0; r.e *= h0; }
 #pragma unroll
-  for (int l = 0; l < MM; ++l)
-    if (l < lmax) { const float beta = rho[l] * dot4(Yr[l], r); axpy4(r, al[l] - beta, Sr[l]); }
+  for (int l = 0; l < MM; ++l) rho_n = (l == len - 1) ? rho[l] : rho_n;
+  if (len > 0) { const float h0 = 1.0f / (rho_n * dot4(Yn, Yn)); r.a *= h0; r.b *= h0; r.c *= h0; r.e *= h0; }
+  else { (void)dot4(Yn, Yn); }
+#pragma unroll
+  for (int l = 0; l < MM; ++l) { const float beta = rho[l] * dot4(Yr[l], r); axpy4(r, al[l] - beta, Sr[l]); }
   Row4 p; p.a = -r.a; p.b = -r.b; p.c = -r.c; p.e = -r.e;
   const float gp = dot4(gam, p);
   bool restart = false;
@@ -243,10 +242,17 @@ cudaError_t launch_release(const State &s, cudaStream_t st) {
 cudaError_t launch_lbfgs_direction(const State &s, const Hyper &h, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
   const int per_block = DIR_WARPS * 2, grid = (s.N + per_block - 1) / per_block;
-  if (s.m <= 4) k_lbfgs_direction<4><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
-  else if (s.m <= 8) k_lbfgs_direction<8><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
-  else if (s.m <= 10) k_lbfgs_direction<10><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
-  else k_lbfgs_direction<16><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+  const bool vec = (s.d & 3) == 0;
+#define CHISAO_DIR(MM)                                                                         \
+  do {                                                                                         \
+    if (vec) k_lbfgs_direction<MM, true><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);               \
+    else k_lbfgs_direction<MM, false><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);                  \
+  } while (0)
+  if (s.m <= 4) CHISAO_DIR(4);
+  else if (s.m <= 8) CHISAO_DIR(8);
+  else if (s.m <= 10) CHISAO_DIR(10);
+  else CHISAO_DIR(16);
+#undef CHISAO_DIR
   return cudaGetLastError();
 }
 cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, cudaStream_t st) {
