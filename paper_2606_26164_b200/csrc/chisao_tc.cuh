@@ -28,7 +28,7 @@ constexpr int TC_REC_BYTES = TC_REC * 4;                 // 33 040 (multiple of 
 constexpr int TC_A_BYTES = TC_GROUP * TC_D * 4;          // 32 768 per operand image
 constexpr int TC_SCRATCH_BYTES = 72 * 1024;               // kernel scratch (FD row patch, HLC normals)
 constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TC_REC_BYTES;   // barriers | scratch | B x2
-constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D 64 | D_hi 64 | D_lo 64
+constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D0 64 | D_hi 64 | D_lo 64 | D1 64
 
 struct TcObj {
   int32_t K, d;
@@ -148,12 +148,43 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
   float m = -INFINITY, s = 0.0f;
   const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
   const uint32_t dcol = tm + (uint32_t)(g * 256), acol_hi = dcol + 64, acol_lo = dcol + 128;
-  const uint32_t taddr = lane_base;
+  float a_prev = 0.0f;
+  // accumulator stage j & 1 of this group -> sum of squares -> online log-sum-exp
+  auto drain = [&](int j, float a_j) {
+    const uint32_t taddr = lane_base + (uint32_t)((j & 1) * 192);
+    uint32_t r[64];
+    tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll
+    for (int n = 0; n < 64; n += 4) {
+      const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
+                  z3 = __uint_as_float(r[n + 3]);
+      q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+    }
+    const float q = (q0 + q1) + (q2 + q3);
+    if constexpr (OBJ == CHISAO_OBJ_QUAD) {
+      s += q;
+    } else {
+      const float v = fmaf(-0.5f, q, a_j);
+      const float mn = fmaxf(m, v);
+      if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
+  };
+  // MMAs of component j have retired: the operand image and B stage j & 1 are free, accumulator stage j & 1 is ready
+  auto retire = [&](int j) {
+    mbar_wait(sm.mbar(g), j & 1);
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (tl == 0) mbar_arrive(sm.fbar(j & 1));
+    __syncwarp();
+  };
   for (int k = 0; k < K; ++k) {
     const int st = k & 1;
     mbar_wait(sm.bbar(st), (k >> 1) & 1);             // W_k hi/lo, mu_k, a_k have landed
     const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(st) + 2 * TC_D * TC_D);
     const float a_k = sm.B(st)[2 * TC_D * TC_D + TC_D];
+    if (k > 0) retire(k - 1);
     // this thread's row of D_hi / D_lo goes straight into its TMEM lane (A operand read from TMEM: the MMA then
     // fetches only W from shared memory)
 #pragma unroll
@@ -183,35 +214,16 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
         const uint64_t b0 = (pr == 2) ? dBl : dBh;
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks)
-          tc_mma_ts(dcol, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
+          tc_mma_ts(dcol + (uint32_t)((k & 1) * 192), a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
       }
       tc_commit(sm.mbar(g));
     }
     __syncwarp();
-    mbar_wait(sm.mbar(g), k & 1);                     // this group's MMAs of component k have retired
-    asm volatile("tcgen05.fence::after_thread_sync;");
-    if (tl == 0) mbar_arrive(sm.fbar(st));            // B stage st is no longer needed by this group
-    __syncwarp();
-    uint32_t r[64];
-    tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
-#pragma unroll
-    for (int n = 0; n < 64; n += 4) {
-      const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
-                  z3 = __uint_as_float(r[n + 3]);
-      q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
-    }
-    const float q = (q0 + q1) + (q2 + q3);
-    if constexpr (OBJ == CHISAO_OBJ_QUAD) {
-      s += q;
-    } else {
-      const float v = fmaf(-0.5f, q, a_k);
-      const float mn = fmaxf(m, v);
-      if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
+    if (k > 0) drain(k - 1, a_prev);                  // overlaps the MMAs of component k (two accumulator stages)
+    a_prev = a_k;
   }
+  retire(K - 1);
+  drain(K - 1, a_prev);
   if constexpr (OBJ == CHISAO_OBJ_QUAD) return -0.5f * s;
   return m + logf(s);
 }
