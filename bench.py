@@ -92,8 +92,8 @@ def oracle_throughput(c: int, steps: int, warmup: int, rank_seed: int = 0):
     from paper_2606_26164_b200 import inputs
     cores = len(os.sched_getaffinity(0))
     full = inputs.config(c)
-    # ~1.7 GFLOP per sample-cycle at C5: a few samples per core keep one step in the 5-15 s range
-    per_core = {1: 256, 2: 64, 3: 6, 4: 8, 5: 1}[c]
+    # ~1.5 s of one core per sample-cycle at C5: 8 samples per core keep one step in the 10-20 s range
+    per_core = {1: 256, 2: 256, 3: 24, 4: 32, 5: 8}[c]
     Ns = min(full.hp.N, max(8, per_core * cores))
     wl = inputs.config(c, N=Ns, n_osc=max(full.hp.n_osc, steps + warmup + 1))
     o = O.Oracle(wl, threads=cores)
