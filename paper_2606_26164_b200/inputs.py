@@ -231,6 +231,25 @@ def config(c: int, N: Optional[int] = None, n_osc: Optional[int] = None, noise: 
     return Workload(f"C{c}", obj, hp, x0)
 
 
+def noise_robustness(sigma_noise: float, trial: int = 0, N: int = 200) -> Workload:
+    """The noise-robustness workload of PAPER.md:523-541 (sec. 5.7, Table 8): 2-mode isotropic Gaussian mixture in
+    d = 6, peaks at +-2 e_1, sigma = 1 (mode separation 4 sigma), Theta = [-10, 10]^6, N = 200 and the
+    defaults of Table 1 (n_osc = 3, n_conv = 10, n_anti = 5, n_cloud = 3, K = 10, m = 10).  The paper does not state
+    the FD step or the thresholds it used under noise; they follow the FD noise floor sigma_noise / (sqrt(2) h) with
+    h = sigma = 1 (DESIGN.md "NEXT-1")."""
+    d = 6
+    means = np.zeros((2, d))
+    means[0, 0], means[1, 0] = 2.0, -2.0
+    obj = gmm_iso(d, 2, 1.0, 10.0, 1, means=means, sigma_noise=sigma_noise)
+    h = 1.0
+    lo, hi = _box(d, 10.0)
+    hp = Hyper(d, N, lo, hi, n_osc=3, n_conv=10, n_anti=5, n_cloud=3, hlc_M=10, lbfgs_m=10, fd_h=h,
+               eps_grad=max(4.0 * sigma_noise / (math.sqrt(2.0) * h), 1e-2), eps_dup=min(3.0, 0.2 + 6.0 * sigma_noise),
+               log_delta=math.log(0.1) - 4.0 * sigma_noise, alpha_anti=0.05, eta_hlc=0.05, sigma_s=1.0, hlc_baseline=1)
+    hp.seed = 500 + trial
+    return Workload(f"noise{sigma_noise:g}", obj, hp, uniform_population(N, lo, hi, 501 + trial))
+
+
 def custom(obj: Objective, box: float, N: int, seed: int = 7, **over) -> Workload:
     """A free-form workload on [-box, box]^d (used by pins and edge-case tests)."""
     lo, hi = _box(obj.d, box)
