@@ -525,10 +525,42 @@ static void phase_reseed(orc_ctx *s) {
  * (Eq. 9): ghat = (1/(M sigma)) sum_k f(x + sigma u_k) u_k, u_k ~ N(0, I) (R-11).
  * hlc_baseline = 1 subtracts the mean of the M values (control variate, same expectation).
  * ---------------------------------------------------------------------------------------------- */
+/* The paper's own form, Eq. 5: theta <- theta + eta (1/K) sum_k grad f(theta + sigma z_k),
+ * z_k ~ N(0, I), with finite-difference gradients: K 2d evaluations per step.  The draws z_k are
+ * the same Philox normals as in the zeroth-order form; evaluation (k, +-h e_j) uses noise slot k 2d + 1 + 2j /
+ * k 2d + 2 + 2j of (phase 5, step t).  Selected by hlc_baseline == 2 (DESIGN.md NEXT-2). */
+static void hlc_sample_eq5(orc_ctx *s, int i, int t) {
+  const int d = s->c.d, M = s->c.hlc_M;
+  const double sig = (double)s->c.sigma_s, eta = (double)s->c.eta_hlc, h = (double)s->c.fd_h;
+  double *gh = s->ghat + (size_t)i * d;
+  for (int j = 0; j < d; ++j) gh[j] = 0.0;
+  if (s->stuck[i] || s->removed[i]) return;            /* "Stuck samples are excluded" PAPER.md:120 */
+  double *x = s->x + (size_t)i * d;
+  double *pt = (double *)alloca(sizeof(double) * d), *xp = (double *)alloca(sizeof(double) * d);
+  for (int k = 0; k < M; ++k) {
+    for (int j = 0; j < d; ++j) {
+      double u = orc_normal(s->c.seed, (uint32_t)i, (uint32_t)s->cycle, tag(5, t, PUR_HLC_U), (uint64_t)k * d + j);
+      pt[j] = (double)(float)(x[j] + sig * u);          /* the perturbed point is an fp32 position like any other */
+    }
+    for (int j = 0; j < d; ++j) {
+      memcpy(xp, pt, sizeof(double) * d);
+      xp[j] = pt[j] + h;
+      double fp = objective(s, xp) + orc_noise(s, s->cycle, i, 5, t, k * 2 * d + 1 + 2 * j);
+      xp[j] = pt[j] - h;
+      double fm = objective(s, xp) + orc_noise(s, s->cycle, i, 5, t, k * 2 * d + 2 + 2 * j);
+      gh[j] += (fp - fm) / (2.0 * h) / M;
+    }
+  }
+#pragma omp atomic
+  s->evals[EV_HLC] += (uint64_t)M * 2 * d;
+  for (int j = 0; j < d; ++j) x[j] = clipf32(x[j] + eta * gh[j], s->lo[j], s->hi[j]);
+}
+
 static void hlc_sample(orc_ctx *s, int i, int t) {
   const int d = s->c.d, M = s->c.hlc_M;
   const double sig = (double)s->c.sigma_s, eta = (double)s->c.eta_hlc;
   double *gh = s->ghat + (size_t)i * d;
+  if (s->c.hlc_baseline == 2) { hlc_sample_eq5(s, i, t); return; }
   for (int j = 0; j < d; ++j) gh[j] = 0.0;
   if (s->stuck[i] || s->removed[i]) return;            /* "Stuck samples are excluded" PAPER.md:120 */
   double *x = s->x + (size_t)i * d;

@@ -465,3 +465,28 @@ def test_modes_equal_brute_force_grid_enumeration_d2(orc):
     assert len(xm) == len(truth_modes) == 4
     for m in truth_modes:
         assert np.min(np.linalg.norm(xm - m[None], axis=1)) < 1e-3
+
+
+def test_hlc_eq5_form_on_a_quadratic_is_the_gradient_at_the_mean_perturbed_point(orc):
+    """Paper form of Hands Like Clouds, Eq. 5: (1/K) sum_k grad f(x + sigma z_k).  On a quadratic the
+    gradient is affine and central differences are exact, so the average equals the analytic gradient at the mean
+    perturbed point -A (mean_k(x + sigma z_k) - c); the step and the evaluation count K 2d follow (Eq. 8)."""
+    obj = inputs.quad(5, 21, lam_max=30.0)
+    wl = inputs.custom(obj, 4.0, 12, hlc_M=7, sigma_s=0.3, eta_hlc=1e-3, fd_h=1e-2, hlc_baseline=2, seed=99)
+    o = orc.Oracle(wl)
+    o.set(orc.CTRL, [2, 1, 0, 0, 0, 0, 0, 0])
+    x0 = o.get(orc.X).copy()
+    stuck = np.zeros(12, np.uint8); stuck[3] = 1
+    o.set(orc.STUCK, stuck)
+    o.phase(orc.PH_HLC_STEP, 1)
+    A, c = obj.truth["A"], obj.truth["c"]
+    tag = orc.tag(5, 1, 2)
+    for i in (0, 5, 11):
+        z = np.array([[orc.normal(99, i, 2, tag, k * 5 + j) for j in range(5)] for k in range(7)])
+        pts = (x0[i][None, :] + float(np.float32(0.3)) * z).astype(np.float32).astype(np.float64)
+        expect = -(A @ (pts.mean(axis=0) - c))
+        gh = o.get(orc.GHAT)[i]
+        assert np.allclose(gh, expect, rtol=1e-7, atol=1e-7)
+        assert np.allclose(o.get(orc.X)[i], np.clip(x0[i] + float(np.float32(1e-3)) * gh, -4, 4).astype(np.float32), atol=1e-7)
+    assert np.array_equal(o.get(orc.X)[3], x0[3]) and not o.get(orc.GHAT)[3].any()
+    assert o.stats().evals[5] == 11 * 7 * 2 * 5
