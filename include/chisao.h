@@ -77,7 +77,8 @@ typedef struct {
   float mu, alpha_anti;     /* Eq. 6 momentum and step */
   float eta_hlc, sigma_s;   /* HLC step size and smoothing scale */
   float ls_c1, ls_shrink;   /* Armijo constant and backtracking factor (R-4) */
-  int32_t hlc_baseline;     /* 0: literal estimator; 1: subtract the mean of the M values (R-11) */
+  int32_t hlc_baseline;     /* 0: literal estimator; 1: subtract the mean of the M values (R-11);
+                               2: the paper's Eq. 5 form, mean of M FD gradients at perturbed points */
   uint32_t phase_mask;      /* bit p (p = 3..6) enables phase p; 0xFFFFFFFF = full algorithm */
   uint64_t seed;            /* Philox key (R-15) */
 } chisao_config;

@@ -221,12 +221,12 @@ struct Scope {   // optional CUDA-event bracket around a launch group
 };
 
 cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const int32_t *count, int mode, float *g_out,
-                    int phase, int iter, int counter) {
+                    int phase, int iter, int counter, int slot_off = 0) {
   const State &s = c->st;
   if (s.N == 0) return cudaSuccess;
   FdArgs a{};
   a.X = X; a.list = list; a.count = count; a.max_count = s.N; a.mode = mode; a.d = s.d; a.cycle = c->cycle;
-  a.phase = phase; a.iter = iter; a.counter = counter; a.g_out = g_out; a.x = s.x; a.v = s.v; a.lo = s.lo; a.hi = s.hi;
+  a.phase = phase; a.iter = iter; a.counter = counter; a.slot_off = slot_off; a.g_out = g_out; a.x = s.x; a.v = s.v; a.lo = s.lo; a.hi = s.hi;
   a.h = c->hp.fd_h; a.mu = c->hp.mu; a.alpha = c->hp.alpha_anti; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
   const int spt = NT / s.d;
   const int grid = (s.N + spt - 1) / spt;
@@ -341,6 +341,16 @@ int run_explore_list(chisao_ctx *ctx) {
 }
 int run_hlc(chisao_ctx *ctx, int t) {
   if (!(ctx->hp.phase_mask & (1u << 5))) return CHISAO_OK;
+  if (ctx->hp.hlc_baseline == 2) {   // the paper's Eq. 5 form: K FD gradients at perturbed points (NEXT-2)
+    const State &s = ctx->st;
+    for (int k = 0; k < ctx->hp.hlc_M; ++k) {
+      { Scope sc(ctx, 2); CK(launch_hlc5(s, ctx->hp, ctx->cycle, t, k, 0, ctx->stream)); ctx->launches += 1; }
+      CK(eval_fd(ctx, s.xt, s.listE, &s.ctrl->nE, FD_GRAD, s.gn, 5, t, EV_HLC, k * 2 * s.d));
+      { Scope sc(ctx, 2); CK(launch_hlc5(s, ctx->hp, ctx->cycle, t, k, 1, ctx->stream)); ctx->launches += 1; }
+    }
+    { Scope sc(ctx, 2); CK(launch_hlc5(s, ctx->hp, ctx->cycle, t, 0, 2, ctx->stream)); ctx->launches += 1; }
+    return CHISAO_OK;
+  }
   CK(hlc_step(ctx, t));
   return CHISAO_OK;
 }

@@ -104,6 +104,8 @@ cudaError_t launch_stick(const State &s, const Hyper &h, cudaStream_t st);      
 cudaError_t launch_dedup(const State &s, const Hyper &h, cudaStream_t st);          // removed + lists + GR state
 cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_t st);
 cudaError_t launch_explore_list(const State &s, cudaStream_t st);
+// paper-form HLC (Eq. 5) helpers: stage 0 perturb (xt = x + sigma z_k), 1 accumulate (ghat += gn / M), 2 apply
+cudaError_t launch_hlc5(const State &s, const Hyper &h, int cycle, int iter, int k, int stage, cudaStream_t st);
 cudaError_t launch_seed_population(const State &s, const Hyper &h, cudaStream_t st);
 cudaError_t launch_gather_rows(const float *x, const int32_t *idx, int n, int d, float *out, cudaStream_t st);
 

@@ -21,6 +21,7 @@ struct FdArgs {
   const int32_t *list;       // sample ids (NULL = identity)
   const int32_t *count;      // device count (NULL = max_count)
   int32_t max_count, mode, d, cycle, phase, iter, counter;
+  int32_t slot_off;          // added to the noise slot (paper-form HLC: draw k uses slots k 2d + 1 ..)
   float *g_out;              // FD_GRAD: [N][d]
   float *x, *v;              // FD_ANTI: updated in place
   const float *lo, *hi;
@@ -70,8 +71,8 @@ __global__ void __launch_bounds__(NT, 2) k_eval_fd(const DevObj o, const FdArgs 
   float fv[PPT];
   eval_tile<OBJ, DP>(o, sm, t, use, fv);
   if (valid) {
-    const float fp = fv[0] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, 1 + 2 * j);
-    const float fm = fv[1] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, 2 + 2 * j);
+    const float fp = fv[0] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, a.slot_off + 1 + 2 * j);
+    const float fm = fv[1] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, a.slot_off + 2 + 2 * j);
     const float g = (fp - fm) / ((xph - xj) + (xj - xmh));
     if (a.mode == FD_GRAD) {
       a.g_out[(size_t)i * d + j] = g;

@@ -391,6 +391,33 @@ cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_
   return cudaGetLastError();
 }
 
+// ---- Hands Like Clouds, the paper's own form, Eq. 5 (DESIGN.md NEXT-2) -----------------------
+// theta <- theta + eta (1/K) sum_k grad f(theta + sigma z_k) with FD gradients: per draw k the host runs
+// [perturb: xt = x + sigma z_k] -> k_eval_fd on xt (noise slots k 2d + ..) -> [accumulate: ghat += gn / K], then
+// [apply].  One thread per (explore-list entry, coordinate).
+__global__ void k_hlc5(State s, Hyper h, int cycle, int iter, int k, int stage) {
+  const int nE = s.ctrl->nE, d = s.d;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= (size_t)nE * d) return;
+  const int q = (int)(e / d), j = (int)(e - (size_t)q * d);
+  const int i = s.listE[q];
+  const size_t o = (size_t)i * d + j;
+  if (stage == 0) {
+    const float u = rng_normal(h.seed, (uint32_t)i, (uint32_t)cycle, rng_tag(5, iter, PUR_HLC_U), (uint32_t)(k * d + j));
+    s.xt[o] = fmaf(h.sigma_s, u, s.x[o]);                 // evaluation points are not clipped (R-12)
+  } else if (stage == 1) {
+    s.ghat[o] = (k == 0 ? 0.0f : s.ghat[o]) + s.gn[o] / (float)h.hlc_M;
+  } else {
+    s.x[o] = clipf(fmaf(h.eta_hlc, s.ghat[o], s.x[o]), s.lo[j], s.hi[j]);
+  }
+}
+cudaError_t launch_hlc5(const State &s, const Hyper &h, int cycle, int iter, int k, int stage, cudaStream_t st) {
+  const size_t n = (size_t)s.N * s.d;
+  if (n == 0) return cudaSuccess;
+  k_hlc5<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s, h, cycle, iter, k, stage);
+  return cudaGetLastError();
+}
+
 // ---- initial population: i.i.d. uniform in Theta (Prop. 2; R-15 purpose INIT, cycle 0) -------
 __global__ void k_seed_population(State s, Hyper h) {
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;

@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
   }
   compute_sync();                        // the scratch rows overlap the operand buffers: everyone has read back
   float f = tc_eval_tile<OBJ>(o, sm, x, t);
-  if (valid) f += eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, 1 + slot);
+  if (valid) f += eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, a.slot_off + 1 + slot);
   // partner lane holds the other sign of the same coordinate
   const float fo = __shfl_xor_sync(0xffffffffu, f, 1);
   const float xo = __shfl_xor_sync(0xffffffffu, xp, 1);

@@ -281,3 +281,30 @@ def test_a7_anti_convergence_step(orc, B, c, N):
         assert np.all(np.max(np.abs(xg - xo), axis=1)[act] <= xt[act])
         assert np.array_equal(xg[~act], x0[~act])              # "Stuck samples are excluded" PAPER.md:129
     assert g.stats().evals[6] == 3 * int(act.sum()) * 2 * hp.d
+
+
+@pytest.mark.parametrize("c,N,M", [(2, 300, 6), (3, 130, 3), (5, 70, 3), (1, 256, 10)])
+def test_a6_hlc_step_paper_form_eq5(orc, B, c, N, M):
+    """NEXT-2: Hands Like Clouds as the paper writes it (Eq. 5): mean of M finite-difference gradients
+    at Gaussian-perturbed points (hlc_baseline = 2): ghat within 1e-3 relative + FD floor, x by rule 4, stuck rows
+    frozen, M 2d evaluations per active sample."""
+    wl = inputs.config(c, N=N, hlc_baseline=2, hlc_M=M)
+    hp = wl.hp
+    o, g = _converged_pair(orc, B, wl, 2)
+    o.phase(orc.PH_STICK)
+    stuck = o.get(orc.STUCK).copy(); stuck[::6] = 1
+    o.set(orc.STUCK, stuck)
+    act = stuck == 0
+    PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+    x0 = o.get(orc.X).copy()
+    o.phase(orc.PH_HLC_STEP, 2); g.phase(B.PH_HLC_STEP, 2)
+    gho, ghg = o.get(orc.GHAT), g.get(B.GHAT).astype(np.float64)
+    floor = PT.fd_floor(np.abs(o.get(orc.F)) + 50.0 * hp.sigma_s ** 2, hp.fd_h, wl.obj.sigma_noise) * 4
+    err = np.max(np.abs(ghg - gho), axis=1)
+    tol = PT.G_REL * np.max(np.abs(gho), axis=1) + floor
+    assert np.all(err[act] <= tol[act]), float(np.max(err[act] / tol[act]))
+    xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
+    xt = PT.x_tol(xo, hp.lo, hp.hi) + hp.eta_hlc * tol
+    assert np.all(np.max(np.abs(xg - xo), axis=1)[act] <= xt[act])
+    assert np.array_equal(xg[~act], x0[~act])
+    assert g.stats().evals[5] == int(act.sum()) * M * 2 * hp.d == o.stats().evals[5]
