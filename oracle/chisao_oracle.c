@@ -32,7 +32,7 @@ struct orc_ctx {
   uint8_t *stuck, *removed, *stalled;
   int32_t cycle, gr_enabled, gr_unproductive, gr_prev_modes, gr_used_last;
   int32_t k_lost, n_stuck, n_active, reseed_strategy;
-  double f_max;
+  double f_max, sigma_eff;
   uint64_t evals[8];
   /* diagnostics */
   double *p, *ls_margin, *asc_margin, *curv_margin, *ghat, *hlc_f, *hlc_u, *rs_margin;
@@ -531,7 +531,7 @@ static void phase_reseed(orc_ctx *s) {
  * k 2d + 2 + 2j of (phase 5, step t).  Selected by hlc_baseline == 2 (DESIGN.md NEXT-2). */
 static void hlc_sample_eq5(orc_ctx *s, int i, int t) {
   const int d = s->c.d, M = s->c.hlc_M;
-  const double sig = (double)s->c.sigma_s, eta = (double)s->c.eta_hlc, h = (double)s->c.fd_h;
+  const double sig = s->sigma_eff, eta = (double)s->c.eta_hlc, h = (double)s->c.fd_h;
   double *gh = s->ghat + (size_t)i * d;
   for (int j = 0; j < d; ++j) gh[j] = 0.0;
   if (s->stuck[i] || s->removed[i]) return;            /* "Stuck samples are excluded" PAPER.md:120 */
@@ -558,7 +558,7 @@ static void hlc_sample_eq5(orc_ctx *s, int i, int t) {
 
 static void hlc_sample(orc_ctx *s, int i, int t) {
   const int d = s->c.d, M = s->c.hlc_M;
-  const double sig = (double)s->c.sigma_s, eta = (double)s->c.eta_hlc;
+  const double sig = s->sigma_eff, eta = (double)s->c.eta_hlc;
   double *gh = s->ghat + (size_t)i * d;
   if (s->c.hlc_baseline == 2) { hlc_sample_eq5(s, i, t); return; }
   for (int j = 0; j < d; ++j) gh[j] = 0.0;
@@ -588,9 +588,26 @@ static void hlc_sample(orc_ctx *s, int i, int t) {
   free(ubuf);
 }
 
+/* Smoothing scale: supplied by the caller (sigma_s > 0), or auto-estimated from the sample spread,
+ * sigma = c std({x_i : not stuck_i}) with c = |sigma_s| (paper default c = 0.1).  Reading R-18: std is the pooled
+ * population standard deviation over all coordinates of the unfrozen samples, re-estimated at the start of every
+ * Hands-Like-Clouds step; sigma = 0 (no spread, or nobody unfrozen) leaves the samples where they are. */
+static void hlc_sigma(orc_ctx *s) {
+  if (s->c.sigma_s > 0.0f) { s->sigma_eff = (double)s->c.sigma_s; return; }
+  const int N = s->c.N, d = s->c.d;
+  double n = 0.0, mean = 0.0, var = 0.0;
+  for (int i = 0; i < N; ++i) if (!s->stuck[i] && !s->removed[i]) for (int j = 0; j < d; ++j) { mean += s->x[(size_t)i * d + j]; n += 1.0; }
+  if (n == 0.0) { s->sigma_eff = 0.0; return; }
+  mean /= n;
+  for (int i = 0; i < N; ++i) if (!s->stuck[i] && !s->removed[i]) for (int j = 0; j < d; ++j) { double t = s->x[(size_t)i * d + j] - mean; var += t * t; }
+  s->sigma_eff = fabs((double)s->c.sigma_s) * sqrt(var / n);
+}
+
 static void phase_hlc_step(orc_ctx *s, int t) {
   const int N = s->c.N;
   if (!(s->c.phase_mask & (1u << 5))) return;
+  hlc_sigma(s);
+  if (s->sigma_eff == 0.0) return;
 #pragma omp parallel for schedule(dynamic, 8) num_threads(s->nthreads)
   for (int i = 0; i < N; ++i) hlc_sample(s, i, t);
 }
@@ -796,6 +813,7 @@ static int xfer_field(orc_ctx *s, int field, void *u, uint64_t bytes, int to_use
   case ORC_RS_SRC: return xfer(s->rs_src, 4 * N, u, bytes, to_user);
   case ORC_RS_CAND: return xfer(s->rs_cand, 4 * N, u, bytes, to_user);
   case ORC_RS_MARGIN: return xfer(s->rs_margin, 8 * N, u, bytes, to_user);
+  case ORC_SIGMA: return to_user ? xfer(&s->sigma_eff, 8, u, bytes, 1) : -1;
   }
   return -1;
 }

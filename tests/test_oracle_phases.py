@@ -490,3 +490,25 @@ def test_hlc_eq5_form_on_a_quadratic_is_the_gradient_at_the_mean_perturbed_point
         assert np.allclose(o.get(orc.X)[i], np.clip(x0[i] + float(np.float32(1e-3)) * gh, -4, 4).astype(np.float32), atol=1e-7)
     assert np.array_equal(o.get(orc.X)[3], x0[3]) and not o.get(orc.GHAT)[3].any()
     assert o.stats().evals[5] == 11 * 7 * 2 * 5
+
+
+def test_hlc_sigma_auto_is_c_times_the_pooled_std_of_the_unfrozen_samples(orc):
+    """sigma = c std({x_i : not stuck_i}), c = 0.1 by default (R-18: pooled population std over all
+    coordinates of the unfrozen samples); sigma_s > 0 is used as given."""
+    obj = inputs.gmm_iso(3, 2, 0.5, 2.0, 5)
+    wl = inputs.custom(obj, 3.0, 50, sigma_s=-0.1, hlc_M=4, eta_hlc=1e-3, seed=31)
+    o = orc.Oracle(wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    stuck = np.zeros(50, np.uint8); stuck[::3] = 1
+    o.set(orc.STUCK, stuck)
+    x0 = o.get(orc.X).copy()
+    o.phase(orc.PH_HLC_STEP, 1)
+    assert abs(o.get(orc.SIGMA)[0] - float(np.float32(0.1)) * np.std(x0[stuck == 0])) < 1e-12
+    assert np.array_equal(o.get(orc.X)[stuck == 1], x0[stuck == 1]) and not np.array_equal(o.get(orc.X), x0)
+    wl2 = inputs.custom(obj, 3.0, 50, sigma_s=0.25, hlc_M=4, seed=31)
+    o2 = orc.Oracle(wl2); o2.phase(orc.PH_HLC_STEP, 1)
+    assert o2.get(orc.SIGMA)[0] == 0.25
+    # nobody unfrozen: sigma = 0 and nothing moves
+    o.set(orc.STUCK, np.ones(50, np.uint8)); x1 = o.get(orc.X).copy()
+    o.phase(orc.PH_HLC_STEP, 2)
+    assert o.get(orc.SIGMA)[0] == 0.0 and np.array_equal(o.get(orc.X), x1)
