@@ -75,7 +75,8 @@ typedef struct {
   float fd_h;               /* central finite-difference step (R-1) */
   float eps_grad, eps_dup, log_delta;            /* Eq. 3 / Eq. 4 thresholds */
   float mu, alpha_anti;     /* Eq. 6 momentum and step */
-  float eta_hlc, sigma_s;   /* HLC step size and smoothing scale */
+  float eta_hlc, sigma_s;   /* HLC step size and smoothing scale; sigma_s < 0: auto-estimate
+                               sigma = |sigma_s| * std of the unfrozen samples (paper default c = 0.1; R-18) */
   float ls_c1, ls_shrink;   /* Armijo constant and backtracking factor (R-4) */
   int32_t hlc_baseline;     /* 0: literal estimator; 1: subtract the mean of the M values (R-11);
                                2: the paper's Eq. 5 form, mean of M FD gradients at perturbed points */
@@ -116,7 +117,8 @@ enum {
   CHISAO_RS_SRC = 27,  /* [N] i32 reseed source (RM: sample, GR: peak), -1 if not reseeded */
   CHISAO_RS_CAND = 28, /* [N] i32 RM: chosen candidate; GR: 2*column + sign */
   CHISAO_XT = 31,      /* [N][d] last line-search trial point */
-  CHISAO_GR_Q = 32     /* [d][d] last Golden-Rooster basis, element (r, c) at r*d + c */
+  CHISAO_GR_Q = 32,    /* [d][d] last Golden-Rooster basis, element (r, c) at r*d + c */
+  CHISAO_SIGMA = 33    /* [1] smoothing scale used by the last Hands-Like-Clouds step */
 };
 
 /* Units for chisao_phase (exactly one unit on the current state; used by teacher-forced parity tests). */

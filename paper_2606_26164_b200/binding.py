@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libchisao.so")
 
 OK, E_INVALID, E_WORKSPACE, E_CAPACITY, E_CUDA, E_STATE = 0, -1, -2, -3, -4, -5
 X, F, G, V, STUCK, REMOVED, HIST_S, HIST_Y, HIST_LEN, STALLED, CTRL = range(11)
-P, LS_B, GHAT, HLC_F, RS_SRC, RS_CAND, XT, GR_Q = 20, 21, 25, 26, 27, 28, 31, 32
+P, LS_B, GHAT, HLC_F, RS_SRC, RS_CAND, XT, GR_Q, SIGMA = 20, 21, 25, 26, 27, 28, 31, 32, 33
 PH_RELEASE_EVAL, PH_STICK, PH_DEDUP, PH_RESEED, PH_HLC_STEP, PH_ANTI_STEP, PH_LBFGS_ITER = 1, 2, 3, 4, 5, 6, 11
 PH_LBFGS_DIRECTION = 12
 TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_update", "select", "reseed")
@@ -214,7 +214,7 @@ class Chisao:
     def _shape(self, field):
         N, d, m, M = self.N, self.d, self.m, self.M
         return {X: (N, d), G: (N, d), V: (N, d), P: (N, d), GHAT: (N, d), XT: (N, d), HIST_S: (m, N, d),
-                HIST_Y: (m, N, d), HLC_F: (N, M), CTRL: (8,), GR_Q: (d, d)}.get(field, (N,))
+                HIST_Y: (m, N, d), HLC_F: (N, M), CTRL: (8,), GR_Q: (d, d), SIGMA: (1,)}.get(field, (N,))
 
     def get(self, field):
         a = np.empty(self._shape(field), _FIELD_DTYPE.get(field, np.float32))

@@ -77,7 +77,7 @@ int validate(const chisao_config *cfg, const chisao_objective *obj, std::string 
   if (cfg->reseed_cands < 1 || cfg->reseed_cands > 16) { why = "reseed_cands must be in 1..16"; return CHISAO_E_INVALID; }
   if (cfg->n_osc < 1 || cfg->n_conv < 0 || cfg->n_anti < 0 || cfg->n_cloud < 0) { why = "negative iteration count"; return CHISAO_E_INVALID; }
   if (!(cfg->fd_h > 0.0f)) { why = "fd_h must be > 0"; return CHISAO_E_INVALID; }
-  if (!(cfg->sigma_s > 0.0f)) { why = "sigma_s must be > 0"; return CHISAO_E_INVALID; }
+  if (!(cfg->sigma_s != 0.0f) || !(fabsf(cfg->sigma_s) < 3.0e38f)) { why = "sigma_s must be > 0 (given) or < 0 (auto, c = |sigma_s|)"; return CHISAO_E_INVALID; }
   if (!cfg->lo || !cfg->hi) { why = "null bounds"; return CHISAO_E_INVALID; }
   for (int j = 0; j < cfg->d; ++j)
     if (!(cfg->lo[j] <= cfg->hi[j])) { why = "lo > hi"; return CHISAO_E_INVALID; }
@@ -284,7 +284,7 @@ cudaError_t hlc_step(chisao_ctx *c, int iter) {
   HlcArgs a{};
   a.list = s.listE; a.count = &s.ctrl->nE; a.max_count = s.N; a.d = s.d; a.M = s.M; a.cycle = c->cycle; a.iter = iter;
   a.baseline = c->hp.hlc_baseline; a.x = s.x; a.ghat = s.ghat; a.hlc_f = s.hlc_f; a.lo = s.lo; a.hi = s.hi;
-  a.sigma = c->hp.sigma_s; a.eta = c->hp.eta_hlc; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
+  a.sigma_dev = &s.ctrl->sigma_eff; a.eta = c->hp.eta_hlc; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
   const int spt = std::min(PTILE / s.M, HLC_MAX_SPT);
   const int grid = (s.N + spt - 1) / spt;
   Scope sc(c, 2);
@@ -341,6 +341,7 @@ int run_explore_list(chisao_ctx *ctx) {
 }
 int run_hlc(chisao_ctx *ctx, int t) {
   if (!(ctx->hp.phase_mask & (1u << 5))) return CHISAO_OK;
+  { Scope sc(ctx, 2); CK(launch_hlc_sigma(ctx->st, ctx->hp, ctx->stream)); ctx->launches += 2; }
   if (ctx->hp.hlc_baseline == 2) {   // the paper's Eq. 5 form: K FD gradients at perturbed points (NEXT-2)
     const State &s = ctx->st;
     for (int k = 0; k < ctx->hp.hlc_M; ++k) {
@@ -589,6 +590,7 @@ static int field_info(chisao_ctx *ctx, int32_t field, void **dev, size_t *bytes)
     case CHISAO_RS_CAND: *dev = s.rs_cand; *bytes = N * 4; return 0;
     case CHISAO_XT: *dev = s.xt; *bytes = N * d * 4; return 0;
     case CHISAO_GR_Q: *dev = s.grQ; *bytes = d * d * 4; return 0;
+    case CHISAO_SIGMA: *dev = &s.ctrl->sigma_eff; *bytes = 4; return 0;
   }
   return -1;
 }

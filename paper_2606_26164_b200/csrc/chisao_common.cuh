@@ -30,8 +30,9 @@ struct Ctrl {
   uint32_t fmax_enc;       // order-preserving image of f_max (0 = nothing finite yet)
   int32_t ls_cnt[3];       // rotating line-search worklist counters
   int32_t fd_cnt;          // samples whose trial was accepted this iteration
-  int32_t pad0;
+  float sigma_eff;         // smoothing scale used by the current HLC step (caller's, or c * std of the unfrozen samples)
   unsigned long long evals[8];
+  double sx, sxx;          // pooled sums for the sigma auto-estimate
 };
 
 // ---- objective parameters packed as fixed-size component records --------------------------------
@@ -105,6 +106,7 @@ cudaError_t launch_dedup(const State &s, const Hyper &h, cudaStream_t st);      
 cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_t st);
 cudaError_t launch_explore_list(const State &s, cudaStream_t st);
 // paper-form HLC (Eq. 5) helpers: stage 0 perturb (xt = x + sigma z_k), 1 accumulate (ghat += gn / M), 2 apply
+cudaError_t launch_hlc_sigma(const State &s, const Hyper &h, cudaStream_t st);   // ctrl->sigma_eff (R-18)
 cudaError_t launch_hlc5(const State &s, const Hyper &h, int cycle, int iter, int k, int stage, cudaStream_t st);
 cudaError_t launch_seed_population(const State &s, const Hyper &h, cudaStream_t st);
 cudaError_t launch_gather_rows(const float *x, const int32_t *idx, int n, int d, float *out, cudaStream_t st);

@@ -172,7 +172,8 @@ struct HlcArgs {
   int32_t max_count, d, M, cycle, iter, baseline;
   float *x, *ghat, *hlc_f;
   const float *lo, *hi;
-  float sigma, eta;
+  const float *sigma_dev;    // ctrl->sigma_eff (caller's sigma_s or the auto-estimate)
+  float eta;
   uint64_t seed;
   unsigned long long *evals;
 };
@@ -189,6 +190,8 @@ __global__ void __launch_bounds__(NT, 2) k_hlc(const DevObj o, const HlcArgs a) 
   float4 *U = reinterpret_cast<float4 *>(sm.extra);                 // [DP/4][PTILE] normals
   float *fvs = reinterpret_cast<float *>(U + (DP / 4) * PTILE);     // [PTILE] values
   const int t = threadIdx.x, d = a.d, M = a.M;
+  const float sigma = *a.sigma_dev;
+  if (sigma == 0.0f) return;                       // no spread among the unfrozen samples: nobody moves (R-18)
   const int spt = min(PTILE / M, HLC_MAX_SPT);
   const int cnt = a.count ? *a.count : a.max_count;
   const int first = blockIdx.x * spt;
@@ -226,7 +229,7 @@ __global__ void __launch_bounds__(NT, 2) k_hlc(const DevObj o, const HlcArgs a) 
             const uint32_t ln = n & 3u;
             const float u = ln == 0u ? z0 : (ln == 1u ? z1 : (ln == 2u ? z2 : z3));
             set4(uv, l, u);
-            set4(pv, l, fmaf(a.sigma, u, get4(xv, l)));   // evaluation points are not clipped (R-12)
+            set4(pv, l, fmaf(sigma, u, get4(xv, l)));   // evaluation points are not clipped (R-12)
           }
         }
         U[c4 * PTILE + p] = uv;
@@ -264,7 +267,7 @@ __global__ void __launch_bounds__(NT, 2) k_hlc(const DevObj o, const HlcArgs a) 
     }
     float acc = 0.0f;
     for (int k = 0; k < M; ++k) acc = fmaf(fvs[s * M + k] - b, get4(U[(j >> 2) * PTILE + s * M + k], j & 3), acc);
-    const float gh = acc / ((float)M * a.sigma);
+    const float gh = acc / ((float)M * sigma);
     a.ghat[(size_t)i * d + j] = gh;
     // x_j of the centre = staged point minus sigma u is not exact; re-read the row (written only here)
     const float xo = a.x[(size_t)i * d + j];

@@ -391,6 +391,45 @@ cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_
   return cudaGetLastError();
 }
 
+// ---- smoothing scale of Hands Like Clouds (R-18): sigma_s > 0 as given, else c * pooled population
+// std over all coordinates of the unfrozen samples (c = |sigma_s|), re-estimated at every step -------------------
+__global__ void __launch_bounds__(256) k_sigma_sum(State s) {
+  __shared__ double shx[8], shxx[8];
+  const int nE = s.ctrl->nE, d = s.d;
+  const size_t n = (size_t)nE * d;
+  double a = 0.0, b = 0.0;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+    const int q = (int)(e / d), j = (int)(e - (size_t)q * d);
+    const double v = (double)s.x[(size_t)s.listE[q] * d + j];
+    a += v; b += v * v;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+  if ((threadIdx.x & 31) == 0) { shx[threadIdx.x >> 5] = a; shxx[threadIdx.x >> 5] = b; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) { a += shx[w]; b += shxx[w]; }
+    atomicAdd(&s.ctrl->sx, a); atomicAdd(&s.ctrl->sxx, b);
+  }
+}
+__global__ void k_sigma_final(State s, Hyper h) {
+  Ctrl *c = s.ctrl;
+  if (h.sigma_s > 0.0f) { c->sigma_eff = h.sigma_s; return; }
+  const double n = (double)c->nE * (double)s.d;
+  if (n == 0.0) { c->sigma_eff = 0.0f; return; }
+  const double mean = c->sx / n, var = fmax(c->sxx / n - mean * mean, 0.0);
+  c->sigma_eff = (float)(fabs((double)h.sigma_s) * sqrt(var));
+}
+cudaError_t launch_hlc_sigma(const State &s, const Hyper &h, cudaStream_t st) {
+  if (h.sigma_s <= 0.0f && s.N > 0) {
+    cudaError_t e = cudaMemsetAsync(&s.ctrl->sx, 0, 2 * sizeof(double), st);
+    if (e != cudaSuccess) return e;
+    k_sigma_sum<<<148, 256, 0, st>>>(s);
+  }
+  k_sigma_final<<<1, 1, 0, st>>>(s, h);
+  return cudaGetLastError();
+}
+
 // ---- Hands Like Clouds, the paper's own form, Eq. 5 (DESIGN.md NEXT-2) -----------------------
 // theta <- theta + eta (1/K) sum_k grad f(theta + sigma z_k) with FD gradients: per draw k the host runs
 // [perturb: xt = x + sigma z_k] -> k_eval_fd on xt (noise slots k 2d + ..) -> [accumulate: ghat += gn / K], then
@@ -398,13 +437,13 @@ cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_
 __global__ void k_hlc5(State s, Hyper h, int cycle, int iter, int k, int stage) {
   const int nE = s.ctrl->nE, d = s.d;
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= (size_t)nE * d) return;
+  if (e >= (size_t)nE * d || s.ctrl->sigma_eff == 0.0f) return;   // sigma = 0: nobody moves (R-18)
   const int q = (int)(e / d), j = (int)(e - (size_t)q * d);
   const int i = s.listE[q];
   const size_t o = (size_t)i * d + j;
   if (stage == 0) {
     const float u = rng_normal(h.seed, (uint32_t)i, (uint32_t)cycle, rng_tag(5, iter, PUR_HLC_U), (uint32_t)(k * d + j));
-    s.xt[o] = fmaf(h.sigma_s, u, s.x[o]);                 // evaluation points are not clipped (R-12)
+    s.xt[o] = fmaf(s.ctrl->sigma_eff, u, s.x[o]);         // evaluation points are not clipped (R-12)
   } else if (stage == 1) {
     s.ghat[o] = (k == 0 ? 0.0f : s.ghat[o]) + s.gn[o] / (float)h.hlc_M;
   } else {

@@ -163,6 +163,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
   const TcSmem sm = tc_carve(tc_smem_raw);
   const int t = threadIdx.x, d = a.d, M = a.M;
+  const float sigma = *a.sigma_dev;
+  if (sigma == 0.0f) return;                       // no spread among the unfrozen samples: nobody moves (R-18)
   const int spt = min(TC_PTS / M, HLC_MAX_SPT);
   const int cnt = a.count ? *a.count : a.max_count;
   const int first = blockIdx.x * spt;
@@ -178,7 +180,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
     hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
     tc_load_row(a.x + (size_t)i * d, d, (d & 3) == 0, x);
 #pragma unroll
-    for (int c = 0; c < TC_D; ++c) x[c] = fmaf(a.sigma, u[c], x[c]);   // evaluation points are not clipped (R-12)
+    for (int c = 0; c < TC_D; ++c) x[c] = fmaf(sigma, u[c], x[c]);   // evaluation points are not clipped (R-12)
   } else {
 #pragma unroll
     for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
@@ -207,7 +209,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
     if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
     float acc = 0.0f;
     for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, Us[(ss * M + kk) * 65 + j], acc);
-    const float gh = acc / ((float)M * a.sigma);
+    const float gh = acc / ((float)M * sigma);
     a.ghat[(size_t)ii * d + j] = gh;
     const float xo = a.x[(size_t)ii * d + j];
     a.x[(size_t)ii * d + j] = clipf(fmaf(a.eta, gh, xo), a.lo[j], a.hi[j]);

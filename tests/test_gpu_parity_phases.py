@@ -308,3 +308,34 @@ def test_a6_hlc_step_paper_form_eq5(orc, B, c, N, M):
     assert np.all(np.max(np.abs(xg - xo), axis=1)[act] <= xt[act])
     assert np.array_equal(xg[~act], x0[~act])
     assert g.stats().evals[5] == int(act.sum()) * M * 2 * hp.d == o.stats().evals[5]
+
+
+@pytest.mark.parametrize("c,N,form", [(2, 500, 1), (5, 150, 1), (3, 200, 2)])
+def test_a6_hlc_sigma_auto_estimate(orc, B, c, N, form):
+    """NEXT-4 / PAPER.md:120: sigma = c std({x_i : not stuck_i}) (sigma_s = -0.1 selects c = 0.1; R-18): the scale
+    matches the oracle to fp32 rounding, and the step taken with it stays within the HLC tolerances."""
+    wl = inputs.config(c, N=N, sigma_s=-0.1, hlc_baseline=form, hlc_M=8)
+    hp = wl.hp
+    o, g = _converged_pair(orc, B, wl, 2)
+    o.phase(orc.PH_STICK)
+    stuck = o.get(orc.STUCK).copy(); stuck[::4] = 1
+    o.set(orc.STUCK, stuck)
+    act = stuck == 0
+    PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+    x0 = o.get(orc.X).copy()
+    o.phase(orc.PH_HLC_STEP, 1); g.phase(B.PH_HLC_STEP, 1)
+    so, sg = float(o.get(orc.SIGMA)[0]), float(g.get(B.SIGMA)[0])
+    assert so > 0 and abs(sg - so) <= 4 * PT.EPS32 * so
+    gho, ghg = o.get(orc.GHAT), g.get(B.GHAT).astype(np.float64)
+    fscale = np.max(np.abs(o.get(orc.HLC_F)), axis=1) if form == 1 else np.abs(o.get(orc.F)) + 50.0 * so ** 2
+    floor = 8 * PT.EPS32 * (fscale + 6 * wl.obj.sigma_noise + 1.0) * (5.5 / so if form == 1 else 4.0 / (2 * hp.fd_h))
+    err = np.max(np.abs(ghg - gho), axis=1)
+    tol = PT.G_REL * np.max(np.abs(gho), axis=1) + floor
+    assert np.all(err[act] <= tol[act]), float(np.max(err[act] / tol[act]))
+    xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
+    assert np.all(np.max(np.abs(xg - xo), axis=1)[act] <= (PT.x_tol(xo, hp.lo, hp.hi) + hp.eta_hlc * tol)[act])
+    assert np.array_equal(xg[~act], x0[~act])
+    # everybody frozen: sigma = 0 and nothing moves on either side
+    g.set(B.STUCK, np.ones(N, np.uint8)); x1 = g.get(B.X).copy()
+    g.phase(B.PH_HLC_STEP, 2)
+    assert float(g.get(B.SIGMA)[0]) == 0.0 and np.array_equal(g.get(B.X), x1)
