@@ -339,3 +339,31 @@ def test_a6_hlc_sigma_auto_estimate(orc, B, c, N, form):
     g.set(B.STUCK, np.ones(N, np.uint8)); x1 = g.get(B.X).copy()
     g.phase(B.PH_HLC_STEP, 2)
     assert float(g.get(B.SIGMA)[0]) == 0.0 and np.array_equal(g.get(B.X), x1)
+
+
+def test_ablation_switches_phase_mask(orc, B):
+    """PAPER.md:498-509 (Table 7 rows): phase_mask bit p off disables phase p on both sides -- no removal (3), no
+    reseeding (4), no HLC move (5), no anti-convergence move (6); the other phases still run."""
+    obj = inputs.gmm_diag(8, 16, 5.0, 1002)
+    for off in (3, 4, 5, 6):
+        wl = inputs.custom(obj, 5.0, 300, eps_dup=0.5, eps_grad=1.0, seed=5, phase_mask=0xFFFFFFFF & ~(1 << off))
+        o, g = _pair(orc, B, wl)
+        rng = np.random.default_rng(off)
+        x = PT.f32(rng.uniform(-5, 5, size=(300, 8))); x[100:200] = PT.f32(x[100] + rng.uniform(-0.01, 0.01, size=(100, 8)))
+        stuck = np.zeros(300, np.uint8); stuck[100:220] = 1
+        f = PT.f32(rng.standard_normal(300))
+        for fo, fg, val in ((orc.X, B.X, x), (orc.F, B.F, f), (orc.STUCK, B.STUCK, stuck), (orc.CTRL, B.CTRL, [1, 1, 0, 0, 0, 0, 120, 180])):
+            o.set(fo, val); g.set(fg, val)
+        o.phase(orc.PH_DEDUP); g.phase(B.PH_DEDUP)
+        assert np.array_equal(g.get(B.REMOVED), o.get(orc.REMOVED))
+        assert (g.get(B.REMOVED).sum() == 0) == (off == 3)
+        o.phase(orc.PH_RESEED); g.phase(B.PH_RESEED)
+        assert g.stats().reseed_strategy == o.stats().reseed_strategy
+        assert (g.stats().reseed_strategy == 0) == (off in (3, 4))
+        x1 = g.get(B.X).copy()
+        g.phase(B.PH_HLC_STEP, 1)
+        moved = not np.array_equal(g.get(B.X), x1)
+        assert moved == (off != 5)
+        x2 = g.get(B.X).copy()
+        g.phase(B.PH_ANTI_STEP, 1)
+        assert (not np.array_equal(g.get(B.X), x2)) == (off != 6)
