@@ -159,6 +159,41 @@ static double objective(const orc_ctx *s, const double *x) {
     }
     return -0.5 * q;
   }
+  /* Appendix D of the paper, "Benchmark Function Definitions", all negated for maximisation */
+  case 5: { /* Rastrigin: f = -[A d + sum (x_i^2 - A cos(2 pi x_i))], A = 10 */
+    double acc = 10.0 * d;
+    for (int j = 0; j < d; ++j) acc += x[j] * x[j] - 10.0 * cos(2.0 * M_PI * x[j]);
+    return -acc;
+  }
+  case 6: { /* Ackley: a = 20, b = 0.2, c = 2 pi */
+    double s2 = 0.0, sc = 0.0;
+    for (int j = 0; j < d; ++j) { s2 += x[j] * x[j]; sc += cos(2.0 * M_PI * x[j]); }
+    return -(-20.0 * exp(-0.2 * sqrt(s2 / d)) - exp(sc / d) + 20.0 + M_E);
+  }
+  case 7: { /* Schwefel: f = -[418.9829 d - sum x_i sin(sqrt|x_i|)] */
+    double acc = 0.0;
+    for (int j = 0; j < d; ++j) acc += x[j] * sin(sqrt(fabs(x[j])));
+    return -(418.9829 * d - acc);
+  }
+  case 8: { /* Styblinski-Tang: f = -1/2 sum (x^4 - 16 x^2 + 5 x) */
+    double acc = 0.0;
+    for (int j = 0; j < d; ++j) { double t = x[j]; acc += t * t * t * t - 16.0 * t * t + 5.0 * t; }
+    return -0.5 * acc;
+  }
+  case 9: { /* Michalewicz: f = sum sin(x_i) sin^{2m}(i x_i^2 / pi), m = 10, i = 1..d */
+    double acc = 0.0;
+    for (int j = 0; j < d; ++j) acc += sin(x[j]) * pow(sin((j + 1) * x[j] * x[j] / M_PI), 20.0);
+    return acc;
+  }
+  case 10: { /* Trid: f = -[sum (x_i - 1)^2 - sum_{i>=2} x_i x_{i-1}] */
+    double acc = 0.0;
+    for (int j = 0; j < d; ++j) acc += (x[j] - 1.0) * (x[j] - 1.0);
+    for (int j = 1; j < d; ++j) acc -= x[j] * x[j - 1];
+    return -acc;
+  }
+  case 11: { /* Bukin N.6, PAPER.md:627 (d = 2): f = -[100 sqrt|y - 0.01 x^2| + 0.01 |x + 10|] */
+    return -(100.0 * sqrt(fabs(x[1] - 0.01 * x[0] * x[0])) + 0.01 * fabs(x[0] + 10.0));
+  }
   }
   return NAN;
 }
@@ -726,6 +761,8 @@ orc_ctx *orc_create(const orc_config *cfg, const orc_objective *obj, const float
   case 2: nmeans = K * d; nmats = K * d * d; na = K; break;
   case 3: nmats = K * d; na = K; nb = K; break;
   case 4: nmeans = d; nmats = d * d; break;
+  case 5: case 6: case 7: case 8: case 9: case 10: break;       /* parameter-free (App. D) */
+  case 11: if (d != 2) { free(s); return NULL; } break;
   default: free(s); return NULL;
   }
   s->means = promote(obj->means, nmeans); s->mats = promote(obj->mats, nmats);

@@ -27,6 +27,9 @@ from typing import Optional
 import numpy as np
 
 OBJ_GMM_ISO, OBJ_GMM_DIAG, OBJ_GMM_FULL, OBJ_RFF, OBJ_QUAD = 0, 1, 2, 3, 4
+# Appendix D of the paper: parameter-free benchmark functions, negated for maximisation
+OBJ_RASTRIGIN, OBJ_ACKLEY, OBJ_SCHWEFEL, OBJ_STYBLINSKI_TANG, OBJ_MICHALEWICZ, OBJ_TRID, OBJ_BUKIN6 = 5, 6, 7, 8, 9, 10, 11
+APPENDIX_D = {"rastrigin": 5, "ackley": 6, "schwefel": 7, "styblinski_tang": 8, "michalewicz": 9, "trid": 10, "bukin6": 11}
 
 
 @dataclass
@@ -248,6 +251,28 @@ def noise_robustness(sigma_noise: float, trial: int = 0, N: int = 200) -> Worklo
                log_delta=math.log(0.1) - 4.0 * sigma_noise, alpha_anti=0.05, eta_hlc=0.05, sigma_s=1.0, hlc_baseline=1)
     hp.seed = 500 + trial
     return Workload(f"noise{sigma_noise:g}", obj, hp, uniform_population(N, lo, hi, 501 + trial))
+
+
+def appendix_d(name: str, d: int, N: int, seed: int = 11, **over) -> Workload:
+    """One of the benchmark functions printed in the paper's Appendix D on its printed domain.
+    Only the seven functions whose definitions are in the paper are available."""
+    oid = APPENDIX_D[name]
+    if name == "bukin6":
+        d = 2
+        lo, hi = np.array([-15.0, -3.0], np.float32), np.array([-5.0, 3.0], np.float32)
+    elif name == "michalewicz":
+        lo, hi = np.zeros(d, np.float32), np.full(d, np.float32(math.pi), np.float32)
+    else:
+        b = {"rastrigin": 5.12, "ackley": 32.768, "schwefel": 500.0, "styblinski_tang": 5.0, "trid": float(d * d)}[name]
+        lo, hi = _box(d, b)
+    obj = Objective(oid, d, 1, np.zeros((1, d), np.float32), np.zeros(1, np.float32), np.zeros(1, np.float32))
+    hp = Hyper(d, N, lo, hi, n_conv=n_conv_default(d))
+    hp.seed = seed
+    for k, v in over.items():
+        if not hasattr(hp, k):
+            raise KeyError(k)
+        setattr(hp, k, v)
+    return Workload(name, obj, hp, uniform_population(N, lo.astype(np.float64), hi.astype(np.float64), seed + 1))
 
 
 def custom(obj: Objective, box: float, N: int, seed: int = 7, **over) -> Workload:
