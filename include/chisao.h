@@ -50,7 +50,16 @@ typedef enum {
   CHISAO_OBJ_GMM_DIAG = 1,  /* log sum_k w_k N(x; mu_k, diag(sigma_k^2))                              */
   CHISAO_OBJ_GMM_FULL = 2,  /* log sum_k w_k N(x; mu_k, Sigma_k), Sigma_k^-1 = W_k^T W_k              */
   CHISAO_OBJ_RFF      = 3,  /* -s0 ||x||^2 + sum_j a_j cos(w_j . x + b_j)                             */
-  CHISAO_OBJ_QUAD     = 4   /* -1/2 ||W (x - c)||^2                                                   */
+  CHISAO_OBJ_QUAD     = 4,  /* -1/2 ||W (x - c)||^2                                                   */
+  /* parameter-free benchmark functions of the paper's Appendix D, negated for maximisation;
+     K must be 1, the parameter pointers are ignored (may be null) */
+  CHISAO_OBJ_RASTRIGIN       = 5,   /* -[10 d + sum (x^2 - 10 cos(2 pi x))] */
+  CHISAO_OBJ_ACKLEY          = 6,   /* a = 20, b = 0.2, c = 2 pi */
+  CHISAO_OBJ_SCHWEFEL        = 7,   /* -[418.9829 d - sum x sin(sqrt|x|)] */
+  CHISAO_OBJ_STYBLINSKI_TANG = 8,   /* -1/2 sum (x^4 - 16 x^2 + 5 x) */
+  CHISAO_OBJ_MICHALEWICZ     = 9,   /* sum sin(x_i) sin^20(i x_i^2 / pi) */
+  CHISAO_OBJ_TRID            = 10,  /* -[sum (x_i - 1)^2 - sum x_i x_{i-1}] */
+  CHISAO_OBJ_BUKIN6          = 11   /* -[100 sqrt|y - 0.01 x^2| + 0.01 |x + 10|], d = 2 */
 } chisao_objective_id;
 
 typedef struct {            /* all arrays HOST, fp32, row-major; copied at init */

@@ -21,7 +21,7 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
 UNITS = [("chisao_api.cu", []), ("chisao_lbfgs.cu", []), ("chisao_select.cu", []), ("chisao_tc_kernels.cu", [])] + \
-        [("chisao_eval_obj.cu", [f"-DCHISAO_OBJ_INST={i}"]) for i in range(5)]
+        [("chisao_eval_obj.cu", [f"-DCHISAO_OBJ_INST={i}"]) for i in range(6)]
 
 
 def _headers():

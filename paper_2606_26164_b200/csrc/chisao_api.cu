@@ -81,13 +81,18 @@ int validate(const chisao_config *cfg, const chisao_objective *obj, std::string 
   if (!cfg->lo || !cfg->hi) { why = "null bounds"; return CHISAO_E_INVALID; }
   for (int j = 0; j < cfg->d; ++j)
     if (!(cfg->lo[j] <= cfg->hi[j])) { why = "lo > hi"; return CHISAO_E_INVALID; }
-  if (obj->id < 0 || obj->id > 4) { why = "unknown objective id"; return CHISAO_E_INVALID; }
+  if (obj->id < 0 || obj->id > CHISAO_OBJ_BUKIN6) { why = "unknown objective id"; return CHISAO_E_INVALID; }
   if (obj->K < 1) { why = "K < 1"; return CHISAO_E_INVALID; }
-  if (obj->id == CHISAO_OBJ_QUAD && obj->K != 1) { why = "QUAD needs K = 1"; return CHISAO_E_INVALID; }
-  if (!obj->mats) { why = "objective.mats is null"; return CHISAO_E_INVALID; }
-  if (obj->id != CHISAO_OBJ_RFF && !obj->means) { why = "objective.means is null"; return CHISAO_E_INVALID; }
-  if (obj->id != CHISAO_OBJ_QUAD && !obj->vec_a) { why = "objective.vec_a is null"; return CHISAO_E_INVALID; }
-  if (obj->id == CHISAO_OBJ_RFF && !obj->vec_b) { why = "objective.vec_b is null"; return CHISAO_E_INVALID; }
+  if (obj->id >= CHISAO_OBJ_RASTRIGIN) {
+    if (obj->K != 1) { why = "Appendix-D objectives need K = 1"; return CHISAO_E_INVALID; }
+    if (obj->id == CHISAO_OBJ_BUKIN6 && obj->d != 2) { why = "Bukin N.6 needs d = 2"; return CHISAO_E_INVALID; }
+  } else {
+    if (obj->id == CHISAO_OBJ_QUAD && obj->K != 1) { why = "QUAD needs K = 1"; return CHISAO_E_INVALID; }
+    if (!obj->mats) { why = "objective.mats is null"; return CHISAO_E_INVALID; }
+    if (obj->id != CHISAO_OBJ_RFF && !obj->means) { why = "objective.means is null"; return CHISAO_E_INVALID; }
+    if (obj->id != CHISAO_OBJ_QUAD && !obj->vec_a) { why = "objective.vec_a is null"; return CHISAO_E_INVALID; }
+    if (obj->id == CHISAO_OBJ_RFF && !obj->vec_b) { why = "objective.vec_b is null"; return CHISAO_E_INVALID; }
+  }
   if (!(obj->sigma_noise >= 0.0f)) { why = "sigma_noise < 0"; return CHISAO_E_INVALID; }
   return CHISAO_OK;
 }
@@ -242,7 +247,8 @@ cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const in
     case 1: return launch_fd_obj_1(c->obj, a, grid, c->stream);
     case 2: return launch_fd_obj_2(c->obj, a, grid, c->stream);
     case 3: return launch_fd_obj_3(c->obj, a, grid, c->stream);
-    default: return launch_fd_obj_4(c->obj, a, grid, c->stream);
+    case 4: return launch_fd_obj_4(c->obj, a, grid, c->stream);
+    default: return launch_fd_obj_5(c->obj, a, grid, c->stream);
   }
 }
 
@@ -274,7 +280,8 @@ cudaError_t eval_points(chisao_ctx *c, int mode, int b, int iter) {
     case 1: return launch_pt_obj_1(c->obj, a, grid, c->stream);
     case 2: return launch_pt_obj_2(c->obj, a, grid, c->stream);
     case 3: return launch_pt_obj_3(c->obj, a, grid, c->stream);
-    default: return launch_pt_obj_4(c->obj, a, grid, c->stream);
+    case 4: return launch_pt_obj_4(c->obj, a, grid, c->stream);
+    default: return launch_pt_obj_5(c->obj, a, grid, c->stream);
   }
 }
 
@@ -295,7 +302,8 @@ cudaError_t hlc_step(chisao_ctx *c, int iter) {
     case 1: return launch_hlc_obj_1(c->obj, a, grid, c->stream);
     case 2: return launch_hlc_obj_2(c->obj, a, grid, c->stream);
     case 3: return launch_hlc_obj_3(c->obj, a, grid, c->stream);
-    default: return launch_hlc_obj_4(c->obj, a, grid, c->stream);
+    case 4: return launch_hlc_obj_4(c->obj, a, grid, c->stream);
+    default: return launch_hlc_obj_5(c->obj, a, grid, c->stream);
   }
 }
 
@@ -442,7 +450,8 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
     case 1: CKI(configure_obj_1()); break;
     case 2: CKI(configure_obj_2()); break;
     case 3: CKI(configure_obj_3()); break;
-    default: CKI(configure_obj_4()); break;
+    case 4: CKI(configure_obj_4()); break;
+    default: CKI(configure_obj_5()); break;
   }
   ctx->use_tc = wants_tc(*obj);
   if (ctx->use_tc) {

@@ -42,6 +42,9 @@ struct Ctrl {
 //   GMM_FULL: W[DP][DP] | mu[DP] | a, 0, 0, 0
 //   RFF     : w[DP] as fp64 (2 DP floats) | a, b, 0, 0    s0 = quadratic coefficient
 //   QUAD    : W[DP][DP] | c[DP] | 0, 0, 0, 0
+//   ids >= 5 (Appendix D): no parameters; the evaluator is instantiated once (template OBJ = CHISAO_OBJ_APPD) and
+//             picks the function from DevObj::id
+constexpr int CHISAO_OBJ_APPD = 5;
 struct DevObj {
   int32_t id, d, K, DP;
   int32_t rec;             // floats per record
@@ -59,7 +62,7 @@ inline int record_floats(int id, int DP) {
     case CHISAO_OBJ_RFF: return 2 * DP + 4;
     case CHISAO_OBJ_QUAD: return DP * DP + DP + 4;
   }
-  return 0;
+  return 4;   // Appendix-D functions carry no parameters (one dummy record keeps the workspace carve uniform)
 }
 
 // ---- device state pointers ------------------------------------------------------------------------

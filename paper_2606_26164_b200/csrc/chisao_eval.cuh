@@ -217,11 +217,94 @@ __device__ __forceinline__ void accum_records(const float *__restrict__ buf, int
   }
 }
 
+// ---- Appendix-D benchmark functions, negated for maximisation ----------------------
+// One staged point (column `col`), function chosen by the objective id (uniform over the launch).  The sums are
+// rearranged so that no large constant is cancelled in fp32 (the rearrangements are exact identities):
+//   Rastrigin  10 d + sum (x^2 - 10 cos 2 pi x)        = sum (x^2 + 20 sin^2(pi x))
+//   Ackley     -20 e^{-0.2 r} - e^{c} + 20 + e          = -20 expm1(-0.2 r) - e expm1(c - 1),
+//              c - 1 = (1/d) sum (cos 2 pi x - 1)       = -(2/d) sum sin^2(pi x)
+// sin(pi x) uses sinpif (exact argument reduction).  Where fp32 cannot deliver the 1e-5 bar on f, the critical
+// sub-expression runs in fp64 (B200 issues DFMA at half the FFMA rate): Schwefel's x sin(sqrt|x|) near x = 421
+// (418.98 - 418.98 at the optimum), Michalewicz's angle i x^2 / pi (up to 200 rad under a 20th power), Trid's
+// O(d^4) products that cancel to O(d^3), Styblinski-Tang's mixed-sign polynomial terms, and Bukin's ridge distance y - 0.01 x^2 under a square root.
+template <int DP>
+__device__ __forceinline__ float appd_point(int id, int d, const float4 *pts, int col) {
+  float x[DP];
+#pragma unroll
+  for (int c4 = 0; c4 < DP / 4; ++c4) {
+    const float4 v = ld_pt(pts, c4, col);
+    x[4 * c4] = v.x; x[4 * c4 + 1] = v.y; x[4 * c4 + 2] = v.z; x[4 * c4 + 3] = v.w;
+  }
+  switch (id) {
+    case CHISAO_OBJ_RASTRIGIN: {
+      float acc = 0.0f;
+#pragma unroll
+      for (int j = 0; j < DP; ++j)
+        if (j < d) { const float sp = sinpif(x[j]); acc = fmaf(x[j], x[j], acc); acc = fmaf(20.0f * sp, sp, acc); }
+      return -acc;
+    }
+    case CHISAO_OBJ_ACKLEY: {
+      float s2 = 0.0f, ss = 0.0f;
+#pragma unroll
+      for (int j = 0; j < DP; ++j)
+        if (j < d) { const float sp = sinpif(x[j]); s2 = fmaf(x[j], x[j], s2); ss = fmaf(sp, sp, ss); }
+      const float inv_d = 1.0f / (float)d;
+      return 20.0f * expm1f(-0.2f * sqrtf(s2 * inv_d)) + 2.7182818284590452f * expm1f(-2.0f * ss * inv_d);
+    }
+    case CHISAO_OBJ_SCHWEFEL: {
+      // rolled loop straight from shared memory (the fp64 sine dominates); sin(a) = sinpi(a / pi), a <= 22.4
+      const float *pf = reinterpret_cast<const float *>(pts + col);
+      double acc = 0.0;
+#pragma unroll 2
+      for (int j = 0; j < d; ++j) {
+        const double t = (double)pf[(j >> 2) * (PTILE * 4) + (j & 3)];
+        acc += 418.9829 - t * sinpi(sqrt(fabs(t)) * 0.3183098861837907);
+      }
+      return (float)(-acc);
+    }
+    case CHISAO_OBJ_STYBLINSKI_TANG: {
+      double acc = 0.0;   // terms of either sign up to 80 cancel across coordinates: three DFMA per coordinate
+#pragma unroll
+      for (int j = 0; j < DP; ++j)
+        if (j < d) { const double t = (double)x[j], t2 = t * t; acc += fma(t2, t2 - 16.0, 5.0 * t); }
+      return (float)(-0.5 * acc);
+    }
+    case CHISAO_OBJ_MICHALEWICZ: {
+      float acc = 0.0f;
+#pragma unroll
+      for (int j = 0; j < DP; ++j)
+        if (j < d) {
+          const double t = (double)x[j];
+          const double turns = (double)(j + 1) * t * t * 0.10132118364233778;   // angle / pi = i x^2 / pi^2
+          const float fr = (float)(turns - 2.0 * rint(0.5 * turns));            // angle / pi reduced to [-1, 1]
+          const float sa = sinpif(fr), s2 = sa * sa, s4 = s2 * s2, s8 = s4 * s4, s16 = s8 * s8;
+          acc = fmaf(sinpif(x[j] * 0.31830988618f), s16 * s4, acc);   // sin(x), x in [0, pi]: no slow-path reduction
+        }
+      return acc;
+    }
+    case CHISAO_OBJ_TRID: {
+      double acc = 0.0, prev = 0.0;
+#pragma unroll
+      for (int j = 0; j < DP; ++j)
+        if (j < d) { const double t = (double)x[j]; acc = fma(t - 1.0, t - 1.0, acc); acc = fma(-t, prev, acc); prev = t; }
+      return (float)(-acc);
+    }
+    default: {  // CHISAO_OBJ_BUKIN6 (d = 2)
+      const double u = (double)x[1] - 0.01 * (double)x[0] * (double)x[0];
+      return -(100.0f * sqrtf((float)fabs(u)) + 0.01f * fabsf(x[0] + 10.0f));
+    }
+  }
+}
+
 // Evaluate the thread's PPT staged points.  Must be called by every thread of the CTA (contains barriers);
 // the points must already be visible in shared memory (caller syncs).  `use` counts bulk copies issued on
 // each mbarrier so far (phase tracking when a kernel evaluates more than one tile).
 template <int OBJ, int DP>
 __device__ __forceinline__ void eval_tile(const DevObj &o, const EvalSmem &sm, int t, uint32_t &use, float (&fout)[PPT]) {
+  if constexpr (OBJ == CHISAO_OBJ_APPD) {   // parameter-free: nothing to stream
+#pragma unroll 1
+    for (int pp = 0; pp < PPT; ++pp) fout[pp] = appd_point<DP>(o.id, o.d, sm.pts, pp * NT + t);
+  } else {
   float m[PPT], s[PPT];
 #pragma unroll
   for (int pp = 0; pp < PPT; ++pp) { m[pp] = -INFINITY; s[pp] = 0.0f; }
@@ -264,6 +347,7 @@ __device__ __forceinline__ void eval_tile(const DevObj &o, const EvalSmem &sm, i
     } else {
       fout[pp] = m[pp] + logf(s[pp]);
     }
+  }
   }
 }
 

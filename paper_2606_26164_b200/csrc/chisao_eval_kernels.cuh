@@ -335,6 +335,6 @@ cudaError_t launch_hlc_obj(const DevObj &o, const HlcArgs &a, int grid, cudaStre
   cudaError_t launch_pt_obj_##ID(const DevObj &, const PtArgs &, int, cudaStream_t);                \
   cudaError_t launch_hlc_obj_##ID(const DevObj &, const HlcArgs &, int, cudaStream_t);              \
   cudaError_t configure_obj_##ID();
-CHISAO_DECL_OBJ(0) CHISAO_DECL_OBJ(1) CHISAO_DECL_OBJ(2) CHISAO_DECL_OBJ(3) CHISAO_DECL_OBJ(4)
+CHISAO_DECL_OBJ(0) CHISAO_DECL_OBJ(1) CHISAO_DECL_OBJ(2) CHISAO_DECL_OBJ(3) CHISAO_DECL_OBJ(4) CHISAO_DECL_OBJ(5)
 
 }  // namespace chisao

@@ -1,5 +1,5 @@
 // chisao_eval_obj.cu -- instantiates the evaluation kernels for ONE objective id
-// (compiled five times with -DCHISAO_OBJ_INST=0..4 so the translation units build in parallel).
+// (compiled six times with -DCHISAO_OBJ_INST=0..5; 5 = the Appendix-D family so the translation units build in parallel).
 #include "chisao_eval_kernels.cuh"
 
 #ifndef CHISAO_OBJ_INST

@@ -83,3 +83,53 @@ def test_bukin6_printed_optimum_and_ridge(orc):
     assert abs(o.values(np.array([-10.0, 2.0]))[0] + 100.0) < 1e-12     # off the ridge by 1: -100 sqrt(1)
     with pytest.raises(ValueError):
         orc.Oracle(type(inputs.appendix_d("bukin6", 2, 4))("b", inputs.Objective(11, 3, 1, np.zeros((1, 3), np.float32), np.zeros(1, np.float32), np.zeros(1, np.float32)), inputs.Hyper(3, 4, np.zeros(3, np.float32), np.ones(3, np.float32)), np.zeros((4, 3), np.float32)))
+
+
+# ---- whole-cycle pins: the mode sets of these functions are known in closed form ---------------------------------
+RUNS = {
+    "rastrigin": dict(d=2, N=512, n_osc=4, n_conv=25, fd_h=1e-3, eps_grad=5e-3, eps_dup=0.1, log_delta=-200.0, sigma_s=0.5),
+    "trid": dict(d=6, N=256, n_osc=2, n_conv=60, fd_h=1e-2, eps_grad=1e-2, eps_dup=0.2, log_delta=-1e9, sigma_s=3.0),
+    "styblinski_tang": dict(d=4, N=512, n_osc=3, n_conv=30, fd_h=1e-3, eps_grad=5e-3, eps_dup=0.1, log_delta=-1e9, sigma_s=0.5),
+    "schwefel": dict(d=2, N=512, n_osc=3, n_conv=30, fd_h=1e-2, eps_grad=1e-3, eps_dup=1.0, log_delta=-1e9, sigma_s=20.0),
+}
+
+
+def _run(orc, name):
+    kw = dict(RUNS[name])
+    wl = inputs.appendix_d(name, kw.pop("d"), kw.pop("N"), **kw)
+    o = orc.Oracle(wl, threads=8)
+    for _ in range(wl.hp.n_osc):
+        o.step()
+    return wl, o.modes()
+
+
+def test_cycle_finds_all_121_rastrigin_maxima_in_2d(orc):
+    """every local maximum of the 2-d Rastrigin function on [-5.12, 5.12]^2 sits next to a lattice point of
+    {-5..5}^2 ("regular grid of local maxima"); the best one is the printed f(0) = 0"""
+    _, (x, f, _) = _run(orc, "rastrigin")
+    assert len(f) == 121 and abs(f[0]) < 1e-6 and np.max(np.abs(x[0])) < 1e-4
+    cells = {tuple(np.rint(r).astype(int)) for r in x}
+    assert len(cells) == 121 and np.max(np.abs(x - np.rint(x))) < 0.03
+
+
+def test_cycle_collapses_trid_to_the_printed_optimum(orc):
+    """Trid is unimodal: one mode at theta*_i = i (d + 1 - i), f* = d (d + 4)(d - 1)/6 = 50 at d = 6"""
+    _, (x, f, _) = _run(orc, "trid")
+    i = np.arange(1, 7)
+    assert len(f) == 1 and abs(f[0] - 50.0) < 1e-6 and np.max(np.abs(x[0] - i * (7 - i))) < 1e-3
+
+
+def test_cycle_finds_the_2_pow_d_styblinski_tang_maxima(orc):
+    """separable with two maxima per coordinate (roots of 4 t^3 - 32 t + 5 with negative curvature of -f): 2^d modes"""
+    _, (x, f, _) = _run(orc, "styblinski_tang")
+    r = np.roots([4.0, 0.0, -32.0, 5.0]).real
+    tops = np.sort(r)[[0, 2]]                                            # -2.9035 and 2.7468
+    assert len(f) == 16
+    assert np.max(np.min(np.abs(x[:, :, None] - tops[None, None, :]), axis=2)) < 1e-3
+    assert abs(f[0] - 4 * 39.16616570377142) < 1e-5
+
+
+def test_cycle_finds_the_schwefel_global_maximum(orc):
+    _, (x, f, _) = _run(orc, "schwefel")
+    assert abs(f[0]) < 1e-3 and np.max(np.abs(x[0] - 420.9687)) < 1e-2  # PAPER.md:619 "near theta_i = 420.97"
+    assert len(f) > 20
