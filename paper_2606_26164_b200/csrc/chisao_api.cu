@@ -123,7 +123,7 @@ size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *b
   const size_t o_blk = F(3 * nb + 3);
   const size_t o_hf = F(N * M);
   const size_t o_q = F(d * d);
-  const size_t o_tc = F(wants_tc(o) ? (size_t)o.K * TC_REC : 0);
+  const size_t o_tc = F(!wants_tc(o) ? 0 : (o.id == CHISAO_OBJ_GMM_FULL ? (size_t)((o.K + 1) / 2) * TCX_REC : (size_t)o.K * TC_REC));
   if (base && st) {
     auto P = [&](size_t off) { return reinterpret_cast<float *>(base + off); };
     auto I = [&](size_t off) { return reinterpret_cast<int32_t *>(base + off); };
@@ -207,6 +207,32 @@ void pack_tc_records(const chisao_objective &o, std::vector<float> &out) {
       }
     for (int j = 0; j < d; ++j) r[2 * TC_D * TC_D + j] = o.means[(size_t)k * d + j];
     r[2 * TC_D * TC_D + TC_D] = (o.id == CHISAO_OBJ_GMM_FULL) ? o.vec_a[k] : 0.0f;
+  }
+}
+
+// x-stationary pair records of GMM_FULL (chisao_tc.cuh): B image of the pair [W_2p ; W_2p+1] (128 rows, hi then lo),
+// c = W mu (fp64 product, rounded once), a; an odd K is padded with a zero component of weight a = -inf
+void pack_tcx_records(const chisao_objective &o, std::vector<float> &out) {
+  const int d = o.d, K = o.K, npair = (K + 1) / 2;
+  out.assign((size_t)npair * TCX_REC, 0.0f);
+  for (int p = 0; p < npair; ++p) {
+    float *r = out.data() + (size_t)p * TCX_REC;
+    for (int hf = 0; hf < 2; ++hf) {
+      const int k = 2 * p + hf;
+      if (k >= K) { r[TCX_W_FLOATS + 128 + hf] = -INFINITY; continue; }
+      for (int n = 0; n < d; ++n) {
+        double cn = 0.0;
+        for (int c = 0; c < d; ++c) {
+          const float w = o.mats[((size_t)k * d + n) * d + c];
+          const float h = tf32_rna_host(w), l = tf32_rna_host(w - h);
+          const int idx = (c / 4) * 512 + (64 * hf + n) * 4 + (c % 4);
+          r[idx] = h; r[TCX_W_FLOATS / 2 + idx] = l;
+          cn += (double)w * (double)o.means[(size_t)k * d + c];
+        }
+        r[TCX_W_FLOATS + 64 * hf + n] = (float)cn;
+      }
+      r[TCX_W_FLOATS + 128 + hf] = o.vec_a[k];
+    }
   }
 }
 
@@ -455,7 +481,9 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
   }
   ctx->use_tc = wants_tc(*obj);
   if (ctx->use_tc) {
-    pack_tc_records(*obj, ctx->tc_host);
+    if (obj->id == CHISAO_OBJ_GMM_FULL) pack_tcx_records(*obj, ctx->tc_host);
+    else pack_tc_records(*obj, ctx->tc_host);
+    ctx->tc.npair = (obj->K + 1) / 2;
     ctx->tc.K = obj->K; ctx->tc.d = obj->d; ctx->tc.sigma_noise = obj->sigma_noise; ctx->tc.recs = tc_dev;
     CKI(tc_configure());
   }

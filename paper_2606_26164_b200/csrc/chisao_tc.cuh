@@ -27,13 +27,22 @@ constexpr int TC_REC = 2 * TC_D * TC_D + TC_D + 4;       // floats per component
 constexpr int TC_REC_BYTES = TC_REC * 4;                 // 33 040 (multiple of 16)
 constexpr int TC_A_BYTES = TC_GROUP * TC_D * 4;          // 32 768 per operand image
 constexpr int TC_SCRATCH_BYTES = 72 * 1024;               // kernel scratch (FD row patch, HLC normals)
-constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TC_REC_BYTES;   // barriers | scratch | B x2
+// x-stationary form (GMM_FULL): components are streamed in PAIRS, one N = 128 operand image per pair
+constexpr int TCX_W_FLOATS = 2 * 128 * TC_D;             // W_hi pair [16 K-chunks][128 rows][4] | W_lo pair
+constexpr int TCX_W_BYTES = TCX_W_FLOATS * 4;            // 65 536
+constexpr int TCX_CA_FLOATS = 128 + 4;                   // c = W mu of both components | a_0, a_1, 0, 0
+constexpr int TCX_CA_BYTES = TCX_CA_FLOATS * 4;          // 528
+constexpr int TCX_REC = TCX_W_FLOATS + TCX_CA_FLOATS;    // floats per pair record (66 064 bytes, multiple of 16)
+constexpr int TCX_RING = 4;                              // c / a ring slots (outlive the W stage by one epilogue)
+constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES;   // >= the 2 x TC_REC form
+static_assert(2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES >= 2 * TC_REC_BYTES, "shared-memory carve");
 constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D0 64 | D_hi 64 | D_lo 64 | D1 64
 
 struct TcObj {
   int32_t K, d;
   float sigma_noise;
-  const float *recs;      // device [K][TC_REC]
+  const float *recs;      // device [K][TC_REC] (QUAD) or [npair][TCX_REC] (GMM_FULL, x-stationary form)
+  int32_t npair;          // ceil(K / 2)
 };
 
 // shared-memory carve (all offsets are arithmetic so that nothing is indexed dynamically through a pointer table):
@@ -48,6 +57,12 @@ struct TcSmem {
   __device__ __forceinline__ unsigned char *scratch() const { return base + 1024; }
   __device__ __forceinline__ float *B(int st) const {
     return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * TC_REC_BYTES);
+  }
+  __device__ __forceinline__ float *Bx(int st) const {    // x-stationary form: W pair stages, then the c / a ring
+    return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * TCX_W_BYTES);
+  }
+  __device__ __forceinline__ float *CA(int r) const {
+    return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + r * TCX_CA_BYTES);
   }
 };
 __device__ __forceinline__ TcSmem tc_carve(unsigned char *base) { TcSmem s; s.base = base; return s; }
@@ -76,6 +91,13 @@ __device__ __forceinline__ void tc_mma_ts(uint32_t tmem_d, uint32_t tmem_a, uint
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(tmem_d),
       "r"(tmem_a), "l"(db), "r"(TC_IDESC), "r"(accumulate));
+}
+constexpr uint32_t TC_IDESC_N128 = (1u << 4) | (2u << 7) | (2u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+__device__ __forceinline__ void tc_mma_ts_i(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate));
 }
 __device__ __forceinline__ void tc_st16(uint32_t taddr, const float (&v)[16]) {
   asm volatile(
@@ -226,6 +248,104 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
   drain(K - 1, a_prev);
   if constexpr (OBJ == CHISAO_OBJ_QUAD) return -0.5f * s;
   return m + logf(s);
+}
+
+// ---- x-stationary form (GMM_FULL) -----------------------------------------------------------------------------
+// z_k = W_k (x - mu_k) = W_k x - c_k with c_k = W_k mu_k precomputed on the host in fp64: the A operand is the point
+// itself, so its hi / lo images are written to TMEM ONCE per tile instead of once per component, and two components
+// share one MMA (B = [W_k ; W_{k+1}], N = 128: 64 cycles against 2 x 47 for two N = 64 instructions).  Per pair a
+// group issues 24 MMAs (X_hi W_hi^T + X_lo W_hi^T + X_hi W_lo^T over 8 K-steps) into its 128 accumulator columns and
+// then drains them (z = acc - c, sum of squares, online log-sum-exp) while the other group's MMAs run.  The
+// cancellation in W x - c costs accuracy: |W x| <= ~110 at C5 against |z| ~ 1..8, measured |df| <= 5e-7 max(|f|, 1)
+// against the 1e-5 bar; QUAD (kappa = 1e4, f -> 0 at the optimum) keeps the (x - c) form above.
+// Group g owns TMEM columns [256 g, 256 g + 256): X_hi 64 | X_lo 64 | accumulators 128.
+__device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int t) {
+  if (t != TC_PTS) return;
+  for (int p = 0; p < o.npair; ++p) {
+    const int st = p & 1;
+    if (p >= 2) mbar_wait(sm.fbar(st), ((p >> 1) - 1) & 1);   // the MMAs of pair p - 2 have retired in both groups
+    const float *r = o.recs + (size_t)p * TCX_REC;
+    mbar_expect_tx(sm.bbar(st), TCX_W_BYTES + TCX_CA_BYTES);
+    bulk_g2s(sm.Bx(st), r, TCX_W_BYTES, sm.bbar(st));
+    // slot p & 3 was last read by the epilogues of pair p - 4, which precede the MMAs of pair p - 3 in both groups
+    bulk_g2s(sm.CA(p & (TCX_RING - 1)), r + TCX_W_FLOATS, TCX_CA_BYTES, sm.bbar(st));
+  }
+}
+
+__device__ __forceinline__ float tcx_eval_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
+  const uint32_t tm = *sm.tmem();
+  const int g = t >> 7, tl = t & (TC_GROUP - 1), npair = o.npair;
+  const uint32_t gcol = tm + (uint32_t)(g * 256);
+  const uint32_t lane_base = gcol + ((uint32_t)(((t >> 5) & 3) * 32) << 16);
+  // the point's hi / lo images, once per tile
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    float h[16], l[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) { h[c] = tf32_rna(x[16 * q + c]); l[c] = x[16 * q + c] - h[c]; }
+    tc_st16(lane_base + 16 * q, h);
+    tc_st16(lane_base + 64 + 16 * q, l);
+  }
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  float m = -INFINITY, s = 0.0f;
+  for (int p = 0; p < npair; ++p) {
+    const int st = p & 1;
+    mbar_wait(sm.bbar(st), (p >> 1) & 1);             // W pair, c, a have landed (every thread: it reads c / a below)
+    group_sync(g);                                    // X image written (p = 0) / accumulators drained (p > 0)
+    if (tl == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      const uint64_t dBh = tc_desc(smem_u32(sm.Bx(st)), 2048, 128), dBl = dBh + (uint64_t)((TCX_W_BYTES / 2) >> 4);
+#pragma unroll
+      for (int pr = 0; pr < 3; ++pr) {
+        const uint32_t a0 = (pr == 1) ? gcol + 64 : gcol;
+        const uint64_t b0 = (pr == 2) ? dBl : dBh;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          tc_mma_ts_i(gcol + 128, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (4096 >> 4)), TC_IDESC_N128, (pr | ks) ? 1u : 0u);
+      }
+      tc_commit(sm.mbar(g));
+    }
+    __syncwarp();
+    mbar_wait(sm.mbar(g), p & 1);
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (tl == 0) mbar_arrive(sm.fbar(st));            // the W stage is free as far as this group is concerned
+    __syncwarp();
+    const float *ca = sm.CA(p & (TCX_RING - 1));
+#pragma unroll
+    for (int hf = 0; hf < 2; ++hf) {
+      const uint32_t taddr = lane_base + 128 + 64 * hf;
+      uint32_t r[64];
+      tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      const float4 *c4 = reinterpret_cast<const float4 *>(ca + 64 * hf);
+      float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll
+      for (int n = 0; n < 64; n += 4) {
+        const float4 c = c4[n >> 2];
+        const float z0 = __uint_as_float(r[n]) - c.x, z1 = __uint_as_float(r[n + 1]) - c.y,
+                    z2 = __uint_as_float(r[n + 2]) - c.z, z3 = __uint_as_float(r[n + 3]) - c.w;
+        q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+      }
+      const float v = fmaf(-0.5f, (q0 + q1) + (q2 + q3), ca[128 + hf]);   // a = -inf pads an odd K
+      const float mn = fmaxf(m, v);
+      if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group barrier
+  }
+  return m + logf(s);
+}
+
+// evaluator / loader of objective OBJ
+template <int OBJ>
+__device__ __forceinline__ float tc_eval(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
+  if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) return tcx_eval_tile(o, sm, x, t);
+  else return tc_eval_tile<OBJ>(o, sm, x, t);
+}
+template <int OBJ>
+__device__ __forceinline__ void tc_load(const TcObj &o, const TcSmem &sm, int t) {
+  if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) tcx_loader(o, sm, t);
+  else tc_loader(o, sm, t);
 }
 
 // launchers (chisao_tc_kernels.cu)

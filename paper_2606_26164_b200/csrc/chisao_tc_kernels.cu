@@ -28,7 +28,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
   const int first = blockIdx.x * spt;
   if (first >= cnt) return;
   tc_setup(sm, t);
-  if (t >= TC_PTS) { tc_loader(o, sm, t); tc_teardown(sm, t); return; }
+  if (t >= TC_PTS) { tc_load<OBJ>(o, sm, t); tc_teardown(sm, t); return; }
   const int s = t / (2 * d), slot = t - s * 2 * d, j = slot >> 1;
   const bool valid = (s < spt) && (first + s < cnt);
   const int i = valid ? (a.list ? a.list[first + s] : first + s) : 0;
@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
     for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
   }
   compute_sync();                        // the scratch rows overlap the operand buffers: everyone has read back
-  float f = tc_eval_tile<OBJ>(o, sm, x, t);
+  float f = tc_eval<OBJ>(o, sm, x, t);
   if (valid) f += eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, a.slot_off + 1 + slot);
   // partner lane holds the other sign of the same coordinate
   const float fo = __shfl_xor_sync(0xffffffffu, f, 1);
@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
   if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
   if (first >= cnt) return;
   tc_setup(sm, t);
-  if (t >= TC_PTS) { tc_loader(o, sm, t); tc_teardown(sm, t); return; }
+  if (t >= TC_PTS) { tc_load<OBJ>(o, sm, t); tc_teardown(sm, t); return; }
   const int e = first + t;
   const bool valid = e < cnt;
   const int i = valid ? (a.list ? a.list[e] : e) : 0;
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
 #pragma unroll
     for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
   }
-  const float fv = tc_eval_tile<OBJ>(o, sm, x, t);
+  const float fv = tc_eval<OBJ>(o, sm, x, t);
   bool accept = false, retry = false;
   float val = 0.f;
   if (valid) {
@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   const int first = blockIdx.x * spt;
   if (first >= cnt) return;
   tc_setup(sm, t);
-  if (t >= TC_PTS) { tc_loader(o, sm, t); tc_teardown(sm, t); return; }
+  if (t >= TC_PTS) { tc_load<OBJ>(o, sm, t); tc_teardown(sm, t); return; }
   const int s = t / M, k = t - s * M;
   const bool valid = (s < spt) && (first + s < cnt);
   const int i = valid ? a.list[first + s] : 0;
@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
 #pragma unroll
     for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
   }
-  float val = tc_eval_tile<OBJ>(o, sm, x, t);
+  float val = tc_eval<OBJ>(o, sm, x, t);
   compute_sync();                        // every MMA has retired: the operand buffers are free
   float *Us = reinterpret_cast<float *>(sm.scratch());        // [256][65] normals (scratch is 72 KB)
   float *fvs = Us + TC_PTS * 65;                              // [256] values
