@@ -21,7 +21,7 @@ namespace chisao {
 
 constexpr int TC_GROUP = 128;                            // threads per group = points per MMA tile = TMEM lanes
 constexpr int TC_PTS = 256;                              // points per CTA tile: two groups ping-pong on the tensor pipe
-constexpr int TC_THREADS = TC_PTS + 32;                  // + one warp that streams the component records
+constexpr int TC_THREADS = TC_PTS + 64;                  // + one warp that streams the records + one that issues MMAs (x-stationary form)
 constexpr int TC_D = 64;
 constexpr int TC_REC = 2 * TC_D * TC_D + TC_D + 4;       // floats per component: W_hi | W_lo | mu | a,0,0,0
 constexpr int TC_REC_BYTES = TC_REC * 4;                 // 33 040 (multiple of 16)
@@ -34,7 +34,8 @@ constexpr int TCX_CA_FLOATS = 128 + 4;                   // c = W mu of both com
 constexpr int TCX_CA_BYTES = TCX_CA_FLOATS * 4;          // 528
 constexpr int TCX_REC = TCX_W_FLOATS + TCX_CA_FLOATS;    // floats per pair record (66 064 bytes, multiple of 16)
 constexpr int TCX_RING = 4;                              // c / a ring slots (outlive the W stage by one epilogue)
-constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES;   // >= the 2 x TC_REC form
+constexpr int TCX_PART_BYTES = 2 * 2 * 2 * TC_GROUP * 8;   // [tile parity][half][group][128] float2
+constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES + TCX_PART_BYTES;   // >= the 2 x TC_REC form
 static_assert(2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES >= 2 * TC_REC_BYTES, "shared-memory carve");
 constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D0 64 | D_hi 64 | D_lo 64 | D1 64
 
@@ -54,6 +55,9 @@ struct TcSmem {
   __device__ __forceinline__ uint64_t *mbar(int g) const { return reinterpret_cast<uint64_t *>(base) + 2 + g; }
   __device__ __forceinline__ uint64_t *fbar(int st) const { return reinterpret_cast<uint64_t *>(base) + 4 + st; }
   __device__ __forceinline__ uint32_t *tmem() const { return reinterpret_cast<uint32_t *>(base + 64); }
+  __device__ __forceinline__ uint64_t *dbar(int g) const { return reinterpret_cast<uint64_t *>(base) + 10 + g; }   // accumulators drained
+  __device__ __forceinline__ uint64_t *cbar(int r) const { return reinterpret_cast<uint64_t *>(base) + 12 + r; }   // c / a ring slot landed
+  __device__ __forceinline__ uint64_t *xbar(int g) const { return reinterpret_cast<uint64_t *>(base) + 16 + g; }   // X image of the tile written
   __device__ __forceinline__ unsigned char *scratch() const { return base + 1024; }
   __device__ __forceinline__ float *B(int st) const {
     return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * TC_REC_BYTES);
@@ -63,6 +67,9 @@ struct TcSmem {
   }
   __device__ __forceinline__ float *CA(int r) const {
     return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + r * TCX_CA_BYTES);
+  }
+  __device__ __forceinline__ float2 *part() const {       // [2 halves][2 groups][128] partial log-sum-exp states
+    return reinterpret_cast<float2 *>(base + 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES);
   }
 };
 __device__ __forceinline__ TcSmem tc_carve(unsigned char *base) { TcSmem s; s.base = base; return s; }
@@ -127,14 +134,16 @@ __device__ __forceinline__ void group_sync(int g) {   // named barrier of the 12
 }
 
 // one-time CTA setup / teardown (all TC_THREADS threads)
-__device__ __forceinline__ void tc_setup(const TcSmem &sm, int t) {
+__device__ __forceinline__ void tc_setup(const TcSmem &sm, int t, int fbar_count) {
   if (t < 32) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(sm.tmem())), "n"(TC_TMEM_COLS));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (t == 32) {
     mbar_init(sm.bbar(0), 1); mbar_init(sm.bbar(1), 1); mbar_init(sm.mbar(0), 1); mbar_init(sm.mbar(1), 1);
-    mbar_init(sm.fbar(0), 2); mbar_init(sm.fbar(1), 2);
+    mbar_init(sm.fbar(0), fbar_count); mbar_init(sm.fbar(1), fbar_count);
+    mbar_init(sm.dbar(0), 8); mbar_init(sm.dbar(1), 8); mbar_init(sm.xbar(0), 4); mbar_init(sm.xbar(1), 4);
+    mbar_init(sm.cbar(0), 1); mbar_init(sm.cbar(1), 1); mbar_init(sm.cbar(2), 1); mbar_init(sm.cbar(3), 1);
     mbar_fence_init();
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
@@ -253,100 +262,189 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
 // ---- x-stationary form (GMM_FULL) -----------------------------------------------------------------------------
 // z_k = W_k (x - mu_k) = W_k x - c_k with c_k = W_k mu_k precomputed on the host in fp64: the A operand is the point
 // itself, so its hi / lo images are written to TMEM ONCE per tile instead of once per component, and two components
-// share one MMA (B = [W_k ; W_{k+1}], N = 128: 64 cycles against 2 x 47 for two N = 64 instructions).  Per pair a
-// group issues 24 MMAs (X_hi W_hi^T + X_lo W_hi^T + X_hi W_lo^T over 8 K-steps) into its 128 accumulator columns and
-// then drains them (z = acc - c, sum of squares, online log-sum-exp) while the other group's MMAs run.  The
-// cancellation in W x - c costs accuracy: |W x| <= ~110 at C5 against |z| ~ 1..8, measured |df| <= 5e-7 max(|f|, 1)
+// share one MMA (B = [W_k ; W_{k+1}], N = 128: 64 cycles against 2 x 47 for two N = 64 instructions).  Per pair and
+// group, 24 MMAs (X_hi W_hi^T + X_lo W_hi^T + X_hi W_lo^T over 8 K-steps) fill the group's 128 accumulator columns.
+// The cancellation in W x - c costs accuracy: |W x| <= ~110 at C5 against |z| ~ 1..8, measured |df| <= 5e-7 max(|f|, 1)
 // against the 1e-5 bar; QUAD (kappa = 1e4, f -> 0 at the optimum) keeps the (x - c) form above.
 // Group g owns TMEM columns [256 g, 256 g + 256): X_hi 64 | X_lo 64 | accumulators 128.
-__device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int t) {
-  if (t != TC_PTS) return;
-  for (int p = 0; p < o.npair; ++p) {
-    const int st = p & 1;
-    if (p >= 2) mbar_wait(sm.fbar(st), ((p >> 1) - 1) & 1);   // the MMAs of pair p - 2 have retired in both groups
+//
+// Roles: warp 8 streams the pair records (W stage ring of 2, c / a ring of 4); warp 9 issues the MMAs (it waits for
+// "W landed", "X image written" and "accumulators of group g drained", issues, and lets tcgen05.commit signal "MMAs of
+// group g retired" and "W stage free"); the 8 compute warps drain BOTH groups' accumulators together -- warp w reads
+// TMEM lanes 32 (w & 3) .. + 31 and the columns of component w >> 2 of the pair -- and hand the accumulators back as
+// soon as the tcgen05.ld has completed, so the tensor pipe only ever waits for one TMEM read, not for the arithmetic.
+// Each thread keeps one online log-sum-exp state per group over "its" components; the two halves of a point meet
+// through shared memory at the end of the tile.
+// The CTA is persistent: it walks tiles blockIdx.x, blockIdx.x + gridDim.x, ...; the record stream simply wraps
+// around, the next tile's points are fetched during the last pair of the current one and written over the X image
+// as soon as that group's last MMAs have retired, and the per-tile epilogue (noise, gradient / line-search / HLC
+// bookkeeping) runs while the tensor pipe is already busy with the next tile.  All mbarrier phases count the
+// CTA-global pair index G = tile_iteration * npair + p.
+__device__ __forceinline__ int tcx_tiles_of_cta(int ntiles) {
+  return ((int)blockIdx.x < ntiles) ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+}
+
+__device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int ntc) {
+  const int total = ntc * o.npair;
+  for (int G = 0, p = 0; G < total; ++G) {
+    const int st = G & 1, rs = G & (TCX_RING - 1);
+    if (G >= 2) mbar_wait(sm.fbar(st), ((G >> 1) - 1) & 1);   // the MMAs of pair G - 2 have retired in both groups
     const float *r = o.recs + (size_t)p * TCX_REC;
-    mbar_expect_tx(sm.bbar(st), TCX_W_BYTES + TCX_CA_BYTES);
+    mbar_expect_tx(sm.bbar(st), TCX_W_BYTES);
     bulk_g2s(sm.Bx(st), r, TCX_W_BYTES, sm.bbar(st));
-    // slot p & 3 was last read by the epilogues of pair p - 4, which precede the MMAs of pair p - 3 in both groups
-    bulk_g2s(sm.CA(p & (TCX_RING - 1)), r + TCX_W_FLOATS, TCX_CA_BYTES, sm.bbar(st));
+    // ring slot rs was last read by the drains of pair G - 4; they precede the MMAs of pair G - 3, whose retirement
+    // the wait above (pair G - 2) implies
+    mbar_expect_tx(sm.cbar(rs), TCX_CA_BYTES);
+    bulk_g2s(sm.CA(rs), r + TCX_W_FLOATS, TCX_CA_BYTES, sm.cbar(rs));
+    if (++p == o.npair) p = 0;
   }
 }
 
-__device__ __forceinline__ float tcx_eval_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
+// one lane of a converged warp (elect.sync): the single-thread tcgen05 instructions are issued under this predicate so
+// that the compiler emits them straight-line (issued from a thread-divergent branch, every UTCHMMA is wrapped in an
+// election loop of ~9 instructions and the issuing thread, not the tensor pipe, sets the pace)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
+// all 32 lanes of warp 9 run the loop (warp-uniform control flow); one elected lane issues
+__device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int ntc) {
   const uint32_t tm = *sm.tmem();
-  const int g = t >> 7, tl = t & (TC_GROUP - 1), npair = o.npair;
-  const uint32_t gcol = tm + (uint32_t)(g * 256);
-  const uint32_t lane_base = gcol + ((uint32_t)(((t >> 5) & 3) * 32) << 16);
-  // the point's hi / lo images, once per tile
-#pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    float h[16], l[16];
-#pragma unroll
-    for (int c = 0; c < 16; ++c) { h[c] = tf32_rna(x[16 * q + c]); l[c] = x[16 * q + c] - h[c]; }
-    tc_st16(lane_base + 16 * q, h);
-    tc_st16(lane_base + 64 + 16 * q, l);
-  }
-  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-  asm volatile("tcgen05.fence::before_thread_sync;");
-  float m = -INFINITY, s = 0.0f;
-  for (int p = 0; p < npair; ++p) {
-    const int st = p & 1;
-    mbar_wait(sm.bbar(st), (p >> 1) & 1);             // W pair, c, a have landed (every thread: it reads c / a below)
-    group_sync(g);                                    // X image written (p = 0) / accumulators drained (p > 0)
-    if (tl == 0) {
-      asm volatile("tcgen05.fence::after_thread_sync;");
+  int G = 0;
+  for (int it = 0; it < ntc; ++it)
+    for (int p = 0; p < o.npair; ++p, ++G) {
+      const int st = G & 1;
+      mbar_wait(sm.bbar(st), (G >> 1) & 1);
       const uint64_t dBh = tc_desc(smem_u32(sm.Bx(st)), 2048, 128), dBl = dBh + (uint64_t)((TCX_W_BYTES / 2) >> 4);
+#pragma unroll 1
+      for (int g = 0; g < 2; ++g) {
+        if (p == 0) mbar_wait(sm.xbar(g), it & 1);              // this tile's X image is in TMEM
+        if (G > 0) mbar_wait(sm.dbar(g), (G - 1) & 1);          // pair G - 1 drained
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        const uint32_t gcol = tm + (uint32_t)(g * 256);
+        if (elect_one()) {
 #pragma unroll
-      for (int pr = 0; pr < 3; ++pr) {
-        const uint32_t a0 = (pr == 1) ? gcol + 64 : gcol;
-        const uint64_t b0 = (pr == 2) ? dBl : dBh;
+          for (int pr = 0; pr < 3; ++pr) {
+            const uint32_t a0 = (pr == 1) ? gcol + 64 : gcol;
+            const uint64_t b0 = (pr == 2) ? dBl : dBh;
 #pragma unroll
-        for (int ks = 0; ks < 8; ++ks)
-          tc_mma_ts_i(gcol + 128, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (4096 >> 4)), TC_IDESC_N128, (pr | ks) ? 1u : 0u);
+            for (int ks = 0; ks < 8; ++ks)
+              tc_mma_ts_i(gcol + 128, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (4096 >> 4)), TC_IDESC_N128, (pr | ks) ? 1u : 0u);
+          }
+          tc_commit(sm.mbar(g));
+          if (g == 1) tc_commit(sm.fbar(st));         // both groups' MMAs of this pair retired: the W stage is free
+        }
+        __syncwarp();
       }
-      tc_commit(sm.mbar(g));
     }
-    __syncwarp();
-    mbar_wait(sm.mbar(g), p & 1);
-    asm volatile("tcgen05.fence::after_thread_sync;");
-    if (tl == 0) mbar_arrive(sm.fbar(st));            // the W stage is free as far as this group is concerned
-    __syncwarp();
-    const float *ca = sm.CA(p & (TCX_RING - 1));
-#pragma unroll
-    for (int hf = 0; hf < 2; ++hf) {
-      const uint32_t taddr = lane_base + 128 + 64 * hf;
-      uint32_t r[64];
-      tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
-      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-      const float4 *c4 = reinterpret_cast<const float4 *>(ca + 64 * hf);
-      float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
-#pragma unroll
-      for (int n = 0; n < 64; n += 4) {
-        const float4 c = c4[n >> 2];
-        const float z0 = __uint_as_float(r[n]) - c.x, z1 = __uint_as_float(r[n + 1]) - c.y,
-                    z2 = __uint_as_float(r[n + 2]) - c.z, z3 = __uint_as_float(r[n + 3]) - c.w;
-        q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
-      }
-      const float v = fmaf(-0.5f, (q0 + q1) + (q2 + q3), ca[128 + hf]);   // a = -inf pads an odd K
-      const float mn = fmaxf(m, v);
-      if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group barrier
-  }
-  return m + logf(s);
 }
 
-// evaluator / loader of objective OBJ
-template <int OBJ>
-__device__ __forceinline__ float tc_eval(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
-  if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) return tcx_eval_tile(o, sm, x, t);
-  else return tc_eval_tile<OBJ>(o, sm, x, t);
+// Compute threads (t < TC_PTS).  load(tile, x) fills the thread's point of that tile (thread t = point t & 127 of
+// group t >> 7; coordinates >= d zero) and returns a small per-tile context; finish(tile, f, ctx) consumes the value.
+// Both are called by all 256 compute threads, in tile order; load(tile + 1) runs before finish(tile).
+template <class Load, class Finish>
+__device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, int t, int ntc, Load load, Finish finish) {
+  const uint32_t tm = *sm.tmem();
+  const int npair = o.npair, w = t >> 5, lane = t & 31, wq = w & 3, hf = w >> 2, own = t >> 7;
+  const uint32_t lanes = tm + ((uint32_t)(wq * 32) << 16);
+  const uint32_t xaddr = lanes + (uint32_t)(own * 256), rd = lanes + (uint32_t)(128 + 64 * hf);
+  auto write_x = [&](const float (&xv)[TC_D]) {        // hi / lo images of the thread's point -> its TMEM lane
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      float h[16], l[16];
+#pragma unroll
+      for (int c = 0; c < 16; ++c) { h[c] = tf32_rna(xv[16 * q + c]); l[c] = xv[16 * q + c] - h[c]; }
+      tc_st16(xaddr + 16 * q, h);
+      tc_st16(xaddr + 64 + 16 * q, l);
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(sm.xbar(own));
+  };
+  float xn[TC_D];
+  auto cn = load((int)blockIdx.x, xn);
+  write_x(xn);
+  int G = 0;
+  for (int it = 0; it < ntc; ++it) {
+    const int tile = (int)blockIdx.x + it * (int)gridDim.x;
+    const bool more = it + 1 < ntc;
+    const auto cc = cn;
+    float m0 = -INFINITY, s0 = 0.0f, m1 = -INFINITY, s1 = 0.0f;
+    for (int p = 0; p < npair; ++p, ++G) {
+      const bool swap = more && (p == npair - 1);
+      if (swap) cn = load(tile + (int)gridDim.x, xn);  // global loads in flight under the waits below
+      const int rs = G & (TCX_RING - 1);
+      mbar_wait(sm.cbar(rs), (G >> 2) & 1);           // c, a of this pair have landed
+      const float *ca = sm.CA(rs);
+      const float4 *c4 = reinterpret_cast<const float4 *>(ca + 64 * hf);
+      const float a_k = ca[128 + hf];                 // a = -inf pads an odd K
+#pragma unroll
+      for (int g = 0; g < 2; ++g) {
+        mbar_wait(sm.mbar(g), G & 1);
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        uint32_t r[64];
+        const uint32_t taddr = rd + (uint32_t)(g * 256);
+        tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.dbar(g));       // accumulators are in registers: the next MMAs may overwrite them
+        if (swap && g == own) write_x(xn);            // this group's last MMAs of the tile have retired
+        float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll
+        for (int n = 0; n < 64; n += 4) {
+          const float4 c = c4[n >> 2];
+          const float z0 = __uint_as_float(r[n]) - c.x, z1 = __uint_as_float(r[n + 1]) - c.y,
+                      z2 = __uint_as_float(r[n + 2]) - c.z, z3 = __uint_as_float(r[n + 3]) - c.w;
+          q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+        }
+        const float v = fmaf(-0.5f, (q0 + q1) + (q2 + q3), a_k);
+        if (g == 0) {
+          const float mn = fmaxf(m0, v);
+          if (mn > -INFINITY) { s0 = s0 * __expf(m0 - mn) + __expf(v - mn); m0 = mn; }
+        } else {
+          const float mn = fmaxf(m1, v);
+          if (mn > -INFINITY) { s1 = s1 * __expf(m1 - mn) + __expf(v - mn); m1 = mn; }
+        }
+      }
+    }
+    // the two component halves of every point meet: part[tile parity][hf][g][point] = (m, s); the barrier of the
+    // next tile separates this tile's reads from the writes of the tile after it
+    float2 *part = sm.part() + (it & 1) * (4 * TC_GROUP);
+    part[(hf * 2 + 0) * TC_GROUP + wq * 32 + lane] = make_float2(m0, s0);
+    part[(hf * 2 + 1) * TC_GROUP + wq * 32 + lane] = make_float2(m1, s1);
+    asm volatile("bar.sync 3, %0;" ::"n"(TC_PTS) : "memory");
+    const float2 pa = part[(0 * 2 + own) * TC_GROUP + (t & (TC_GROUP - 1))];
+    const float2 pb = part[(1 * 2 + own) * TC_GROUP + (t & (TC_GROUP - 1))];
+    const float mm = fmaxf(pa.x, pb.x);
+    const float f = (mm > -INFINITY) ? mm + logf(pa.y * __expf(pa.x - mm) + pb.y * __expf(pb.x - mm)) : -INFINITY;
+    finish(tile, f, cc);
+  }
+}
+
+// Run the evaluator over `ntiles` tiles of 256 points; called by every thread of the CTA after tc_begin.
+//   GMM_FULL: persistent x-stationary form, any grid <= ntiles;  QUAD: one tile per CTA (grid = ntiles).
+template <int OBJ, class Load, class Finish>
+__device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish) {
+  if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) {
+    const int ntc = tcx_tiles_of_cta(ntiles);
+    const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+    if (warp < TC_PTS / 32) tcx_compute(o, sm, t, ntc, load, finish);
+    else if (warp == TC_PTS / 32) { if (t == TC_PTS) tcx_loader(o, sm, ntc); }
+    else tcx_issuer(o, sm, ntc);
+  } else {
+    if (t >= TC_PTS) { tc_loader(o, sm, t); return; }
+    float x[TC_D];
+    const auto c = load((int)blockIdx.x, x);
+    const float f = tc_eval_tile<OBJ>(o, sm, x, t);
+    finish((int)blockIdx.x, f, c);
+  }
 }
 template <int OBJ>
-__device__ __forceinline__ void tc_load(const TcObj &o, const TcSmem &sm, int t) {
-  if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) tcx_loader(o, sm, t);
-  else tc_loader(o, sm, t);
-}
+__device__ __forceinline__ void tc_begin(const TcSmem &sm, int t) { tc_setup(sm, t, OBJ == CHISAO_OBJ_GMM_FULL ? 1 : 2); }
 
 // launchers (chisao_tc_kernels.cu)
 struct FdArgs; struct PtArgs; struct HlcArgs;

@@ -18,6 +18,7 @@ __device__ __forceinline__ void tc_load_row(const float *row, int d, bool vec, f
 }
 
 // thread t -> (sample t / 2d of the tile, slot t % 2d); slot 2j = x + h e_j, 2j + 1 = x - h e_j
+struct FdCtx { int i; float xj, xp; bool valid; };
 template <int OBJ>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, const FdArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
@@ -25,111 +26,122 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
   const int t = threadIdx.x, d = a.d;
   const int spt = TC_PTS / (2 * d);
   const int cnt = a.count ? *a.count : a.max_count;
-  const int first = blockIdx.x * spt;
-  if (first >= cnt) return;
-  tc_setup(sm, t);
-  if (t >= TC_PTS) { tc_load<OBJ>(o, sm, t); tc_teardown(sm, t); return; }
+  const int ntiles = (cnt + spt - 1) / spt;
+  if ((int)blockIdx.x >= ntiles) return;
+  tc_begin<OBJ>(sm, t);
   const int s = t / (2 * d), slot = t - s * 2 * d, j = slot >> 1;
-  const bool valid = (s < spt) && (first + s < cnt);
-  const int i = valid ? (a.list ? a.list[first + s] : first + s) : 0;
-  float x[TC_D];
-  float xj = 0.f, xp = 0.f;
-  if (valid) {
-    const float *row = a.X + (size_t)i * d;
-    tc_load_row(row, d, (d & 3) == 0, x);
-    xj = row[j];
-    xp = (slot & 1) ? xj - a.h : xj + a.h;
-    // replace coordinate j through a shared-memory round trip of the thread's own row: a dynamically indexed
-    // register array would be lowered to a branch tree over j, and the warp-collective tcgen05 instructions
-    // below need every lane on the same path
-    float *own = reinterpret_cast<float *>(sm.scratch()) + t * 68;
+  auto load = [&](int tile, float (&x)[TC_D]) -> FdCtx {
+    FdCtx c;
+    const int first = tile * spt;
+    c.valid = (s < spt) && (first + s < cnt);
+    c.i = c.valid ? (a.list ? a.list[first + s] : first + s) : 0;
+    c.xj = 0.f; c.xp = 0.f;
+    if (c.valid) {
+      const float *row = a.X + (size_t)c.i * d;
+      tc_load_row(row, d, (d & 3) == 0, x);
+      c.xj = row[j];
+      c.xp = (slot & 1) ? c.xj - a.h : c.xj + a.h;
+      // replace coordinate j through a shared-memory round trip of the thread's own row: a dynamically indexed
+      // register array would be lowered to a branch tree over j, and the warp-collective tcgen05 instructions
+      // of the evaluator need every lane on the same path
+      float *own = reinterpret_cast<float *>(sm.scratch()) + t * 68;
 #pragma unroll
-    for (int c4 = 0; c4 < TC_D / 4; ++c4)
-      *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
-    own[j] = xp;                         // same thread writes and reads its row: program order suffices
+      for (int c4 = 0; c4 < TC_D / 4; ++c4)
+        *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
+      own[j] = c.xp;                       // same thread writes and reads its row: program order suffices
 #pragma unroll
-    for (int c4 = 0; c4 < TC_D / 4; ++c4) {
-      const float4 v = *reinterpret_cast<const float4 *>(own + 4 * c4);
-      x[4 * c4] = v.x; x[4 * c4 + 1] = v.y; x[4 * c4 + 2] = v.z; x[4 * c4 + 3] = v.w;
+      for (int c4 = 0; c4 < TC_D / 4; ++c4) {
+        const float4 v = *reinterpret_cast<const float4 *>(own + 4 * c4);
+        x[4 * c4] = v.x; x[4 * c4 + 1] = v.y; x[4 * c4 + 2] = v.z; x[4 * c4 + 3] = v.w;
+      }
+    } else {
+#pragma unroll
+      for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
     }
-  } else {
-#pragma unroll
-    for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
-  }
-  compute_sync();                        // the scratch rows overlap the operand buffers: everyone has read back
-  float f = tc_eval<OBJ>(o, sm, x, t);
-  if (valid) f += eval_noise(o.sigma_noise, a.seed, a.cycle, i, a.phase, a.iter, a.slot_off + 1 + slot);
-  // partner lane holds the other sign of the same coordinate
-  const float fo = __shfl_xor_sync(0xffffffffu, f, 1);
-  const float xo = __shfl_xor_sync(0xffffffffu, xp, 1);
-  if (valid && !(slot & 1)) {
-    const float g = (f - fo) / ((xp - xj) + (xj - xo));
-    if (a.mode == FD_GRAD) {
-      a.g_out[(size_t)i * d + j] = g;
-    } else {   // Eq. 6
-      const float vo = (a.iter == 1) ? 0.0f : a.v[(size_t)i * d + j];
-      const float vn = fmaf(a.mu, vo, -a.alpha * g);
-      a.v[(size_t)i * d + j] = vn;
-      a.x[(size_t)i * d + j] = clipf(xj + vn, a.lo[j], a.hi[j]);
+    return c;
+  };
+  auto finish = [&](int tile, float f, const FdCtx &c) {
+    if (c.valid) f += eval_noise(o.sigma_noise, a.seed, a.cycle, c.i, a.phase, a.iter, a.slot_off + 1 + slot);
+    // partner lane holds the other sign of the same coordinate
+    const float fo = __shfl_xor_sync(0xffffffffu, f, 1);
+    const float xo = __shfl_xor_sync(0xffffffffu, c.xp, 1);
+    if (c.valid && !(slot & 1)) {
+      const float g = (f - fo) / ((c.xp - c.xj) + (c.xj - xo));
+      if (a.mode == FD_GRAD) {
+        a.g_out[(size_t)c.i * d + j] = g;
+      } else {   // Eq. 6
+        const float vo = (a.iter == 1) ? 0.0f : a.v[(size_t)c.i * d + j];
+        const float vn = fmaf(a.mu, vo, -a.alpha * g);
+        a.v[(size_t)c.i * d + j] = vn;
+        a.x[(size_t)c.i * d + j] = clipf(c.xj + vn, a.lo[j], a.hi[j]);
+      }
     }
-  }
-  if (t == 0) atomicAdd(&a.evals[a.counter], (unsigned long long)min(spt, cnt - first) * 2ull * d);
+    if (t == 0) atomicAdd(&a.evals[a.counter], (unsigned long long)min(spt, cnt - tile * spt) * 2ull * d);
+  };
+  tc_run<OBJ>(o, sm, t, ntiles, load, finish);
   tc_teardown(sm, t);
 }
 
+struct PtCtx { int i; bool valid; };
 template <int OBJ>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o, const PtArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
   const TcSmem sm = tc_carve(tc_smem_raw);
   const int t = threadIdx.x, d = a.d;
   const int cnt = a.count ? *a.count : a.max_count;
-  const int first = blockIdx.x * TC_PTS;
+  const int ntiles = (cnt + TC_PTS - 1) / TC_PTS;
   if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
-  if (first >= cnt) return;
-  tc_setup(sm, t);
-  if (t >= TC_PTS) { tc_load<OBJ>(o, sm, t); tc_teardown(sm, t); return; }
-  const int e = first + t;
-  const bool valid = e < cnt;
-  const int i = valid ? (a.list ? a.list[e] : e) : 0;
-  float x[TC_D];
-  if (valid) tc_load_row(a.X + (size_t)i * d, d, (d & 3) == 0, x);
-  else {
+  if ((int)blockIdx.x >= ntiles) return;
+  tc_begin<OBJ>(sm, t);
+  auto load = [&](int tile, float (&x)[TC_D]) -> PtCtx {
+    PtCtx c;
+    const int e = tile * TC_PTS + t;
+    c.valid = e < cnt;
+    c.i = c.valid ? (a.list ? a.list[e] : e) : 0;
+    if (c.valid) tc_load_row(a.X + (size_t)c.i * d, d, (d & 3) == 0, x);
+    else {
 #pragma unroll
-    for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
-  }
-  const float fv = tc_eval<OBJ>(o, sm, x, t);
-  bool accept = false, retry = false;
-  float val = 0.f;
-  if (valid) {
-    if (a.mode == PT_CENTRE) {
-      a.f[i] = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, 0, 0);
-    } else {
-      val = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + a.b);
-      const float phit = -val, phi = -a.f[i];
-      const float rhs = fmaf(a.c1, a.dec[i], phi);
-      accept = (fabsf(phit) <= 3.0e38f) && (phit <= rhs);
-      retry = !accept && (a.b < a.ls_max);
+      for (int k = 0; k < TC_D; ++k) x[k] = 0.f;
     }
-  }
-  if (a.mode == PT_LS) {
-    const int sa = warp_append(a.fd_cnt, accept);
-    if (accept) { a.fd_list[sa] = i; a.ls_b[i] = a.b; a.ft[i] = val; }
-    const int sr = warp_append(a.next_cnt, retry);
-    if (retry) {
-      a.next_list[sr] = i;
-      const float tn = a.tcur[i] * a.shrink;
-      a.tcur[i] = tn;
-      float dsum = 0.0f;
-      for (int j = 0; j < d; ++j) {
-        const float xo = a.x[(size_t)i * d + j];
-        const float xn = clipf(fmaf(tn, a.p[(size_t)i * d + j], xo), a.lo[j], a.hi[j]);
-        a.xt[(size_t)i * d + j] = xn;
-        dsum = fmaf(-a.g[(size_t)i * d + j], xn - xo, dsum);
+    return c;
+  };
+  auto finish = [&](int tile, float fv, const PtCtx &c) {
+    const int i = c.i;
+    bool accept = false, retry = false;
+    float val = 0.f;
+    if (c.valid) {
+      if (a.mode == PT_CENTRE) {
+        a.f[i] = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, 0, 0);
+      } else {
+        val = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + a.b);
+        const float phit = -val, phi = -a.f[i];
+        const float rhs = fmaf(a.c1, a.dec[i], phi);
+        accept = (fabsf(phit) <= 3.0e38f) && (phit <= rhs);
+        retry = !accept && (a.b < a.ls_max);
       }
-      a.dec[i] = dsum;
     }
-  }
-  if (t == 0) atomicAdd(&a.evals[a.mode == PT_CENTRE ? EV_INIT : EV_LS], (unsigned long long)min(TC_PTS, cnt - first));
+    if (a.mode == PT_LS) {
+      const int sa = warp_append(a.fd_cnt, accept);
+      if (accept) { a.fd_list[sa] = i; a.ls_b[i] = a.b; a.ft[i] = val; }
+      const int sr = warp_append(a.next_cnt, retry);
+      if (retry) {
+        a.next_list[sr] = i;
+        const float tn = a.tcur[i] * a.shrink;
+        a.tcur[i] = tn;
+        float dsum = 0.0f;
+        for (int j = 0; j < d; ++j) {
+          const float xo = a.x[(size_t)i * d + j];
+          const float xn = clipf(fmaf(tn, a.p[(size_t)i * d + j], xo), a.lo[j], a.hi[j]);
+          a.xt[(size_t)i * d + j] = xn;
+          dsum = fmaf(-a.g[(size_t)i * d + j], xn - xo, dsum);
+        }
+        a.dec[i] = dsum;
+      }
+    }
+    if (t == 0)
+      atomicAdd(&a.evals[a.mode == PT_CENTRE ? EV_INIT : EV_LS], (unsigned long long)min(TC_PTS, cnt - tile * TC_PTS));
+  };
+  tc_run<OBJ>(o, sm, t, ntiles, load, finish);
   tc_teardown(sm, t);
 }
 
@@ -158,6 +170,7 @@ __device__ __forceinline__ void hlc_normals(uint64_t seed, int i, int cycle, int
 }
 
 // Hands Like Clouds on the tensor-core evaluator: point t of the tile = (sample t / M, draw t % M), M <= 128
+struct HlcCtx { int i; bool valid; };
 template <int OBJ>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const HlcArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
@@ -167,60 +180,75 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   if (sigma == 0.0f) return;                       // no spread among the unfrozen samples: nobody moves (R-18)
   const int spt = min(TC_PTS / M, HLC_MAX_SPT);
   const int cnt = a.count ? *a.count : a.max_count;
-  const int first = blockIdx.x * spt;
-  if (first >= cnt) return;
-  tc_setup(sm, t);
-  if (t >= TC_PTS) { tc_load<OBJ>(o, sm, t); tc_teardown(sm, t); return; }
+  const int ntiles = (cnt + spt - 1) / spt;
+  if ((int)blockIdx.x >= ntiles) return;
+  tc_begin<OBJ>(sm, t);
   const int s = t / M, k = t - s * M;
-  const bool valid = (s < spt) && (first + s < cnt);
-  const int i = valid ? a.list[first + s] : 0;
-  float x[TC_D];
-  if (valid) {
-    float u[TC_D];
-    hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
-    tc_load_row(a.x + (size_t)i * d, d, (d & 3) == 0, x);
+  auto load = [&](int tile, float (&x)[TC_D]) -> HlcCtx {
+    HlcCtx c;
+    const int first = tile * spt;
+    c.valid = (s < spt) && (first + s < cnt);
+    c.i = c.valid ? a.list[first + s] : 0;
+    if (c.valid) {
+      float u[TC_D];
+      hlc_normals(a.seed, c.i, a.cycle, a.iter, k, d, u);
+      tc_load_row(a.x + (size_t)c.i * d, d, (d & 3) == 0, x);
 #pragma unroll
-    for (int c = 0; c < TC_D; ++c) x[c] = fmaf(sigma, u[c], x[c]);   // evaluation points are not clipped (R-12)
-  } else {
+      for (int q = 0; q < TC_D; ++q) x[q] = fmaf(sigma, u[q], x[q]);   // evaluation points are not clipped (R-12)
+    } else {
 #pragma unroll
-    for (int c = 0; c < TC_D; ++c) x[c] = 0.f;
-  }
-  float val = tc_eval<OBJ>(o, sm, x, t);
-  compute_sync();                        // every MMA has retired: the operand buffers are free
-  float *Us = reinterpret_cast<float *>(sm.scratch());        // [256][65] normals (scratch is 72 KB)
-  float *fvs = Us + TC_PTS * 65;                              // [256] values
-  if (valid) {
-    val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
-    a.hlc_f[(size_t)i * M + k] = val;
-    float u[TC_D];
-    hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
+      for (int q = 0; q < TC_D; ++q) x[q] = 0.f;
+    }
+    return c;
+  };
+  // Positions are only written by the tile that owns the sample, after every point of that tile has been read
+  // (load of the tile precedes its finish); tiles own disjoint samples.
+  auto finish = [&](int tile, float val, const HlcCtx &c) {
+    const int first = tile * spt, i = c.i;
+    compute_sync();                        // the previous tile's estimate has been read out of the scratch
+    float *Us = reinterpret_cast<float *>(sm.scratch());        // [256][65] normals (scratch is 72 KB)
+    float *fvs = Us + TC_PTS * 65;                              // [256] values
+    if (c.valid) {
+      val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
+      a.hlc_f[(size_t)i * M + k] = val;
+      float u[TC_D];
+      hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
 #pragma unroll
-    for (int c = 0; c < TC_D; ++c) Us[t * 65 + c] = u[c];
-  } else {
-    val = 0.f;
-  }
-  fvs[t] = val;
-  compute_sync();
-  const int nval = min(spt, cnt - first);
-  for (int item = t; item < nval * d; item += TC_PTS) {
-    const int ss = item / d, j = item - ss * d;
-    const int ii = a.list[first + ss];
-    float b = 0.0f;
-    if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
-    float acc = 0.0f;
-    for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, Us[(ss * M + kk) * 65 + j], acc);
-    const float gh = acc / ((float)M * sigma);
-    a.ghat[(size_t)ii * d + j] = gh;
-    const float xo = a.x[(size_t)ii * d + j];
-    a.x[(size_t)ii * d + j] = clipf(fmaf(a.eta, gh, xo), a.lo[j], a.hi[j]);
-  }
-  if (t == 0) atomicAdd(&a.evals[EV_HLC], (unsigned long long)nval * (unsigned long long)M);
+      for (int q = 0; q < TC_D; ++q) Us[t * 65 + q] = u[q];
+    } else {
+      val = 0.f;
+    }
+    fvs[t] = val;
+    compute_sync();
+    const int nval = min(spt, cnt - first);
+    for (int item = t; item < nval * d; item += TC_PTS) {
+      const int ss = item / d, j = item - ss * d;
+      const int ii = a.list[first + ss];
+      float b = 0.0f;
+      if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
+      float acc = 0.0f;
+      for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, Us[(ss * M + kk) * 65 + j], acc);
+      const float gh = acc / ((float)M * sigma);
+      a.ghat[(size_t)ii * d + j] = gh;
+      const float xo = a.x[(size_t)ii * d + j];
+      a.x[(size_t)ii * d + j] = clipf(fmaf(a.eta, gh, xo), a.lo[j], a.hi[j]);
+    }
+    if (t == 0) atomicAdd(&a.evals[EV_HLC], (unsigned long long)nval * (unsigned long long)M);
+  };
+  tc_run<OBJ>(o, sm, t, ntiles, load, finish);
   tc_teardown(sm, t);
 }
 
 // ---- launchers ------------------------------------------------------------------------------------------------
+static int g_tc_sms = 148;
+static inline int tc_grid(int obj_id, int ntiles) {   // GMM_FULL runs persistent CTAs, one per SM
+  return (obj_id == CHISAO_OBJ_GMM_FULL && ntiles > g_tc_sms) ? g_tc_sms : ntiles;
+}
 cudaError_t tc_configure() {
   cudaError_t e;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+    g_tc_sms = sms;
 #define CFG(K) if ((e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES)) != cudaSuccess) return e;
   CFG(k_eval_fd_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_fd_tc<CHISAO_OBJ_QUAD>)
   CFG(k_eval_points_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_points_tc<CHISAO_OBJ_QUAD>)
@@ -230,20 +258,20 @@ cudaError_t tc_configure() {
 }
 cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samples, cudaStream_t st) {
   const int spt = TC_PTS / (2 * a.d);
-  const int grid = (n_samples + spt - 1) / spt;
+  const int grid = tc_grid(obj_id, (n_samples + spt - 1) / spt);
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_fd_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_eval_fd_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
 cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samples, cudaStream_t st) {
-  const int grid = (n_samples + TC_PTS - 1) / TC_PTS;
+  const int grid = tc_grid(obj_id, (n_samples + TC_PTS - 1) / TC_PTS);
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
 cudaError_t launch_hlc_tc(int obj_id, const TcObj &o, const HlcArgs &a, int n_samples, cudaStream_t st) {
   const int spt = TC_PTS / a.M < HLC_MAX_SPT ? TC_PTS / a.M : HLC_MAX_SPT;
-  const int grid = (n_samples + spt - 1) / spt;
+  const int grid = tc_grid(obj_id, (n_samples + spt - 1) / spt);
   if (obj_id == CHISAO_OBJ_QUAD) k_hlc_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_hlc_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
