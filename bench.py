@@ -55,7 +55,7 @@ class ClockSampler(threading.Thread):
     def run(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
             for line in self.proc.stdout:
                 self.rows.append([s.strip() for s in line.split(",")])
         except Exception:
@@ -73,8 +73,15 @@ class ClockSampler(threading.Thread):
                         reasons.add(name)
             except Exception:
                 continue
+        pw = []
+        for r in self.rows:
+            try:
+                pw.append(float(r[2]))
+            except Exception:
+                continue
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "samples": len(sm), "sm_mhz_min": float(np.min(sm)) if sm else None,
+                "power_w": float(np.median(pw)) if pw else None}
 
 
 def measured_peaks():
@@ -214,6 +221,11 @@ def run_ours(args, rank, local_rank, world):
                     "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(c),
                     "peak_source": f"bf16_tflops_sustained ({peaks_src} MEASURED_PEAKS.json) x 1.1/2.25 (tf32:bf16 nominal)",
                     "executed_tensor_tflops": executed, "executed_frac": executed / peak,
+                    # the pipe's own rate: one 128x128x8 kind::tf32 MMA per 64 clocks per SM (measured, _work microbench
+                    # and DESIGN.md section 7) = 4096 flop/clk/SM, at the SM clock sampled during the timed region --
+                    # the kernel runs into the 1000 W power cap, so that clock is well below sm_max_mhz
+                    "tensor_peak_at_sampled_clock": (4096 * 148 * clocks["sm_mhz"] * 1e6 / 1e12) if clocks.get("sm_mhz") else None,
+                    "executed_frac_at_sampled_clock": (executed / (4096 * 148 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
                     "fp32_alu_peak_tflops": alu_peak, "vs_fp32_alu_peak": achieved / alu_peak}
     else:
         roofline = {"bound": "alu", "kernel": "k_eval_fd", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",

@@ -126,6 +126,15 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[64], int q
       : "r"(taddr + 16 * q));
 }
 
+// one lane of a converged warp (elect.sync): the single-thread tcgen05 instructions are issued under this predicate so
+// that the compiler emits them straight-line (issued from a thread-divergent branch, every UTCHMMA is wrapped in an
+// election loop of ~9 instructions and the issuing thread, not the tensor pipe, sets the pace)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -176,6 +185,7 @@ template <int OBJ>
 __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
   const uint32_t tm = *sm.tmem();
   const int K = o.K, g = t >> 7, tl = t & (TC_GROUP - 1);
+  const bool wg0 = __shfl_sync(0xffffffffu, tl >> 5, 0) == 0;   // provably warp-uniform
   float m = -INFINITY, s = 0.0f;
   const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
   const uint32_t dcol = tm + (uint32_t)(g * 256), acol_hi = dcol + 64, acol_lo = dcol + 128;
@@ -236,7 +246,7 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;");
     group_sync(g);
-    if (tl == 0) {
+    if (wg0 && elect_one()) {                         // one lane of the group's first warp (straight-line UTCHMMA)
       asm volatile("tcgen05.fence::after_thread_sync;");
       const uint64_t dBh = tc_desc(smem_u32(sm.B(st)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
 #pragma unroll
@@ -298,15 +308,6 @@ __device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int
     bulk_g2s(sm.CA(rs), r + TCX_W_FLOATS, TCX_CA_BYTES, sm.cbar(rs));
     if (++p == o.npair) p = 0;
   }
-}
-
-// one lane of a converged warp (elect.sync): the single-thread tcgen05 instructions are issued under this predicate so
-// that the compiler emits them straight-line (issued from a thread-divergent branch, every UTCHMMA is wrapped in an
-// election loop of ~9 instructions and the issuing thread, not the tensor pipe, sets the pace)
-__device__ __forceinline__ bool elect_one() {
-  uint32_t pred;
-  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
-  return pred != 0;
 }
 
 // all 32 lanes of warp 9 run the loop (warp-uniform control flow); one elected lane issues
