@@ -1,19 +1,18 @@
 // chisao_tc.cuh -- tensor-core evaluator for the dense objectives at d > 32 (GMM_FULL, QUAD; DP = 64).
 //
 // The quadratic forms q_k(x) = || W_k (x - mu_k) ||^2 of a group of 128 points are a dense contraction
-// Z_k[128 x 64] = D_k[128 x 64] * W_k^T[64 x 64] (BASELINE.json north_star: "tensor cores ... full-covariance
-// mixture quadratic forms").  It runs on the 5th-generation tensor cores: tcgen05.mma kind::tf32, M = 128,
-// N = 64, K = 8 per instruction, accumulators in TMEM, fp32 accuracy by the 3xTF32 split
-//     D W^T ~= D_hi W_hi^T + D_lo W_hi^T + D_hi W_lo^T          (hi = rna-tf32(v), lo = v - hi),
-// 24 MMAs per component.  Thread t of a group owns point t (= TMEM lane t): it writes its row of D_hi / D_lo
-// straight into its TMEM lane with tcgen05.st (the A operand is read from TMEM, element c in column c, so the
-// MMA fetches only W from shared memory), one thread issues the MMAs, and every thread reads its 64
-// accumulators back with tcgen05.ld for the epilogue (sum of squares, online log-sum-exp).  W_k hi/lo are split
-// and laid out on the host once in the canonical K-major no-swizzle UMMA layout (16-byte K-chunks of 8 rows form
-// a 128-byte core matrix; byte offset of (n, c) = (c/4)*1024 + n*16 + (c%4)*4) and streamed by a dedicated warp
-// through two stages with the bulk-copy engine.
-// A CTA evaluates 256 points as two groups of 128 threads; each group has its own operand buffers, accumulator
-// columns and MMA mbarrier, so one group's MMAs run while the other builds operands / drains its accumulators.
+// (BASELINE.json north_star: "tensor cores ... full-covariance mixture quadratic forms").  It runs on the
+// 5th-generation tensor cores: tcgen05.mma kind::tf32, M = 128, K = 8 per instruction, accumulators in TMEM, fp32
+// accuracy by the 3xTF32 split
+//     A B^T ~= A_hi B_hi^T + A_lo B_hi^T + A_hi B_lo^T          (hi = rna-tf32(v), lo = v - hi).
+// Thread t of a group owns point t (= TMEM lane t): it writes its row of A_hi / A_lo straight into its TMEM lane
+// with tcgen05.st (the A operand is read from TMEM, element c in column c, so the MMA fetches only W from shared
+// memory).  W hi/lo are split and laid out on the host once in the canonical K-major no-swizzle UMMA layout (16-byte
+// K-chunks of 8 rows form a 128-byte core matrix) and streamed through shared memory with the bulk-copy engine.
+// A CTA evaluates 256 points as two groups of 128 that alternate on the tensor pipe.  Two forms:
+//   QUAD     (K = 1): A = x - c per component, N = 64, one tile per CTA                      -> tc_eval_tile
+//   GMM_FULL        : A = x once per tile, z = W x - W mu, two components per N = 128 MMA,
+//                     persistent CTAs with loader and MMA-issuer warps                       -> tcx_* below
 #pragma once
 #include "chisao_device.cuh"
 
