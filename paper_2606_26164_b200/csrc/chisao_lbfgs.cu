@@ -106,14 +106,17 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 2) k_lbfgs_direction(State s, 
   __syncthreads();
   const bool in = i < N;
   const size_t ro = (size_t)(in ? i : 0) * d;
+  // one round trip for everything the activity test needs (the flags are read whether or not the sample turns out
+  // to be active: three dependent round trips -> two)
   Row4 g = ld_row4h(s.g + ro, hl, d, vec);
+  const int stalled_i = s.stalled[in ? i : 0], len_i = s.hist_len[in ? i : 0], head_i = s.hist_head[in ? i : 0];
   if (!in) { g.a = g.b = g.c = g.e = 0.f; }
   const float ginf = half_max(fmaxf(fmaxf(fabsf(g.a), fabsf(g.b)), fmaxf(fabsf(g.c), fabsf(g.e))));
   // (i) stationary (Eq. 3's gradient test) or stalled: no work, no evaluations (R-6)
-  const bool act = in && !(s.stalled[in ? i : 0] || !(ginf >= h.eps_grad));
-  int len = act ? s.hist_len[i] : 0;
+  const bool act = in && !(stalled_i || !(ginf >= h.eps_grad));
+  int len = act ? len_i : 0;
   const int len_read = len;
-  const int head = act ? s.hist_head[i] : 0;
+  const int head = act ? head_i : 0;
   Row4 Sr[MM], Yr[MM];
 #pragma unroll
   for (int l = 0; l < MM; ++l) {
@@ -126,8 +129,25 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 2) k_lbfgs_direction(State s, 
       Sr[l].a = Sr[l].b = Sr[l].c = Sr[l].e = 0.f; Yr[l] = Sr[l];
     }
   }
-  const Row4 x = ld_row4h(s.x + ro, hl, d, vec);
+  Row4 x; x.a = x.b = x.c = x.e = 0.f;
+  if (act) x = ld_row4h(s.x + ro, hl, d, vec);
+  // block-aggregated append of the searching samples to line-search worklist 0, and the byte counter: the one
+  // returning global atomic per CTA is issued here, under the history loads, not at the end of the CTA's life
+  int my_slot = 0;
+  if (act && hl == 0) my_slot = atomicAdd(&sh_cnt, 1);
+  if (in && hl == 0) atomicAdd(&sh_bytes, (2u * d + (act ? 2u * (unsigned)len_read * d + 2u * d : 0u)) * 4u);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (sh_cnt > 0) sh_base = atomicAdd(&s.ctrl->ls_cnt[0], sh_cnt);
+    if (sh_bytes) atomicAdd(&s.ctrl->evals[7], (unsigned long long)sh_bytes);   // g read, p written (+ pairs, x, x_t)
+  }
   Row4 gam; gam.a = -g.a; gam.b = -g.b; gam.c = -g.c; gam.e = -g.e;
+  // a warp none of whose two samples is active skips the recursion altogether (late in phase 2 most are stationary)
+  Row4 p, xt;
+  p.a = p.b = p.c = p.e = 0.f; xt = p;
+  bool restart = false;
+  float t0 = 0.f, dec = 0.f;
+  if (__any_sync(0xffffffffu, act)) {
   const float gn2 = dot4(g, g);
   // straight-line code over all MM slots: rows beyond len are zero and rho = 0 there, so they contribute nothing,
   // and no shuffle sits under a branch (the compiler would otherwise wrap each one in a convergence region)
@@ -151,22 +171,20 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 2) k_lbfgs_direction(State s, 
   else { (void)dot4(Yn, Yn); }
 #pragma unroll
   for (int l = 0; l < MM; ++l) { const float beta = rho[l] * dot4(Yr[l], r); axpy4(r, al[l] - beta, Sr[l]); }
-  Row4 p; p.a = -r.a; p.b = -r.b; p.c = -r.c; p.e = -r.e;
+  p.a = -r.a; p.b = -r.b; p.c = -r.c; p.e = -r.e;
   const float gp = dot4(gam, p);
-  bool restart = false;
+  restart = false;
   if (len > 0 && !(gp < 0.0f)) { restart = true; len = 0; }   // not a descent direction for phi = -f: steepest restart
   if (len_read == 0 || restart) { p.a = -gam.a; p.b = -gam.b; p.c = -gam.c; p.e = -gam.e; }
   // (iii) first trial step; (iv) trial point projected on Theta, Armijo linear term gamma.(x_t - x)
-  const float t0 = (len > 0) ? 1.0f : fminf(1.0f, 1.0f / sqrtf(gn2));
+  t0 = (len > 0) ? 1.0f : fminf(1.0f, 1.0f / sqrtf(gn2));
   const Row4 lo = ld_row4h(s.lo, hl, d, vec), hi = ld_row4h(s.hi, hl, d, vec);
-  Row4 xt;
   xt.a = clipf(fmaf(t0, p.a, x.a), lo.a, hi.a); xt.b = clipf(fmaf(t0, p.b, x.b), lo.b, hi.b);
   xt.c = clipf(fmaf(t0, p.c, x.c), lo.c, hi.c); xt.e = clipf(fmaf(t0, p.e, x.e), lo.e, hi.e);
   Row4 dx; dx.a = xt.a - x.a; dx.b = xt.b - x.b; dx.c = xt.c - x.c; dx.e = xt.e - x.e;
-  const float dec = dot4(gam, dx);
-  unsigned int my_bytes = 0u;   // algorithmic HBM bytes of this sample (rows read and written)
+  dec = dot4(gam, dx);
+  }
   if (in) {
-    my_bytes = 2u * d * 4u;                               // g read, p written
     if (act) {
       st_row4h(s.xt + ro, hl, d, vec, xt);
       st_row4h(s.p + ro, hl, d, vec, p);
@@ -174,21 +192,13 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 2) k_lbfgs_direction(State s, 
         s.dec[i] = dec; s.tcur[i] = t0; s.ls_b[i] = -1;
         if (restart) { s.hist_len[i] = 0; s.hist_head[i] = 0; }
       }
-      my_bytes += (2u * (unsigned)len_read * d + 2u * d) * 4u;   // history pairs + x read, x_t written
     } else {
       Row4 z; z.a = z.b = z.c = z.e = 0.f;
       st_row4h(s.p + ro, hl, d, vec, z);
       if (hl == 0) s.ls_b[i] = -2;
     }
   }
-  // block-aggregated append of the searching samples to line-search worklist 0
-  int my_slot = 0;
-  if (act && hl == 0) my_slot = atomicAdd(&sh_cnt, 1);
-  if (hl == 0 && my_bytes) atomicAdd(&sh_bytes, my_bytes);
-  __syncthreads();
-  if (threadIdx.x == 0 && sh_cnt > 0) sh_base = atomicAdd(&s.ctrl->ls_cnt[0], sh_cnt);
-  if (threadIdx.x == 0 && sh_bytes) atomicAdd(&s.ctrl->evals[7], (unsigned long long)sh_bytes);
-  __syncthreads();
+  __syncthreads();                     // sh_base (written by thread 0 after its atomic returned)
   if (act && hl == 0) s.ls_list[0][sh_base + my_slot] = i;
 }
 
