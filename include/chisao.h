@@ -182,6 +182,15 @@ CHISAO_API int chisao_phase(chisao_ctx *ctx, int32_t phase_id, int32_t iter);
 /* Fill *stats from the device control block (synchronises). */
 CHISAO_API int chisao_get_stats(chisao_ctx *ctx, chisao_stats *stats);
 
+/* Options outside the paper's parameter list.  CHISAO_OPT_STENCIL_AWARE (value 0 / 1, default 0): finite-difference
+ * gradients of the dense objectives (GMM_FULL, QUAD) are computed by the stencil-aware evaluator, which shares
+ * W (x - mu), |.|^2 and W^T W (x - mu) between the 2d stencil points of a sample (q(x +- h e_j) = q0 +- 2 h t_j +
+ * h^2 cc_j).  It returns the same 2d values within rounding and counts
+ * the same evaluations, but it is NOT a black-box evaluation of f: numbers obtained with it are
+ * reported separately.  CHISAO_E_INVALID for other objectives or unknown options. */
+#define CHISAO_OPT_STENCIL_AWARE 1
+CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value);
+
 /* Number of kernel launches this context has enqueued so far (host counter). */
 CHISAO_API uint64_t chisao_launch_count(const chisao_ctx *ctx);
 

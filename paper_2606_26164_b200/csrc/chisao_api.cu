@@ -42,6 +42,7 @@ struct chisao_ctx {
   std::vector<float> lo, hi, recs_host, tc_host;
   TcObj tc;
   bool use_tc = false;   // dense objective at d > 32: tensor-core evaluator (chisao_tc.cuh)
+  bool stencil_aware = false;   // chisao_set_option(CHISAO_OPT_STENCIL_AWARE): FD gradients by chisao_stencil.cu
   std::string err;
   uint64_t launches = 0;
   bool timing = false;
@@ -263,6 +264,7 @@ cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const in
   const int grid = (s.N + spt - 1) / spt;
   Scope sc(c, 0);
   c->launches += 1;
+  if (c->stencil_aware) return launch_fd_stencil(c->obj, a, s.N, c->stream);   // opt-in, dense objectives only (NEXT-5)
   if (c->use_tc) {
     cudaError_t e = launch_fd_tc(c->obj.id, c->tc, a, s.N, c->stream);
     if (getenv("CHISAO_DEBUG")) { fprintf(stderr, "[chisao] fd_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] fd_tc done (%s)\n", cudaGetErrorString(e)); }
@@ -702,6 +704,17 @@ int chisao_set_state(chisao_ctx *ctx, int32_t field, const void *src, size_t byt
   if (bytes) CK(cudaMemcpyAsync(dev, src, bytes, cudaMemcpyHostToDevice, ctx->stream));
   CK(cudaStreamSynchronize(ctx->stream));
   return CHISAO_OK;
+}
+
+int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  if (option == CHISAO_OPT_STENCIL_AWARE) {
+    if (value && !fd_stencil_supported(ctx->obj))
+      return fail(ctx, CHISAO_E_INVALID, "the stencil-aware FD evaluator exists for GMM_FULL and QUAD only");
+    ctx->stencil_aware = value != 0;
+    return CHISAO_OK;
+  }
+  return fail(ctx, CHISAO_E_INVALID, "unknown option");
 }
 
 uint64_t chisao_launch_count(const chisao_ctx *ctx) { return ctx ? ctx->launches : 0; }

@@ -30,6 +30,10 @@ struct FdArgs {
   unsigned long long *evals;
 };
 
+// stencil-aware FD evaluator for the dense objectives (chisao_stencil.cu; opt-in)
+bool fd_stencil_supported(const DevObj &o);
+cudaError_t launch_fd_stencil(const DevObj &o, const FdArgs &a, int n_samples, cudaStream_t st);
+
 // ---- central finite differences: 2d stencil points per sample (R-1) ---------------
 // thread t -> (sample t / d of the tile, coordinate j = t % d); it evaluates both x + h e_j and x - h e_j
 // (noise slots 1 + 2j and 2 + 2j, R-2) and forms g_j with the step actually taken in fp32.
