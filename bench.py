@@ -214,18 +214,23 @@ def run_ours(args, rank, local_rank, world):
         # kind::tf32 peak = measured bf16 cuBLAS throughput (sustained: the kernel is timed inside a long step) x the
         # guide's nominal tf32 : bf16 ratio 1.1 : 2.25.  The 3xTF32 split executes three tensor flops per
         # algorithmic flop of the contraction, so frac <= 1/3 by construction; executed_frac says how busy the pipe is.
-        peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * 1.1 / 2.25
+        ev_mode = g.evaluator()                                # 1, 2: kind::tf32;  3: kind::f16 (fp16 hi / lo operands)
+        f16 = ev_mode == 3
+        peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * (1.0 if f16 else 1.1 / 2.25)
+        pipe_rate = 8192 if f16 else 4096                      # flop / clk / SM: one 128x128x16 f16 (x8 tf32) MMA per 64 clocks
         contraction = wl.obj.K * 2.0 * hp.d * hp.d
         executed = 3.0 * fd_evals * contraction / (fd_ms * 1e-3) / 1e12 if fd_ms > 0 else 0.0
         roofline = {"bound": "tensor", "kernel": "k_eval_fd_tc", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                     "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(c),
-                    "peak_source": f"bf16_tflops_sustained ({peaks_src} MEASURED_PEAKS.json) x 1.1/2.25 (tf32:bf16 nominal)",
+                    "evaluator": B.EVALUATOR_NAMES[ev_mode],
+                    "peak_source": f"bf16_tflops_sustained ({peaks_src} MEASURED_PEAKS.json)" + ("" if f16 else " x 1.1/2.25 (tf32:bf16 nominal)")
+                                   + "; the hi/lo split executes 3 tensor flops per algorithmic flop",
                     "executed_tensor_tflops": executed, "executed_frac": executed / peak,
-                    # the pipe's own rate: one 128x128x8 kind::tf32 MMA per 64 clocks per SM (measured, _work microbench
-                    # and DESIGN.md section 7) = 4096 flop/clk/SM, at the SM clock sampled during the timed region --
+                    # the pipe's own rate: one 128x128x8 kind::tf32 (128x128x16 kind::f16) MMA per 64 clocks per SM
+                    # = 4096 (8192) flop/clk/SM, at the SM clock sampled during the timed region --
                     # the kernel runs into the 1000 W power cap, so that clock is well below sm_max_mhz
-                    "tensor_peak_at_sampled_clock": (4096 * 148 * clocks["sm_mhz"] * 1e6 / 1e12) if clocks.get("sm_mhz") else None,
-                    "executed_frac_at_sampled_clock": (executed / (4096 * 148 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
+                    "tensor_peak_at_sampled_clock": (pipe_rate * 148 * clocks["sm_mhz"] * 1e6 / 1e12) if clocks.get("sm_mhz") else None,
+                    "executed_frac_at_sampled_clock": (executed / (pipe_rate * 148 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
                     "fp32_alu_peak_tflops": alu_peak, "vs_fp32_alu_peak": achieved / alu_peak}
     else:
         roofline = {"bound": "alu", "kernel": "k_eval_fd", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",

@@ -191,6 +191,13 @@ CHISAO_API int chisao_get_stats(chisao_ctx *ctx, chisao_stats *stats);
 #define CHISAO_OPT_STENCIL_AWARE 1
 CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value);
 
+/* Which evaluator the context runs (decided at chisao_init from the objective, d and the value ranges):
+ * CHISAO_INFO_EVALUATOR -> 0 FP32-FMA evaluator; 1 tensor cores, 3xTF32, A = x - c per component (QUAD at d > 32);
+ * 2 tensor cores, x-stationary form with tf32 hi / lo operands; 3 the same with fp16 hi / lo operands (kind::f16; chosen
+ * for GMM_FULL at d > 32 when max |W| and the box radius lie in [2^-3, 2^13]). */
+#define CHISAO_INFO_EVALUATOR 1
+CHISAO_API int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value);
+
 /* Number of kernel launches this context has enqueued so far (host counter). */
 CHISAO_API uint64_t chisao_launch_count(const chisao_ctx *ctx);
 

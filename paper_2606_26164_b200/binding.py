@@ -21,11 +21,13 @@ P, LS_B, GHAT, HLC_F, RS_SRC, RS_CAND, XT, GR_Q, SIGMA = 20, 21, 25, 26, 27, 28,
 PH_RELEASE_EVAL, PH_STICK, PH_DEDUP, PH_RESEED, PH_HLC_STEP, PH_ANTI_STEP, PH_LBFGS_ITER = 1, 2, 3, 4, 5, 6, 11
 PH_LBFGS_DIRECTION = 12
 OPT_STENCIL_AWARE = 1
+INFO_EVALUATOR = 1
+EVALUATOR_NAMES = ("fp32-fma", "tcgen05 3xTF32 (x - c)", "tcgen05 x-stationary tf32 hi/lo", "tcgen05 x-stationary fp16 hi/lo")
 TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_update", "select", "reseed")
 
 EXPORTS = ("chisao_workspace_bytes", "chisao_init", "chisao_seed_population", "chisao_step", "chisao_step_host",
            "chisao_modes", "chisao_get_state", "chisao_set_state", "chisao_phase", "chisao_get_stats",
-           "chisao_set_option", "chisao_launch_count", "chisao_timing_enable", "chisao_timing_reset", "chisao_timing_get",
+           "chisao_set_option", "chisao_get_info", "chisao_launch_count", "chisao_timing_enable", "chisao_timing_reset", "chisao_timing_get",
            "chisao_last_error", "chisao_destroy")
 
 _fp = C.POINTER(C.c_float)
@@ -86,6 +88,7 @@ def load_library(path: Optional[str] = None):
     L.chisao_phase.argtypes = [vp, C.c_int32, C.c_int32]
     L.chisao_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.chisao_set_option.argtypes = [vp, C.c_int32, C.c_int32]
+    L.chisao_get_info.argtypes = [vp, C.c_int32, C.POINTER(C.c_int32)]
     L.chisao_launch_count.argtypes = [vp]
     L.chisao_launch_count.restype = C.c_uint64
     L.chisao_timing_enable.argtypes = [vp, C.c_int32]
@@ -198,6 +201,12 @@ class Chisao:
     def set_option(self, option: int, value: int):
         """chisao_set_option (OPT_STENCIL_AWARE: opt-in stencil-aware FD evaluator, reported separately)."""
         self._ck(self._L.chisao_set_option(self._h, int(option), int(value)))
+
+    def evaluator(self) -> int:
+        """chisao_get_info(INFO_EVALUATOR): index into EVALUATOR_NAMES"""
+        v = C.c_int32(0)
+        self._ck(self._L.chisao_get_info(self._h, INFO_EVALUATOR, C.byref(v)))
+        return int(v.value)
 
     def stats(self) -> Stats:
         st = Stats()

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "chisao_eval_kernels.cuh"
+#include <cuda_fp16.h>
 #include "chisao_tc.cuh"
 
 using namespace chisao;
@@ -235,6 +236,43 @@ void pack_tcx_records(const chisao_objective &o, std::vector<float> &out) {
       r[TCX_W_FLOATS + 128 + hf] = o.vec_a[k];
     }
   }
+}
+
+// the same pair records with fp16 hi / lo images (kind::f16): element (n, c) of an image at byte (c/8)*2048 + n*16 +
+// (c%8)*2, hi image then lo image (16 KB each) at the start of the record; c and a as above
+void pack_tcx16_records(const chisao_objective &o, std::vector<float> &out) {
+  const int d = o.d, K = o.K, npair = (K + 1) / 2;
+  out.assign((size_t)npair * TCX_REC, 0.0f);
+  for (int p = 0; p < npair; ++p) {
+    float *r = out.data() + (size_t)p * TCX_REC;
+    uint16_t *img = reinterpret_cast<uint16_t *>(r);
+    for (int hf = 0; hf < 2; ++hf) {
+      const int k = 2 * p + hf;
+      if (k >= K) { r[TCX_W_FLOATS + 128 + hf] = -INFINITY; continue; }
+      for (int n = 0; n < d; ++n) {
+        double cn = 0.0;
+        for (int c = 0; c < d; ++c) {
+          const float w = o.mats[((size_t)k * d + n) * d + c];
+          const __half h = __float2half_rn(w), l = __float2half_rn(w - __half2float(h));
+          const size_t idx = (size_t)(c / 8) * 1024 + (size_t)(64 * hf + n) * 8 + (c % 8);   // in 16-bit elements
+          img[idx] = __half_as_ushort(h); img[8192 + idx] = __half_as_ushort(l);
+          cn += (double)w * (double)o.means[(size_t)k * d + c];
+        }
+        r[TCX_W_FLOATS + 64 * hf + n] = (float)cn;
+      }
+      r[TCX_W_FLOATS + 128 + hf] = o.vec_a[k];
+    }
+  }
+}
+// fp16 hi / lo carries 22 bits like tf32 hi / lo as long as nothing overflows (65504) and the lo parts stay above the
+// fp16 subnormal spacing 2^-24: max |W| and the box radius (plus the HLC spread) must lie in [2^-3, 2^13]
+bool fp16_split_ok(const chisao_objective &o, const chisao_config &c) {
+  float wmax = 0.f, xmax = 0.f;
+  for (size_t e = 0; e < (size_t)o.K * o.d * o.d; ++e) wmax = std::max(wmax, std::fabs(o.mats[e]));
+  for (int j = 0; j < c.d; ++j) xmax = std::max(xmax, std::max(std::fabs(c.lo[j]), std::fabs(c.hi[j])));
+  xmax += 8.0f * std::fabs(c.sigma_s) + std::fabs(c.fd_h);
+  const float lo = 0.125f, hi = 8192.0f;
+  return wmax >= lo && wmax <= hi && xmax >= lo && xmax <= hi && !getenv("CHISAO_TC_TF32");
 }
 
 struct Scope {   // optional CUDA-event bracket around a launch group
@@ -483,7 +521,9 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
   }
   ctx->use_tc = wants_tc(*obj);
   if (ctx->use_tc) {
-    if (obj->id == CHISAO_OBJ_GMM_FULL) pack_tcx_records(*obj, ctx->tc_host);
+    ctx->tc.f16 = (obj->id == CHISAO_OBJ_GMM_FULL && fp16_split_ok(*obj, *cfg)) ? 1 : 0;
+    if (ctx->tc.f16) pack_tcx16_records(*obj, ctx->tc_host);
+    else if (obj->id == CHISAO_OBJ_GMM_FULL) pack_tcx_records(*obj, ctx->tc_host);
     else pack_tc_records(*obj, ctx->tc_host);
     ctx->tc.npair = (obj->K + 1) / 2;
     ctx->tc.K = obj->K; ctx->tc.d = obj->d; ctx->tc.sigma_noise = obj->sigma_noise; ctx->tc.recs = tc_dev;
@@ -715,6 +755,12 @@ int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value) {
     return CHISAO_OK;
   }
   return fail(ctx, CHISAO_E_INVALID, "unknown option");
+}
+
+int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value) {
+  if (!ctx || !value || which != CHISAO_INFO_EVALUATOR) return CHISAO_E_INVALID;
+  *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_QUAD ? 1 : (ctx->tc.f16 ? 3 : 2));
+  return CHISAO_OK;
 }
 
 uint64_t chisao_launch_count(const chisao_ctx *ctx) { return ctx ? ctx->launches : 0; }

@@ -14,6 +14,7 @@
 //   GMM_FULL        : A = x once per tile, z = W x - W mu, two components per N = 128 MMA,
 //                     persistent CTAs with loader and MMA-issuer warps                       -> tcx_* below
 #pragma once
+#include <cuda_fp16.h>
 #include "chisao_device.cuh"
 
 namespace chisao {
@@ -43,6 +44,7 @@ struct TcObj {
   float sigma_noise;
   const float *recs;      // device [K][TC_REC] (QUAD) or [npair][TCX_REC] (GMM_FULL, x-stationary form)
   int32_t npair;          // ceil(K / 2)
+  int32_t f16;            // x-stationary form: operands split into fp16 hi / lo (kind::f16) instead of tf32 hi / lo
 };
 
 // shared-memory carve (all offsets are arithmetic so that nothing is indexed dynamically through a pointer table):
@@ -104,6 +106,21 @@ __device__ __forceinline__ void tc_mma_ts_i(uint32_t tmem_d, uint32_t tmem_a, ui
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(tmem_d),
       "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate));
+}
+__device__ __forceinline__ void tc_mma_ts_f16(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate));
+}
+// D = F32, A = B = F16 (format 0), both K-major, N = 128, M = 128; K = 16 per instruction
+constexpr uint32_t TC_IDESC_F16_N128 = (1u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+__device__ __forceinline__ void tc_st16u(uint32_t taddr, const uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+      "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+      "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+      : "memory");
 }
 __device__ __forceinline__ void tc_st16(uint32_t taddr, const float (&v)[16]) {
   asm volatile(
@@ -299,8 +316,9 @@ __device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int
     const int st = G & 1, rs = G & (TCX_RING - 1);
     if (G >= 2) mbar_wait(sm.fbar(st), ((G >> 1) - 1) & 1);   // the MMAs of pair G - 2 have retired in both groups
     const float *r = o.recs + (size_t)p * TCX_REC;
-    mbar_expect_tx(sm.bbar(st), TCX_W_BYTES);
-    bulk_g2s(sm.Bx(st), r, TCX_W_BYTES, sm.bbar(st));
+    const uint32_t wbytes = o.f16 ? TCX_W_BYTES / 2 : TCX_W_BYTES;   // fp16 images are half the size (same record stride)
+    mbar_expect_tx(sm.bbar(st), wbytes);
+    bulk_g2s(sm.Bx(st), r, wbytes, sm.bbar(st));
     // ring slot rs was last read by the drains of pair G - 4; they precede the MMAs of pair G - 3, whose retirement
     // the wait above (pair G - 2) implies
     mbar_expect_tx(sm.cbar(rs), TCX_CA_BYTES);
@@ -325,6 +343,17 @@ __device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int
         asm volatile("tcgen05.fence::after_thread_sync;");
         const uint32_t gcol = tm + (uint32_t)(g * 256);
         if (elect_one()) {
+          if (o.f16) {   // fp16 hi / lo: K = 16 per MMA (8 packed columns of A, two 8-element K-chunks of B), 4 K-steps
+            const uint64_t dBl16 = dBh + (uint64_t)((TCX_W_BYTES / 4) >> 4);
+#pragma unroll
+            for (int pr = 0; pr < 3; ++pr) {
+              const uint32_t a0 = (pr == 1) ? gcol + 32 : gcol;
+              const uint64_t b0 = (pr == 2) ? dBl16 : dBh;
+#pragma unroll
+              for (int ks = 0; ks < 4; ++ks)
+                tc_mma_ts_f16(gcol + 128, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (4096 >> 4)), TC_IDESC_F16_N128, (pr | ks) ? 1u : 0u);
+            }
+          } else {
 #pragma unroll
           for (int pr = 0; pr < 3; ++pr) {
             const uint32_t a0 = (pr == 1) ? gcol + 64 : gcol;
@@ -332,6 +361,7 @@ __device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int
 #pragma unroll
             for (int ks = 0; ks < 8; ++ks)
               tc_mma_ts_i(gcol + 128, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (4096 >> 4)), TC_IDESC_N128, (pr | ks) ? 1u : 0u);
+          }
           }
           tc_commit(sm.mbar(g));
           if (g == 1) tc_commit(sm.fbar(st));         // both groups' MMAs of this pair retired: the W stage is free
@@ -351,6 +381,22 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
   const uint32_t lanes = tm + ((uint32_t)(wq * 32) << 16);
   const uint32_t xaddr = lanes + (uint32_t)(own * 256), rd = lanes + (uint32_t)(128 + 64 * hf);
   auto write_x = [&](const float (&xv)[TC_D]) {        // hi / lo images of the thread's point -> its TMEM lane
+    if (o.f16) {   // two fp16 per 32-bit column (element 2c in the low half): hi in columns [0, 32), lo in [32, 64)
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        uint32_t h[16], l[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+          const float x0 = xv[32 * q + 2 * c], x1 = xv[32 * q + 2 * c + 1];
+          const __half h0 = __float2half_rn(x0), h1 = __float2half_rn(x1);
+          const __half l0 = __float2half_rn(x0 - __half2float(h0)), l1 = __float2half_rn(x1 - __half2float(h1));
+          h[c] = (uint32_t)__half_as_ushort(h0) | ((uint32_t)__half_as_ushort(h1) << 16);
+          l[c] = (uint32_t)__half_as_ushort(l0) | ((uint32_t)__half_as_ushort(l1) << 16);
+        }
+        tc_st16u(xaddr + 16 * q, h);
+        tc_st16u(xaddr + 32 + 16 * q, l);
+      }
+    } else {
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       float h[16], l[16];
@@ -358,6 +404,7 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
       for (int c = 0; c < 16; ++c) { h[c] = tf32_rna(xv[16 * q + c]); l[c] = xv[16 * q + c] - h[c]; }
       tc_st16(xaddr + 16 * q, h);
       tc_st16(xaddr + 64 + 16 * q, l);
+    }
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;");

@@ -367,3 +367,28 @@ def test_ablation_switches_phase_mask(orc, B):
         x2 = g.get(B.X).copy()
         g.phase(B.PH_ANTI_STEP, 1)
         assert (not np.array_equal(g.get(B.X), x2)) == (off != 6)
+
+
+def test_tensor_evaluator_selection_and_tf32_fallback(orc, B, monkeypatch):
+    """chisao_get_info: which evaluator chisao_init chose; the tf32 hi/lo form (forced by CHISAO_TC_TF32, or chosen
+    when the box radius leaves fp16's range) passes the same a1 parity as the fp16 hi/lo form"""
+    for c, want in ((5, 3), (4, 1), (3, 0), (1, 0)):
+        g = B.Chisao(inputs.config(c, N=64))
+        assert g.evaluator() == want, (c, g.evaluator())
+        g.close()
+    monkeypatch.setenv("CHISAO_TC_TF32", "1")
+    g = B.Chisao(inputs.config(5, N=64))
+    assert g.evaluator() == 2
+    g.close()
+    test_a1_eval_and_fd_gradient(orc, B, 5, 200)
+    monkeypatch.delenv("CHISAO_TC_TF32")
+    # a box of radius 9000 > 2^13: fp16 would overflow -> tf32 operands, same tolerances
+    wl = inputs.custom(inputs.gmm_full(40, 3, 3.0, 77), 9000.0, 300, seed=5, fd_h=4.0)
+    o, g = _pair(orc, B, wl)
+    assert g.evaluator() == 2
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0]); g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL); g.phase(B.PH_RELEASE_EVAL)
+    fo, fg = o.get(orc.F), g.get(B.F).astype(np.float64)
+    assert np.all(np.abs(fg - fo) <= PT.f_tol(fo)), float(np.max(np.abs(fg - fo) / np.maximum(np.abs(fo), 1)))
+    ok, err, tol = PT.grad_ok(g.get(B.G).astype(np.float64), o.get(orc.G), fo, wl.hp.fd_h)
+    assert np.all(ok), float(np.max(err / tol))
