@@ -259,6 +259,13 @@ void pack_tcx16_records(const chisao_objective &o, std::vector<float> &out) {
           cn += (double)w * (double)o.means[(size_t)k * d + c];
         }
         r[TCX_W_FLOATS + 64 * hf + n] = (float)cn;
+        // -c_n as three fp16 pieces (33 bits) in K positions 0..2 of the extra K = 16 step, 32 KB into the record
+        const __half c1 = __float2half_rn((float)-cn);
+        const double r1 = -cn - (double)__half2float(c1);
+        const __half c2 = __float2half_rn((float)r1);
+        const __half c3 = __float2half_rn((float)(r1 - (double)__half2float(c2)));
+        uint16_t *cimg = img + 16384 + (size_t)(64 * hf + n) * 8;
+        cimg[0] = __half_as_ushort(c1); cimg[1] = __half_as_ushort(c2); cimg[2] = __half_as_ushort(c3);
       }
       r[TCX_W_FLOATS + 128 + hf] = o.vec_a[k];
     }
@@ -272,7 +279,14 @@ bool fp16_split_ok(const chisao_objective &o, const chisao_config &c) {
   for (int j = 0; j < c.d; ++j) xmax = std::max(xmax, std::max(std::fabs(c.lo[j]), std::fabs(c.hi[j])));
   xmax += 8.0f * std::fabs(c.sigma_s) + std::fabs(c.fd_h);
   const float lo = 0.125f, hi = 8192.0f;
-  return wmax >= lo && wmax <= hi && xmax >= lo && xmax <= hi && !getenv("CHISAO_TC_TF32");
+  double cmax = 0.0;                                   // c = W mu goes through the pipe as fp16 pieces as well
+  for (int k = 0; k < o.K; ++k)
+    for (int n = 0; n < o.d; ++n) {
+      double cn = 0.0;
+      for (int c2 = 0; c2 < o.d; ++c2) cn += (double)o.mats[((size_t)k * o.d + n) * o.d + c2] * (double)o.means[(size_t)k * o.d + c2];
+      cmax = std::max(cmax, std::fabs(cn));
+    }
+  return wmax >= lo && wmax <= hi && xmax >= lo && xmax <= hi && cmax <= 32768.0 && !getenv("CHISAO_TC_TF32");
 }
 
 struct Scope {   // optional CUDA-event bracket around a launch group

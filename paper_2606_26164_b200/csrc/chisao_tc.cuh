@@ -33,10 +33,12 @@ constexpr int TCX_W_BYTES = TCX_W_FLOATS * 4;            // 65 536
 constexpr int TCX_CA_FLOATS = 128 + 4;                   // c = W mu of both components | a_0, a_1, 0, 0
 constexpr int TCX_CA_BYTES = TCX_CA_FLOATS * 4;          // 528
 constexpr int TCX_REC = TCX_W_FLOATS + TCX_CA_FLOATS;    // floats per pair record (66 064 bytes, multiple of 16)
+constexpr int TCX16_W_BYTES = TCX_W_BYTES / 2 + 4096;    // fp16 form: W_hi 16 KB | W_lo 16 KB | one K = 16 step holding -c (4 KB)
 constexpr int TCX_RING = 4;                              // c / a ring slots (outlive the W stage by one epilogue)
 constexpr int TCX_PART_BYTES = 2 * 2 * 2 * TC_GROUP * 8;   // [tile parity][half][group][128] float2
 constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES + TCX_PART_BYTES;   // >= the 2 x TC_REC form
 static_assert(2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES >= 2 * TC_REC_BYTES, "shared-memory carve");
+static_assert(3 * TCX16_W_BYTES <= 2 * TCX_W_BYTES, "three fp16 stages fit the two tf32 stages");
 constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D0 64 | D_hi 64 | D_lo 64 | D1 64
 
 struct TcObj {
@@ -63,9 +65,13 @@ struct TcSmem {
   __device__ __forceinline__ float *B(int st) const {
     return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * TC_REC_BYTES);
   }
-  __device__ __forceinline__ float *Bx(int st) const {    // x-stationary form: W pair stages, then the c / a ring
-    return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * TCX_W_BYTES);
+  // x-stationary form: a ring of W pair stages (2 x 64 KB with tf32 operands, 3 x 36 KB with fp16 operands) with its own
+  // "landed" / "free" barriers, then the c / a ring
+  __device__ __forceinline__ float *Bx(int st, int stage_bytes) const {
+    return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * stage_bytes);
   }
+  __device__ __forceinline__ uint64_t *bbarx(int st) const { return reinterpret_cast<uint64_t *>(base) + 18 + st; }
+  __device__ __forceinline__ uint64_t *fbarx(int st) const { return reinterpret_cast<uint64_t *>(base) + 21 + st; }
   __device__ __forceinline__ float *CA(int r) const {
     return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + r * TCX_CA_BYTES);
   }
@@ -169,6 +175,7 @@ __device__ __forceinline__ void tc_setup(const TcSmem &sm, int t, int fbar_count
     mbar_init(sm.fbar(0), fbar_count); mbar_init(sm.fbar(1), fbar_count);
     mbar_init(sm.dbar(0), 8); mbar_init(sm.dbar(1), 8); mbar_init(sm.xbar(0), 4); mbar_init(sm.xbar(1), 4);
     mbar_init(sm.cbar(0), 1); mbar_init(sm.cbar(1), 1); mbar_init(sm.cbar(2), 1); mbar_init(sm.cbar(3), 1);
+    for (int st = 0; st < 3; ++st) { mbar_init(sm.bbarx(st), 1); mbar_init(sm.fbarx(st), 1); }
     mbar_fence_init();
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
@@ -312,30 +319,32 @@ __device__ __forceinline__ int tcx_tiles_of_cta(int ntiles) {
 
 __device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int ntc) {
   const int total = ntc * o.npair;
-  for (int G = 0, p = 0; G < total; ++G) {
-    const int st = G & 1, rs = G & (TCX_RING - 1);
-    if (G >= 2) mbar_wait(sm.fbar(st), ((G >> 1) - 1) & 1);   // the MMAs of pair G - 2 have retired in both groups
+  const int nst = o.f16 ? 3 : 2;
+  const uint32_t wbytes = o.f16 ? TCX16_W_BYTES : TCX_W_BYTES;       // fp16 images: hi | lo | -c (same record stride)
+  for (int G = 0, p = 0, st = 0, lap = 0; G < total; ++G) {
+    const int rs = G & (TCX_RING - 1);
+    if (lap > 0) mbar_wait(sm.fbarx(st), (lap - 1) & 1);      // the MMAs of pair G - nst have retired in both groups
     const float *r = o.recs + (size_t)p * TCX_REC;
-    const uint32_t wbytes = o.f16 ? TCX_W_BYTES / 2 : TCX_W_BYTES;   // fp16 images are half the size (same record stride)
-    mbar_expect_tx(sm.bbar(st), wbytes);
-    bulk_g2s(sm.Bx(st), r, wbytes, sm.bbar(st));
+    mbar_expect_tx(sm.bbarx(st), wbytes);
+    bulk_g2s(sm.Bx(st, (int)wbytes), r, wbytes, sm.bbarx(st));
     // ring slot rs was last read by the drains of pair G - 4; they precede the MMAs of pair G - 3, whose retirement
-    // the wait above (pair G - 2) implies
+    // the wait above (pair G - 2 or G - 3) implies
     mbar_expect_tx(sm.cbar(rs), TCX_CA_BYTES);
     bulk_g2s(sm.CA(rs), r + TCX_W_FLOATS, TCX_CA_BYTES, sm.cbar(rs));
     if (++p == o.npair) p = 0;
+    if (++st == nst) { st = 0; ++lap; }
   }
 }
 
 // all 32 lanes of warp 9 run the loop (warp-uniform control flow); one elected lane issues
 __device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int ntc) {
   const uint32_t tm = *sm.tmem();
-  int G = 0;
+  const int nst = o.f16 ? 3 : 2, stage_bytes = o.f16 ? TCX16_W_BYTES : TCX_W_BYTES;
+  int G = 0, st = 0, lap = 0;
   for (int it = 0; it < ntc; ++it)
     for (int p = 0; p < o.npair; ++p, ++G) {
-      const int st = G & 1;
-      mbar_wait(sm.bbar(st), (G >> 1) & 1);
-      const uint64_t dBh = tc_desc(smem_u32(sm.Bx(st)), 2048, 128), dBl = dBh + (uint64_t)((TCX_W_BYTES / 2) >> 4);
+      mbar_wait(sm.bbarx(st), lap & 1);
+      const uint64_t dBh = tc_desc(smem_u32(sm.Bx(st, stage_bytes)), 2048, 128), dBl = dBh + (uint64_t)((TCX_W_BYTES / 2) >> 4);
 #pragma unroll 1
       for (int g = 0; g < 2; ++g) {
         if (p == 0) mbar_wait(sm.xbar(g), it & 1);              // this tile's X image is in TMEM
@@ -353,6 +362,9 @@ __device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int
               for (int ks = 0; ks < 4; ++ks)
                 tc_mma_ts_f16(gcol + 128, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (4096 >> 4)), TC_IDESC_F16_N128, (pr | ks) ? 1u : 0u);
             }
+            // thirteenth step: A = (1, 1, 1, 0, ...) in columns [64, 72), B rows = the three fp16 pieces of -c_n, so the
+            // accumulators hold z = W x - c and the drain has nothing to subtract
+            tc_mma_ts_f16(gcol + 128, gcol + 64, dBh + (uint64_t)((TCX_W_BYTES / 2) >> 4), TC_IDESC_F16_N128, 1u);
           } else {
 #pragma unroll
           for (int pr = 0; pr < 3; ++pr) {
@@ -364,10 +376,11 @@ __device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int
           }
           }
           tc_commit(sm.mbar(g));
-          if (g == 1) tc_commit(sm.fbar(st));         // both groups' MMAs of this pair retired: the W stage is free
+          if (g == 1) tc_commit(sm.fbarx(st));        // both groups' MMAs of this pair retired: the W stage is free
         }
         __syncwarp();
       }
+      if (++st == nst) { st = 0; ++lap; }
     }
 }
 
@@ -411,6 +424,13 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
     __syncwarp();
     if (lane == 0) mbar_arrive(sm.xbar(own));
   };
+  if (o.f16) {   // the constant operand row (1, 1, 1, 0, ...) of the -c step: columns [64, 80) of the thread's own lane, once
+    uint32_t one[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) one[c] = 0u;
+    one[0] = 0x3C003C00u; one[1] = 0x00003C00u;
+    tc_st16u(xaddr + 64, one);
+  }
   float xn[TC_D];
   auto cn = load((int)blockIdx.x, xn);
   write_x(xn);
@@ -441,12 +461,21 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
         if (lane == 0) mbar_arrive(sm.dbar(g));       // accumulators are in registers: the next MMAs may overwrite them
         if (swap && g == own) write_x(xn);            // this group's last MMAs of the tile have retired
         float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+        if (o.f16) {                                  // -c went through the tensor pipe
 #pragma unroll
-        for (int n = 0; n < 64; n += 4) {
-          const float4 c = c4[n >> 2];
-          const float z0 = __uint_as_float(r[n]) - c.x, z1 = __uint_as_float(r[n + 1]) - c.y,
-                      z2 = __uint_as_float(r[n + 2]) - c.z, z3 = __uint_as_float(r[n + 3]) - c.w;
-          q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+          for (int n = 0; n < 64; n += 4) {
+            const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
+                        z3 = __uint_as_float(r[n + 3]);
+            q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+          }
+        } else {
+#pragma unroll
+          for (int n = 0; n < 64; n += 4) {
+            const float4 c = c4[n >> 2];
+            const float z0 = __uint_as_float(r[n]) - c.x, z1 = __uint_as_float(r[n + 1]) - c.y,
+                        z2 = __uint_as_float(r[n + 2]) - c.z, z3 = __uint_as_float(r[n + 3]) - c.w;
+            q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+          }
         }
         const float v = fmaf(-0.5f, (q0 + q1) + (q2 + q3), a_k);
         if (g == 0) {
