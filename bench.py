@@ -327,7 +327,7 @@ def run_ours(args, rank, local_rank, world):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_eval_fd launch from the committed `ncu --set full`
 # capture (profiles/); None until a capture of that workload exists.
-TRAFFIC_BYTES_PER_LAUNCH = {5: 1.9e7}   # profiles/r1_evalfd_c5_tc.md (full-size launch: 18.96 MB read, 0 written)
+TRAFFIC_BYTES_PER_LAUNCH = {5: 1.84e7}  # profiles/r1_evalfd_c5_f16.md (full-size launch: 18.35 MB read, 0.07 MB written)
 
 
 def main():
