@@ -12,7 +12,9 @@
 // A CTA evaluates 256 points as two groups of 128 that alternate on the tensor pipe.  Two forms:
 //   QUAD     (K = 1): A = x - c per component, N = 64, one tile per CTA                      -> tc_eval_tile
 //   GMM_FULL        : A = x once per tile, z = W x - W mu, two components per N = 128 MMA,
-//                     persistent CTAs with loader and MMA-issuer warps                       -> tcx_* below
+//                     persistent CTAs with loader and MMA-issuer warps; operands as fp16 hi / lo
+//                     (kind::f16, K = 16, -c as a 13th K-step) when the value ranges allow,
+//                     else tf32 hi / lo                                                      -> tcx_* below
 #pragma once
 #include <cuda_fp16.h>
 #include "chisao_device.cuh"
@@ -297,9 +299,10 @@ __device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, 
 // itself, so its hi / lo images are written to TMEM ONCE per tile instead of once per component, and two components
 // share one MMA (B = [W_k ; W_{k+1}], N = 128: 64 cycles against 2 x 47 for two N = 64 instructions).  Per pair and
 // group, 24 MMAs (X_hi W_hi^T + X_lo W_hi^T + X_hi W_lo^T over 8 K-steps) fill the group's 128 accumulator columns.
-// The cancellation in W x - c costs accuracy: |W x| <= ~110 at C5 against |z| ~ 1..8, measured |df| <= 5e-7 max(|f|, 1)
-// against the 1e-5 bar; QUAD (kappa = 1e4, f -> 0 at the optimum) keeps the (x - c) form above.
-// Group g owns TMEM columns [256 g, 256 g + 256): X_hi 64 | X_lo 64 | accumulators 128.
+// The cancellation in W x - c costs accuracy: |W x| <= ~110 at C5 against |z| ~ 1..8, measured |df| <= 3.8e-6 max(|f|, 1)
+// near the modes (6.1e-6 with tf32 operands) against the 1e-5 bar; QUAD (kappa = 1e4, f -> 0 at the optimum) keeps the (x - c) form above.
+// Group g owns TMEM columns [256 g, 256 g + 256): X_hi 64 | X_lo 64 | accumulators 128 (fp16 form: X_hi 32 | X_lo 32 |
+// ones 16 | unused | accumulators 128).
 //
 // Roles: warp 8 streams the pair records (W stage ring of 2, c / a ring of 4); warp 9 issues the MMAs (it waits for
 // "W landed", "X image written" and "accumulators of group g drained", issues, and lets tcgen05.commit signal "MMAs of
