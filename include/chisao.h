@@ -194,7 +194,10 @@ CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value)
 /* Which evaluator the context runs (decided at chisao_init from the objective, d and the value ranges):
  * CHISAO_INFO_EVALUATOR -> 0 FP32-FMA evaluator; 1 tensor cores, 3xTF32, A = x - c per component (QUAD at d > 32);
  * 2 tensor cores, x-stationary form with tf32 hi / lo operands; 3 the same with fp16 hi / lo operands (kind::f16; chosen
- * for GMM_FULL at d > 32 when max |W| and the box radius lie in [2^-3, 2^13]). */
+ * for GMM_FULL at d > 32 when max |W| and the box radius lie in [2^-3, 2^13]); 4 tensor cores,
+ * random-Fourier phases w_j . x as an exact contraction of 10-bit fixed-point fp16 pieces (RFF at d <= 32, K <= 256
+ * with max |w| and the box radius + 8 sigma_s + h in [2^-7, 2^10]; CHISAO_RFF_FP64 in the environment keeps the
+ * FP32-FMA evaluator with fp64 phases). */
 #define CHISAO_INFO_EVALUATOR 1
 CHISAO_API int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value);
 

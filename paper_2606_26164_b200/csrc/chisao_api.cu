@@ -100,8 +100,28 @@ int validate(const chisao_config *cfg, const chisao_objective *obj, std::string 
 }
 
 // workspace carve; fills st pointers relative to `base` (may be null when only sizing)
-inline bool wants_tc(const chisao_objective &o) {
-  return (o.id == CHISAO_OBJ_GMM_FULL || o.id == CHISAO_OBJ_QUAD) && o.d > 32;
+// RFF on the tensor cores (chisao_tc.cuh, tc_rff_tile): d <= 32, K <= 256 and value ranges inside the fixed-point
+// split: |x| < 2^ex (box radius + HLC spread + FD step), |w| < 2^ew, with ex, ew in [-6, 10]
+bool rff_tc_scales(const chisao_objective &o, const chisao_config &c, int *ex_out, int *ew_out) {
+  if (o.id != CHISAO_OBJ_RFF || o.d > RFF_TC_D || o.K > RFF_TC_K || getenv("CHISAO_RFF_FP64")) return false;
+  float wmax = 0.f, rad = 0.f;
+  for (size_t e = 0; e < (size_t)o.K * o.d; ++e) wmax = std::max(wmax, std::fabs(o.mats[e]));
+  for (int j = 0; j < c.d; ++j) rad = std::max(rad, std::max(std::fabs(c.lo[j]), std::fabs(c.hi[j])));
+  // auto sigma (sigma_s < 0): |sigma_s| x pooled std of the unfrozen samples <= |sigma_s| x box diameter
+  const float sig = c.sigma_s > 0.0f ? c.sigma_s : 2.0f * rad * std::fabs(c.sigma_s);
+  const float xmax = rad + 8.0f * sig + std::fabs(c.fd_h);
+  if (!(wmax > 0.f) || !(xmax > 0.f) || !(wmax < 3.0e38f) || !(xmax < 3.0e38f)) return false;
+  int ex = 0, ew = 0;
+  std::frexp(xmax, &ex);   // xmax = m 2^ex, m in [0.5, 1): xmax < 2^ex (or = 2^(ex-1): still inside the 4x headroom)
+  std::frexp(wmax, &ew);
+  ew += 0;
+  if (ex < -6 || ex > 10 || ew < -6 || ew > 10) return false;
+  if (ex_out) *ex_out = ex;
+  if (ew_out) *ew_out = ew;
+  return true;
+}
+inline bool wants_tc(const chisao_objective &o, const chisao_config &c) {
+  return ((o.id == CHISAO_OBJ_GMM_FULL || o.id == CHISAO_OBJ_QUAD) && o.d > 32) || rff_tc_scales(o, c, nullptr, nullptr);
 }
 
 size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *base, State *st, const float **recs_dev,
@@ -125,7 +145,7 @@ size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *b
   const size_t o_blk = F(3 * nb + 3);
   const size_t o_hf = F(N * M);
   const size_t o_q = F(d * d);
-  const size_t o_tc = F(!wants_tc(o) ? 0 : (o.id == CHISAO_OBJ_GMM_FULL ? (size_t)((o.K + 1) / 2) * TCX_REC : (size_t)o.K * TC_REC));
+  const size_t o_tc = F(!wants_tc(o, c) ? 0 : (o.id == CHISAO_OBJ_RFF ? (size_t)RFF_REC_FLOATS : (o.id == CHISAO_OBJ_GMM_FULL ? (size_t)((o.K + 1) / 2) * TCX_REC : (size_t)o.K * TC_REC)));
   if (base && st) {
     auto P = [&](size_t off) { return reinterpret_cast<float *>(base + off); };
     auto I = [&](size_t off) { return reinterpret_cast<int32_t *>(base + off); };
@@ -269,6 +289,28 @@ void pack_tcx16_records(const chisao_objective &o, std::vector<float> &out) {
       }
       r[TCX_W_FLOATS + 128 + hf] = o.vec_a[k];
     }
+  }
+}
+// RFF record (chisao_tc.cuh, tc_rff_tile): the frequencies cut into three 10-bit fixed-point pieces
+// w = 2^(ew-9) (m0 + 2^-10 m1 + 2^-20 m2) (fp64 arithmetic on the fp32 inputs: every step exact), stored as the fp16
+// images m0 | m1 | 2^-10 m2, element (n, c) of an image at 16-bit index (c/8)*2048 + n*8 + (c%8); then (a_n, b_n)
+void pack_rff_records(const chisao_objective &o, int ew, std::vector<float> &out) {
+  out.assign(RFF_REC_FLOATS, 0.0f);
+  uint16_t *img = reinterpret_cast<uint16_t *>(out.data());
+  const double S0 = std::ldexp(1.0, 9 - ew);
+  for (int n = 0; n < o.K; ++n) {
+    for (int c = 0; c < o.d; ++c) {
+      const double w = (double)o.mats[(size_t)n * o.d + c];
+      const double m0 = std::nearbyint(w * S0), r1 = w - m0 / S0;
+      const double m1 = std::nearbyint(r1 * S0 * 1024.0), r2 = r1 - m1 / (S0 * 1024.0);
+      const double m2 = std::nearbyint(r2 * S0 * 1048576.0);
+      const size_t idx = (size_t)(c / 8) * 2048 + (size_t)n * 8 + (c % 8);
+      img[idx] = __half_as_ushort(__float2half_rn((float)m0));
+      img[8192 + idx] = __half_as_ushort(__float2half_rn((float)m1));
+      img[16384 + idx] = __half_as_ushort(__float2half_rn((float)(m2 / 1024.0)));
+    }
+    out[RFF_W_BYTES / 4 + 2 * n] = o.vec_a[n];
+    out[RFF_W_BYTES / 4 + 2 * n + 1] = o.vec_b[n];
   }
 }
 // fp16 hi / lo carries 22 bits like tf32 hi / lo as long as nothing overflows (65504) and the lo parts stay above the
@@ -533,10 +575,16 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
     case 4: CKI(configure_obj_4()); break;
     default: CKI(configure_obj_5()); break;
   }
-  ctx->use_tc = wants_tc(*obj);
+  ctx->use_tc = wants_tc(*obj, *cfg);
   if (ctx->use_tc) {
     ctx->tc.f16 = (obj->id == CHISAO_OBJ_GMM_FULL && fp16_split_ok(*obj, *cfg)) ? 1 : 0;
-    if (ctx->tc.f16) pack_tcx16_records(*obj, ctx->tc_host);
+    if (obj->id == CHISAO_OBJ_RFF) {
+      int ex = 0, ew = 0;
+      rff_tc_scales(*obj, *cfg, &ex, &ew);
+      pack_rff_records(*obj, ew, ctx->tc_host);
+      ctx->tc.rff_S0 = std::ldexp(1.0f, 9 - ex); ctx->tc.rff_uA = std::ldexp(1.0f, ex + ew - 18);
+      ctx->tc.rff_s0 = obj->scalar0; ctx->tc.nchunk = (obj->K + 63) / 64;
+    } else if (ctx->tc.f16) pack_tcx16_records(*obj, ctx->tc_host);
     else if (obj->id == CHISAO_OBJ_GMM_FULL) pack_tcx_records(*obj, ctx->tc_host);
     else pack_tc_records(*obj, ctx->tc_host);
     ctx->tc.npair = (obj->K + 1) / 2;
@@ -773,7 +821,7 @@ int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value) {
 
 int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value) {
   if (!ctx || !value || which != CHISAO_INFO_EVALUATOR) return CHISAO_E_INVALID;
-  *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_QUAD ? 1 : (ctx->tc.f16 ? 3 : 2));
+  *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_RFF ? 4 : (ctx->obj.id == CHISAO_OBJ_QUAD ? 1 : (ctx->tc.f16 ? 3 : 2)));
   return CHISAO_OK;
 }
 

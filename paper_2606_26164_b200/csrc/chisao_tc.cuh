@@ -41,6 +41,13 @@ constexpr int TCX_PART_BYTES = 2 * 2 * 2 * TC_GROUP * 8;   // [tile parity][half
 constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES + TCX_PART_BYTES;   // >= the 2 x TC_REC form
 static_assert(2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES >= 2 * TC_REC_BYTES, "shared-memory carve");
 static_assert(3 * TCX16_W_BYTES <= 2 * TCX_W_BYTES, "three fp16 stages fit the two tf32 stages");
+// RFF form: three fixed-point fp16 images of the frequencies [3][4 K-chunks][256 rows][8], then (a_j, b_j) pairs
+constexpr int RFF_TC_D = 32, RFF_TC_K = 256;
+constexpr int RFF_W_BYTES = 3 * RFF_TC_K * RFF_TC_D * 2;   // 49 152
+constexpr int RFF_REC_BYTES = RFF_W_BYTES + RFF_TC_K * 8;  // 51 200
+constexpr int RFF_REC_FLOATS = RFF_REC_BYTES / 4;
+constexpr int RFF_X_BYTES = 4 * TC_GROUP * RFF_TC_D * 2;   // four point images of a group (canonical K-major layout), 32 768
+static_assert(RFF_REC_BYTES + 2 * RFF_X_BYTES <= 2 * TCX_W_BYTES, "RFF carve fits the W stage region");
 constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D0 64 | D_hi 64 | D_lo 64 | D1 64
 
 struct TcObj {
@@ -49,6 +56,11 @@ struct TcObj {
   const float *recs;      // device [K][TC_REC] (QUAD) or [npair][TCX_REC] (GMM_FULL, x-stationary form)
   int32_t npair;          // ceil(K / 2)
   int32_t f16;            // x-stationary form: operands split into fp16 hi / lo (kind::f16) instead of tf32 hi / lo
+  // RFF form (tc_rff_tile): fixed-point scales of the operand pieces and the -s0 ||x||^2 coefficient
+  float rff_S0;           // 2^(9 - ex): x * S0 rounds to the first 10-bit piece (|x| < 2^ex)
+  float rff_uA;           // 2^(ex + ew - 18): value of one unit of the exact accumulator (|w| < 2^ew)
+  float rff_s0;           // coefficient of -||x||^2
+  int32_t nchunk;         // ceil(K / 64) feature chunks
 };
 
 // shared-memory carve (all offsets are arithmetic so that nothing is indexed dynamically through a pointer table):
@@ -121,6 +133,13 @@ __device__ __forceinline__ void tc_mma_ts_f16(uint32_t tmem_d, uint32_t tmem_a, 
       "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(tmem_d),
       "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate));
 }
+__device__ __forceinline__ void tc_mma_ss_f16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate));
+}
+constexpr uint32_t TC_IDESC_F16_N64 = (1u << 4) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
 // D = F32, A = B = F16 (format 0), both K-major, N = 128, M = 128; K = 16 per instruction
 constexpr uint32_t TC_IDESC_F16_N128 = (1u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
 __device__ __forceinline__ void tc_st16u(uint32_t taddr, const uint32_t (&v)[16]) {
@@ -148,6 +167,16 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[64], int q
         "=r"(r[16 * q + 10]), "=r"(r[16 * q + 11]), "=r"(r[16 * q + 12]), "=r"(r[16 * q + 13]), "=r"(r[16 * q + 14]),
         "=r"(r[16 * q + 15])
       : "r"(taddr + 16 * q));
+}
+
+__device__ __forceinline__ void tc_ld16s(uint32_t taddr, uint32_t (&r)[64], int q) {   // 16 columns at taddr -> r[16 q ..]
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[16 * q + 0]), "=r"(r[16 * q + 1]), "=r"(r[16 * q + 2]), "=r"(r[16 * q + 3]), "=r"(r[16 * q + 4]),
+        "=r"(r[16 * q + 5]), "=r"(r[16 * q + 6]), "=r"(r[16 * q + 7]), "=r"(r[16 * q + 8]), "=r"(r[16 * q + 9]),
+        "=r"(r[16 * q + 10]), "=r"(r[16 * q + 11]), "=r"(r[16 * q + 12]), "=r"(r[16 * q + 13]), "=r"(r[16 * q + 14]),
+        "=r"(r[16 * q + 15])
+      : "r"(taddr));
 }
 
 // one lane of a converged warp (elect.sync): the single-thread tcgen05 instructions are issued under this predicate so
@@ -504,6 +533,127 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
   }
 }
 
+// ---- random-Fourier form (RFF at d <= 32, K <= 256) ---------------------------------------------------------------
+// The phases t_j = w_j . x of a group of 128 points are the dense contraction X W^T (128 x 32 by 32 x 256).  f needs
+// them to ~1e-6 absolute at |t| up to ~100 (the cosine passes a phase error straight on to f), which an fp32 running
+// sum does not give; the FFMA evaluator therefore accumulates in fp64.  Here the contraction runs EXACTLY on the
+// tensor cores instead: x and w are cut into three 10-bit fixed-point pieces each,
+//     x = 2^(ex-9) (n0 + 2^-10 n1 + 2^-20 n2),   w = 2^(ew-9) (m0 + 2^-10 m1 + 2^-20 m2),   |n|, |m| <= 512 integers,
+// every piece is an integer-valued fp16 (exact), every product is an integer below 2^18 and a sum of 32 of them stays
+// below 2^23: the fp32 accumulators hold exact integers whatever the order of summation.  Two accumulators per
+// feature:   A = sum n0 m0   and   BC = sum n0 m1 + n1 m0 + 2^-10 (n1 m1 + n0 m2 + n2 m0)   (12 K = 16 MMAs per 64 features),
+// t = 2^(ex+ew-18) (A + 2^-10 BC) + b; dropped: 2^-30 (n1 m2 + n2 m1 + ...), below 1e-6 |x|max |w|max.  The range
+// reduction t - 2 pi k is exact on the A part (Cody-Waite with 2 pi = 201/32 + rest), so the angle handed to the
+// hardware cosine carries one fp32 rounding, like the fp64 path's.  Point images go to shared memory in the canonical
+// K-major layout (generic stores + fence.proxy.async); the frequencies' images and (a, b) are loaded once per CTA
+// (persistent over tiles).  Group g: accumulator stages s = 0, 1 at TMEM columns 256 g + 128 s (A 64 | BC 64); chunk
+// c + 1 is issued before chunk c is drained, and the other group's MMAs run under this group's arithmetic.
+// round to nearest integer for |v| < 2^22: two full-rate additions instead of a conversion-pipe FRND
+__device__ __forceinline__ float rint_magic(float v) { return (v + 12582912.0f) - 12582912.0f; }
+__device__ __forceinline__ void rff_split(float v, float S0, float U0, float &n0, float &n1, float &n2) {
+  n0 = rint_magic(fminf(fmaxf(v * S0, -2047.0f), 2047.0f));
+  const float r1 = fmaf(-n0, U0, v);                                   // exact
+  n1 = rint_magic(fminf(fmaxf(r1 * (S0 * 1024.0f), -2047.0f), 2047.0f));
+  const float r2 = fmaf(-n1, U0 * (1.0f / 1024.0f), r1);               // exact
+  n2 = rint_magic(fminf(fmaxf(r2 * (S0 * 1048576.0f), -2047.0f), 2047.0f));
+}
+__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
+  const __half2 h = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t *>(&h);
+}
+__device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t, uint32_t (&use)[2]) {
+  const uint32_t tm = *sm.tmem();
+  const int g = t >> 7, tl = t & (TC_GROUP - 1);
+  const bool wg0 = __shfl_sync(0xffffffffu, tl >> 5, 0) == 0;   // provably warp-uniform
+  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
+  const uint32_t gcol = tm + (uint32_t)(g * 256);
+  unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
+  unsigned char *ximg = wbase + RFF_REC_BYTES + g * RFF_X_BYTES;
+  const float2 *ab2 = reinterpret_cast<const float2 *>(wbase + RFF_W_BYTES);
+  const float S0 = o.rff_S0, U0 = 1.0f / S0;
+  float nrm = 0.0f;
+  // the thread's row of the four point images: n0 | n1 | 2^-10 n1 | 2^-10 n2
+#pragma unroll
+  for (int kc = 0; kc < RFF_TC_D / 8; ++kc) {
+    uint32_t i0[4], i1[4], i1s[4], i2s[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const float xa = x[8 * kc + 2 * e], xb = x[8 * kc + 2 * e + 1];
+      nrm = fmaf(xa, xa, nrm); nrm = fmaf(xb, xb, nrm);
+      float a0, a1, a2, b0, b1, b2;
+      rff_split(xa, S0, U0, a0, a1, a2);
+      rff_split(xb, S0, U0, b0, b1, b2);
+      i0[e] = pack_h2(a0, b0); i1[e] = pack_h2(a1, b1);
+      i1s[e] = pack_h2(a1 * (1.0f / 1024.0f), b1 * (1.0f / 1024.0f));
+      i2s[e] = pack_h2(a2 * (1.0f / 1024.0f), b2 * (1.0f / 1024.0f));
+    }
+    unsigned char *dst = ximg + kc * 2048 + tl * 16;
+    *reinterpret_cast<uint4 *>(dst) = make_uint4(i0[0], i0[1], i0[2], i0[3]);
+    *reinterpret_cast<uint4 *>(dst + 8192) = make_uint4(i1[0], i1[1], i1[2], i1[3]);
+    *reinterpret_cast<uint4 *>(dst + 16384) = make_uint4(i1s[0], i1s[1], i1s[2], i1s[3]);
+    *reinterpret_cast<uint4 *>(dst + 24576) = make_uint4(i2s[0], i2s[1], i2s[2], i2s[3]);
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core's reads
+  const float uA = o.rff_uA, uB = o.rff_uA * (1.0f / 1024.0f);
+  float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+  auto drain = [&](int c) {
+    const int st = c & 1;
+    mbar_wait(sm.cbar(2 * g + st), use[st] & 1);
+    use[st] += 1;
+    asm volatile("tcgen05.fence::after_thread_sync;");
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+      uint32_t r[64];
+      const uint32_t ta = lane_base + (uint32_t)(128 * st + 32 * hh);
+      tc_ld16s(ta, r, 0); tc_ld16s(ta + 16, r, 1); tc_ld16s(ta + 64, r, 2); tc_ld16s(ta + 80, r, 3);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      const float2 *ab = ab2 + 64 * c + 32 * hh;
+#pragma unroll
+      for (int n = 0; n < 32; ++n) {
+        const float2 p = ab[n];                                       // a_j, b_j (broadcast)
+        const float rest = fmaf(__uint_as_float(r[32 + n]), uB, p.y);
+        const float tA = __uint_as_float(r[n]) * uA;                  // exact
+        const float kq = rint_magic((tA + rest) * 0.15915494309189535f);
+        float red = fmaf(-kq, 6.28125f, tA);                          // exact: multiples of min(uA, 2^-5), |red| small
+        red = fmaf(-kq, 1.9353071795864769e-3f, red);
+        const float cs = __cosf(red + rest);
+        if ((n & 3) == 0) s0 = fmaf(p.x, cs, s0);
+        else if ((n & 3) == 1) s1 = fmaf(p.x, cs, s1);
+        else if ((n & 3) == 2) s2 = fmaf(p.x, cs, s2);
+        else s3 = fmaf(p.x, cs, s3);
+      }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
+  };
+  const int nch = o.nchunk;
+  for (int c = 0; c < nch; ++c) {
+    group_sync(g);   // c = 0: the images of all 128 rows are written; c >= 2: every thread has drained chunk c - 2
+    if (wg0 && elect_one()) {
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      const uint64_t dX = tc_desc(smem_u32(ximg), 2048, 128);
+      const uint64_t dW = tc_desc(smem_u32(wbase) + (uint32_t)(c * 1024), 4096, 128);
+      const uint32_t accA = gcol + (uint32_t)(128 * (c & 1)), accBC = accA + 64;
+#pragma unroll
+      for (int ks = 0; ks < 2; ++ks)
+        tc_mma_ss_f16(accA, dX + (uint64_t)(ks * 256), dW + (uint64_t)(ks * 512), TC_IDESC_F16_N64, ks ? 1u : 0u);
+#pragma unroll
+      for (int pr = 0; pr < 5; ++pr) {
+        const int xp = (pr == 0 || pr == 3) ? 0 : (pr == 1 ? 1 : (pr == 2 ? 2 : 3));
+        const int wp = (pr == 0 || pr == 2) ? 1 : (pr == 3 ? 2 : 0);
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks)
+          tc_mma_ss_f16(accBC, dX + (uint64_t)(xp * 512 + ks * 256), dW + (uint64_t)(wp * 1024 + ks * 512), TC_IDESC_F16_N64,
+                        (pr | ks) ? 1u : 0u);
+      }
+      tc_commit(sm.cbar(2 * g + (c & 1)));
+    }
+    __syncwarp();
+    if (c > 0) drain(c - 1);
+  }
+  drain(nch - 1);
+  return fmaf(-o.rff_s0, nrm, (s0 + s1) + (s2 + s3));
+}
+
 // Run the evaluator over `ntiles` tiles of 256 points; called by every thread of the CTA after tc_begin.
 //   GMM_FULL: persistent x-stationary form, any grid <= ntiles;  QUAD: one tile per CTA (grid = ntiles).
 template <int OBJ, class Load, class Finish>
@@ -514,6 +664,25 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
     if (warp < TC_PTS / 32) tcx_compute(o, sm, t, ntc, load, finish);
     else if (warp == TC_PTS / 32) { if (t == TC_PTS) tcx_loader(o, sm, ntc); }
     else tcx_issuer(o, sm, ntc);
+  } else if constexpr (OBJ == CHISAO_OBJ_RFF) {
+    // persistent over tiles; the frequencies' images and (a, b) land once (51 200 bytes)
+    if (t >= TC_PTS) {
+      if (t == TC_PTS) {
+        mbar_expect_tx(sm.bbar(0), RFF_REC_BYTES);
+        bulk_g2s(sm.Bx(0, 0), o.recs, RFF_REC_BYTES, sm.bbar(0));
+      }
+      return;
+    }
+    mbar_wait(sm.bbar(0), 0);
+    const int ntc = tcx_tiles_of_cta(ntiles);
+    uint32_t use[2] = {0u, 0u};
+    for (int it = 0; it < ntc; ++it) {
+      const int tile = (int)blockIdx.x + it * (int)gridDim.x;
+      float x[TC_D];
+      const auto c = load(tile, x);
+      const float f = tc_rff_tile(o, sm, x, t, use);
+      finish(tile, f, c);
+    }
   } else {
     if (t >= TC_PTS) { tc_loader(o, sm, t); return; }
     float x[TC_D];

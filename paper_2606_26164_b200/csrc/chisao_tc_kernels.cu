@@ -1,5 +1,5 @@
 // chisao_tc_kernels.cu -- the three evaluation kernels (FD stencil, one point per sample, Hands Like Clouds)
-// on the tensor-core evaluator of chisao_tc.cuh, for GMM_FULL and QUAD at 32 < d <= 64.  Same arguments, same
+// on the tensor-core evaluator of chisao_tc.cuh, for GMM_FULL and QUAD at 32 < d <= 64 and RFF at d <= 32, K <= 256.  Same arguments, same
 // noise slots, same epilogues as the FFMA kernels of chisao_eval_kernels.cuh; one point per compute thread, 256
 // points per CTA (two groups of 128 ping-pong on the tensor pipe) plus one warp that streams the parameters.  Citations: PAPER.md:62, :555 (FD), :75-82 (line search), :113-120 + Eq. 9 :577 (HLC), Eq. 6 :126.
 #include "chisao_eval_kernels.cuh"
@@ -250,8 +250,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
 
 // ---- launchers ------------------------------------------------------------------------------------------------
 static int g_tc_sms = 148;
-static inline int tc_grid(int obj_id, int ntiles) {   // GMM_FULL runs persistent CTAs, one per SM
-  return (obj_id == CHISAO_OBJ_GMM_FULL && ntiles > g_tc_sms) ? g_tc_sms : ntiles;
+static inline int tc_grid(int obj_id, int ntiles) {   // GMM_FULL and RFF run persistent CTAs, one per SM
+  return ((obj_id == CHISAO_OBJ_GMM_FULL || obj_id == CHISAO_OBJ_RFF) && ntiles > g_tc_sms) ? g_tc_sms : ntiles;
 }
 cudaError_t tc_configure() {
   cudaError_t e;
@@ -262,6 +262,7 @@ cudaError_t tc_configure() {
   CFG(k_eval_fd_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_fd_tc<CHISAO_OBJ_QUAD>)
   CFG(k_eval_points_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_points_tc<CHISAO_OBJ_QUAD>)
   CFG(k_hlc_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_hlc_tc<CHISAO_OBJ_QUAD>)
+  CFG(k_eval_fd_tc<CHISAO_OBJ_RFF>) CFG(k_eval_points_tc<CHISAO_OBJ_RFF>) CFG(k_hlc_tc<CHISAO_OBJ_RFF>)
 #undef CFG
   return cudaSuccess;
 }
@@ -269,12 +270,14 @@ cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samp
   const int spt = TC_PTS / (2 * a.d);
   const int grid = tc_grid(obj_id, (n_samples + spt - 1) / spt);
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_fd_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
+  else if (obj_id == CHISAO_OBJ_RFF) k_eval_fd_tc<CHISAO_OBJ_RFF><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_eval_fd_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
 cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samples, cudaStream_t st) {
   const int grid = tc_grid(obj_id, (n_samples + TC_PTS - 1) / TC_PTS);
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
+  else if (obj_id == CHISAO_OBJ_RFF) k_eval_points_tc<CHISAO_OBJ_RFF><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
@@ -282,6 +285,7 @@ cudaError_t launch_hlc_tc(int obj_id, const TcObj &o, const HlcArgs &a, int n_sa
   const int spt = TC_PTS / a.M < HLC_MAX_SPT ? TC_PTS / a.M : HLC_MAX_SPT;
   const int grid = tc_grid(obj_id, (n_samples + spt - 1) / spt);
   if (obj_id == CHISAO_OBJ_QUAD) k_hlc_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
+  else if (obj_id == CHISAO_OBJ_RFF) k_hlc_tc<CHISAO_OBJ_RFF><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_hlc_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }

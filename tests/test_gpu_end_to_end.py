@@ -245,12 +245,14 @@ def test_step_host_matches_device_resident_step(B):
     assert list(sa.evals) == list(sb.evals)
 
 
-@pytest.mark.parametrize("obj_id,d,K,N", [(2, 40, 3, 300), (2, 64, 1, 130), (2, 33, 2, 257), (4, 50, 1, 260), (2, 64, 5, 513)])
+@pytest.mark.parametrize("obj_id,d,K,N", [(2, 40, 3, 300), (2, 64, 1, 130), (2, 33, 2, 257), (4, 50, 1, 260), (2, 64, 5, 513),
+                                          (3, 32, 256, 300), (3, 5, 10, 130), (3, 17, 200, 257), (3, 24, 64, 513)])
 def test_tensor_core_evaluator_shapes(orc, B, obj_id, d, K, N):
-    """dense objectives at 32 < d <= 64 run on the tcgen05 evaluator (256-point tiles, two groups): d not a
-    multiple of 4 or 8 (zero-padded to 64), one / odd numbers of components, ragged last tile; f, g, one L-BFGS
+    """dense objectives at 32 < d <= 64 (and the random-Fourier objective at d <= 32, K <= 256) run on the tcgen05
+    evaluator (256-point tiles, two groups): d not a multiple of 4 or 8 (zero-padded), one / odd numbers of
+    components, feature counts that are not a multiple of the 64-feature chunk, ragged last tile; f, g, one L-BFGS
     iteration, one HLC and one anti-convergence step against the oracle."""
-    obj = inputs.gmm_full(d, K, 3.0, 70 + d + K) if obj_id == 2 else inputs.quad(d, 71 + d, lam_max=50.0)
+    obj = inputs.gmm_full(d, K, 3.0, 70 + d + K) if obj_id == 2 else (inputs.rff(d, K, 72 + d + K) if obj_id == 3 else inputs.quad(d, 71 + d, lam_max=50.0))
     wl = inputs.custom(obj, 4.0, N, seed=123 + d, hlc_M=12, n_conv=3, fd_h=5e-2, eps_grad=1e-3, n_osc=2, hlc_baseline=1,
                        sigma_s=0.5, eta_hlc=1e-3, alpha_anti=1e-3)
     o, g = orc.Oracle(wl, threads=8), B.Chisao(wl)

@@ -372,10 +372,22 @@ def test_ablation_switches_phase_mask(orc, B):
 def test_tensor_evaluator_selection_and_tf32_fallback(orc, B, monkeypatch):
     """chisao_get_info: which evaluator chisao_init chose; the tf32 hi/lo form (forced by CHISAO_TC_TF32, or chosen
     when the box radius leaves fp16's range) passes the same a1 parity as the fp16 hi/lo form"""
-    for c, want in ((5, 3), (4, 1), (3, 0), (1, 0)):
+    for c, want in ((5, 3), (4, 1), (3, 4), (1, 0)):
         g = B.Chisao(inputs.config(c, N=64))
         assert g.evaluator() == want, (c, g.evaluator())
         g.close()
+    # random-Fourier objective: exact fixed-point contraction on the tensor cores at d <= 32, K <= 256; the fp64-phase
+    # FFMA evaluator otherwise (or when CHISAO_RFF_FP64 is set), same tolerances
+    for d, K, want in ((32, 256, 4), (33, 16, 0), (8, 257, 0)):
+        g = B.Chisao(inputs.custom(inputs.rff(d, K, 5), 5.0, 64))
+        assert g.evaluator() == want, (d, K, g.evaluator())
+        g.close()
+    monkeypatch.setenv("CHISAO_RFF_FP64", "1")
+    g = B.Chisao(inputs.config(3, N=64))
+    assert g.evaluator() == 0
+    g.close()
+    test_a1_eval_and_fd_gradient(orc, B, 3, 200)
+    monkeypatch.delenv("CHISAO_RFF_FP64")
     monkeypatch.setenv("CHISAO_TC_TF32", "1")
     g = B.Chisao(inputs.config(5, N=64))
     assert g.evaluator() == 2
