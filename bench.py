@@ -209,22 +209,23 @@ def run_ours(args, rank, local_rank, world):
     fd_ms, fd_n = phase_ms["eval_fd"]
     alu_peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12   # TFLOP/s, FP32 FMA lanes x clock
     achieved = fd_evals * fpe / (fd_ms * 1e-3) / 1e12 if fd_ms > 0 else 0.0
-    on_tensor = wl.obj.id in (2, 4) and hp.d > 32          # dense objectives at d > 32 run on tcgen05 (chisao_tc.cuh)
+    on_tensor = g.evaluator() != 0                          # dense objectives at d > 32 and RFF at d <= 32 run on tcgen05 (chisao_tc.cuh)
     if on_tensor:
         # kind::tf32 peak = measured bf16 cuBLAS throughput (sustained: the kernel is timed inside a long step) x the
         # guide's nominal tf32 : bf16 ratio 1.1 : 2.25.  The 3xTF32 split executes three tensor flops per
         # algorithmic flop of the contraction, so frac <= 1/3 by construction; executed_frac says how busy the pipe is.
         ev_mode = g.evaluator()                                # 1, 2: kind::tf32;  3: kind::f16 (fp16 hi / lo operands)
-        f16 = ev_mode == 3
+        f16 = ev_mode in (3, 4)                                # 4: random-Fourier phases, six products of 10-bit fp16 pieces
         peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * (1.0 if f16 else 1.1 / 2.25)
         pipe_rate = 8192 if f16 else 4096                      # flop / clk / SM: one 128x128x16 f16 (x8 tf32) MMA per 64 clocks
-        contraction = wl.obj.K * 2.0 * hp.d * hp.d
-        executed = 3.0 * fd_evals * contraction / (fd_ms * 1e-3) / 1e12 if fd_ms > 0 else 0.0
+        contraction = wl.obj.K * 2.0 * hp.d * (1 if ev_mode == 4 else hp.d)
+        nprod = 6.0 if ev_mode == 4 else 3.0                   # tensor flops executed per algorithmic flop of the contraction
+        executed = nprod * fd_evals * contraction / (fd_ms * 1e-3) / 1e12 if fd_ms > 0 else 0.0
         roofline = {"bound": "tensor", "kernel": "k_eval_fd_tc", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                     "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(c),
                     "evaluator": B.EVALUATOR_NAMES[ev_mode],
                     "peak_source": f"bf16_tflops_sustained ({peaks_src} MEASURED_PEAKS.json)" + ("" if f16 else " x 1.1/2.25 (tf32:bf16 nominal)")
-                                   + "; the hi/lo split executes 3 tensor flops per algorithmic flop",
+                                   + f"; the operand split executes {nprod:.0f} tensor flops per algorithmic flop of the contraction",
                     "executed_tensor_tflops": executed, "executed_frac": executed / peak,
                     # the pipe's own rate: one 128x128x8 kind::tf32 (128x128x16 kind::f16) MMA per 64 clocks per SM
                     # = 4096 (8192) flop/clk/SM, at the SM clock sampled during the timed region --

@@ -9,8 +9,10 @@
 // with tcgen05.st (the A operand is read from TMEM, element c in column c, so the MMA fetches only W from shared
 // memory).  W hi/lo are split and laid out on the host once in the canonical K-major no-swizzle UMMA layout (16-byte
 // K-chunks of 8 rows form a 128-byte core matrix) and streamed through shared memory with the bulk-copy engine.
-// A CTA evaluates 256 points as two groups of 128 that alternate on the tensor pipe.  Two forms:
-//   QUAD     (K = 1): A = x - c per component, N = 64, one tile per CTA                      -> tc_eval_tile
+// A CTA evaluates 256 points as two groups of 128 that alternate on the tensor pipe; CTAs are persistent (one per SM,
+// walking tiles).  Three forms:
+//   QUAD     (K = 1): A = x - c, N = 64, the record resident in shared memory                -> tc_quad_run
+//   RFF  (d <= 32)  : phases w_j . x as an EXACT contraction of 10-bit fixed-point fp16 pieces -> tc_rff_tile
 //   GMM_FULL        : A = x once per tile, z = W x - W mu, two components per N = 128 MMA,
 //                     persistent CTAs with loader and MMA-issuer warps; operands as fp16 hi / lo
 //                     (kind::f16, K = 16, -c as a 13th K-step) when the value ranges allow,
@@ -217,110 +219,6 @@ __device__ __forceinline__ void tc_teardown(const TcSmem &sm, int t) {
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
   if (t < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*sm.tmem()), "n"(TC_TMEM_COLS));
-}
-
-// Streams the K component records through the two B stages (called by the loader warp, t >= TC_PTS).
-__device__ __forceinline__ void tc_loader(const TcObj &o, const TcSmem &sm, int t) {
-  if (t != TC_PTS) return;
-  for (int k = 0; k < o.K; ++k) {
-    const int st = k & 1;
-    if (k >= 2) mbar_wait(sm.fbar(st), ((k >> 1) - 1) & 1);   // both groups are done with component k - 2
-    mbar_expect_tx(sm.bbar(st), TC_REC_BYTES);
-    bulk_g2s(sm.B(st), o.recs + (size_t)k * TC_REC, TC_REC_BYTES, sm.bbar(st));
-  }
-}
-
-// Evaluate the calling thread's point x[64] (coordinates >= d must be zero).  Called by the 256 compute threads
-// (t < TC_PTS) while the loader warp runs tc_loader; tc_setup must have run.  Group g = t / 128 owns operand
-// TMEM columns [256 g, 256 g + 192) (accumulator | D_hi | D_lo) and mbarrier mbar(g); the two groups share the B stages
-// and alternate on the tensor pipe: while one group's 24 MMAs run, the other builds its next operand / reads its
-// accumulators.  OBJ is CHISAO_OBJ_GMM_FULL or CHISAO_OBJ_QUAD.
-template <int OBJ>
-__device__ __forceinline__ float tc_eval_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
-  const uint32_t tm = *sm.tmem();
-  const int K = o.K, g = t >> 7, tl = t & (TC_GROUP - 1);
-  const bool wg0 = __shfl_sync(0xffffffffu, tl >> 5, 0) == 0;   // provably warp-uniform
-  float m = -INFINITY, s = 0.0f;
-  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
-  const uint32_t dcol = tm + (uint32_t)(g * 256), acol_hi = dcol + 64, acol_lo = dcol + 128;
-  float a_prev = 0.0f;
-  // accumulator stage j & 1 of this group -> sum of squares -> online log-sum-exp
-  auto drain = [&](int j, float a_j) {
-    const uint32_t taddr = lane_base + (uint32_t)((j & 1) * 192);
-    uint32_t r[64];
-    tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
-#pragma unroll
-    for (int n = 0; n < 64; n += 4) {
-      const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
-                  z3 = __uint_as_float(r[n + 3]);
-      q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
-    }
-    const float q = (q0 + q1) + (q2 + q3);
-    if constexpr (OBJ == CHISAO_OBJ_QUAD) {
-      s += q;
-    } else {
-      const float v = fmaf(-0.5f, q, a_j);
-      const float mn = fmaxf(m, v);
-      if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
-  };
-  // MMAs of component j have retired: the operand image and B stage j & 1 are free, accumulator stage j & 1 is ready
-  auto retire = [&](int j) {
-    mbar_wait(sm.mbar(g), j & 1);
-    asm volatile("tcgen05.fence::after_thread_sync;");
-    if (tl == 0) mbar_arrive(sm.fbar(j & 1));
-    __syncwarp();
-  };
-  for (int k = 0; k < K; ++k) {
-    const int st = k & 1;
-    mbar_wait(sm.bbar(st), (k >> 1) & 1);             // W_k hi/lo, mu_k, a_k have landed
-    const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(st) + 2 * TC_D * TC_D);
-    const float a_k = sm.B(st)[2 * TC_D * TC_D + TC_D];
-    if (k > 0) retire(k - 1);
-    // this thread's row of D_hi / D_lo goes straight into its TMEM lane (A operand read from TMEM: the MMA then
-    // fetches only W from shared memory)
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      float h[16], l[16];
-#pragma unroll
-      for (int c4 = 0; c4 < 4; ++c4) {
-        const float4 mu = mu4[4 * q + c4];
-        const int c = 16 * q + 4 * c4;
-        const float d0 = x[c] - mu.x, d1 = x[c + 1] - mu.y, d2 = x[c + 2] - mu.z, d3 = x[c + 3] - mu.w;
-        h[4 * c4] = tf32_rna(d0); h[4 * c4 + 1] = tf32_rna(d1); h[4 * c4 + 2] = tf32_rna(d2); h[4 * c4 + 3] = tf32_rna(d3);
-        // d - hi is exact in fp32 with at most 13 significant bits; the MMA reads its top 11 (residual 2^-22 |d|)
-        l[4 * c4] = d0 - h[4 * c4]; l[4 * c4 + 1] = d1 - h[4 * c4 + 1]; l[4 * c4 + 2] = d2 - h[4 * c4 + 2]; l[4 * c4 + 3] = d3 - h[4 * c4 + 3];
-      }
-      tc_st16(lane_base + 64 + 16 * q, h);
-      tc_st16(lane_base + 128 + 16 * q, l);
-    }
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-    asm volatile("tcgen05.fence::before_thread_sync;");
-    group_sync(g);
-    if (wg0 && elect_one()) {                         // one lane of the group's first warp (straight-line UTCHMMA)
-      asm volatile("tcgen05.fence::after_thread_sync;");
-      const uint64_t dBh = tc_desc(smem_u32(sm.B(st)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
-#pragma unroll
-      for (int pr = 0; pr < 3; ++pr) {
-        const uint32_t a0 = (pr == 1) ? acol_lo : acol_hi;
-        const uint64_t b0 = (pr == 2) ? dBl : dBh;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks)
-          tc_mma_ts(dcol + (uint32_t)((k & 1) * 192), a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
-      }
-      tc_commit(sm.mbar(g));
-    }
-    __syncwarp();
-    if (k > 0) drain(k - 1, a_prev);                  // overlaps the MMAs of component k (two accumulator stages)
-    a_prev = a_k;
-  }
-  retire(K - 1);
-  drain(K - 1, a_prev);
-  if constexpr (OBJ == CHISAO_OBJ_QUAD) return -0.5f * s;
-  return m + logf(s);
 }
 
 // ---- x-stationary form (GMM_FULL) -----------------------------------------------------------------------------
@@ -654,6 +552,76 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
   return fmaf(-o.rff_s0, nrm, (s0 + s1) + (s2 + s3));
 }
 
+// ---- QUAD (K = 1), persistent form ----------------------------------------------------------------------------------
+// One record (W hi / lo, c) stays resident in shared memory; the CTA walks tiles blockIdx.x, blockIdx.x + gridDim.x, ...
+// Per tile a thread writes A = x - c (tf32 hi / lo) into its TMEM lane, the group's 24 MMAs (3xTF32, M128 N64 K8) fill
+// its 64 accumulator columns, and the next tile's point is fetched while they run.  The two groups alternate on the
+// tensor pipe.  TMEM per group (256 g): accumulators 64 | A_hi 64 | A_lo 64.
+template <class Load, class Finish>
+__device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish) {
+  const uint32_t tm = *sm.tmem();
+  const int g = t >> 7, tl = t & (TC_GROUP - 1);
+  const bool wg0 = __shfl_sync(0xffffffffu, tl >> 5, 0) == 0;   // provably warp-uniform
+  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
+  const uint32_t dcol = tm + (uint32_t)(g * 256), acol_hi = dcol + 64, acol_lo = dcol + 128;
+  const int ntc = tcx_tiles_of_cta(ntiles);
+  mbar_wait(sm.bbar(0), 0);                                      // W hi / lo and c have landed (once)
+  const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(0) + 2 * TC_D * TC_D);
+  const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
+  float x[TC_D];
+  auto cn = load((int)blockIdx.x, x);
+  for (int it = 0; it < ntc; ++it) {
+    const int tile = (int)blockIdx.x + it * (int)gridDim.x;
+    const auto cc = cn;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      float h[16], l[16];
+#pragma unroll
+      for (int c4 = 0; c4 < 4; ++c4) {
+        const float4 mu = mu4[4 * q + c4];
+        const int c = 16 * q + 4 * c4;
+        const float d0 = x[c] - mu.x, d1 = x[c + 1] - mu.y, d2 = x[c + 2] - mu.z, d3 = x[c + 3] - mu.w;
+        h[4 * c4] = tf32_rna(d0); h[4 * c4 + 1] = tf32_rna(d1); h[4 * c4 + 2] = tf32_rna(d2); h[4 * c4 + 3] = tf32_rna(d3);
+        // d - hi is exact in fp32 with at most 13 significant bits; the MMA reads its top 11 (residual 2^-22 |d|)
+        l[4 * c4] = d0 - h[4 * c4]; l[4 * c4 + 1] = d1 - h[4 * c4 + 1]; l[4 * c4 + 2] = d2 - h[4 * c4 + 2]; l[4 * c4 + 3] = d3 - h[4 * c4 + 3];
+      }
+      tc_st16(lane_base + 64 + 16 * q, h);
+      tc_st16(lane_base + 128 + 16 * q, l);
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    group_sync(g);   // all 128 rows of the operand are written; every thread has read the previous tile's accumulators
+    if (wg0 && elect_one()) {
+      asm volatile("tcgen05.fence::after_thread_sync;");
+#pragma unroll
+      for (int pr = 0; pr < 3; ++pr) {
+        const uint32_t a0 = (pr == 1) ? acol_lo : acol_hi;
+        const uint64_t b0 = (pr == 2) ? dBl : dBh;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          tc_mma_ts(dcol, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
+      }
+      tc_commit(sm.mbar(g));
+    }
+    __syncwarp();
+    if (it + 1 < ntc) cn = load(tile + (int)gridDim.x, x);   // global loads in flight under the MMAs
+    mbar_wait(sm.mbar(g), it & 1);
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    uint32_t r[64];
+    tc_ld16(lane_base, r, 0); tc_ld16(lane_base, r, 1); tc_ld16(lane_base, r, 2); tc_ld16(lane_base, r, 3);
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll
+    for (int n = 0; n < 64; n += 4) {
+      const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
+                  z3 = __uint_as_float(r[n + 3]);
+      q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+    }
+    finish(tile, -0.5f * ((q0 + q1) + (q2 + q3)), cc);
+  }
+}
+
 // Run the evaluator over `ntiles` tiles of 256 points; called by every thread of the CTA after tc_begin.
 //   GMM_FULL: persistent x-stationary form, any grid <= ntiles;  QUAD: one tile per CTA (grid = ntiles).
 template <int OBJ, class Load, class Finish>
@@ -683,12 +651,15 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
       const float f = tc_rff_tile(o, sm, x, t, use);
       finish(tile, f, c);
     }
-  } else {
-    if (t >= TC_PTS) { tc_loader(o, sm, t); return; }
-    float x[TC_D];
-    const auto c = load((int)blockIdx.x, x);
-    const float f = tc_eval_tile<OBJ>(o, sm, x, t);
-    finish((int)blockIdx.x, f, c);
+  } else {   // QUAD: persistent, the record is loaded once
+    if (t >= TC_PTS) {
+      if (t == TC_PTS) {
+        mbar_expect_tx(sm.bbar(0), TC_REC_BYTES);
+        bulk_g2s(sm.B(0), o.recs, TC_REC_BYTES, sm.bbar(0));
+      }
+      return;
+    }
+    tc_quad_run(o, sm, t, ntiles, load, finish);
   }
 }
 template <int OBJ>

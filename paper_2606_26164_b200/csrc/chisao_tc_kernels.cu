@@ -250,8 +250,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
 
 // ---- launchers ------------------------------------------------------------------------------------------------
 static int g_tc_sms = 148;
-static inline int tc_grid(int obj_id, int ntiles) {   // GMM_FULL and RFF run persistent CTAs, one per SM
-  return ((obj_id == CHISAO_OBJ_GMM_FULL || obj_id == CHISAO_OBJ_RFF) && ntiles > g_tc_sms) ? g_tc_sms : ntiles;
+static inline int tc_grid(int obj_id, int ntiles) {   // persistent CTAs, one per SM
+  (void)obj_id;
+  return ntiles > g_tc_sms ? g_tc_sms : ntiles;
 }
 cudaError_t tc_configure() {
   cudaError_t e;
