@@ -148,7 +148,7 @@ def run_ours(args, rank, local_rank, world):
     K, W, c = args.steps, args.warmup, args.config
     full = inputs.config(c)
     N = args.N or full.hp.N
-    n_osc = max(full.hp.n_osc, K + W + 1)                   # timed cycles are all full cycles (phases 1-6)
+    n_osc = max(full.hp.n_osc, 2 * K + W + 1)               # timed cycles are all full cycles (phases 1-6)
     wl = replicas.replica_workload(c, rank, N=N, n_osc=n_osc)
     hp = wl.hp
 
@@ -157,7 +157,9 @@ def run_ours(args, rank, local_rank, world):
     for _ in range(W):
         g.step(stats=False)
     st0 = g.stats()
-    g.timing_enable(True); g.timing_reset()
+    # only the two roofline kernels are bracketed with events inside the timed region (two event records per launch
+    # are measurable on the launch-bound configurations); the full per-phase table comes from a second pass below
+    g.timing_enable(("eval_fd", "lbfgs_direction")); g.timing_reset()
     l0 = g.launch_count()
     sampler = ClockSampler(local_rank); sampler.start()
     time.sleep(0.25)
@@ -177,6 +179,10 @@ def run_ours(args, rank, local_rank, world):
     launches = g.launch_count() - l0
     st1 = g.stats()
     phase_ms = g.timing()
+    g.timing_enable(True); g.timing_reset()                 # second pass: K more cycles with every kernel class bracketed
+    for _ in range(K):
+        g.step(stats=False)
+    phase_all = g.timing()
     g.timing_enable(False)
     evals = np.array(st1.evals[:], np.int64) - np.array(st0.evals[:], np.int64)
     ms_max = replicas.max_over_ranks(ms, dist if world > 1 else None, dev)
@@ -316,7 +322,8 @@ def run_ours(args, rank, local_rank, world):
             "e2e": {"value": world * hp.N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo},
             "gpu_launches": int(launches),
             "roofline": roofline, "hbm_kernel": hbm, "hbm_kernel_full_history": hbm_full,
-            "phase_ms_per_step": {k: round(v[0] / K, 4) for k, v in phase_ms.items()},
+            "phase_ms_per_step": {k: round(v[0] / K, 4) for k, v in phase_all.items()},
+            "phase_ms_note": "second pass of K cycles with every kernel class bracketed by events (not the timed region)",
             "cpu_baseline": cpu,
             "stencil_aware_separately": stencil,
         }

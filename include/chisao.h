@@ -205,9 +205,11 @@ CHISAO_API int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *va
 CHISAO_API uint64_t chisao_launch_count(const chisao_ctx *ctx);
 
 /* Device time in ms accumulated by the kernel class `which` since chisao_timing_reset, measured with CUDA
- * events on the context's stream when timing is enabled (chisao_timing_enable(ctx, 1)); also returns the
- * launch count of that class.  Classes: 0 eval_fd, 1 eval_points, 2 hlc, 3 lbfgs_direction,
- * 4 lbfgs_update, 5 stick/dedup/lists, 6 reseed.  Synchronises. */
+ * events on the context's stream when timing is enabled; also returns the launch count of that class.
+ * chisao_timing_enable(ctx, on): on = 0 off, 1 every class, otherwise a mask with bit k + 1 selecting class k
+ * (bracketing costs two event records per launch: measurable on the launch-bound configurations).
+ * Classes: 0 eval_fd, 1 eval_points, 2 hlc, 3 lbfgs_direction, 4 lbfgs_update, 5 stick/dedup/lists,
+ * 6 reseed.  chisao_timing_get synchronises. */
 CHISAO_API int chisao_timing_enable(chisao_ctx *ctx, int32_t on);
 CHISAO_API int chisao_timing_reset(chisao_ctx *ctx);
 CHISAO_API int chisao_timing_get(chisao_ctx *ctx, int32_t which, double *ms, uint64_t *launches);

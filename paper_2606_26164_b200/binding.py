@@ -245,8 +245,13 @@ class Chisao:
     def launch_count(self) -> int:
         return int(self._L.chisao_launch_count(self._h))
 
-    def timing_enable(self, on: bool = True):
-        self._ck(self._L.chisao_timing_enable(self._h, 1 if on else 0))
+    def timing_enable(self, on=True):
+        """on: False / True (every kernel class) or an iterable of class names from TIMING_CLASSES"""
+        if isinstance(on, (bool, int)):
+            v = 1 if on else 0
+        else:
+            v = sum(1 << (TIMING_CLASSES.index(name) + 1) for name in on)
+        self._ck(self._L.chisao_timing_enable(self._h, v))
 
     def timing_reset(self):
         self._ck(self._L.chisao_timing_reset(self._h))

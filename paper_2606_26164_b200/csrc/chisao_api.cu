@@ -46,7 +46,7 @@ struct chisao_ctx {
   bool stencil_aware = false;   // chisao_set_option(CHISAO_OPT_STENCIL_AWARE): FD gradients by chisao_stencil.cu
   std::string err;
   uint64_t launches = 0;
-  bool timing = false;
+  uint32_t timing = 0;   // bit k: kernel class k is bracketed with CUDA events
   std::vector<TimedRec> recs;
   std::vector<cudaEvent_t> pool;
   size_t ws_bytes = 0;
@@ -115,7 +115,7 @@ bool rff_tc_scales(const chisao_objective &o, const chisao_config &c, int *ex_ou
   std::frexp(xmax, &ex);   // xmax = m 2^ex, m in [0.5, 1): xmax < 2^ex (or = 2^(ex-1): still inside the 4x headroom)
   std::frexp(wmax, &ew);
   ew += 0;
-  if (ex < -6 || ex > 10 || ew < -6 || ew > 10) return false;
+  if (ex < -6 || ex > 10 || ew < -6 || ew > 10 || ex + ew > 14) return false;   // uA = 2^(ex+ew-18) <= 1/16: 2 pi / uA > 100
   if (ex_out) *ex_out = ex;
   if (ew_out) *ew_out = ew;
   return true;
@@ -293,7 +293,7 @@ void pack_tcx16_records(const chisao_objective &o, std::vector<float> &out) {
 }
 // RFF record (chisao_tc.cuh, tc_rff_tile): the frequencies cut into three 10-bit fixed-point pieces
 // w = 2^(ew-9) (m0 + 2^-10 m1 + 2^-20 m2) (fp64 arithmetic on the fp32 inputs: every step exact), stored as the fp16
-// images m0 | m1 | 2^-10 m2, element (n, c) of an image at 16-bit index (c/8)*2048 + n*8 + (c%8); then (a_n, b_n)
+// images m0 | m1 | 2^-10 m2, element (n, c) of an image at 16-bit index (c/8)*2048 + n*8 + (c%8); then the constants
 void pack_rff_records(const chisao_objective &o, int ew, std::vector<float> &out) {
   out.assign(RFF_REC_FLOATS, 0.0f);
   uint16_t *img = reinterpret_cast<uint16_t *>(out.data());
@@ -309,8 +309,10 @@ void pack_rff_records(const chisao_objective &o, int ew, std::vector<float> &out
       img[8192 + idx] = __half_as_ushort(__float2half_rn((float)m1));
       img[16384 + idx] = __half_as_ushort(__float2half_rn((float)(m2 / 1024.0)));
     }
-    out[RFF_W_BYTES / 4 + 2 * n] = o.vec_a[n];
-    out[RFF_W_BYTES / 4 + 2 * n + 1] = o.vec_b[n];
+    float *pr = out.data() + RFF_W_BYTES / 4 + 8 * (n / 2);   // per feature pair: (b0/2pi, b1/2pi, b0, b1) (a0, a1, 0, 0)
+    pr[n & 1] = (float)((double)o.vec_b[n] / 6.283185307179586476925);
+    pr[2 + (n & 1)] = o.vec_b[n];
+    pr[4 + (n & 1)] = o.vec_a[n];
   }
 }
 // fp16 hi / lo carries 22 bits like tf32 hi / lo as long as nothing overflows (65504) and the lo parts stay above the
@@ -334,7 +336,7 @@ bool fp16_split_ok(const chisao_objective &o, const chisao_config &c) {
 struct Scope {   // optional CUDA-event bracket around a launch group
   chisao_ctx *c; int cls; cudaEvent_t a = nullptr, b = nullptr;
   Scope(chisao_ctx *ctx, int k) : c(ctx), cls(k) {
-    if (!c->timing) return;
+    if (!(c->timing & (1u << k))) return;
     auto get = [&]() { cudaEvent_t e; if (!c->pool.empty()) { e = c->pool.back(); c->pool.pop_back(); } else cudaEventCreate(&e); return e; };
     a = get(); b = get();
     cudaEventRecord(a, c->stream);
@@ -584,6 +586,8 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
       pack_rff_records(*obj, ew, ctx->tc_host);
       ctx->tc.rff_S0 = std::ldexp(1.0f, 9 - ex); ctx->tc.rff_uA = std::ldexp(1.0f, ex + ew - 18);
       ctx->tc.rff_s0 = obj->scalar0; ctx->tc.nchunk = (obj->K + 63) / 64;
+      const double uA = std::ldexp(1.0, ex + ew - 18), P = 6.283185307179586476925 / uA, Phi = std::nearbyint(P);
+      ctx->tc.rff_cA = (float)(uA / 6.283185307179586476925); ctx->tc.rff_Phi = (float)Phi; ctx->tc.rff_cL = (float)(-(P - Phi) * uA);
     } else if (ctx->tc.f16) pack_tcx16_records(*obj, ctx->tc_host);
     else if (obj->id == CHISAO_OBJ_GMM_FULL) pack_tcx_records(*obj, ctx->tc_host);
     else pack_tc_records(*obj, ctx->tc_host);
@@ -829,7 +833,7 @@ uint64_t chisao_launch_count(const chisao_ctx *ctx) { return ctx ? ctx->launches
 
 int chisao_timing_enable(chisao_ctx *ctx, int32_t on) {
   if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
-  ctx->timing = on != 0;
+  ctx->timing = on == 1 ? 0xFFFFFFFFu : (on <= 0 ? 0u : ((uint32_t)on >> 1));   // 1: every class; else bit k + 1 selects class k
   return CHISAO_OK;
 }
 int chisao_timing_reset(chisao_ctx *ctx) {

@@ -43,10 +43,10 @@ constexpr int TCX_PART_BYTES = 2 * 2 * 2 * TC_GROUP * 8;   // [tile parity][half
 constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES + TCX_PART_BYTES;   // >= the 2 x TC_REC form
 static_assert(2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES >= 2 * TC_REC_BYTES, "shared-memory carve");
 static_assert(3 * TCX16_W_BYTES <= 2 * TCX_W_BYTES, "three fp16 stages fit the two tf32 stages");
-// RFF form: three fixed-point fp16 images of the frequencies [3][4 K-chunks][256 rows][8], then (a_j, b_j) pairs
+// RFF form: three fixed-point fp16 images of the frequencies [3][4 K-chunks][256 rows][8], then the per-feature constants
 constexpr int RFF_TC_D = 32, RFF_TC_K = 256;
 constexpr int RFF_W_BYTES = 3 * RFF_TC_K * RFF_TC_D * 2;   // 49 152
-constexpr int RFF_REC_BYTES = RFF_W_BYTES + RFF_TC_K * 8;  // 51 200
+constexpr int RFF_REC_BYTES = RFF_W_BYTES + RFF_TC_K * 16; // 53 248: + per feature pair (b0/2pi, b1/2pi, b0, b1) (a0, a1, 0, 0)
 constexpr int RFF_REC_FLOATS = RFF_REC_BYTES / 4;
 constexpr int RFF_X_BYTES = 4 * TC_GROUP * RFF_TC_D * 2;   // four point images of a group (canonical K-major layout), 32 768
 static_assert(RFF_REC_BYTES + 2 * RFF_X_BYTES <= 2 * TCX_W_BYTES, "RFF carve fits the W stage region");
@@ -62,6 +62,7 @@ struct TcObj {
   float rff_S0;           // 2^(9 - ex): x * S0 rounds to the first 10-bit piece (|x| < 2^ex)
   float rff_uA;           // 2^(ex + ew - 18): value of one unit of the exact accumulator (|w| < 2^ew)
   float rff_s0;           // coefficient of -||x||^2
+  float rff_cA, rff_Phi, rff_cL;   // uA / 2 pi;  P_hi = rint(2 pi / uA);  -(2 pi / uA - P_hi) uA   (range reduction, tc_rff_tile)
   int32_t nchunk;         // ceil(K / 64) feature chunks
 };
 
@@ -77,6 +78,7 @@ struct TcSmem {
   __device__ __forceinline__ uint64_t *dbar(int g) const { return reinterpret_cast<uint64_t *>(base) + 10 + g; }   // accumulators drained
   __device__ __forceinline__ uint64_t *cbar(int r) const { return reinterpret_cast<uint64_t *>(base) + 12 + r; }   // c / a ring slot landed
   __device__ __forceinline__ uint64_t *xbar(int g) const { return reinterpret_cast<uint64_t *>(base) + 16 + g; }   // X image of the tile written
+  __device__ __forceinline__ uint64_t *rdbar(int gs) const { return reinterpret_cast<uint64_t *>(base) + 24 + gs; }  // RFF: stage (g, s) read out (4 warps)
   __device__ __forceinline__ unsigned char *scratch() const { return base + 1024; }
   __device__ __forceinline__ float *B(int st) const {
     return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * TC_REC_BYTES);
@@ -209,6 +211,7 @@ __device__ __forceinline__ void tc_setup(const TcSmem &sm, int t, int fbar_count
     mbar_init(sm.dbar(0), 8); mbar_init(sm.dbar(1), 8); mbar_init(sm.xbar(0), 4); mbar_init(sm.xbar(1), 4);
     mbar_init(sm.cbar(0), 1); mbar_init(sm.cbar(1), 1); mbar_init(sm.cbar(2), 1); mbar_init(sm.cbar(3), 1);
     for (int st = 0; st < 3; ++st) { mbar_init(sm.bbarx(st), 1); mbar_init(sm.fbarx(st), 1); }
+    for (int gs = 0; gs < 4; ++gs) mbar_init(sm.rdbar(gs), 4);
     mbar_fence_init();
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
@@ -443,9 +446,10 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
 // t = 2^(ex+ew-18) (A + 2^-10 BC) + b; dropped: 2^-30 (n1 m2 + n2 m1 + ...), below 1e-6 |x|max |w|max.  The range
 // reduction t - 2 pi k is exact on the A part (Cody-Waite with 2 pi = 201/32 + rest), so the angle handed to the
 // hardware cosine carries one fp32 rounding, like the fp64 path's.  Point images go to shared memory in the canonical
-// K-major layout (generic stores + fence.proxy.async); the frequencies' images and (a, b) are loaded once per CTA
-// (persistent over tiles).  Group g: accumulator stages s = 0, 1 at TMEM columns 256 g + 128 s (A 64 | BC 64); chunk
-// c + 1 is issued before chunk c is drained, and the other group's MMAs run under this group's arithmetic.
+// K-major layout (generic stores + fence.proxy.async); the frequencies' images and the per-feature constants are loaded
+// once per CTA (persistent over tiles).  Group g: accumulator stages s = 0, 1 at TMEM columns 256 g + 128 s (A 64 | BC 64).
+// Warp 9 issues the MMAs (rff_issuer) one stage ahead of the drain; the compute warps never meet at a barrier: they wait
+// on "MMAs retired" and arrive on "stage read out" / "images written" mbarriers, warp by warp.
 // round to nearest integer for |v| < 2^22: two full-rate additions instead of a conversion-pipe FRND
 __device__ __forceinline__ float rint_magic(float v) { return (v + 12582912.0f) - 12582912.0f; }
 __device__ __forceinline__ void rff_split(float v, float S0, float U0, float &n0, float &n1, float &n2) {
@@ -459,15 +463,77 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
   const __half2 h = __floats2half2_rn(lo, hi);
   return *reinterpret_cast<const uint32_t *>(&h);
 }
+// packed fp32 pairs (sm_100 FFMA2 / FADD2: two IEEE fma / add per issue slot)
+__device__ __forceinline__ uint64_t pk2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+
+// MMA issuer of the RFF form (warp 9, warp-uniform control flow, one elected lane issues): chunk c of group g goes to
+// accumulator stage c & 1 as soon as the group's point images are written (xbar) and that stage has been read out
+// (rdbar); tcgen05.commit signals cbar(2 g + stage).
+__device__ __forceinline__ void rff_issuer(const TcObj &o, const TcSmem &sm, int ntc) {
+  mbar_wait(sm.bbar(0), 0);                                      // the frequencies' images have landed
+  const uint32_t tm = *sm.tmem();
+  const int nch = o.nchunk;
+  unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
+  const uint32_t wa = smem_u32(wbase), xa = wa + RFF_REC_BYTES;
+  for (int it = 0; it < ntc; ++it)
+    for (int c = 0; c < nch; ++c) {
+      const int st = c & 1;
+      const int n = it * (st ? nch / 2 : (nch + 1) / 2) + (c >> 1);   // earlier issues into this stage
+      const uint64_t dW = tc_desc(wa + (uint32_t)(c * 1024), 4096, 128);
+#pragma unroll 1
+      for (int g = 0; g < 2; ++g) {
+        if (c == 0) mbar_wait(sm.xbar(g), it & 1);
+        if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        if (elect_one()) {
+          const uint64_t dX = tc_desc(xa + (uint32_t)(g * RFF_X_BYTES), 2048, 128);
+          const uint32_t accA = tm + (uint32_t)(g * 256 + 128 * st), accBC = accA + 64;
+#pragma unroll
+          for (int ks = 0; ks < 2; ++ks)
+            tc_mma_ss_f16(accA, dX + (uint64_t)(ks * 256), dW + (uint64_t)(ks * 512), TC_IDESC_F16_N64, ks ? 1u : 0u);
+#pragma unroll
+          for (int pr = 0; pr < 5; ++pr) {   // (n0, m1) (n1, m0) (2^-10 n1, m1) (n0, 2^-10 m2) (2^-10 n2, m0)
+            const int xp = (pr == 0 || pr == 3) ? 0 : (pr == 1 ? 1 : (pr == 2 ? 2 : 3));
+            const int wp = (pr == 0 || pr == 2) ? 1 : (pr == 3 ? 2 : 0);
+#pragma unroll
+            for (int ks = 0; ks < 2; ++ks)
+              tc_mma_ss_f16(accBC, dX + (uint64_t)(xp * 512 + ks * 256), dW + (uint64_t)(wp * 1024 + ks * 512), TC_IDESC_F16_N64,
+                            (pr | ks) ? 1u : 0u);
+          }
+          tc_commit(sm.cbar(2 * g + st));
+        }
+        __syncwarp();
+      }
+    }
+}
+
+// compute side of one tile: the thread's point -> its row of the four images; then per 64-feature chunk: wait for the
+// MMAs, read A and BC out of TMEM (the stage is handed back as soon as the second half is in registers), and per
+// feature pair (packed fp32):  k = rint(A cA + b / 2 pi);  r = A - k P_hi (exact integers);
+//                              angle = r uA + (k cL + (BC uB + b));  s += a cos(angle)
+// with P_hi = rint(2 pi / uA), cL = -(2 pi / uA - P_hi) uA, cA = uA / 2 pi.
 __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t, uint32_t (&use)[2]) {
   const uint32_t tm = *sm.tmem();
-  const int g = t >> 7, tl = t & (TC_GROUP - 1);
-  const bool wg0 = __shfl_sync(0xffffffffu, tl >> 5, 0) == 0;   // provably warp-uniform
+  const int g = t >> 7, tl = t & (TC_GROUP - 1), lane = t & 31;
   const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
-  const uint32_t gcol = tm + (uint32_t)(g * 256);
   unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
   unsigned char *ximg = wbase + RFF_REC_BYTES + g * RFF_X_BYTES;
-  const float2 *ab2 = reinterpret_cast<const float2 *>(wbase + RFF_W_BYTES);
+  const float4 *prm = reinterpret_cast<const float4 *>(wbase + RFF_W_BYTES);   // per feature pair: (bt0, bt1, b0, b1) (a0, a1, 0, 0)
   const float S0 = o.rff_S0, U0 = 1.0f / S0;
   float nrm = 0.0f;
   // the thread's row of the four point images: n0 | n1 | 2^-10 n1 | 2^-10 n2
@@ -492,9 +558,14 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
     *reinterpret_cast<uint4 *>(dst + 24576) = make_uint4(i2s[0], i2s[1], i2s[2], i2s[3]);
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core's reads
-  const float uA = o.rff_uA, uB = o.rff_uA * (1.0f / 1024.0f);
-  float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-  auto drain = [&](int c) {
+  __syncwarp();
+  if (lane == 0) mbar_arrive(sm.xbar(g));
+  const uint64_t cA2 = pk2(o.rff_cA, o.rff_cA), nP2 = pk2(-o.rff_Phi, -o.rff_Phi), cL2 = pk2(o.rff_cL, o.rff_cL);
+  const uint64_t uA2 = pk2(o.rff_uA, o.rff_uA), uB2 = pk2(o.rff_uA * (1.0f / 1024.0f), o.rff_uA * (1.0f / 1024.0f));
+  const uint64_t mg2 = pk2(12582912.0f, 12582912.0f), nmg2 = pk2(-12582912.0f, -12582912.0f);
+  uint64_t sA = pk2(0.f, 0.f), sB = pk2(0.f, 0.f);
+  const int nch = o.nchunk;
+  for (int c = 0; c < nch; ++c) {
     const int st = c & 1;
     mbar_wait(sm.cbar(2 * g + st), use[st] & 1);
     use[st] += 1;
@@ -505,51 +576,32 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
       const uint32_t ta = lane_base + (uint32_t)(128 * st + 32 * hh);
       tc_ld16s(ta, r, 0); tc_ld16s(ta + 16, r, 1); tc_ld16s(ta + 64, r, 2); tc_ld16s(ta + 80, r, 3);
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-      const float2 *ab = ab2 + 64 * c + 32 * hh;
+      if (hh == 1) {   // both halves are out of TMEM: the issuer may overwrite this stage
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.rdbar(2 * g + st));
+      }
+      const float4 *pp = prm + 2 * (32 * c + 16 * hh);
 #pragma unroll
-      for (int n = 0; n < 32; ++n) {
-        const float2 p = ab[n];                                       // a_j, b_j (broadcast)
-        const float rest = fmaf(__uint_as_float(r[32 + n]), uB, p.y);
-        const float tA = __uint_as_float(r[n]) * uA;                  // exact
-        const float kq = rint_magic((tA + rest) * 0.15915494309189535f);
-        float red = fmaf(-kq, 6.28125f, tA);                          // exact: multiples of min(uA, 2^-5), |red| small
-        red = fmaf(-kq, 1.9353071795864769e-3f, red);
-        const float cs = __cosf(red + rest);
-        if ((n & 3) == 0) s0 = fmaf(p.x, cs, s0);
-        else if ((n & 3) == 1) s1 = fmaf(p.x, cs, s1);
-        else if ((n & 3) == 2) s2 = fmaf(p.x, cs, s2);
-        else s3 = fmaf(p.x, cs, s3);
+      for (int n = 0; n < 32; n += 2) {
+        const float4 p0 = pp[n], p1 = pp[n + 1];                       // (bt0, bt1, b0, b1), (a0, a1, -, -): broadcast
+        const uint64_t A2 = pk2(__uint_as_float(r[n]), __uint_as_float(r[n + 1]));
+        const uint64_t B2 = pk2(__uint_as_float(r[32 + n]), __uint_as_float(r[33 + n]));
+        const uint64_t kq = add2(add2(fma2(A2, cA2, pk2(p0.x, p0.y)), mg2), nmg2);
+        const uint64_t red = fma2(kq, nP2, A2);                        // exact (integers below 2^24)
+        const uint64_t rest = fma2(B2, uB2, pk2(p0.z, p0.w));
+        const uint64_t ang = fma2(red, uA2, fma2(kq, cL2, rest));
+        float g0, g1;
+        upk2(ang, g0, g1);
+        const uint64_t cs = pk2(__cosf(g0), __cosf(g1));
+        if (n & 2) sB = fma2(pk2(p1.x, p1.y), cs, sB);
+        else sA = fma2(pk2(p1.x, p1.y), cs, sA);
       }
     }
-    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
-  };
-  const int nch = o.nchunk;
-  for (int c = 0; c < nch; ++c) {
-    group_sync(g);   // c = 0: the images of all 128 rows are written; c >= 2: every thread has drained chunk c - 2
-    if (wg0 && elect_one()) {
-      asm volatile("tcgen05.fence::after_thread_sync;");
-      const uint64_t dX = tc_desc(smem_u32(ximg), 2048, 128);
-      const uint64_t dW = tc_desc(smem_u32(wbase) + (uint32_t)(c * 1024), 4096, 128);
-      const uint32_t accA = gcol + (uint32_t)(128 * (c & 1)), accBC = accA + 64;
-#pragma unroll
-      for (int ks = 0; ks < 2; ++ks)
-        tc_mma_ss_f16(accA, dX + (uint64_t)(ks * 256), dW + (uint64_t)(ks * 512), TC_IDESC_F16_N64, ks ? 1u : 0u);
-#pragma unroll
-      for (int pr = 0; pr < 5; ++pr) {
-        const int xp = (pr == 0 || pr == 3) ? 0 : (pr == 1 ? 1 : (pr == 2 ? 2 : 3));
-        const int wp = (pr == 0 || pr == 2) ? 1 : (pr == 3 ? 2 : 0);
-#pragma unroll
-        for (int ks = 0; ks < 2; ++ks)
-          tc_mma_ss_f16(accBC, dX + (uint64_t)(xp * 512 + ks * 256), dW + (uint64_t)(wp * 1024 + ks * 512), TC_IDESC_F16_N64,
-                        (pr | ks) ? 1u : 0u);
-      }
-      tc_commit(sm.cbar(2 * g + (c & 1)));
-    }
-    __syncwarp();
-    if (c > 0) drain(c - 1);
   }
-  drain(nch - 1);
-  return fmaf(-o.rff_s0, nrm, (s0 + s1) + (s2 + s3));
+  float a0, a1, b0, b1;
+  upk2(sA, a0, a1); upk2(sB, b0, b1);
+  return fmaf(-o.rff_s0, nrm, (a0 + a1) + (b0 + b1));
 }
 
 // ---- QUAD (K = 1), persistent form ----------------------------------------------------------------------------------
@@ -633,16 +685,18 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
     else if (warp == TC_PTS / 32) { if (t == TC_PTS) tcx_loader(o, sm, ntc); }
     else tcx_issuer(o, sm, ntc);
   } else if constexpr (OBJ == CHISAO_OBJ_RFF) {
-    // persistent over tiles; the frequencies' images and (a, b) land once (51 200 bytes)
-    if (t >= TC_PTS) {
+    // persistent over tiles; the frequencies' images and the per-feature constants land once (53 248 bytes)
+    const int ntc = tcx_tiles_of_cta(ntiles);
+    const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+    if (warp == TC_PTS / 32) {
       if (t == TC_PTS) {
         mbar_expect_tx(sm.bbar(0), RFF_REC_BYTES);
         bulk_g2s(sm.Bx(0, 0), o.recs, RFF_REC_BYTES, sm.bbar(0));
       }
       return;
     }
+    if (warp > TC_PTS / 32) { rff_issuer(o, sm, ntc); return; }
     mbar_wait(sm.bbar(0), 0);
-    const int ntc = tcx_tiles_of_cta(ntiles);
     uint32_t use[2] = {0u, 0u};
     for (int it = 0; it < ntc; ++it) {
       const int tile = (int)blockIdx.x + it * (int)gridDim.x;
