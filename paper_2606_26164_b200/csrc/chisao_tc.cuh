@@ -173,13 +173,13 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[64], int q
       : "r"(taddr + 16 * q));
 }
 
-__device__ __forceinline__ void tc_ld16s(uint32_t taddr, uint32_t (&r)[64], int q) {   // 16 columns at taddr -> r[16 q ..]
+__device__ __forceinline__ void tc_ld16h(uint32_t taddr, uint32_t (&r)[32], int h) {   // 16 columns at taddr -> r[16 h ..]
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-      : "=r"(r[16 * q + 0]), "=r"(r[16 * q + 1]), "=r"(r[16 * q + 2]), "=r"(r[16 * q + 3]), "=r"(r[16 * q + 4]),
-        "=r"(r[16 * q + 5]), "=r"(r[16 * q + 6]), "=r"(r[16 * q + 7]), "=r"(r[16 * q + 8]), "=r"(r[16 * q + 9]),
-        "=r"(r[16 * q + 10]), "=r"(r[16 * q + 11]), "=r"(r[16 * q + 12]), "=r"(r[16 * q + 13]), "=r"(r[16 * q + 14]),
-        "=r"(r[16 * q + 15])
+      : "=r"(r[16 * h + 0]), "=r"(r[16 * h + 1]), "=r"(r[16 * h + 2]), "=r"(r[16 * h + 3]), "=r"(r[16 * h + 4]),
+        "=r"(r[16 * h + 5]), "=r"(r[16 * h + 6]), "=r"(r[16 * h + 7]), "=r"(r[16 * h + 8]), "=r"(r[16 * h + 9]),
+        "=r"(r[16 * h + 10]), "=r"(r[16 * h + 11]), "=r"(r[16 * h + 12]), "=r"(r[16 * h + 13]), "=r"(r[16 * h + 14]),
+        "=r"(r[16 * h + 15])
       : "r"(taddr));
 }
 
@@ -527,7 +527,7 @@ __device__ __forceinline__ void rff_issuer(const TcObj &o, const TcSmem &sm, int
 // feature pair (packed fp32):  k = rint(A cA + b / 2 pi);  r = A - k P_hi (exact integers);
 //                              angle = r uA + (k cL + (BC uB + b));  s += a cos(angle)
 // with P_hi = rint(2 pi / uA), cL = -(2 pi / uA - P_hi) uA, cA = uA / 2 pi.
-__device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t, uint32_t (&use)[2]) {
+__device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t, int it) {
   const uint32_t tm = *sm.tmem();
   const int g = t >> 7, tl = t & (TC_GROUP - 1), lane = t & 31;
   const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
@@ -567,26 +567,30 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
   const int nch = o.nchunk;
   for (int c = 0; c < nch; ++c) {
     const int st = c & 1;
-    mbar_wait(sm.cbar(2 * g + st), use[st] & 1);
-    use[st] += 1;
+    const int nuse = it * (st ? nch / 2 : (nch + 1) / 2) + (c >> 1);   // earlier uses of this stage (as in rff_issuer)
+    mbar_wait(sm.cbar(2 * g + st), nuse & 1);
     asm volatile("tcgen05.fence::after_thread_sync;");
+    // 16 features at a time, the next 16 in flight from TMEM while these are worked on
+    uint32_t rb[2][32];
+    const uint32_t ta = lane_base + (uint32_t)(128 * st);
+    tc_ld16h(ta, rb[0], 0); tc_ld16h(ta + 64, rb[0], 1);
 #pragma unroll
-    for (int hh = 0; hh < 2; ++hh) {
-      uint32_t r[64];
-      const uint32_t ta = lane_base + (uint32_t)(128 * st + 32 * hh);
-      tc_ld16s(ta, r, 0); tc_ld16s(ta + 16, r, 1); tc_ld16s(ta + 64, r, 2); tc_ld16s(ta + 80, r, 3);
+    for (int q = 0; q < 4; ++q) {
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-      if (hh == 1) {   // both halves are out of TMEM: the issuer may overwrite this stage
+      if (q < 3) {
+        tc_ld16h(ta + 16 * (q + 1), rb[(q + 1) & 1], 0); tc_ld16h(ta + 64 + 16 * (q + 1), rb[(q + 1) & 1], 1);
+      } else {         // the whole stage is in registers: the issuer may overwrite it
         asm volatile("tcgen05.fence::before_thread_sync;");
         __syncwarp();
         if (lane == 0) mbar_arrive(sm.rdbar(2 * g + st));
       }
-      const float4 *pp = prm + 2 * (32 * c + 16 * hh);
+      const uint32_t (&r)[32] = rb[q & 1];
+      const float4 *pp = prm + 2 * (32 * c + 8 * q);
 #pragma unroll
-      for (int n = 0; n < 32; n += 2) {
+      for (int n = 0; n < 16; n += 2) {
         const float4 p0 = pp[n], p1 = pp[n + 1];                       // (bt0, bt1, b0, b1), (a0, a1, -, -): broadcast
         const uint64_t A2 = pk2(__uint_as_float(r[n]), __uint_as_float(r[n + 1]));
-        const uint64_t B2 = pk2(__uint_as_float(r[32 + n]), __uint_as_float(r[33 + n]));
+        const uint64_t B2 = pk2(__uint_as_float(r[16 + n]), __uint_as_float(r[17 + n]));
         const uint64_t kq = add2(add2(fma2(A2, cA2, pk2(p0.x, p0.y)), mg2), nmg2);
         const uint64_t red = fma2(kq, nP2, A2);                        // exact (integers below 2^24)
         const uint64_t rest = fma2(B2, uB2, pk2(p0.z, p0.w));
@@ -697,12 +701,11 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
     }
     if (warp > TC_PTS / 32) { rff_issuer(o, sm, ntc); return; }
     mbar_wait(sm.bbar(0), 0);
-    uint32_t use[2] = {0u, 0u};
     for (int it = 0; it < ntc; ++it) {
       const int tile = (int)blockIdx.x + it * (int)gridDim.x;
       float x[TC_D];
       const auto c = load(tile, x);
-      const float f = tc_rff_tile(o, sm, x, t, use);
+      const float f = tc_rff_tile(o, sm, x, t, it);
       finish(tile, f, c);
     }
   } else {   // QUAD: persistent, the record is loaded once
