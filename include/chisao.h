@@ -189,6 +189,12 @@ CHISAO_API int chisao_get_stats(chisao_ctx *ctx, chisao_stats *stats);
  * the same evaluations, but it is NOT a black-box evaluation of f: numbers obtained with it are
  * reported separately.  CHISAO_E_INVALID for other objectives or unknown options. */
 #define CHISAO_OPT_STENCIL_AWARE 1
+/* CHISAO_OPT_CUDA_GRAPH (default 1): chisao_step submits the cycle as ONE CUDA graph launch.  The launch sequence of a
+ * cycle is static (every kernel reads its counts from the device control block); it is captured on an internal stream
+ * that is forked from and joined to the caller's stream with events, and applied to the instantiated graph with
+ * cudaGraphExecUpdate (the cycle index is a kernel argument).  Results are identical to direct submission; direct
+ * submission is used while per-launch timing is enabled, by chisao_phase, and if the graph machinery fails. */
+#define CHISAO_OPT_CUDA_GRAPH 2
 CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value);
 
 /* Which evaluator the context runs (decided at chisao_init from the objective, d and the value ranges):
@@ -199,6 +205,7 @@ CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value)
  * with max |w| and the box radius + 8 sigma_s + h in [2^-7, 2^10]; CHISAO_RFF_FP64 in the environment keeps the
  * FP32-FMA evaluator with fp64 phases). */
 #define CHISAO_INFO_EVALUATOR 1
+#define CHISAO_INFO_GRAPH_LAUNCHES 2   /* cycles submitted as a CUDA graph so far */
 CHISAO_API int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value);
 
 /* Number of kernel launches this context has enqueued so far (host counter). */

@@ -21,7 +21,9 @@ P, LS_B, GHAT, HLC_F, RS_SRC, RS_CAND, XT, GR_Q, SIGMA = 20, 21, 25, 26, 27, 28,
 PH_RELEASE_EVAL, PH_STICK, PH_DEDUP, PH_RESEED, PH_HLC_STEP, PH_ANTI_STEP, PH_LBFGS_ITER = 1, 2, 3, 4, 5, 6, 11
 PH_LBFGS_DIRECTION = 12
 OPT_STENCIL_AWARE = 1
+OPT_CUDA_GRAPH = 2
 INFO_EVALUATOR = 1
+INFO_GRAPH_LAUNCHES = 2
 EVALUATOR_NAMES = ("fp32-fma", "tcgen05 3xTF32 (x - c)", "tcgen05 x-stationary tf32 hi/lo", "tcgen05 x-stationary fp16 hi/lo",
                    "tcgen05 exact fixed-point fp16 pieces (random-Fourier phases)")
 TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_update", "select", "reseed")
@@ -200,13 +202,20 @@ class Chisao:
         self._ck(self._L.chisao_phase(self._h, phase_id, it))
 
     def set_option(self, option: int, value: int):
-        """chisao_set_option (OPT_STENCIL_AWARE: opt-in stencil-aware FD evaluator, reported separately)."""
+        """chisao_set_option (OPT_STENCIL_AWARE: opt-in stencil-aware FD evaluator, reported separately;
+        OPT_CUDA_GRAPH: submit each cycle as one CUDA graph launch, default on)."""
         self._ck(self._L.chisao_set_option(self._h, int(option), int(value)))
 
     def evaluator(self) -> int:
         """chisao_get_info(INFO_EVALUATOR): index into EVALUATOR_NAMES"""
         v = C.c_int32(0)
         self._ck(self._L.chisao_get_info(self._h, INFO_EVALUATOR, C.byref(v)))
+        return int(v.value)
+
+    def graph_launches(self) -> int:
+        """chisao_get_info(INFO_GRAPH_LAUNCHES): cycles submitted as one CUDA graph launch so far"""
+        v = C.c_int32(0)
+        self._ck(self._L.chisao_get_info(self._h, INFO_GRAPH_LAUNCHES, C.byref(v)))
         return int(v.value)
 
     def stats(self) -> Stats:

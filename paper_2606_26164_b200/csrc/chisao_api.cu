@@ -50,6 +50,14 @@ struct chisao_ctx {
   std::vector<TimedRec> recs;
   std::vector<cudaEvent_t> pool;
   size_t ws_bytes = 0;
+  // one cycle as a CUDA graph (chisao_step): captured on an internal stream that is forked from / joined to the
+  // caller's stream with events, re-captured every cycle (the cycle index is a kernel argument) and applied to the
+  // instantiated graph with cudaGraphExecUpdate; slot 0 = full cycle, 1 = the short last cycle
+  bool graph_on = true;
+  cudaStream_t gstream = nullptr;
+  cudaEvent_t gfork = nullptr, gjoin = nullptr;
+  cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+  uint64_t graph_launches = 0;
 };
 
 namespace {
@@ -618,10 +626,8 @@ int chisao_seed_population(chisao_ctx *ctx) {
   return CHISAO_OK;
 }
 
-int chisao_step(chisao_ctx *ctx, chisao_stats *stats) {
-  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
-  if (ctx->cycle >= ctx->hp.n_osc) return fail(ctx, CHISAO_E_STATE, "all n_osc cycles already done");
-  ctx->cycle += 1;                                    // "for k = 1..n_osc" (PAPER.md:147)
+// the launch sequence of one cycle k = ctx->cycle on ctx->stream (Algorithm 1)
+static int enqueue_cycle(chisao_ctx *ctx) {
   int rc;
   if ((rc = run_release_eval(ctx))) return rc;        // Phase 1: release all, then converge
   for (int it = 1; it <= ctx->hp.n_conv; ++it)
@@ -637,6 +643,68 @@ int chisao_step(chisao_ctx *ctx, chisao_stats *stats) {
     for (int t = 1; t <= ctx->hp.n_anti; ++t)         // Phase 6
       if ((rc = run_anti(ctx, t))) return rc;
   }
+  return CHISAO_OK;
+}
+
+// The same sequence submitted as ONE graph launch: every launch already reads its counts from the device control
+// block, so the sequence is static; only the cycle index (a kernel argument) changes, hence capture + ExecUpdate per
+// cycle (host cost ~1 us per node instead of a launch each; the GPU runs the nodes back to back).  Any failure of the
+// graph machinery switches it off for the context and the cycle is submitted directly.
+static int step_graph(chisao_ctx *ctx) {
+  cudaStream_t user = ctx->stream;
+  auto give_up = [&]() { ctx->graph_on = false; cudaGetLastError(); return enqueue_cycle(ctx); };
+  if (!ctx->gstream) {
+    if (cudaStreamCreateWithFlags(&ctx->gstream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->gfork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->gjoin, cudaEventDisableTiming) != cudaSuccess)
+      return give_up();
+  }
+  if (cudaStreamBeginCapture(ctx->gstream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) return give_up();
+  ctx->stream = ctx->gstream;
+  const uint64_t l0 = ctx->launches;
+  const int rc = enqueue_cycle(ctx);
+  ctx->stream = user;
+  cudaGraph_t graph = nullptr;
+  const cudaError_t ec = cudaStreamEndCapture(ctx->gstream, &graph);
+  if (rc || ec != cudaSuccess || !graph) {
+    if (graph) cudaGraphDestroy(graph);
+    ctx->launches = l0;
+    if (rc) { ctx->graph_on = false; cudaGetLastError(); return rc; }
+    return give_up();
+  }
+  const int slot = ctx->cycle < ctx->hp.n_osc ? 0 : 1;
+  if (ctx->gexec[slot]) {
+    cudaGraphExecUpdateResultInfo info;
+    if (cudaGraphExecUpdate(ctx->gexec[slot], graph, &info) != cudaSuccess) {
+      cudaGetLastError();
+      cudaGraphExecDestroy(ctx->gexec[slot]);
+      ctx->gexec[slot] = nullptr;
+    }
+  }
+  if (!ctx->gexec[slot] && cudaGraphInstantiate(&ctx->gexec[slot], graph, 0) != cudaSuccess) {
+    ctx->gexec[slot] = nullptr;
+    cudaGraphDestroy(graph);
+    ctx->launches = l0;
+    return give_up();
+  }
+  cudaGraphDestroy(graph);
+  CK(cudaEventRecord(ctx->gfork, user));
+  CK(cudaStreamWaitEvent(ctx->gstream, ctx->gfork, 0));
+  CK(cudaGraphLaunch(ctx->gexec[slot], ctx->gstream));
+  CK(cudaEventRecord(ctx->gjoin, ctx->gstream));
+  CK(cudaStreamWaitEvent(user, ctx->gjoin, 0));
+  ctx->graph_launches += 1;
+  return CHISAO_OK;
+}
+
+int chisao_step(chisao_ctx *ctx, chisao_stats *stats) {
+  if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
+  if (ctx->cycle >= ctx->hp.n_osc) return fail(ctx, CHISAO_E_STATE, "all n_osc cycles already done");
+  ctx->cycle += 1;                                    // "for k = 1..n_osc" (PAPER.md:147)
+  // per-launch event bracketing (chisao_timing_enable) and CHISAO_DEBUG need the launches on the stream itself
+  const bool graph = ctx->graph_on && ctx->timing == 0 && ctx->st.N > 0 && !getenv("CHISAO_DEBUG");
+  const int rc = graph ? step_graph(ctx) : enqueue_cycle(ctx);
+  if (rc) return rc;
   if (stats) return read_stats(ctx, stats);
   return CHISAO_OK;
 }
@@ -820,10 +888,12 @@ int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value) {
     ctx->stencil_aware = value != 0;
     return CHISAO_OK;
   }
+  if (option == CHISAO_OPT_CUDA_GRAPH) { ctx->graph_on = value != 0; return CHISAO_OK; }
   return fail(ctx, CHISAO_E_INVALID, "unknown option");
 }
 
 int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value) {
+  if (ctx && value && which == CHISAO_INFO_GRAPH_LAUNCHES) { *value = (int32_t)ctx->graph_launches; return CHISAO_OK; }
   if (!ctx || !value || which != CHISAO_INFO_EVALUATOR) return CHISAO_E_INVALID;
   *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_RFF ? 4 : (ctx->obj.id == CHISAO_OBJ_QUAD ? 1 : (ctx->tc.f16 ? 3 : 2)));
   return CHISAO_OK;
@@ -864,6 +934,10 @@ void chisao_destroy(chisao_ctx *ctx) {
   if (!ctx) return;
   for (auto &r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto &e : ctx->pool) cudaEventDestroy(e);
+  for (auto &ge : ctx->gexec) if (ge) cudaGraphExecDestroy(ge);
+  if (ctx->gfork) cudaEventDestroy(ctx->gfork);
+  if (ctx->gjoin) cudaEventDestroy(ctx->gjoin);
+  if (ctx->gstream) cudaStreamDestroy(ctx->gstream);
   delete ctx;
 }
 

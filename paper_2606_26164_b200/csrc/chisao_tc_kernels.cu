@@ -149,12 +149,16 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
 __device__ __forceinline__ void hlc_normals(uint64_t seed, int i, int cycle, int iter, int k, int d, float (&u)[TC_D]) {
   const uint32_t tg = rng_tag(5, iter, PUR_HLC_U);
   const uint32_t n0 = (uint32_t)k * (uint32_t)d;
-  if (d == TC_D) {   // the draw's 64 normals are 16 whole Philox blocks: independent chains the scheduler can interleave
+  if ((d & 3) == 0) {   // the draw's d normals are d / 4 whole Philox blocks: independent chains the scheduler can interleave
 #pragma unroll
     for (int b = 0; b < TC_D / 4; ++b) {
-      const uint4 w = philox_block(seed, (n0 >> 2) + (uint32_t)b, (uint32_t)i, (uint32_t)cycle, tg);
-      box_muller(w.x, w.y, u[4 * b], u[4 * b + 1]);
-      box_muller(w.z, w.w, u[4 * b + 2], u[4 * b + 3]);
+      if (4 * b < d) {    // warp-uniform
+        const uint4 w = philox_block(seed, (n0 >> 2) + (uint32_t)b, (uint32_t)i, (uint32_t)cycle, tg);
+        box_muller(w.x, w.y, u[4 * b], u[4 * b + 1]);
+        box_muller(w.z, w.w, u[4 * b + 2], u[4 * b + 3]);
+      } else {
+        u[4 * b] = 0.f; u[4 * b + 1] = 0.f; u[4 * b + 2] = 0.f; u[4 * b + 3] = 0.f;
+      }
     }
     return;
   }

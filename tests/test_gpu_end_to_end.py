@@ -299,3 +299,21 @@ def test_next1_noise_robustness_workload(orc, B, sigma_noise, paper_err):
     for name in ("gpu", "orc"):
         assert np.mean(errs[name]) <= 6.0 * paper_err + 0.01, (name, float(np.mean(errs[name])))
     assert abs(np.mean(errs["gpu"]) - np.mean(errs["orc"])) <= 0.5 * max(np.mean(errs["orc"]), 0.01) + 0.02
+
+
+@pytest.mark.parametrize("c,N", [(1, 256), (2, 700), (3, 300), (5, 300)])
+def test_cycle_as_cuda_graph_is_bit_identical_to_direct_submission(B, c, N):
+    """chisao_step submits the cycle as one CUDA graph launch (captured per cycle, cudaGraphExecUpdate); the state
+    after every cycle, including the short last one (a second graph topology), equals direct submission bit for bit"""
+    wl = inputs.config(c, N=N, n_osc=4)
+    a, b = B.Chisao(wl), B.Chisao(wl)
+    b.set_option(B.OPT_CUDA_GRAPH, 0)
+    for k in range(4):
+        sa, sb = a.step(), b.step()
+        for fld in (B.X, B.F, B.G, B.STUCK):
+            assert np.array_equal(a.get(fld), b.get(fld)), (k, fld)
+        assert (sa.n_stuck, sa.k_lost, sa.n_active) == (sb.n_stuck, sb.k_lost, sb.n_active)
+        assert list(sa.evals) == list(sb.evals)
+    assert a.graph_launches() == 4 and b.graph_launches() == 0
+    assert a.launch_count() == b.launch_count()
+    a.close(); b.close()
