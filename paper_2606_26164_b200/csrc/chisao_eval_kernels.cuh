@@ -105,6 +105,43 @@ struct PtArgs {
   unsigned long long *evals;
 };
 
+// Line-search retry (R-4): the shrunk trial point x_t = clip(x + t p) of sample i and the directional decrease
+// -g . (x_t - x), accumulated in coordinate order.  Rows are fetched eight coordinates at a time (independent loads in
+// flight) before anything is stored: a scalar loop serialises on the L2 latency of every coordinate.
+__device__ __forceinline__ float ls_retry_row(const PtArgs &a, int i, int d, float tn) {
+  const float *__restrict__ xr = a.x + (size_t)i * d;
+  const float *__restrict__ pr = a.p + (size_t)i * d;
+  const float *__restrict__ gr = a.g + (size_t)i * d;
+  float *xt = a.xt + (size_t)i * d;
+  float dsum = 0.0f;
+  int j = 0;
+  if ((d & 3) == 0) {
+    for (; j + 8 <= d; j += 8) {
+      const float4 x0 = *reinterpret_cast<const float4 *>(xr + j), x1 = *reinterpret_cast<const float4 *>(xr + j + 4);
+      const float4 p0 = *reinterpret_cast<const float4 *>(pr + j), p1 = *reinterpret_cast<const float4 *>(pr + j + 4);
+      const float4 g0 = *reinterpret_cast<const float4 *>(gr + j), g1 = *reinterpret_cast<const float4 *>(gr + j + 4);
+      const float xo[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+      const float pv[8] = {p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w};
+      const float gv[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+      float xn[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        xn[e] = clipf(fmaf(tn, pv[e], xo[e]), a.lo[j + e], a.hi[j + e]);
+        dsum = fmaf(-gv[e], xn[e] - xo[e], dsum);
+      }
+      *reinterpret_cast<float4 *>(xt + j) = make_float4(xn[0], xn[1], xn[2], xn[3]);
+      *reinterpret_cast<float4 *>(xt + j + 4) = make_float4(xn[4], xn[5], xn[6], xn[7]);
+    }
+  }
+  for (; j < d; ++j) {
+    const float xo = xr[j];
+    const float xn = clipf(fmaf(tn, pr[j], xo), a.lo[j], a.hi[j]);
+    xt[j] = xn;
+    dsum = fmaf(-gr[j], xn - xo, dsum);
+  }
+  return dsum;
+}
+
 // ---- one point per sample: cycle-start centre value, or line-search trial b (R-4) ---------------------
 template <int OBJ, int DP>
 __global__ void __launch_bounds__(NT, 2) k_eval_points(const DevObj o, const PtArgs a) {
@@ -156,14 +193,7 @@ __global__ void __launch_bounds__(NT, 2) k_eval_points(const DevObj o, const PtA
         a.next_list[sr] = i;
         const float tn = a.tcur[i] * a.shrink;
         a.tcur[i] = tn;
-        float dsum = 0.0f;
-        for (int j = 0; j < d; ++j) {
-          const float xo = a.x[(size_t)i * d + j];
-          const float xn = clipf(fmaf(tn, a.p[(size_t)i * d + j], xo), a.lo[j], a.hi[j]);
-          a.xt[(size_t)i * d + j] = xn;
-          dsum = fmaf(-a.g[(size_t)i * d + j], xn - xo, dsum);
-        }
-        a.dec[i] = dsum;
+        a.dec[i] = ls_retry_row(a, i, d, tn);
       }
     }
   }

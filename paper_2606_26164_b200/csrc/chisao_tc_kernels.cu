@@ -128,14 +128,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
         a.next_list[sr] = i;
         const float tn = a.tcur[i] * a.shrink;
         a.tcur[i] = tn;
-        float dsum = 0.0f;
-        for (int j = 0; j < d; ++j) {
-          const float xo = a.x[(size_t)i * d + j];
-          const float xn = clipf(fmaf(tn, a.p[(size_t)i * d + j], xo), a.lo[j], a.hi[j]);
-          a.xt[(size_t)i * d + j] = xn;
-          dsum = fmaf(-a.g[(size_t)i * d + j], xn - xo, dsum);
-        }
-        a.dec[i] = dsum;
+        a.dec[i] = ls_retry_row(a, i, d, tn);
       }
     }
     if (t == 0)
