@@ -173,6 +173,15 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[64], int q
       : "r"(taddr + 16 * q));
 }
 
+__device__ __forceinline__ void tc_ld16s64(uint32_t taddr, uint32_t (&r)[64], int q) {   // 16 columns at taddr -> r[16 q ..]
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[16 * q + 0]), "=r"(r[16 * q + 1]), "=r"(r[16 * q + 2]), "=r"(r[16 * q + 3]), "=r"(r[16 * q + 4]),
+        "=r"(r[16 * q + 5]), "=r"(r[16 * q + 6]), "=r"(r[16 * q + 7]), "=r"(r[16 * q + 8]), "=r"(r[16 * q + 9]),
+        "=r"(r[16 * q + 10]), "=r"(r[16 * q + 11]), "=r"(r[16 * q + 12]), "=r"(r[16 * q + 13]), "=r"(r[16 * q + 14]),
+        "=r"(r[16 * q + 15])
+      : "r"(taddr));
+}
 __device__ __forceinline__ void tc_ld16h(uint32_t taddr, uint32_t (&r)[32], int h) {   // 16 columns at taddr -> r[16 h ..]
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
@@ -610,25 +619,50 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
 
 // ---- QUAD (K = 1), persistent form ----------------------------------------------------------------------------------
 // One record (W hi / lo, c) stays resident in shared memory; the CTA walks tiles blockIdx.x, blockIdx.x + gridDim.x, ...
-// Per tile a thread writes A = x - c (tf32 hi / lo) into its TMEM lane, the group's 24 MMAs (3xTF32, M128 N64 K8) fill
-// its 64 accumulator columns, and the next tile's point is fetched while they run.  The two groups alternate on the
-// tensor pipe.  TMEM per group (256 g): accumulators 64 | A_hi 64 | A_lo 64.
+// Per tile a thread writes A = x - c (tf32 hi / lo) into its TMEM lane and the group's 24 MMAs (3xTF32, M128 N64 K8) fill
+// one of the group's two accumulator stages.  Warp 9 issues (quad_issuer): tile n + 1 of a group is issued as soon as
+// its operand image is written (xbar) and its stage has been read out (rdbar), i.e. while the compute warps still
+// square, sum and finish tile n.  The compute warps never meet at a barrier; the point of tile n + 2 is fetched from
+// global memory right after tile n is finished and consumed after the wait for the MMAs of tile n + 1.  TMEM per group (256 g): A_hi 64 | A_lo 64 | accumulators 2 x 64.
+__device__ __forceinline__ void quad_issuer(const TcSmem &sm, int ntc) {
+  mbar_wait(sm.bbar(0), 0);                                      // W hi / lo and c have landed (once)
+  const uint32_t tm = *sm.tmem();
+  const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
+  for (int it = 0; it < ntc; ++it) {
+    const int st = it & 1, n = it >> 1;                          // n earlier issues into this stage
+#pragma unroll 1
+    for (int g = 0; g < 2; ++g) {
+      mbar_wait(sm.xbar(g), it & 1);                             // operand image of tile `it` written by the group's 4 warps
+      if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);   // accumulators of tile it - 2 are in registers
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      if (elect_one()) {
+        const uint32_t gcol = tm + (uint32_t)(g * 256), acc = gcol + 128 + (uint32_t)(64 * st);
+#pragma unroll
+        for (int pr = 0; pr < 3; ++pr) {
+          const uint32_t a0 = (pr == 1) ? gcol + 64 : gcol;
+          const uint64_t b0 = (pr == 2) ? dBl : dBh;
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks)
+            tc_mma_ts(acc, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
+        }
+        tc_commit(sm.cbar(2 * g + st));
+      }
+      __syncwarp();
+    }
+  }
+}
+
 template <class Load, class Finish>
 __device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish) {
   const uint32_t tm = *sm.tmem();
-  const int g = t >> 7, tl = t & (TC_GROUP - 1);
-  const bool wg0 = __shfl_sync(0xffffffffu, tl >> 5, 0) == 0;   // provably warp-uniform
+  const int g = t >> 7, lane = t & 31;
   const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
-  const uint32_t dcol = tm + (uint32_t)(g * 256), acol_hi = dcol + 64, acol_lo = dcol + 128;
   const int ntc = tcx_tiles_of_cta(ntiles);
-  mbar_wait(sm.bbar(0), 0);                                      // W hi / lo and c have landed (once)
+  const int stride = (int)gridDim.x;
+  mbar_wait(sm.bbar(0), 0);                                      // c has landed
   const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(0) + 2 * TC_D * TC_D);
-  const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
   float x[TC_D];
-  auto cn = load((int)blockIdx.x, x);
-  for (int it = 0; it < ntc; ++it) {
-    const int tile = (int)blockIdx.x + it * (int)gridDim.x;
-    const auto cc = cn;
+  auto write_a = [&]() {                                         // A = x - c as tf32 hi / lo -> the thread's TMEM lane
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       float h[16], l[16];
@@ -641,32 +675,30 @@ __device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, in
         // d - hi is exact in fp32 with at most 13 significant bits; the MMA reads its top 11 (residual 2^-22 |d|)
         l[4 * c4] = d0 - h[4 * c4]; l[4 * c4 + 1] = d1 - h[4 * c4 + 1]; l[4 * c4 + 2] = d2 - h[4 * c4 + 2]; l[4 * c4 + 3] = d3 - h[4 * c4 + 3];
       }
-      tc_st16(lane_base + 64 + 16 * q, h);
-      tc_st16(lane_base + 128 + 16 * q, l);
+      tc_st16(lane_base + 16 * q, h);
+      tc_st16(lane_base + 64 + 16 * q, l);
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;");
-    group_sync(g);   // all 128 rows of the operand are written; every thread has read the previous tile's accumulators
-    if (wg0 && elect_one()) {
-      asm volatile("tcgen05.fence::after_thread_sync;");
-#pragma unroll
-      for (int pr = 0; pr < 3; ++pr) {
-        const uint32_t a0 = (pr == 1) ? acol_lo : acol_hi;
-        const uint64_t b0 = (pr == 2) ? dBl : dBh;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks)
-          tc_mma_ts(dcol, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
-      }
-      tc_commit(sm.mbar(g));
-    }
     __syncwarp();
-    if (it + 1 < ntc) cn = load(tile + (int)gridDim.x, x);   // global loads in flight under the MMAs
-    mbar_wait(sm.mbar(g), it & 1);
+    if (lane == 0) mbar_arrive(sm.xbar(g));
+  };
+  auto c0 = load((int)blockIdx.x, x);                            // context of the tile being finished
+  write_a();
+  auto c1 = c0;                                                  // context of the tile whose operand is written next
+  if (ntc > 1) c1 = load((int)blockIdx.x + stride, x);
+  for (int it = 0; it < ntc; ++it) {
+    const int tile = (int)blockIdx.x + it * stride, st = it & 1;
+    mbar_wait(sm.cbar(2 * g + st), (it >> 1) & 1);               // MMAs of tile `it` retired: the operand image is free
     asm volatile("tcgen05.fence::after_thread_sync;");
+    if (it + 1 < ntc) write_a();                                 // tile it + 1 (x was fetched one iteration ago)
     uint32_t r[64];
-    tc_ld16(lane_base, r, 0); tc_ld16(lane_base, r, 1); tc_ld16(lane_base, r, 2); tc_ld16(lane_base, r, 3);
+    const uint32_t ta = lane_base + 128 + (uint32_t)(64 * st);
+    tc_ld16s64(ta, r, 0); tc_ld16s64(ta + 16, r, 1); tc_ld16s64(ta + 32, r, 2); tc_ld16s64(ta + 48, r, 3);
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-    asm volatile("tcgen05.fence::before_thread_sync;");   // accumulator reads ordered before the next group_sync
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(sm.rdbar(2 * g + st));            // the stage may be overwritten (tile it + 2)
     float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
 #pragma unroll
     for (int n = 0; n < 64; n += 4) {
@@ -674,7 +706,9 @@ __device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, in
                   z3 = __uint_as_float(r[n + 3]);
       q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
     }
-    finish(tile, -0.5f * ((q0 + q1) + (q2 + q3)), cc);
+    finish(tile, -0.5f * ((q0 + q1) + (q2 + q3)), c0);
+    c0 = c1;
+    if (it + 2 < ntc) c1 = load(tile + 2 * stride, x);           // consumed one iteration later, after the wait for the MMAs
   }
 }
 
@@ -709,13 +743,15 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
       finish(tile, f, c);
     }
   } else {   // QUAD: persistent, the record is loaded once
-    if (t >= TC_PTS) {
+    const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+    if (warp == TC_PTS / 32) {
       if (t == TC_PTS) {
         mbar_expect_tx(sm.bbar(0), TC_REC_BYTES);
         bulk_g2s(sm.B(0), o.recs, TC_REC_BYTES, sm.bbar(0));
       }
       return;
     }
+    if (warp > TC_PTS / 32) { quad_issuer(sm, tcx_tiles_of_cta(ntiles)); return; }
     tc_quad_run(o, sm, t, ntiles, load, finish);
   }
 }

@@ -41,18 +41,26 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
       tc_load_row(row, d, (d & 3) == 0, x);
       c.xj = row[j];
       c.xp = (slot & 1) ? c.xj - a.h : c.xj + a.h;
-      // replace coordinate j through a shared-memory round trip of the thread's own row: a dynamically indexed
-      // register array would be lowered to a branch tree over j, and the warp-collective tcgen05 instructions
-      // of the evaluator need every lane on the same path
-      float *own = reinterpret_cast<float *>(sm.scratch()) + t * 68;
+      // replace coordinate j by compare-and-select over the whole row: every lane runs the same straight-line code (a
+      // dynamically indexed register array would be lowered to a branch tree over j, and the warp-collective tcgen05
+      // instructions of the evaluator need every lane on the same path), and nothing waits for the row here -- the
+      // global loads stay in flight until the evaluator first touches x
+      if constexpr (OBJ != CHISAO_OBJ_GMM_FULL) {
 #pragma unroll
-      for (int c4 = 0; c4 < TC_D / 4; ++c4)
-        *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
-      own[j] = c.xp;                       // same thread writes and reads its row: program order suffices
+        for (int q = 0; q < TC_D; ++q) x[q] = (q == j) ? c.xp : x[q];
+      } else {
+        // GMM_FULL (the row is consumed within the same pair iteration anyway; 64 selects cost registers there): the
+        // thread's own row goes through shared memory and comes back with coordinate j patched
+        float *own = reinterpret_cast<float *>(sm.scratch()) + t * 68;
 #pragma unroll
-      for (int c4 = 0; c4 < TC_D / 4; ++c4) {
-        const float4 v = *reinterpret_cast<const float4 *>(own + 4 * c4);
-        x[4 * c4] = v.x; x[4 * c4 + 1] = v.y; x[4 * c4 + 2] = v.z; x[4 * c4 + 3] = v.w;
+        for (int c4 = 0; c4 < TC_D / 4; ++c4)
+          *reinterpret_cast<float4 *>(own + 4 * c4) = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
+        own[j] = c.xp;                       // same thread writes and reads its row: program order suffices
+#pragma unroll
+        for (int c4 = 0; c4 < TC_D / 4; ++c4) {
+          const float4 v = *reinterpret_cast<const float4 *>(own + 4 * c4);
+          x[4 * c4] = v.x; x[4 * c4 + 1] = v.y; x[4 * c4 + 2] = v.z; x[4 * c4 + 3] = v.w;
+        }
       }
     } else {
 #pragma unroll
