@@ -335,7 +335,9 @@ def run_ours(args, rank, local_rank, world):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_eval_fd launch from the committed `ncu --set full`
 # capture (profiles/); None until a capture of that workload exists.
-TRAFFIC_BYTES_PER_LAUNCH = {5: 1.84e7}  # profiles/r1_evalfd_c5_f16.md (full-size launch: 18.35 MB read, 0.07 MB written)
+TRAFFIC_BYTES_PER_LAUNCH = {5: 1.84e7,   # profiles/r1_evalfd_c5_f16.md (full-size launch: 18.35 MB read, 0.07 MB written)
+                            3: 2.26e6,   # profiles/r1_evalfd_c3_rfftc.md (2.26 MB read, 0 written: the gradient stays in L2)
+                            4: 4.33e6}   # profiles/r1_evalfd_c4_quad.md (4.33 MB read, 0 written)
 
 
 def main():
