@@ -35,6 +35,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
     const int first = tile * spt;
     c.valid = (s < spt) && (first + s < cnt);
     c.i = c.valid ? (a.list ? a.list[first + s] : first + s) : 0;
+    // the CTA's next tile: its worklist entry is pulled into L1 now, so that the dependent load in front of the row
+    // loads is a hit by then
+    if (OBJ != CHISAO_OBJ_GMM_FULL && a.list && s < spt) {   // (GMM_FULL fetches its next tile a whole tile ahead)
+      const int nf = (tile + (int)gridDim.x) * spt + s;
+      if (nf < cnt) asm volatile("prefetch.global.L1 [%0];" ::"l"(a.list + nf));
+    }
     c.xj = 0.f; c.xp = 0.f;
     if (c.valid) {
       const float *row = a.X + (size_t)c.i * d;
