@@ -58,6 +58,7 @@ struct chisao_ctx {
   cudaEvent_t gfork = nullptr, gjoin = nullptr;
   cudaGraphExec_t gexec[2] = {nullptr, nullptr};
   uint64_t graph_launches = 0;
+  bool debug = false;    // CHISAO_DEBUG in the environment at chisao_init: synchronise and report after every tensor-core launch
 };
 
 namespace {
@@ -371,7 +372,7 @@ cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const in
   if (c->stencil_aware) return launch_fd_stencil(c->obj, a, s.N, c->stream);   // opt-in, dense objectives only (NEXT-5)
   if (c->use_tc) {
     cudaError_t e = launch_fd_tc(c->obj.id, c->tc, a, s.N, c->stream);
-    if (getenv("CHISAO_DEBUG")) { fprintf(stderr, "[chisao] fd_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] fd_tc done (%s)\n", cudaGetErrorString(e)); }
+    if (c->debug) { fprintf(stderr, "[chisao] fd_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] fd_tc done (%s)\n", cudaGetErrorString(e)); }
     return e;
   }
   switch (c->obj.id) {
@@ -404,7 +405,7 @@ cudaError_t eval_points(chisao_ctx *c, int mode, int b, int iter) {
   c->launches += 1;
   if (c->use_tc) {
     cudaError_t e = launch_pt_tc(c->obj.id, c->tc, a, s.N, c->stream);
-    if (getenv("CHISAO_DEBUG")) { fprintf(stderr, "[chisao] pt_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] pt_tc done (%s)\n", cudaGetErrorString(e)); }
+    if (c->debug) { fprintf(stderr, "[chisao] pt_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] pt_tc done (%s)\n", cudaGetErrorString(e)); }
     return e;
   }
   switch (c->obj.id) {
@@ -541,6 +542,7 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
   if (e != cudaSuccess || ndev == 0) return cuda_fail(nullptr, e == cudaSuccess ? cudaErrorNoDevice : e, "no CUDA device");
 
   chisao_ctx *ctx = new chisao_ctx();
+  ctx->debug = getenv("CHISAO_DEBUG") != nullptr;
   ctx->cfg = *cfg;
   ctx->stream = reinterpret_cast<cudaStream_t>(stream);
   ctx->ws_bytes = need;
@@ -702,7 +704,7 @@ int chisao_step(chisao_ctx *ctx, chisao_stats *stats) {
   if (ctx->cycle >= ctx->hp.n_osc) return fail(ctx, CHISAO_E_STATE, "all n_osc cycles already done");
   ctx->cycle += 1;                                    // "for k = 1..n_osc"
   // per-launch event bracketing (chisao_timing_enable) and CHISAO_DEBUG need the launches on the stream itself
-  const bool graph = ctx->graph_on && ctx->timing == 0 && ctx->st.N > 0 && !getenv("CHISAO_DEBUG");
+  const bool graph = ctx->graph_on && ctx->timing == 0 && ctx->st.N > 0 && !ctx->debug;
   const int rc = graph ? step_graph(ctx) : enqueue_cycle(ctx);
   if (rc) return rc;
   if (stats) return read_stats(ctx, stats);
