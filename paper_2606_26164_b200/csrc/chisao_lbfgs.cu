@@ -92,9 +92,9 @@ __device__ __forceinline__ void axpy4(Row4 &r, float c, Row4 v) {
 // A half-warp owns one sample (two samples per warp, float4 per lane: one 512-byte contiguous request per warp
 // and history plane); MM = compile-time bound on the history length, so the pair loops unroll over registers.
 // Every shuffle is executed by all 32 lanes: inactive samples run with len = 0 and predicated stores.
-constexpr int DIR_WARPS = 8;   // measured: 8 warps x 1 CTA per SM (2759 GB/s at C5, full history) beats 4 warps x 3 CTAs (2258 GB/s)
+constexpr int DIR_WARPS = 4;   // measured at C5, full history: 4 warps x 4 CTAs per SM 4023 GB/s, 2 x 8 4025, 8 x 2 3884 (finer CTA turnover: less lockstep between load and recursion phases)
 template <int MM, bool VEC>
-__global__ void __launch_bounds__(DIR_WARPS * 32, 2) k_lbfgs_direction(State s, Hyper h) {
+__global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_direction(State s, Hyper h) {
   __shared__ int sh_cnt, sh_base;
   __shared__ unsigned int sh_bytes;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, hl = lane & 15, half = lane >> 4;
