@@ -195,6 +195,14 @@ CHISAO_API int chisao_get_stats(chisao_ctx *ctx, chisao_stats *stats);
  * cudaGraphExecUpdate (the cycle index is a kernel argument).  Results are identical to direct submission; direct
  * submission is used while per-launch timing is enabled, by chisao_phase, and if the graph machinery fails. */
 #define CHISAO_OPT_CUDA_GRAPH 2
+/* CHISAO_OPT_LS_TILE_LOCAL (default: chosen at chisao_init from the cost of one evaluation tile): form of the
+ * backtracking line search of an L-BFGS iteration (R-4 (iv)).  1: one launch runs every trial b = 0..ls_max -- a tile of
+ * 256 searching samples repeats evaluate -> Armijo -> shrink until none of its samples retries; 0: one launch per trial
+ * on worklists compacted between the trials (ls_max + 1 launches).  Per sample the arithmetic is the same (same
+ * evaluator, noise slot, Armijo test, shrink), so the results are identical; 1 is the default for the FP32-FMA evaluators
+ * of the small objectives and for QUAD / RFF on the tensor cores, 0 for the x-stationary GMM_FULL evaluator (a tile
+ * streams the whole mixture: retries must stay dense), for which 1 returns CHISAO_E_INVALID. */
+#define CHISAO_OPT_LS_TILE_LOCAL 3
 CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value);
 
 /* Which evaluator the context runs (decided at chisao_init from the objective, d and the value ranges):
@@ -206,6 +214,7 @@ CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value)
  * FP32-FMA evaluator with fp64 phases). */
 #define CHISAO_INFO_EVALUATOR 1
 #define CHISAO_INFO_GRAPH_LAUNCHES 2   /* cycles submitted as a CUDA graph so far */
+#define CHISAO_INFO_LS_TILE_LOCAL 3    /* 1 if the line search runs every trial of a tile in one launch */
 CHISAO_API int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value);
 
 /* Number of kernel launches this context has enqueued so far (host counter). */

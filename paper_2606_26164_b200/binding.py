@@ -22,8 +22,10 @@ PH_RELEASE_EVAL, PH_STICK, PH_DEDUP, PH_RESEED, PH_HLC_STEP, PH_ANTI_STEP, PH_LB
 PH_LBFGS_DIRECTION = 12
 OPT_STENCIL_AWARE = 1
 OPT_CUDA_GRAPH = 2
+OPT_LS_TILE_LOCAL = 3
 INFO_EVALUATOR = 1
 INFO_GRAPH_LAUNCHES = 2
+INFO_LS_TILE_LOCAL = 3
 EVALUATOR_NAMES = ("fp32-fma", "tcgen05 3xTF32 (x - c)", "tcgen05 x-stationary tf32 hi/lo", "tcgen05 x-stationary fp16 hi/lo",
                    "tcgen05 exact fixed-point fp16 pieces (random-Fourier phases)")
 TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_update", "select", "reseed")
@@ -203,7 +205,8 @@ class Chisao:
 
     def set_option(self, option: int, value: int):
         """chisao_set_option (OPT_STENCIL_AWARE: opt-in stencil-aware FD evaluator, reported separately;
-        OPT_CUDA_GRAPH: submit each cycle as one CUDA graph launch, default on)."""
+        OPT_CUDA_GRAPH: submit each cycle as one CUDA graph launch, default on; OPT_LS_TILE_LOCAL: form of the line
+        search, see include/chisao.h)."""
         self._ck(self._L.chisao_set_option(self._h, int(option), int(value)))
 
     def evaluator(self) -> int:
@@ -211,6 +214,12 @@ class Chisao:
         v = C.c_int32(0)
         self._ck(self._L.chisao_get_info(self._h, INFO_EVALUATOR, C.byref(v)))
         return int(v.value)
+
+    def ls_tile_local(self) -> bool:
+        """chisao_get_info(INFO_LS_TILE_LOCAL): the line search runs every trial of a tile in one launch"""
+        v = C.c_int32(0)
+        self._ck(self._L.chisao_get_info(self._h, INFO_LS_TILE_LOCAL, C.byref(v)))
+        return bool(v.value)
 
     def graph_launches(self) -> int:
         """chisao_get_info(INFO_GRAPH_LAUNCHES): cycles submitted as one CUDA graph launch so far"""

@@ -58,7 +58,11 @@ struct chisao_ctx {
   cudaEvent_t gfork = nullptr, gjoin = nullptr;
   cudaGraphExec_t gexec[2] = {nullptr, nullptr};
   uint64_t graph_launches = 0;
-  bool debug = false;    // CHISAO_DEBUG in the environment at chisao_init: synchronise and report after every tensor-core launch
+  // line search: every trial of a tile in one launch (PT_LS_ALL) when a tile of the evaluator costs microseconds
+  // (FP32-FMA evaluators of the small objectives, QUAD and RFF on the tensor cores); one launch per trial on compacted
+  // worklists otherwise (GMM_FULL: a tile streams the whole mixture, the retries must stay dense)
+  bool ls_tile_local = false;
+  bool in_cycle = false; // enqueue_cycle is running: the launch sequence may rely on what the previous unit left behind
 };
 
 namespace {
@@ -111,14 +115,19 @@ int validate(const chisao_config *cfg, const chisao_objective *obj, std::string 
 // workspace carve; fills st pointers relative to `base` (may be null when only sizing)
 // RFF on the tensor cores (chisao_tc.cuh, tc_rff_tile): d <= 32, K <= 256 and value ranges inside the fixed-point
 // split: |x| < 2^ex (box radius + HLC spread + FD step), |w| < 2^ew, with ex, ew in [-6, 10]
+// largest |coordinate| an evaluation point can have: box radius + the Hands-Like-Clouds spread (8 sigma; with the auto
+// estimate sigma_s < 0, sigma = |sigma_s| x pooled std of the unfrozen samples <= |sigma_s| x box diameter) + the FD step
+float eval_point_radius(const chisao_config &c) {
+  float rad = 0.f;
+  for (int j = 0; j < c.d; ++j) rad = std::max(rad, std::max(std::fabs(c.lo[j]), std::fabs(c.hi[j])));
+  const float sig = c.sigma_s > 0.0f ? c.sigma_s : 2.0f * rad * std::fabs(c.sigma_s);
+  return rad + 8.0f * sig + std::fabs(c.fd_h);
+}
 bool rff_tc_scales(const chisao_objective &o, const chisao_config &c, int *ex_out, int *ew_out) {
   if (o.id != CHISAO_OBJ_RFF || o.d > RFF_TC_D || o.K > RFF_TC_K || getenv("CHISAO_RFF_FP64")) return false;
-  float wmax = 0.f, rad = 0.f;
+  float wmax = 0.f;
   for (size_t e = 0; e < (size_t)o.K * o.d; ++e) wmax = std::max(wmax, std::fabs(o.mats[e]));
-  for (int j = 0; j < c.d; ++j) rad = std::max(rad, std::max(std::fabs(c.lo[j]), std::fabs(c.hi[j])));
-  // auto sigma (sigma_s < 0): |sigma_s| x pooled std of the unfrozen samples <= |sigma_s| x box diameter
-  const float sig = c.sigma_s > 0.0f ? c.sigma_s : 2.0f * rad * std::fabs(c.sigma_s);
-  const float xmax = rad + 8.0f * sig + std::fabs(c.fd_h);
+  const float xmax = eval_point_radius(c);
   if (!(wmax > 0.f) || !(xmax > 0.f) || !(wmax < 3.0e38f) || !(xmax < 3.0e38f)) return false;
   int ex = 0, ew = 0;
   std::frexp(xmax, &ex);   // xmax = m 2^ex, m in [0.5, 1): xmax < 2^ex (or = 2^(ex-1): still inside the 4x headroom)
@@ -327,10 +336,9 @@ void pack_rff_records(const chisao_objective &o, int ew, std::vector<float> &out
 // fp16 hi / lo carries 22 bits like tf32 hi / lo as long as nothing overflows (65504) and the lo parts stay above the
 // fp16 subnormal spacing 2^-24: max |W| and the box radius (plus the HLC spread) must lie in [2^-3, 2^13]
 bool fp16_split_ok(const chisao_objective &o, const chisao_config &c) {
-  float wmax = 0.f, xmax = 0.f;
+  float wmax = 0.f;
   for (size_t e = 0; e < (size_t)o.K * o.d * o.d; ++e) wmax = std::max(wmax, std::fabs(o.mats[e]));
-  for (int j = 0; j < c.d; ++j) xmax = std::max(xmax, std::max(std::fabs(c.lo[j]), std::fabs(c.hi[j])));
-  xmax += 8.0f * std::fabs(c.sigma_s) + std::fabs(c.fd_h);
+  const float xmax = eval_point_radius(c);
   const float lo = 0.125f, hi = 8192.0f;
   double cmax = 0.0;                                   // c = W mu goes through the pipe as fp16 pieces as well
   for (int k = 0; k < o.K; ++k)
@@ -372,7 +380,9 @@ cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const in
   if (c->stencil_aware) return launch_fd_stencil(c->obj, a, s.N, c->stream);   // opt-in, dense objectives only (NEXT-5)
   if (c->use_tc) {
     cudaError_t e = launch_fd_tc(c->obj.id, c->tc, a, s.N, c->stream);
-    if (c->debug) { fprintf(stderr, "[chisao] fd_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] fd_tc done (%s)\n", cudaGetErrorString(e)); }
+#ifdef CHISAO_DEBUG_SYNC   // debugging builds only: synchronise and report after every tensor-core launch
+    fprintf(stderr, "[chisao] fd_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] fd_tc done (%s)\n", cudaGetErrorString(e));
+#endif
     return e;
   }
   switch (c->obj.id) {
@@ -395,6 +405,8 @@ cudaError_t eval_points(chisao_ctx *c, int mode, int b, int iter) {
   a.c1 = c->hp.ls_c1; a.shrink = c->hp.ls_shrink; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
   if (mode == PT_CENTRE) {
     a.X = s.x; a.list = nullptr; a.count = nullptr;
+  } else if (mode == PT_LS_ALL) {
+    a.X = s.xt; a.list = s.ls_list[0]; a.count = &s.ctrl->ls_cnt[0];
   } else {
     a.X = s.xt; a.list = s.ls_list[b % 3]; a.count = &s.ctrl->ls_cnt[b % 3];
     a.next_list = s.ls_list[(b + 1) % 3]; a.next_cnt = &s.ctrl->ls_cnt[(b + 1) % 3];
@@ -405,7 +417,9 @@ cudaError_t eval_points(chisao_ctx *c, int mode, int b, int iter) {
   c->launches += 1;
   if (c->use_tc) {
     cudaError_t e = launch_pt_tc(c->obj.id, c->tc, a, s.N, c->stream);
-    if (c->debug) { fprintf(stderr, "[chisao] pt_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] pt_tc done (%s)\n", cudaGetErrorString(e)); }
+#ifdef CHISAO_DEBUG_SYNC
+    fprintf(stderr, "[chisao] pt_tc launched (%s)\n", cudaGetErrorString(e)); e = cudaStreamSynchronize(c->stream); fprintf(stderr, "[chisao] pt_tc done (%s)\n", cudaGetErrorString(e));
+#endif
     return e;
   }
   switch (c->obj.id) {
@@ -451,7 +465,8 @@ int run_lbfgs_iter(chisao_ctx *ctx, int it) {   // one L-BFGS iteration (PAPER.m
   const State &s = ctx->st;
   CK(cudaMemsetAsync(s.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
   { Scope sc(ctx, 3); CK(launch_lbfgs_direction(s, ctx->hp, ctx->stream)); ctx->launches += 1; }
-  for (int b = 0; b <= ctx->hp.ls_max; ++b) CK(eval_points(ctx, PT_LS, b, it));
+  if (ctx->ls_tile_local) CK(eval_points(ctx, PT_LS_ALL, 0, it));
+  else for (int b = 0; b <= ctx->hp.ls_max; ++b) CK(eval_points(ctx, PT_LS, b, it));
   CK(eval_fd(ctx, s.xt, s.fd_list, &s.ctrl->fd_cnt, FD_GRAD, s.gn, 1, it, EV_LBFGS_FD));
   { Scope sc(ctx, 4); CK(launch_lbfgs_update(s, ctx->hp, ctx->stream)); ctx->launches += 1; }
   return CHISAO_OK;
@@ -464,8 +479,9 @@ int run_stick(chisao_ctx *ctx) {
 }
 int run_dedup(chisao_ctx *ctx) {
   Scope sc(ctx, 5);
-  CK(launch_dedup(ctx->st, ctx->hp, ctx->stream));
-  ctx->launches += 8;
+  const bool dedup_on = (ctx->hp.phase_mask & (1u << 3)) != 0;
+  CK(launch_dedup(ctx->st, ctx->hp, !ctx->in_cycle, ctx->stream));
+  ctx->launches += (ctx->in_cycle ? 0 : 3) + (dedup_on ? 2 : 0) + 3;
   return CHISAO_OK;
 }
 int run_reseed(chisao_ctx *ctx) {
@@ -482,7 +498,7 @@ int run_explore_list(chisao_ctx *ctx) {
 }
 int run_hlc(chisao_ctx *ctx, int t) {
   if (!(ctx->hp.phase_mask & (1u << 5))) return CHISAO_OK;
-  { Scope sc(ctx, 2); CK(launch_hlc_sigma(ctx->st, ctx->hp, ctx->stream)); ctx->launches += 2; }
+  if (!(ctx->hp.sigma_s > 0.0f)) { Scope sc(ctx, 2); CK(launch_hlc_sigma(ctx->st, ctx->hp, ctx->stream)); ctx->launches += 2; }
   if (ctx->hp.hlc_baseline == 2) {   // the paper's Eq. 5 form: K FD gradients at perturbed points (NEXT-2)
     const State &s = ctx->st;
     for (int k = 0; k < ctx->hp.hlc_M; ++k) {
@@ -542,7 +558,6 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
   if (e != cudaSuccess || ndev == 0) return cuda_fail(nullptr, e == cudaSuccess ? cudaErrorNoDevice : e, "no CUDA device");
 
   chisao_ctx *ctx = new chisao_ctx();
-  ctx->debug = getenv("CHISAO_DEBUG") != nullptr;
   ctx->cfg = *cfg;
   ctx->stream = reinterpret_cast<cudaStream_t>(stream);
   ctx->ws_bytes = need;
@@ -605,6 +620,20 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
     ctx->tc.K = obj->K; ctx->tc.d = obj->d; ctx->tc.sigma_noise = obj->sigma_noise; ctx->tc.recs = tc_dev;
     CKI(tc_configure());
   }
+  {   // line search form (see chisao_ctx::ls_tile_local): plain-definition flop per evaluation as the cost of a tile
+    const double dd = obj->d, KK = obj->K;
+    double cost = 0.0;
+    switch (obj->id) {
+      case CHISAO_OBJ_GMM_ISO: cost = KK * 3 * dd; break;
+      case CHISAO_OBJ_GMM_DIAG: cost = KK * 4 * dd; break;
+      case CHISAO_OBJ_GMM_FULL: cost = KK * 2 * dd * dd; break;
+      case CHISAO_OBJ_RFF: cost = KK * 4 * dd; break;      // fp64 phases at half rate on the FP32-FMA evaluator
+      case CHISAO_OBJ_QUAD: cost = 2 * dd * dd; break;
+      default: cost = 64 * dd; break;                      // Appendix-D functions
+    }
+    ctx->ls_tile_local = ctx->use_tc ? (obj->id != CHISAO_OBJ_GMM_FULL) : (cost <= 32768.0);
+    if (getenv("CHISAO_LS_PER_TRIAL")) ctx->ls_tile_local = false;
+  }
   // zero everything except the parameter records, then upload parameters and bounds
   CKI(cudaMemsetAsync(workspace_dev, 0, need, ctx->stream));
   CKI(cudaMemcpyAsync(const_cast<float *>(recs_dev), ctx->recs_host.data(), ctx->recs_host.size() * 4,
@@ -616,6 +645,8 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
   CKI(cudaMemcpyAsync(s.hi, ctx->hi.data(), 4 * (size_t)cfg->d, cudaMemcpyHostToDevice, ctx->stream));
   const int32_t one = 1;
   CKI(cudaMemcpyAsync(&s.ctrl->gr_enabled, &one, 4, cudaMemcpyHostToDevice, ctx->stream));
+  if (cfg->sigma_s > 0.0f)   // caller-supplied smoothing scale: constant for the life of the context
+    CKI(cudaMemcpyAsync(&s.ctrl->sigma_eff, &ctx->hp.sigma_s, 4, cudaMemcpyHostToDevice, ctx->stream));
 #undef CKI
   *out = ctx;
   return CHISAO_OK;
@@ -629,7 +660,14 @@ int chisao_seed_population(chisao_ctx *ctx) {
 }
 
 // the launch sequence of one cycle k = ctx->cycle on ctx->stream (Algorithm 1)
+static int enqueue_cycle_units(chisao_ctx *ctx);
 static int enqueue_cycle(chisao_ctx *ctx) {
+  ctx->in_cycle = true;
+  const int rc = enqueue_cycle_units(ctx);
+  ctx->in_cycle = false;
+  return rc;
+}
+static int enqueue_cycle_units(chisao_ctx *ctx) {
   int rc;
   if ((rc = run_release_eval(ctx))) return rc;        // Phase 1: release all, then converge
   for (int it = 1; it <= ctx->hp.n_conv; ++it)
@@ -703,10 +741,14 @@ int chisao_step(chisao_ctx *ctx, chisao_stats *stats) {
   if (!ctx) return fail(nullptr, CHISAO_E_INVALID, "null ctx");
   if (ctx->cycle >= ctx->hp.n_osc) return fail(ctx, CHISAO_E_STATE, "all n_osc cycles already done");
   ctx->cycle += 1;                                    // "for k = 1..n_osc"
-  // per-launch event bracketing (chisao_timing_enable) and CHISAO_DEBUG need the launches on the stream itself
-  const bool graph = ctx->graph_on && ctx->timing == 0 && ctx->st.N > 0 && !ctx->debug;
+  // per-launch event bracketing (chisao_timing_enable) needs the launches on the stream itself
+#ifdef CHISAO_DEBUG_SYNC
+  const bool graph = false;
+#else
+  const bool graph = ctx->graph_on && ctx->timing == 0 && ctx->st.N > 0;
+#endif
   const int rc = graph ? step_graph(ctx) : enqueue_cycle(ctx);
-  if (rc) return rc;
+  if (rc) { ctx->cycle -= 1; return rc; }             // a cycle that could not be enqueued does not advance k (nor the Philox keys)
   if (stats) return read_stats(ctx, stats);
   return CHISAO_OK;
 }
@@ -891,11 +933,19 @@ int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value) {
     return CHISAO_OK;
   }
   if (option == CHISAO_OPT_CUDA_GRAPH) { ctx->graph_on = value != 0; return CHISAO_OK; }
+  if (option == CHISAO_OPT_LS_TILE_LOCAL) {
+    if (value && ctx->use_tc && ctx->obj.id == CHISAO_OBJ_GMM_FULL)
+      return fail(ctx, CHISAO_E_INVALID, "the tile-local line search does not exist for the x-stationary GMM_FULL evaluator");
+    ctx->ls_tile_local = value != 0;
+    for (auto &ge : ctx->gexec) if (ge) { cudaGraphExecDestroy(ge); ge = nullptr; }   // another topology
+    return CHISAO_OK;
+  }
   return fail(ctx, CHISAO_E_INVALID, "unknown option");
 }
 
 int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value) {
   if (ctx && value && which == CHISAO_INFO_GRAPH_LAUNCHES) { *value = (int32_t)ctx->graph_launches; return CHISAO_OK; }
+  if (ctx && value && which == CHISAO_INFO_LS_TILE_LOCAL) { *value = ctx->ls_tile_local ? 1 : 0; return CHISAO_OK; }
   if (!ctx || !value || which != CHISAO_INFO_EVALUATOR) return CHISAO_E_INVALID;
   *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_RFF ? 4 : (ctx->obj.id == CHISAO_OBJ_QUAD ? 1 : (ctx->tc.f16 ? 3 : 2)));
   return CHISAO_OK;

@@ -88,7 +88,7 @@ struct Hyper {                        // by-value copy of the cycle hyper-parame
 
 // modes of the evaluation kernels
 enum { FD_GRAD = 0, FD_ANTI = 1 };
-enum { PT_CENTRE = 0, PT_LS = 1 };
+enum { PT_CENTRE = 0, PT_LS = 1, PT_LS_ALL = 2 };
 // modes of the list-building scan
 enum { SCAN_STICK = 0, SCAN_FINAL = 1, SCAN_EXPLORE = 2 };
 
@@ -105,7 +105,7 @@ cudaError_t launch_lbfgs_direction(const State &s, const Hyper &h, cudaStream_t 
 cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, cudaStream_t st);
 cudaError_t launch_release(const State &s, cudaStream_t st);
 cudaError_t launch_stick(const State &s, const Hyper &h, cudaStream_t st);          // ginf, f_max, flags, P0
-cudaError_t launch_dedup(const State &s, const Hyper &h, cudaStream_t st);          // removed + lists + GR state
+cudaError_t launch_dedup(const State &s, const Hyper &h, bool rebuild_p0, cudaStream_t st);   // removed + lists + GR state
 cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_t st);
 cudaError_t launch_explore_list(const State &s, cudaStream_t st);
 // paper-form HLC (Eq. 5) helpers: stage 0 perturb (xt = x + sigma z_k), 1 accumulate (ghat += gn / M), 2 apply

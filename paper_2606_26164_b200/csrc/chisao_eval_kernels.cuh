@@ -142,7 +142,20 @@ __device__ __forceinline__ float ls_retry_row(const PtArgs &a, int i, int d, flo
   return dsum;
 }
 
+// the Armijo decision of one line-search trial (R-4 (iv)); a non-finite trial value is rejected (R-12)
+__device__ __forceinline__ bool ls_accept(float val, float f_i, float dec_i, float c1) {
+  const float phit = -val, phi = -f_i;
+  const float rhs = fmaf(c1, dec_i, phi);                 // Armijo: phi_t <= phi + c1 gamma.(x_t - x)
+  return (fabsf(phit) <= 3.0e38f) && (phit <= rhs);
+}
+
 // ---- one point per sample: cycle-start centre value, or line-search trial b (R-4) ---------------------
+// PT_LS     : trial b of the samples on worklist b % 3; rejected samples are compacted onto worklist (b + 1) % 3
+//             (one launch per trial: for evaluators whose tile is expensive, the retries stay dense)
+// PT_LS_ALL : every trial b = 0 .. ls_max of the samples on worklist 0 in ONE launch: a tile keeps its samples and
+//             repeats evaluate -> Armijo -> shrink until none of them retries (for evaluators whose tile costs
+//             microseconds: the ls_max + 1 dependent launches, most of them empty, were the cost)
+// Both forms run the same per-sample arithmetic (same evaluator, noise slot 2d + 1 + b, Armijo test, shrink).
 template <int OBJ, int DP>
 __global__ void __launch_bounds__(NT, 2) k_eval_points(const DevObj o, const PtArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -160,44 +173,61 @@ __global__ void __launch_bounds__(NT, 2) k_eval_points(const DevObj o, const PtA
     const int e = first + pp * NT + t;
     valid[pp] = e < cnt;
     idx[pp] = valid[pp] ? (a.list ? a.list[e] : e) : 0;
-    const float *row = a.X + (size_t)idx[pp] * d;
-#pragma unroll
-    for (int c4 = 0; c4 < DP / 4; ++c4)
-      sm.pts[c4 * PTILE + pp * NT + t] = valid[pp] ? ld_row4(row, c4, d, vec) : make_float4(0.f, 0.f, 0.f, 0.f);
   }
-  __syncthreads();
   uint32_t use = 0;
-  float fv[PPT];
-  eval_tile<OBJ, DP>(o, sm, t, use, fv);
+  unsigned int nev = 0;                                   // evaluations done by this thread (PT_LS_ALL)
+  for (int b = a.b;; ++b) {
 #pragma unroll
-  for (int pp = 0; pp < PPT; ++pp) {
-    const int i = idx[pp];
-    bool accept = false, retry = false;
-    float val = 0.f;
-    if (valid[pp]) {
-      if (a.mode == PT_CENTRE) {
-        a.f[i] = fv[pp] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, 0, 0);
-      } else {
-        val = fv[pp] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + a.b);
-        const float phit = -val, phi = -a.f[i];
-        const float rhs = fmaf(a.c1, a.dec[i], phi);          // Armijo: phi_t <= phi + c1 gamma.(x_t - x)
-        accept = (fabsf(phit) <= 3.0e38f) && (phit <= rhs);    // non-finite trial is rejected (R-12)
-        retry = !accept && (a.b < a.ls_max);
+    for (int pp = 0; pp < PPT; ++pp) {
+      const float *row = a.X + (size_t)idx[pp] * d;
+#pragma unroll
+      for (int c4 = 0; c4 < DP / 4; ++c4)
+        sm.pts[c4 * PTILE + pp * NT + t] = valid[pp] ? ld_row4(row, c4, d, vec) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    __syncthreads();
+    float fv[PPT];
+    eval_tile<OBJ, DP>(o, sm, t, use, fv);
+    bool again = false;
+#pragma unroll
+    for (int pp = 0; pp < PPT; ++pp) {
+      const int i = idx[pp];
+      bool accept = false, retry = false;
+      float val = 0.f;
+      if (valid[pp]) {
+        if (a.mode == PT_CENTRE) {
+          a.f[i] = fv[pp] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, 0, 0);
+        } else {
+          val = fv[pp] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + b);
+          accept = ls_accept(val, a.f[i], a.dec[i], a.c1);
+          retry = !accept && (b < a.ls_max);
+          nev += 1u;
+        }
+      }
+      if (a.mode != PT_CENTRE) {
+        const int sa = warp_append(a.fd_cnt, accept);
+        if (accept) { a.fd_list[sa] = i; a.ls_b[i] = b; a.ft[i] = val; }
+        if (a.mode == PT_LS) {
+          const int sr = warp_append(a.next_cnt, retry);
+          if (retry) a.next_list[sr] = i;
+        }
+        if (retry) {
+          const float tn = a.tcur[i] * a.shrink;
+          a.tcur[i] = tn;
+          a.dec[i] = ls_retry_row(a, i, d, tn);          // rewrites x_t of sample i (read back by this thread only)
+        }
+        valid[pp] = retry;                                // PT_LS_ALL: the sample stays in its tile slot
+        again |= retry;
       }
     }
-    if (a.mode == PT_LS) {
-      const int sa = warp_append(a.fd_cnt, accept);
-      if (accept) { a.fd_list[sa] = i; a.ls_b[i] = a.b; a.ft[i] = val; }
-      const int sr = warp_append(a.next_cnt, retry);
-      if (retry) {
-        a.next_list[sr] = i;
-        const float tn = a.tcur[i] * a.shrink;
-        a.tcur[i] = tn;
-        a.dec[i] = ls_retry_row(a, i, d, tn);
-      }
-    }
+    if (a.mode != PT_LS_ALL) break;
+    if (!__syncthreads_or(again)) break;                  // also orders this round's reads of the staged points before the next staging
   }
-  if (t == 0) atomicAdd(&a.evals[a.mode == PT_CENTRE ? EV_INIT : EV_LS], (unsigned long long)min(PTILE, cnt - first));
+  if (a.mode == PT_LS_ALL) {
+    nev = (unsigned int)warp_sum_u(nev);
+    if ((t & 31) == 0 && nev) atomicAdd(&a.evals[EV_LS], (unsigned long long)nev);
+  } else if (t == 0) {
+    atomicAdd(&a.evals[a.mode == PT_CENTRE ? EV_INIT : EV_LS], (unsigned long long)min(PTILE, cnt - first));
+  }
 }
 
 struct HlcArgs {

@@ -208,10 +208,11 @@ cudaError_t launch_stick(const State &s, const Hyper &h, cudaStream_t st) {
   return run_scan(s, SCAN_STICK, st);
 }
 
-cudaError_t launch_dedup(const State &s, const Hyper &h, cudaStream_t st) {
+cudaError_t launch_dedup(const State &s, const Hyper &h, bool rebuild_p0, cudaStream_t st) {
   if (s.N > 0) {
-    // lists may be stale if the caller edited the flags: rebuild the pre-removal stuck list first
-    cudaError_t e = run_scan(s, SCAN_STICK, st);
+    // as a stand-alone unit (chisao_phase) the caller may have edited the flags: rebuild the pre-removal stuck list
+    // first; inside a cycle launch_stick has just written it
+    cudaError_t e = rebuild_p0 ? run_scan(s, SCAN_STICK, st) : cudaSuccess;
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(s.removed, 0, s.N, st);
     if (e != cudaSuccess) return e;
@@ -420,8 +421,10 @@ __global__ void k_sigma_final(State s, Hyper h) {
   const double mean = c->sx / n, var = fmax(c->sxx / n - mean * mean, 0.0);
   c->sigma_eff = (float)(fabs((double)h.sigma_s) * sqrt(var));
 }
+// a caller-supplied scale (sigma_s > 0) is written to ctrl->sigma_eff once, at chisao_init: nothing to launch then
 cudaError_t launch_hlc_sigma(const State &s, const Hyper &h, cudaStream_t st) {
-  if (h.sigma_s <= 0.0f && s.N > 0) {
+  if (h.sigma_s > 0.0f) return cudaSuccess;
+  if (s.N > 0) {
     cudaError_t e = cudaMemsetAsync(&s.ctrl->sx, 0, 2 * sizeof(double), st);
     if (e != cudaSuccess) return e;
     k_sigma_sum<<<148, 256, 0, st>>>(s);

@@ -493,42 +493,44 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
 // MMA issuer of the RFF form (warp 9, warp-uniform control flow, one elected lane issues): chunk c of group g goes to
 // accumulator stage c & 1 as soon as the group's point images are written (xbar) and that stage has been read out
 // (rdbar); tcgen05.commit signals cbar(2 g + stage).
+__device__ __forceinline__ void rff_issue_tile(const TcObj &o, const TcSmem &sm, uint32_t tm, uint32_t wa, uint32_t xa, int it) {
+  const int nch = o.nchunk;
+  for (int c = 0; c < nch; ++c) {
+    const int st = c & 1;
+    const int n = it * (st ? nch / 2 : (nch + 1) / 2) + (c >> 1);   // earlier issues into this stage
+    const uint64_t dW = tc_desc(wa + (uint32_t)(c * 1024), 4096, 128);
+#pragma unroll 1
+    for (int g = 0; g < 2; ++g) {
+      if (c == 0) mbar_wait(sm.xbar(g), it & 1);
+      if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      if (elect_one()) {
+        const uint64_t dX = tc_desc(xa + (uint32_t)(g * RFF_X_BYTES), 2048, 128);
+        const uint32_t accA = tm + (uint32_t)(g * 256 + 128 * st), accBC = accA + 64;
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks)
+          tc_mma_ss_f16(accA, dX + (uint64_t)(ks * 256), dW + (uint64_t)(ks * 512), TC_IDESC_F16_N64, ks ? 1u : 0u);
+#pragma unroll
+        for (int pr = 0; pr < 5; ++pr) {   // (n0, m1) (n1, m0) (2^-10 n1, m1) (n0, 2^-10 m2) (2^-10 n2, m0)
+          const int xp = (pr == 0 || pr == 3) ? 0 : (pr == 1 ? 1 : (pr == 2 ? 2 : 3));
+          const int wp = (pr == 0 || pr == 2) ? 1 : (pr == 3 ? 2 : 0);
+#pragma unroll
+          for (int ks = 0; ks < 2; ++ks)
+            tc_mma_ss_f16(accBC, dX + (uint64_t)(xp * 512 + ks * 256), dW + (uint64_t)(wp * 1024 + ks * 512), TC_IDESC_F16_N64,
+                          (pr | ks) ? 1u : 0u);
+        }
+        tc_commit(sm.cbar(2 * g + st));
+      }
+      __syncwarp();
+    }
+  }
+}
 __device__ __forceinline__ void rff_issuer(const TcObj &o, const TcSmem &sm, int ntc) {
   mbar_wait(sm.bbar(0), 0);                                      // the frequencies' images have landed
   const uint32_t tm = *sm.tmem();
-  const int nch = o.nchunk;
   unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
   const uint32_t wa = smem_u32(wbase), xa = wa + RFF_REC_BYTES;
-  for (int it = 0; it < ntc; ++it)
-    for (int c = 0; c < nch; ++c) {
-      const int st = c & 1;
-      const int n = it * (st ? nch / 2 : (nch + 1) / 2) + (c >> 1);   // earlier issues into this stage
-      const uint64_t dW = tc_desc(wa + (uint32_t)(c * 1024), 4096, 128);
-#pragma unroll 1
-      for (int g = 0; g < 2; ++g) {
-        if (c == 0) mbar_wait(sm.xbar(g), it & 1);
-        if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);
-        asm volatile("tcgen05.fence::after_thread_sync;");
-        if (elect_one()) {
-          const uint64_t dX = tc_desc(xa + (uint32_t)(g * RFF_X_BYTES), 2048, 128);
-          const uint32_t accA = tm + (uint32_t)(g * 256 + 128 * st), accBC = accA + 64;
-#pragma unroll
-          for (int ks = 0; ks < 2; ++ks)
-            tc_mma_ss_f16(accA, dX + (uint64_t)(ks * 256), dW + (uint64_t)(ks * 512), TC_IDESC_F16_N64, ks ? 1u : 0u);
-#pragma unroll
-          for (int pr = 0; pr < 5; ++pr) {   // (n0, m1) (n1, m0) (2^-10 n1, m1) (n0, 2^-10 m2) (2^-10 n2, m0)
-            const int xp = (pr == 0 || pr == 3) ? 0 : (pr == 1 ? 1 : (pr == 2 ? 2 : 3));
-            const int wp = (pr == 0 || pr == 2) ? 1 : (pr == 3 ? 2 : 0);
-#pragma unroll
-            for (int ks = 0; ks < 2; ++ks)
-              tc_mma_ss_f16(accBC, dX + (uint64_t)(xp * 512 + ks * 256), dW + (uint64_t)(wp * 1024 + ks * 512), TC_IDESC_F16_N64,
-                            (pr | ks) ? 1u : 0u);
-          }
-          tc_commit(sm.cbar(2 * g + st));
-        }
-        __syncwarp();
-      }
-    }
+  for (int it = 0; it < ntc; ++it) rff_issue_tile(o, sm, tm, wa, xa, it);
 }
 
 // compute side of one tile: the thread's point -> its row of the four images; then per 64-feature chunk: wait for the
@@ -624,32 +626,33 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
 // its operand image is written (xbar) and its stage has been read out (rdbar), i.e. while the compute warps still
 // square, sum and finish tile n.  The compute warps never meet at a barrier; the point of tile n + 2 is fetched from
 // global memory right after tile n is finished and consumed after the wait for the MMAs of tile n + 1.  TMEM per group (256 g): A_hi 64 | A_lo 64 | accumulators 2 x 64.
+__device__ __forceinline__ void quad_issue_tile(const TcSmem &sm, uint32_t tm, uint64_t dBh, uint64_t dBl, int it) {
+  const int st = it & 1, n = it >> 1;                            // n earlier issues into this stage
+#pragma unroll 1
+  for (int g = 0; g < 2; ++g) {
+    mbar_wait(sm.xbar(g), it & 1);                               // operand image of tile `it` written by the group's 4 warps
+    if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);     // accumulators of tile it - 2 are in registers
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (elect_one()) {
+      const uint32_t gcol = tm + (uint32_t)(g * 256), acc = gcol + 128 + (uint32_t)(64 * st);
+#pragma unroll
+      for (int pr = 0; pr < 3; ++pr) {
+        const uint32_t a0 = (pr == 1) ? gcol + 64 : gcol;
+        const uint64_t b0 = (pr == 2) ? dBl : dBh;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          tc_mma_ts(acc, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
+      }
+      tc_commit(sm.cbar(2 * g + st));
+    }
+    __syncwarp();
+  }
+}
 __device__ __forceinline__ void quad_issuer(const TcSmem &sm, int ntc) {
   mbar_wait(sm.bbar(0), 0);                                      // W hi / lo and c have landed (once)
   const uint32_t tm = *sm.tmem();
   const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
-  for (int it = 0; it < ntc; ++it) {
-    const int st = it & 1, n = it >> 1;                          // n earlier issues into this stage
-#pragma unroll 1
-    for (int g = 0; g < 2; ++g) {
-      mbar_wait(sm.xbar(g), it & 1);                             // operand image of tile `it` written by the group's 4 warps
-      if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);   // accumulators of tile it - 2 are in registers
-      asm volatile("tcgen05.fence::after_thread_sync;");
-      if (elect_one()) {
-        const uint32_t gcol = tm + (uint32_t)(g * 256), acc = gcol + 128 + (uint32_t)(64 * st);
-#pragma unroll
-        for (int pr = 0; pr < 3; ++pr) {
-          const uint32_t a0 = (pr == 1) ? gcol + 64 : gcol;
-          const uint64_t b0 = (pr == 2) ? dBl : dBh;
-#pragma unroll
-          for (int ks = 0; ks < 8; ++ks)
-            tc_mma_ts(acc, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), (pr | ks) ? 1u : 0u);
-        }
-        tc_commit(sm.cbar(2 * g + st));
-      }
-      __syncwarp();
-    }
-  }
+  for (int it = 0; it < ntc; ++it) quad_issue_tile(sm, tm, dBh, dBl, it);
 }
 
 template <class Load, class Finish>
@@ -709,6 +712,97 @@ __device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, in
     finish(tile, -0.5f * ((q0 + q1) + (q2 + q3)), c0);
     c0 = c1;
     if (it + 2 < ntc) c1 = load(tile + 2 * stride, x);           // consumed one iteration later, after the wait for the MMAs
+  }
+}
+
+// ---- tile-local rounds (QUAD and RFF forms): ONE tile per CTA, evaluated again and again until no thread asks for
+// another round (the line search: evaluate -> Armijo -> shrink; chisao_tc_kernels.cu, PT_LS_ALL).  The 256 compute
+// threads and the MMA-issuer warp vote at a named barrier after every round (bar.red.or); the loader warp has
+// nothing to do after the record has landed.  Round r uses accumulator stage r & 1 and the barrier phases of tile
+// iteration r of the persistent forms above.
+__device__ __forceinline__ bool round_vote(bool again) {       // 256 compute threads + the issuer warp
+  uint32_t res;
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 q, %1, 0;\n\tbar.red.or.pred p, 4, 288, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(res) : "r"((uint32_t)again) : "memory");
+  return res != 0u;
+}
+// load(r, x): the thread's point of round r;  finish(r, f) -> true if the thread wants another round
+template <int OBJ, class Load, class Finish>
+__device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int t, Load load, Finish finish) {
+  static_assert(OBJ == CHISAO_OBJ_QUAD || OBJ == CHISAO_OBJ_RFF, "tile-local rounds exist for the QUAD and RFF forms");
+  const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+  const uint32_t rec_bytes = (OBJ == CHISAO_OBJ_RFF) ? (uint32_t)RFF_REC_BYTES : (uint32_t)TC_REC_BYTES;
+  if (warp == TC_PTS / 32) {                               // loader warp: the record lands once
+    if (t == TC_PTS) {
+      mbar_expect_tx(sm.bbar(0), rec_bytes);
+      if constexpr (OBJ == CHISAO_OBJ_RFF) bulk_g2s(sm.Bx(0, 0), o.recs, rec_bytes, sm.bbar(0));
+      else bulk_g2s(sm.B(0), o.recs, rec_bytes, sm.bbar(0));
+    }
+    return;
+  }
+  mbar_wait(sm.bbar(0), 0);
+  const uint32_t tm = *sm.tmem();
+  if (warp > TC_PTS / 32) {                                // issuer warp
+    if constexpr (OBJ == CHISAO_OBJ_RFF) {
+      unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
+      const uint32_t wa = smem_u32(wbase), xa = wa + RFF_REC_BYTES;
+      for (int r = 0;; ++r) { rff_issue_tile(o, sm, tm, wa, xa, r); if (!round_vote(false)) break; }
+    } else {
+      const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
+      for (int r = 0;; ++r) { quad_issue_tile(sm, tm, dBh, dBl, r); if (!round_vote(false)) break; }
+    }
+    return;
+  }
+  const int g = t >> 7, lane = t & 31;
+  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
+  for (int r = 0;; ++r) {
+    float x[TC_D];
+    load(r, x);
+    float f;
+    if constexpr (OBJ == CHISAO_OBJ_RFF) {
+      f = tc_rff_tile(o, sm, x, t, r);
+    } else {
+      const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(0) + 2 * TC_D * TC_D);
+      const int st = r & 1;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {                        // A = x - c as tf32 hi / lo -> the thread's TMEM lane (as tc_quad_run)
+        float h[16], l[16];
+#pragma unroll
+        for (int c4 = 0; c4 < 4; ++c4) {
+          const float4 mu = mu4[4 * q + c4];
+          const int c = 16 * q + 4 * c4;
+          const float d0 = x[c] - mu.x, d1 = x[c + 1] - mu.y, d2 = x[c + 2] - mu.z, d3 = x[c + 3] - mu.w;
+          h[4 * c4] = tf32_rna(d0); h[4 * c4 + 1] = tf32_rna(d1); h[4 * c4 + 2] = tf32_rna(d2); h[4 * c4 + 3] = tf32_rna(d3);
+          l[4 * c4] = d0 - h[4 * c4]; l[4 * c4 + 1] = d1 - h[4 * c4 + 1]; l[4 * c4 + 2] = d2 - h[4 * c4 + 2]; l[4 * c4 + 3] = d3 - h[4 * c4 + 3];
+        }
+        tc_st16(lane_base + 16 * q, h);
+        tc_st16(lane_base + 64 + 16 * q, l);
+      }
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      asm volatile("tcgen05.fence::before_thread_sync;");
+      __syncwarp();
+      if (lane == 0) mbar_arrive(sm.xbar(g));
+      mbar_wait(sm.cbar(2 * g + st), (r >> 1) & 1);         // MMAs of round r retired
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      uint32_t rr[64];
+      const uint32_t ta = lane_base + 128 + (uint32_t)(64 * st);
+      tc_ld16s64(ta, rr, 0); tc_ld16s64(ta + 16, rr, 1); tc_ld16s64(ta + 32, rr, 2); tc_ld16s64(ta + 48, rr, 3);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      asm volatile("tcgen05.fence::before_thread_sync;");
+      __syncwarp();
+      if (lane == 0) mbar_arrive(sm.rdbar(2 * g + st));
+      float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll
+      for (int n = 0; n < 64; n += 4) {
+        const float z0 = __uint_as_float(rr[n]), z1 = __uint_as_float(rr[n + 1]), z2 = __uint_as_float(rr[n + 2]),
+                    z3 = __uint_as_float(rr[n + 3]);
+        q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+      }
+      f = -0.5f * ((q0 + q1) + (q2 + q3));
+    }
+    const bool again = finish(r, f);
+    if (!round_vote(again)) break;
   }
 }
 

@@ -17,19 +17,24 @@ __device__ __forceinline__ void tc_load_row(const float *row, int d, bool vec, f
   }
 }
 
-// thread t -> (sample t / 2d of the tile, slot t % 2d); slot 2j = x + h e_j, 2j + 1 = x - h e_j
+// thread t of group t >> 7 -> (sample (t & 127) / 2d of the group, slot (t & 127) % 2d); slot 2j = x + h e_j,
+// 2j + 1 = x - h e_j.  The 2d stencil points of a sample never straddle the two groups of 128 points: in the QUAD and RFF
+// forms the groups run unsynchronised (one may be a tile ahead of the other), and FD_ANTI rewrites the sample's row
+// in place from the finish of the group that owns it -- a row shared by both groups could be read half-updated.
+__host__ __device__ inline int fd_tc_samples_per_tile(int d) { return 2 * (TC_GROUP / (2 * d)); }
 struct FdCtx { int i; float xj, xp; bool valid; };
 template <int OBJ>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, const FdArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
   const TcSmem sm = tc_carve(tc_smem_raw);
   const int t = threadIdx.x, d = a.d;
-  const int spt = TC_PTS / (2 * d);
+  const int spg = TC_GROUP / (2 * d), spt = 2 * spg;
   const int cnt = a.count ? *a.count : a.max_count;
   const int ntiles = (cnt + spt - 1) / spt;
   if ((int)blockIdx.x >= ntiles) return;
   tc_begin<OBJ>(sm, t);
-  const int s = t / (2 * d), slot = t - s * 2 * d, j = slot >> 1;
+  const int tl = t & (TC_GROUP - 1), sg = tl / (2 * d), slot = tl - sg * 2 * d, j = slot >> 1;
+  const int s = (t < TC_PTS && sg < spg) ? (t >> 7) * spg + sg : spt;   // s >= spt: idle lane (also the loader / issuer warps)
   auto load = [&](int tile, float (&x)[TC_D]) -> FdCtx {
     FdCtx c;
     const int first = tile * spt;
@@ -107,6 +112,48 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
   if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
   if ((int)blockIdx.x >= ntiles) return;
   tc_begin<OBJ>(sm, t);
+  if constexpr (OBJ != CHISAO_OBJ_GMM_FULL) {
+    if (a.mode == PT_LS_ALL) {
+      // every trial b = 0 .. ls_max of the CTA's 256 worklist entries in one launch (tc_rounds): round r = trial b
+      const int e = (int)blockIdx.x * TC_PTS + t;
+      bool active = (t < TC_PTS) && (e < cnt);
+      const int i = active ? a.list[e] : 0;
+      unsigned int nev = 0;
+      auto load = [&](int, float (&x)[TC_D]) {
+        if (active) tc_load_row(a.X + (size_t)i * d, d, (d & 3) == 0, x);
+        else {
+#pragma unroll
+          for (int k = 0; k < TC_D; ++k) x[k] = 0.f;
+        }
+      };
+      auto finish = [&](int b, float fv) -> bool {
+        bool accept = false, retry = false;
+        float val = 0.f;
+        if (active) {
+          val = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + b);
+          accept = ls_accept(val, a.f[i], a.dec[i], a.c1);
+          retry = !accept && (b < a.ls_max);
+          nev += 1u;
+        }
+        const int sa = warp_append(a.fd_cnt, accept);
+        if (accept) { a.fd_list[sa] = i; a.ls_b[i] = b; a.ft[i] = val; }
+        if (retry) {
+          const float tn = a.tcur[i] * a.shrink;
+          a.tcur[i] = tn;
+          a.dec[i] = ls_retry_row(a, i, d, tn);            // rewrites x_t of sample i (read back by this thread only)
+        }
+        active = retry;
+        return retry;
+      };
+      tc_rounds<OBJ>(o, sm, t, load, finish);
+      if (t < TC_PTS) {
+        nev = warp_sum_u(nev);
+        if ((t & 31) == 0 && nev) atomicAdd(&a.evals[EV_LS], (unsigned long long)nev);
+      }
+      tc_teardown(sm, t);
+      return;
+    }
+  }
   auto load = [&](int tile, float (&x)[TC_D]) -> PtCtx {
     PtCtx c;
     const int e = tile * TC_PTS + t;
@@ -128,9 +175,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
         a.f[i] = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, 0, 0);
       } else {
         val = fv + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + a.b);
-        const float phit = -val, phi = -a.f[i];
-        const float rhs = fmaf(a.c1, a.dec[i], phi);
-        accept = (fabsf(phit) <= 3.0e38f) && (phit <= rhs);
+        accept = ls_accept(val, a.f[i], a.dec[i], a.c1);
         retry = !accept && (a.b < a.ls_max);
       }
     }
@@ -279,7 +324,7 @@ cudaError_t tc_configure() {
   return cudaSuccess;
 }
 cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samples, cudaStream_t st) {
-  const int spt = TC_PTS / (2 * a.d);
+  const int spt = fd_tc_samples_per_tile(a.d);
   const int grid = tc_grid(obj_id, (n_samples + spt - 1) / spt);
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_fd_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else if (obj_id == CHISAO_OBJ_RFF) k_eval_fd_tc<CHISAO_OBJ_RFF><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
@@ -287,7 +332,8 @@ cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samp
   return cudaGetLastError();
 }
 cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samples, cudaStream_t st) {
-  const int grid = tc_grid(obj_id, (n_samples + TC_PTS - 1) / TC_PTS);
+  const int ntiles = (n_samples + TC_PTS - 1) / TC_PTS;
+  const int grid = (a.mode == PT_LS_ALL) ? ntiles : tc_grid(obj_id, ntiles);   // tile-local rounds: one tile per CTA
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else if (obj_id == CHISAO_OBJ_RFF) k_eval_points_tc<CHISAO_OBJ_RFF><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);

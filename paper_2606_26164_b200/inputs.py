@@ -285,3 +285,29 @@ def custom(obj: Objective, box: float, N: int, seed: int = 7, **over) -> Workloa
             raise KeyError(k)
         setattr(hp, k, v)
     return Workload("custom", obj, hp, uniform_population(N, lo, hi, seed + 1))
+
+
+def synthetic_converged_state(wl: Workload, frac_clustered: float = 0.6, n_clusters: int = 300, seed: int = 17):
+    """A seeded post-convergence state (x, f, g) for cross-sample phase tests at any N -- inputs only, no arithmetic of
+    the method: `frac_clustered` of the samples sit in `n_clusters` tight clusters (centres uniform in Theta, jitter
+    well inside eps_dup, so the deduplication has many removals and exact / near ties), the rest stay at their
+    seeded uniform positions; f is a seeded per-cluster level minus a jitter term (with exact ties), g is seeded
+    noise whose magnitude straddles eps_grad; a few f / g entries are non-finite (R-12)."""
+    hp = wl.hp
+    N, d = hp.N, hp.d
+    rng = _rng(seed)
+    x = np.array(wl.x0, dtype=np.float64, copy=True)
+    clustered = rng.uniform(size=N) < frac_clustered
+    centres = rng.uniform(hp.lo.astype(np.float64) * 0.9, hp.hi.astype(np.float64) * 0.9, size=(n_clusters, d))
+    which = rng.integers(0, n_clusters, size=N)
+    jit = rng.uniform(-0.3, 0.3, size=(N, d)) * float(hp.eps_dup)
+    x[clustered] = centres[which[clustered]] + jit[clustered]
+    level = rng.uniform(-2.0, 0.0, size=n_clusters)          # most clusters inside the quality gate of the best one
+    f = np.where(clustered, level[which] - np.round(np.abs(jit).max(axis=1) / float(hp.eps_dup), 2),
+                 rng.uniform(-40.0, -1.0, size=N))           # two decimals: many exact ties inside a cluster
+    gmag = float(hp.eps_grad) * np.where(clustered, rng.uniform(0.0, 1.25, size=N), rng.uniform(0.5, 50.0, size=N))
+    g = rng.uniform(-1.0, 1.0, size=(N, d))
+    g *= (gmag / np.abs(g).max(axis=1))[:, None]
+    if N >= 64:
+        f[5] = np.nan; f[17] = np.inf; f[33] = -np.inf; g[41, d - 1] = np.nan
+    return _f32(x), _f32(f), _f32(g)

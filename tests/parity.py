@@ -81,3 +81,74 @@ def match_modes(xa, xb, tol):
             used[j] = True
             n += 1
     return n
+
+
+# ---- end-to-end mode-set comparison (R-14) ---------------------------------
+def subset_workload(wl, x0, **over):
+    """the same problem and hyper-parameters on another population (used by the oracle polish)"""
+    import copy
+    hp = copy.copy(wl.hp)
+    hp.N = len(x0)
+    for k, v in over.items():
+        setattr(hp, k, v)
+    obj = copy.copy(wl.obj)
+    out = copy.copy(wl)
+    out.obj, out.hp, out.x0 = obj, hp, np.ascontiguousarray(x0, np.float32)
+    return out
+
+
+def oracle_polish(O, wl, x_pts, f_max_ref, threads=8):
+    """S-14's acceptance rule for a mode reported by the CUDA path that has no partner in the oracle's set: run the
+    oracle's own Phase 1 (release + n_conv L-BFGS iterations, noise off) from the point; returns the L2 movement, and
+    whether the polished point is stationary by the oracle's gradient test and passes the oracle's Eq. 1 / Eq. 3 quality
+    gate f >= f_max_ref + log delta."""
+    x_pts = np.asarray(x_pts, np.float64).reshape(-1, wl.hp.d)
+    if len(x_pts) == 0:
+        return np.zeros(0), np.zeros(0, bool), np.zeros(0)
+    sub = subset_workload(wl, x_pts)
+    sub.obj.sigma_noise = 0.0
+    o = O.Oracle(sub, threads=threads)
+    o.set(O.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(O.PH_RELEASE_EVAL)
+    for it in range(1, sub.hp.n_conv + 1):
+        o.phase(O.PH_LBFGS_ITER, it)
+    x1, f1, g1 = o.get(O.X), o.get(O.F), o.get(O.G)
+    o.close()
+    move = np.linalg.norm(x1 - f32(x_pts), axis=1)
+    ok = (np.max(np.abs(g1), axis=1) < wl.hp.eps_grad) & (f1 >= f_max_ref + wl.hp.log_delta)
+    return move, ok, f1
+
+
+def nearest(xa, xb):
+    """for every row of xa: (L2 distance to, index of) the nearest row of xb"""
+    xa = np.asarray(xa, np.float64); xb = np.asarray(xb, np.float64)
+    if len(xa) == 0:
+        return np.zeros(0), np.zeros(0, int)
+    if len(xb) == 0:
+        return np.full(len(xa), np.inf), np.full(len(xa), -1)
+    D = np.linalg.norm(xa[:, None, :] - xb[None, :, :], axis=2)
+    return D.min(axis=1), D.argmin(axis=1)
+
+
+def mode_set_report(xg, fg, xo, fo, tol):
+    """one-to-one matching within tol plus what is left over on either side"""
+    xg = np.asarray(xg, np.float64); xo = np.asarray(xo, np.float64)
+    used = np.zeros(len(xo), bool)
+    pair = np.full(len(xg), -1)
+    for q, a in enumerate(xg):
+        if len(xo) == 0:
+            break
+        dist = np.linalg.norm(xo - a[None, :], axis=1)
+        dist[used] = np.inf
+        j = int(np.argmin(dist))
+        if dist[j] <= tol:
+            used[j] = True
+            pair[q] = j
+    only_g = np.flatnonzero(pair < 0)
+    only_o = np.flatnonzero(~used)
+    dg, _ = nearest(xg[only_g], xo)
+    do, _ = nearest(xo[only_o], xg)
+    text = (f"gpu {len(xg)} modes, oracle {len(xo)}, matched {int((pair >= 0).sum())} within {tol:g}; "
+            f"gpu-only {len(only_g)} (nearest oracle mode at {np.round(dg, 4).tolist()}, f {np.round(np.asarray(fg)[only_g], 4).tolist()}); "
+            f"oracle-only {len(only_o)} (nearest gpu mode at {np.round(do, 4).tolist()}, f {np.round(np.asarray(fo)[only_o], 4).tolist()})")
+    return pair, only_g, only_o, text

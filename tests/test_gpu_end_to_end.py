@@ -45,20 +45,133 @@ def test_c1_full_run_recovers_the_oracles_mode_set(orc, B):
     assert ei.value.code == B.E_STATE
 
 
-@pytest.mark.parametrize("c,N,cycles,tol", [(2, 1024, 6, 1e-3), (5, 256, 4, 1e-3)])
-def test_noise_free_mixtures_recover_the_same_modes(orc, B, c, N, cycles, tol):
-    """C2 / C5 with sigma_noise = 0 at reduced N (R-14): every mode of one side has a partner on the
-    other within 1e-3 L2 after the final cycle; noise-free thresholds follow the fp32 FD floor."""
-    # eps_grad bounds the position error of a frozen sample by eps_grad / curvature: 5e-4 keeps it under 1e-3 L2
-    over = dict(eps_grad=5e-4, eps_dup=1e-2, log_delta=float(np.log(1e-3)), n_conv=30) if c == 2 else \
-        dict(eps_grad=5e-4, eps_dup=1e-2, log_delta=-30.0, n_conv=60)
-    wl = inputs.config(c, N=N, n_osc=cycles, noise=0.0, **over)
+# noise-free thresholds of the end-to-end runs on the separated mixtures (R-14): eps_grad bounds the position
+# error of a frozen sample by eps_grad / curvature, so 5e-4 keeps it under 1e-3 L2; log_delta keeps every component peak
+# inside the quality gate of Eq. 1 so that the set does not hinge on one peak height
+E2E_NOISE_FREE = {2: dict(eps_grad=5e-4, eps_dup=1e-2, log_delta=float(np.log(1e-3)), n_conv=30),
+                  5: dict(eps_grad=5e-4, eps_dup=1e-2, log_delta=-30.0, n_conv=60)}
+
+
+def _explain_leftovers(orc, wl, xg, fg, xo, fo, only_g, only_o):
+    """S-14 diagnosis of unmatched modes: for the CUDA path's extra modes the oracle polish (movement, gate)"""
+    f_ref = float(np.max(fo)) if len(fo) else -np.inf
+    move, ok, f1 = PT.oracle_polish(orc, wl, xg[only_g], f_ref)
+    return (f"gpu-only modes under the oracle polish: moved {np.round(move, 5).tolist()}, oracle-stationary and inside the oracle's "
+            f"gate {ok.tolist()}, polished f {np.round(f1, 4).tolist()} (oracle f_max {f_ref:.4f}, log delta {wl.hp.log_delta:.3f})"), move, ok
+
+
+@pytest.mark.parametrize("c,N,cycles", [(2, 1024, 6), (5, 256, 4)])
+def test_noise_free_mixtures_recover_the_same_modes(orc, B, c, N, cycles):
+    """C2 / C5 with sigma_noise = 0 at reduced N (R-14): the mode sets are EQUAL -- every mode of one side has
+    its own partner on the other within 1e-3 L2 (north_star) -- and the values agree."""
+    wl = inputs.config(c, N=N, n_osc=cycles, noise=0.0, **E2E_NOISE_FREE[c])
     o, g, hist = _run_both(orc, B, wl)
     xo, fo, _ = o.modes()
     xg, fg, _, n = g.modes()
     assert n >= 1 and len(fo) >= 1
-    both = PT.match_modes(xg, xo, tol)
-    assert both >= 0.9 * max(n, len(fo)), (both, n, len(fo))
+    pair, only_g, only_o, text = PT.mode_set_report(xg, fg, xo, fo, 1e-3)
+    print(f"C{c} noise-free N={N}, {cycles} cycles: {text}")
+    why = _explain_leftovers(orc, wl, xg.astype(np.float64), fg, xo, fo, only_g, only_o)[0] if len(only_g) else ""
+    assert len(only_g) == 0 and len(only_o) == 0, text + " | " + why
+    m = pair >= 0
+    assert np.all(np.abs(fg.astype(np.float64)[m] - fo[pair[m]]) <= 1e-4 * np.maximum(np.abs(fo[pair[m]]), 1.0))
+
+
+def _read_golden(path):
+    rows = [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")]
+    idx = np.array([int(r[0]) for r in rows]); f = np.array([float(r[1]) for r in rows])
+    x = np.array([[float(v) for v in r[2:]] for r in rows])
+    return x, f, idx
+
+
+def test_c5_n4096_ten_cycles_recovers_the_oracles_stored_mode_set(orc, B):
+    """end-to-end parity at C5 on the reduced run "same d, K; N = 4096, 10 cycles", noise-free.
+    The oracle's mode set of this run is stored (tests/golden/c5_n4096_oracle_modes.txt, written by
+    tests/golden/make_c5_n4096_modes.py, which calls only oracle/: two hours of host time); the CUDA path must return
+    the same set, matched one to one within 1e-3 L2 (north_star)."""
+    import os
+    here = os.path.dirname(os.path.abspath(__file__))
+    sys_path_golden = os.path.join(here, "golden")
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_c5", os.path.join(sys_path_golden, "make_c5_n4096_modes.py"))
+    mk = importlib.util.module_from_spec(spec); spec.loader.exec_module(mk)
+    xo, fo, _ = _read_golden(mk.OUT)
+    wl = inputs.config(5, N=mk.E2E_N, n_osc=mk.E2E_CYCLES, noise=0.0, **mk.E2E_OVERRIDES)
+    g = B.Chisao(wl)
+    per_cycle = [g.step() for _ in range(mk.E2E_CYCLES)]
+    xg, fg, _, n = g.modes()
+    pair, only_g, only_o, text = PT.mode_set_report(xg, fg, xo, fo, 1e-3)
+    print(f"C5 noise-free N=4096, 10 cycles: {text}; gpu n_stuck per cycle {[s.n_stuck for s in per_cycle]}")
+    why = _explain_leftovers(orc, wl, xg.astype(np.float64), fg, xo, fo, only_g, only_o)[0] if len(only_g) else ""
+    assert len(only_g) == 0 and len(only_o) == 0, text + " | " + why
+    m = pair >= 0
+    assert np.all(np.abs(fg.astype(np.float64)[m] - fo[pair[m]]) <= 1e-4 * np.maximum(np.abs(fo[pair[m]]), 1.0))
+
+
+def test_c3_modes_are_modes_of_the_oracle(orc, B):
+    """C3 (random-Fourier landscape, d = 32): a landscape with very many near-equal local maxima, on which free-running
+    fp32 and fp64 trajectories end in different maxima, so the sets themselves differ (S-14 (c)).  Acceptance rule of
+    SURVEY.md S-14: a mode of the CUDA path is matched by an oracle mode within 1e-3 L2, or an oracle L-BFGS polish started
+    from it moves < 1e-3 and the polished point passes the oracle's own stick test and quality gate.  With the
+    config's n_conv = 15 nothing converges on either side (both return the empty set: checked), so the run uses
+    n_conv = 150."""
+    wl0 = inputs.config(3, N=512, n_osc=2)
+    o0, g0, _ = _run_both(orc, B, wl0)
+    assert len(o0.modes()[1]) == 0 and g0.modes()[3] == 0       # the configured C3: empty mode set on both sides
+    wl = inputs.config(3, N=1024, n_osc=4, n_conv=150)
+    o, g, hist = _run_both(orc, B, wl)
+    xo, fo, _ = o.modes()
+    xg, fg, _, n = g.modes()
+    xg = xg.astype(np.float64)
+    assert n >= 5 and len(fo) >= 5
+    pair, only_g, only_o, text = PT.mode_set_report(xg, fg, xo, fo, 1e-3)
+    why, move, ok = _explain_leftovers(orc, wl, xg, fg, xo, fo, only_g, only_o)
+    print(f"C3 N=1024, 4 cycles, n_conv=150: {text} | {why}")
+    # the quality gate is relative to each side's own f_max (Eq. 3): a gpu-only mode may sit below the oracle's gate only
+    # if the oracle's best mode is better than the CUDA path's best by more than that margin
+    f_ref = float(np.max(fo))
+    below = (np.asarray(fg, np.float64)[only_g] < f_ref + wl.hp.log_delta)
+    bad = ~ok & ~below
+    assert np.all(move < 1e-3), (int(np.sum(move >= 1e-3)), float(move.max()))
+    assert not bad.any(), why
+    assert below.sum() <= 0.1 * max(n, 1), (int(below.sum()), n, float(np.max(fg)), f_ref)
+    # same order of magnitude of modes, same best value within the tolerance on f
+    assert 0.5 * len(fo) <= n <= 2.0 * len(fo), (n, len(fo))
+    for so, sg in hist:
+        assert abs(sg.n_stuck - so.n_stuck) <= max(5, 0.25 * so.n_stuck), (sg.n_stuck, so.n_stuck)
+
+
+@pytest.mark.parametrize("c,N,cycles", [(2, 2048, 6), (5, 512, 4)])
+def test_noisy_mixtures_recover_the_same_components(orc, B, c, N, cycles):
+    """C2 / C5 as configured (sigma_noise = 0.1 / 1.0) at reduced N: under evaluation noise a frozen sample jitters inside
+    its peak, so modes are matched within the config's eps_dup sqrt(d) (S-14); every mode of one side must have a partner
+    on the other, except modes whose noise-free height lies within the noise of that side's quality gate
+    f_max + log delta (Eq. 3; f_max itself is a noisy maximum) -- those decisions are inside the noise band, are counted,
+    and must stay rare."""
+    wl = inputs.config(c, N=N, n_osc=cycles)
+    hp = wl.hp
+    o, g, hist = _run_both(orc, B, wl)
+    xo, fo, _ = o.modes()
+    xg, fg, _, n = g.modes()
+    xg = xg.astype(np.float64)
+    assert n >= 1 and len(fo) >= 1
+    tol = hp.eps_dup * np.sqrt(hp.d)
+    dg, _ = PT.nearest(xg, xo); do, _ = PT.nearest(xo, xg)
+    lone_g, lone_o = np.flatnonzero(dg > tol), np.flatnonzero(do > tol)
+    sn = wl.obj.sigma_noise
+    band = 6.0 * sn                                            # noise of f_i and of the maximum over the population
+    gate_g, gate_o = float(np.max(fg)) + hp.log_delta, float(np.max(fo)) + hp.log_delta
+    ft_g, ft_o = o.values(xg[lone_g]), o.values(xo[lone_o])    # noise-free heights of the unmatched modes
+    near_g = np.abs(ft_g - gate_o) <= band                     # the OTHER side's gate decides whether it could report it
+    near_o = np.abs(ft_o - gate_g) <= band
+    text = (f"C{c} noisy N={N}, {cycles} cycles: gpu {n} modes, oracle {len(fo)}, tolerance {tol:.3f}; gpu-only {len(lone_g)} "
+            f"(noise-free f {np.round(ft_g, 3).tolist()}, oracle gate {gate_o:.3f}), oracle-only {len(lone_o)} "
+            f"(noise-free f {np.round(ft_o, 3).tolist()}, gpu gate {gate_g:.3f}); band {band:.2f}")
+    print(text)
+    assert near_g.all() and near_o.all(), text
+    assert len(lone_g) + len(lone_o) <= max(1, 0.1 * max(n, len(fo))), text
+    for so, sg in hist:
+        assert sg.reseed_strategy == so.reseed_strategy or min(so.n_active, sg.n_active) < 10
 
 
 def test_c4_side_run_unimodal_collapses_to_the_maximiser(orc, B):
@@ -141,9 +254,13 @@ def test_ragged_and_degenerate_shapes_match_the_oracle(orc, B, d, N, M, m):
     fo = o.get(orc.HLC_F)
     assert np.all(np.abs(g.get(B.HLC_F) - fo) <= PT.F_REL * np.maximum(np.abs(fo), 1.0))
     PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+    x_before = o.get(orc.X).copy()
     o.phase(orc.PH_ANTI_STEP, 1); g.phase(B.PH_ANTI_STEP, 1)
     xo = o.get(orc.X)
-    assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1) <= 10 * PT.x_tol(xo, wl.hp.lo, wl.hp.hi))
+    # rule 4 with the gradient computed inside the unit: 1e-4 of the domain + 1e-3 of the step + alpha x the FD floor
+    step = np.max(np.abs(xo - x_before), axis=1)
+    floor = wl.hp.alpha_anti * PT.fd_floor(np.abs(o.values(x_before)), wl.hp.fd_h) * 4
+    assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1) <= PT.x_tol(xo, wl.hp.lo, wl.hp.hi, step, grad_inside=True) + floor)
 
 
 def test_empty_population(B):
@@ -273,9 +390,13 @@ def test_tensor_core_evaluator_shapes(orc, B, obj_id, d, K, N):
     ho = o.get(orc.HLC_F)
     assert np.all(np.abs(g.get(B.HLC_F) - ho) <= PT.F_REL * np.maximum(np.abs(ho), 1.0))
     PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+    x_before = o.get(orc.X).copy()
     o.phase(orc.PH_ANTI_STEP, 1); g.phase(B.PH_ANTI_STEP, 1)
     xo = o.get(orc.X)
-    assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1) <= 10 * PT.x_tol(xo, wl.hp.lo, wl.hp.hi))
+    # rule 4 with the gradient computed inside the unit: 1e-4 of the domain + 1e-3 of the step + alpha x the FD floor
+    step = np.max(np.abs(xo - x_before), axis=1)
+    floor = wl.hp.alpha_anti * PT.fd_floor(np.abs(o.values(x_before)), wl.hp.fd_h) * 4
+    assert np.all(np.max(np.abs(g.get(B.X) - xo), axis=1) <= PT.x_tol(xo, wl.hp.lo, wl.hp.hi, step, grad_inside=True) + floor)
 
 
 @pytest.mark.parametrize("sigma_noise,paper_err", [(1e-3, 2.1e-3), (0.1, 0.17), (0.5, 0.73)])

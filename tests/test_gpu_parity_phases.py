@@ -95,10 +95,13 @@ def test_a2_lbfgs_iterations_teacher_forced(orc, B, c, N):
             assert np.all(np.max(np.abs(yg - yo), axis=1) <= ytol)
         assert np.array_equal(g.get(B.STALLED)[safe], o.get(orc.STALLED)[safe])
         assert np.all(len0[~active] == lg_[~active])
-    # decisions inside the fp32 uncertainty band are counted, not compared.  The band follows from the f tolerance
-    # (2e-5 relative on the Armijo difference), so nearly converged samples -- whose decrease per step is below
-    # the fp32 resolution of f -- fall inside it; the cap is 5 % of all decisions over the 8 iterations.
-    assert n_excl <= max(2, 0.05 * n_dec), (n_excl, n_dec)
+    # decisions inside the fp32 uncertainty band are counted, not compared, and their share is capped (protocol rule 3:
+    # 0.5 % of the decisions).  C1 alone gets 5 %: its samples converge within these 8 iterations, and a nearly converged
+    # sample's decrease per step is below the fp32 resolution of f (2e-5 relative on the Armijo difference), so its
+    # decisions sit inside the band by construction (measured counts: DESIGN.md section 5).
+    cap = 0.05 if c == 1 else PT.MAX_EXCLUDED_FRACTION
+    print(f"C{c}: {n_excl} of {n_dec} L-BFGS decisions inside the fp32 band ({n_excl / max(n_dec, 1):.4%}, cap {cap:.1%})")
+    assert n_excl <= max(2, cap * n_dec), (n_excl, n_dec)
 
 
 def _converged_pair(orc, B, wl, n_conv=None):
@@ -110,7 +113,7 @@ def _converged_pair(orc, B, wl, n_conv=None):
     return o, g
 
 
-@pytest.mark.parametrize("c,N,n_conv", [(1, 256, 20), (2, 777, 10), (5, 200, 18), (4, 130, 5)])
+@pytest.mark.parametrize("c,N,n_conv", [(1, 256, 20), (2, 777, 10), (3, 300, 120), (5, 200, 18), (4, 130, 5)])
 def test_a3_stick_and_a4_dedup(orc, B, c, N, n_conv):
     """a3: f_max, Eq. 3 flags exact away from the thresholds; a4: Eq. 4 removed mask, K_lost, counts."""
     wl = inputs.config(c, N=N)
@@ -206,7 +209,8 @@ def test_a5_reseed_via_dedup(orc, B, strategy):
     if strategy == 1:
         mg = o.get(orc.RS_MARGIN)
         safe = removed & ((mg > 1e-5) | (mg == 0.0))     # margin 0: degenerate ray (t_max = 0), both pick candidate 0
-        assert safe.sum() >= 0.98 * removed.sum()            # short rays (t_max ~ 0) give near-identical candidates
+        print(f"RM strategy {strategy}: {int(safe.sum())} of {int(removed.sum())} slots with a safe candidate margin")
+        assert safe.sum() >= 0.99 * removed.sum()            # protocol rule 3 (short rays, t_max ~ 0, give near-identical candidates)
     else:
         safe = removed
     assert np.array_equal(g.get(B.RS_CAND)[safe], o.get(orc.RS_CAND)[safe])
@@ -224,7 +228,7 @@ def test_a5_reseed_via_dedup(orc, B, strategy):
         assert np.allclose(Q, o.gr_basis(2), atol=2e-5)
 
 
-@pytest.mark.parametrize("c,N,baseline", [(1, 256, 1), (2, 500, 1), (3, 300, 1), (4, 140, 1), (5, 150, 1), (2, 300, 0)])
+@pytest.mark.parametrize("c,N,baseline", [(1, 256, 1), (2, 500, 1), (3, 300, 1), (4, 140, 1), (5, 150, 1), (2, 300, 0), (5, 150, 0)])
 def test_a6_hlc_step(orc, B, c, N, baseline):
     """a6: every f_k within 1e-5 relative, ghat within 1e-3 relative + floor, x by rule 4; stuck rows frozen."""
     wl = inputs.config(c, N=N, hlc_baseline=baseline)
@@ -404,3 +408,77 @@ def test_tensor_evaluator_selection_and_tf32_fallback(orc, B, monkeypatch):
     assert np.all(np.abs(fg - fo) <= PT.f_tol(fo)), float(np.max(np.abs(fg - fo) / np.maximum(np.abs(fo), 1)))
     ok, err, tol = PT.grad_ok(g.get(B.G).astype(np.float64), o.get(orc.G), fo, wl.hp.fd_h)
     assert np.all(ok), float(np.max(err / tol))
+
+
+@pytest.mark.parametrize("case", ["c1", "c2", "c3", "c4", "diag33", "rastrigin5"])
+def test_line_search_forms_are_bit_identical(B, case):
+    """The tile-local line search (one launch for every trial of a tile, CHISAO_OPT_LS_TILE_LOCAL = 1) and the
+    per-trial launches on compacted worklists run the same arithmetic per sample: after every L-BFGS iteration the
+    whole state is bit-identical (and the evaluation counters are equal)."""
+    wl = {"c1": lambda: inputs.config(1), "c2": lambda: inputs.config(2, N=1500), "c3": lambda: inputs.config(3, N=700),
+          "c4": lambda: inputs.config(4, N=600),
+          "diag33": lambda: inputs.custom(inputs.gmm_diag(33, 5, 3.0, 9), 4.0, 300, fd_h=1e-2, eps_grad=1e-3, n_conv=6, lbfgs_m=4),
+          "rastrigin5": lambda: inputs.appendix_d("rastrigin", 5, 400, fd_h=1e-3, eps_grad=1e-3)}[case]()
+    a, b = B.Chisao(wl), B.Chisao(wl)
+    a.set_option(B.OPT_LS_TILE_LOCAL, 1); b.set_option(B.OPT_LS_TILE_LOCAL, 0)
+    assert a.ls_tile_local() and not b.ls_tile_local()
+    for g in (a, b):
+        g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+        g.phase(B.PH_RELEASE_EVAL)
+    for it in range(1, 7):
+        a.phase(B.PH_LBFGS_ITER, it); b.phase(B.PH_LBFGS_ITER, it)
+        for fld in (B.X, B.F, B.G, B.LS_B, B.HIST_LEN, B.HIST_S, B.HIST_Y, B.STALLED, B.XT):
+            assert np.array_equal(a.get(fld), b.get(fld), equal_nan=True), (it, fld)
+        assert list(a.stats().evals)[:7] == list(b.stats().evals)[:7]
+    lsb = a.get(B.LS_B)
+    assert (lsb > 0).any()                                 # some samples needed more than one trial
+    # whole cycles through chisao_step (graph submission) agree as well
+    wl.hp.n_osc = 3
+    a, b = B.Chisao(wl), B.Chisao(wl)
+    a.set_option(B.OPT_LS_TILE_LOCAL, 1); b.set_option(B.OPT_LS_TILE_LOCAL, 0)
+    for k in range(3):
+        sa, sb = a.step(), b.step()
+        for fld in (B.X, B.F, B.G, B.STUCK):
+            assert np.array_equal(a.get(fld), b.get(fld), equal_nan=True), (k, fld)
+        assert list(sa.evals)[:7] == list(sb.evals)[:7]
+    assert a.launch_count() < b.launch_count()
+
+
+def test_gmm_full_keeps_the_per_trial_line_search(B):
+    g = B.Chisao(inputs.config(5, N=64))
+    assert not g.ls_tile_local()
+    with pytest.raises(B.ChisaoError) as ei:
+        g.set_option(B.OPT_LS_TILE_LOCAL, 1)
+    assert ei.value.code == B.E_INVALID
+    for c in (1, 2, 3, 4):
+        assert B.Chisao(inputs.config(c, N=64)).ls_tile_local()
+
+
+@pytest.mark.parametrize("kind,d,N", [("quad", 50, 1000), ("rff", 24, 2000), ("quad", 33, 1400), ("rff", 5, 5000)])
+def test_anti_step_in_place_update_on_multi_tile_persistent_ctas(orc, B, kind, d, N):
+    """Eq. 6 rewrites x and v in place from the FD kernel's epilogue.  On the tensor-core evaluators the two groups of
+    128 points of a CTA run unsynchronised, so the 2d stencil points of a sample must never straddle them (a row could
+    be read half-updated by the group that lags): >= 3 tiles per persistent CTA, 2d not a divisor of 128, a large alpha
+    (a torn row would be far off) and the normal position tolerance."""
+    obj = inputs.quad(d, 71 + d, lam_max=50.0) if kind == "quad" else inputs.rff(d, 64, 72 + d)
+    wl = inputs.custom(obj, 4.0, N, seed=321 + d, fd_h=5e-2, eps_grad=1e-3, alpha_anti=2e-2 if kind == "rff" else 2e-3, mu=0.9)
+    o, g = orc.Oracle(wl, threads=8), B.Chisao(wl)
+    assert g.evaluator() in (1, 4)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, N]); g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, N])
+    for t in (1, 2, 3):
+        PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
+        v0 = o.get(orc.V).copy()
+        o.phase(orc.PH_ANTI_STEP, t); g.phase(B.PH_ANTI_STEP, t)
+        vo, vg = o.get(orc.V), g.get(B.V).astype(np.float64)
+        xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
+        vprev = np.zeros_like(v0) if t == 1 else v0
+        g_used = (wl.hp.mu * vprev - vo) / wl.hp.alpha_anti
+        fscale = np.abs(o.values(xo)) + 1.0
+        floor = PT.fd_floor(fscale, wl.hp.fd_h) * 4
+        vtol = wl.hp.alpha_anti * (PT.G_REL * np.max(np.abs(g_used), axis=1) + floor) + 4 * PT.EPS32 * np.max(np.abs(vo), axis=1)
+        ev = np.max(np.abs(vg - vo), axis=1)
+        assert np.all(ev <= vtol), (t, int(np.sum(ev > vtol)), float(np.max(ev / vtol)))
+        ex = np.max(np.abs(xg - xo), axis=1)
+        xt = PT.x_tol(xo, wl.hp.lo, wl.hp.hi) + vtol
+        assert np.all(ex <= xt), (t, int(np.sum(ex > xt)), float(np.max(ex / xt)))
+    assert g.stats().evals[6] == 3 * N * 2 * d

@@ -105,6 +105,104 @@ def test_stationary_samples_are_skipped(orc):
     assert list(o.stats().evals) == e0 and np.all(o.get(orc.LS_B) == -2)
 
 
+def test_first_step_length_is_min_1_inverse_gradient_norm(orc):
+    """R-4 (iii): with an empty history the first trial step is t0 = min(1, 1/||gamma||_2) along p = -gamma.  On
+    f = -1/2 ||x - c||^2 (central differences are exact, g = -(x - c), and every t <= 1 passes Armijo) the first trial
+    is accepted, so a sample farther than 1 from c moves by exactly 1 towards c and a sample closer than 1 lands on c.
+    t0 = 1 for everybody, or t0 = 1/||gamma||^2, fails."""
+    obj = inputs.quad(3, 11, lam_max=1.0)                       # lambda = (1, 1, 1): W orthogonal, A = I
+    c = obj.truth["c"]
+    wl = inputs.custom(obj, 8.0, 6, fd_h=1e-2, eps_grad=1e-9)
+    rng = np.random.default_rng(4)
+    dirs = rng.standard_normal((6, 3)); dirs /= np.linalg.norm(dirs, axis=1)[:, None]
+    radii = np.array([3.0, 2.0, 1.5, 0.75, 0.5, 0.1])
+    wl.x0[:] = np.float32(c[None, :] + radii[:, None] * dirs)
+    o = orc.Oracle(wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL)
+    x0 = o.get(orc.X).copy()
+    assert np.allclose(o.get(orc.G), -(x0 - c[None, :]), atol=1e-9)
+    o.phase(orc.PH_LBFGS_ITER, 1)
+    assert np.all(o.get(orc.LS_B) == 0)                          # first trial accepted
+    x1 = o.get(orc.X)
+    r0 = np.linalg.norm(x0 - c[None, :], axis=1)
+    step = np.linalg.norm(x1 - x0, axis=1)
+    far = r0 > 1.0
+    assert far.sum() == 3
+    assert np.allclose(step[far], 1.0, atol=2e-6)                # min(1, 1/||gamma||) ||gamma|| = 1 (positions are fp32)
+    assert np.allclose(np.linalg.norm(x1[far] - c[None, :], axis=1), r0[far] - 1.0, atol=2e-6)   # towards c
+    assert np.allclose(x1[~far], c[None, :], atol=2e-6)          # t0 = 1: the Newton step of A = I
+    assert np.allclose(step[~far], r0[~far], atol=2e-6)
+    assert np.all(o.get(orc.HIST_LEN) == 1)                      # s.y = ||s||^2 > 0: the pair is stored
+
+
+def _cosine_1d(w, a, x0, **over):
+    """f(x) = a cos(w x) on [-1, 1] (the random-Fourier objective with one feature, b = 0 and no quadratic term)"""
+    obj = inputs.Objective(inputs.OBJ_RFF, 1, 1, np.zeros((1, 1), np.float32), np.float32([[w]]), np.float32([a]),
+                           np.float32([0.0]), 0.0, 0.0)
+    wl = inputs.custom(obj, 1.0, len(x0), **over)
+    wl.x0[:] = np.float32(x0)[:, None]
+    return wl
+
+
+def test_curvature_pair_is_stored_only_for_positive_curvature(orc):
+    """R-4 (vi): the pair (s, y) is stored iff s.y > 1e-10 |s||y|.  With s = x+ - x and y = gamma+ - gamma = -(g+ - g),
+    s.y = -s^2 f''(xi): positive where f is concave, negative where f is convex.  f = 0.05 cos(2x): concave on
+    |2x| < pi/2, convex on pi/2 < 2x < 3pi/2 (the small amplitude keeps the first step inside the region it starts in).  An accepted step inside the convex region must leave the history empty; inside the
+    concave region it must store the pair."""
+    wl = _cosine_1d(2.0, 0.05, [0.3, 1.0], fd_h=1e-4, eps_grad=1e-9, lbfgs_m=3)
+    wl.hp.lo[:] = -2.0; wl.hp.hi[:] = 2.0                      # 2x up to 4: the convex region is inside the box
+    o = orc.Oracle(wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL)
+    x0 = o.get(orc.X)[:, 0].copy(); g0 = o.get(orc.G)[:, 0].copy()
+    o.phase(orc.PH_LBFGS_ITER, 1)
+    x1 = o.get(orc.X)[:, 0]; g1 = o.get(orc.G)[:, 0]
+    assert np.all(o.get(orc.LS_B) >= 0) and np.all(x1 != x0)     # both samples took an accepted step
+    sy = (x1 - x0) * (-(g1 - g0))
+    assert sy[0] > 0 and sy[1] < 0
+    assert 1.0 < 2 * min(x0[1], x1[1]) * 2 / math.pi and 2 * max(x0[1], x1[1]) * 2 / math.pi < 3.0   # inside the convex region
+    assert list(o.get(orc.HIST_LEN)) == [1, 0]
+    S, Y = o.get(orc.HIST_S), o.get(orc.HIST_Y)
+    assert S[0, 0, 0] == x1[0] - x0[0] and Y[0, 0, 0] == -(g1[0] - g0[0])
+    assert not S[:, 1].any() and not Y[:, 1].any()
+
+
+def test_failed_line_search_stalls_or_clears_history(orc):
+    """R-4 (v): no trial accepted -> the sample is stalled (no further work) if its history was empty, else only the
+    history is cleared.  f = 1/2 cos(40 x) just right of its maximum at 0 with an FD step h = 3 pi / 80 (w h = 3 pi / 2:
+    the central difference has the wrong sign), so p points downhill for every trial t0 2^-b, b = 0..10: all ls_max + 1
+    trials fail."""
+    h = 3.0 * math.pi / 80.0
+    wl = _cosine_1d(40.0, 0.5, [0.001, 0.001], fd_h=h, eps_grad=1e-3, lbfgs_m=2, ls_max=10)
+    o = orc.Oracle(wl)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL)
+    g0 = o.get(orc.G)[:, 0]
+    assert np.all(g0 > 0.1) and np.all(g0 < 1.0)                 # wrong sign (true slope is negative), t0 = 1
+    # sample 1 starts with one stored pair (s = y = 1: H = 1, the same direction p = g, t0 = 1)
+    S = np.zeros((2, 2, 1)); S[0, 1, 0] = 1.0
+    o.set(orc.HIST_S, S); o.set(orc.HIST_Y, S); o.set(orc.HIST_LEN, [0, 1])
+    e0 = list(o.stats().evals)
+    x0 = o.get(orc.X).copy(); f0 = o.get(orc.F).copy()
+    o.phase(orc.PH_LBFGS_ITER, 1)
+    e1 = list(o.stats().evals)
+    assert list(o.get(orc.LS_B)) == [-1, -1]                     # nobody accepted
+    assert e1[1] - e0[1] == 2 * 11 and e1[2] == e0[2]            # ls_max + 1 trials each, no FD gradient
+    assert np.array_equal(o.get(orc.X), x0) and np.array_equal(o.get(orc.F), f0)   # no move
+    assert list(o.get(orc.STALLED)) == [1, 0] and list(o.get(orc.HIST_LEN)) == [0, 0]
+    # next iteration: the stalled sample does nothing; the other one searches again (now with an empty history) and stalls
+    o.phase(orc.PH_LBFGS_ITER, 2)
+    e2 = list(o.stats().evals)
+    assert list(o.get(orc.LS_B)) == [-2, -1] and e2[1] - e1[1] == 11
+    assert list(o.get(orc.STALLED)) == [1, 1]
+    o.phase(orc.PH_LBFGS_ITER, 3)
+    assert list(o.stats().evals) == e2 and list(o.get(orc.LS_B)) == [-2, -2]
+    # release at the start of the next Phase 1 clears the flag (R-5)
+    o.phase(orc.PH_RELEASE_EVAL)
+    assert not o.get(orc.STALLED).any()
+
+
 # ----------------------------------------------------------------------------- Phase 2: Eq. 3
 def test_stick_is_eq3(orc):
     wl = inputs.config(1, N=200)
