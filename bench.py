@@ -92,18 +92,20 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-def oracle_throughput(c: int, steps: int, warmup: int, rank_seed: int = 0):
-    """Time the oracle as it stands on a bounded sample of workload `c` (host cores of this box)."""
+def oracle_throughput(c: int, steps: int, warmup: int, threads: int = 0):
+    """Time the oracle as it stands on a bounded sample of workload `c` (host cores of this box): `warmup` untimed
+    cycles, then `steps` timed ones; OpenMP over the samples with `threads` threads (0 = every core of the box)."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle as O
     from paper_2606_26164_b200 import inputs
     cores = len(os.sched_getaffinity(0))
+    threads = threads or cores
     full = inputs.config(c)
-    # ~1.5 s of one core per sample-cycle at C5: 8 samples per core keep one step in the 10-20 s range
-    per_core = {1: 256, 2: 256, 3: 24, 4: 32, 5: 8}[c]
-    Ns = min(full.hp.N, max(8, per_core * cores))
+    # ~1.5 s of one core per sample-cycle at C5: 8 samples per thread keep one step in the 10-20 s range
+    per_thread = {1: 256, 2: 256, 3: 24, 4: 32, 5: 8}[c]
+    Ns = min(full.hp.N, max(8, per_thread * threads))
     wl = inputs.config(c, N=Ns, n_osc=max(full.hp.n_osc, steps + warmup + 1))
-    o = O.Oracle(wl, threads=cores)
+    o = O.Oracle(wl, threads=threads)
     for _ in range(warmup):
         o.step()
     ev0 = sum(o.stats().evals)
@@ -113,9 +115,9 @@ def oracle_throughput(c: int, steps: int, warmup: int, rank_seed: int = 0):
     dt = time.perf_counter() - t0
     ev = sum(o.stats().evals) - ev0
     o.close()
-    return {"value": Ns * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+    return {"value": Ns * steps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": f"{Ns} of {full.hp.N} samples x {steps} full cycle(s) after {warmup} warm-up cycle(s), fp64, "
-                      f"OpenMP over samples; per-sample cost is N-independent except deduplication",
+                      f"OpenMP over samples on {threads} of {cores} host cores; per-sample cost is N-independent except deduplication",
             "f_evals_per_sec": ev / dt, "seconds": dt}, wl
 
 
@@ -123,9 +125,10 @@ def run_reference(args, rank, world):
     if rank != 0:
         return
     # the oracle is slow by design: one warm-up cycle is enough to page everything in
-    res, wl = oracle_throughput(args.config, max(1, args.steps), min(args.warmup, 1))
+    res, wl = oracle_throughput(args.config, max(3, args.steps), max(1, min(args.warmup, 1)))
+    steps = max(3, args.steps)
     line = {"impl": "reference", "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * res["seconds"] / max(1, args.steps),
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * res["seconds"] / steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD_TEXT[args.config], "sampled": res["sample"]},
             "cpu_baseline": {k: res[k] for k in ("value", "unit", "cores", "kind", "sample")},
@@ -134,33 +137,33 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def run_ours(args, rank, local_rank, world):
-    import torch
-    import torch.distributed as dist
-    from paper_2606_26164_b200 import binding as B, inputs, replicas
+def measured_alu_peaks(dev):
+    """FP32 FMA (TFLOP/s) and SFU (T op/s) rates of this GPU, measured now by the library's probe kernels
+    (chisao_measure_peak: include/chisao.h); they are the denominators of the "alu" rooflines."""
+    from paper_2606_26164_b200 import binding as B
+    return {"fp32_fma_tflops": B.measure_peak(B.PEAK_FP32_FMA, dev), "sfu_tops": B.measure_peak(B.PEAK_SFU, dev),
+            "source": "measured in this run: chisao_measure_peak (FFMA / MUFU.EX2 micro-benchmark kernels, best of 5)"}
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    K, W, c = args.steps, args.warmup, args.config
+
+def measure_config(c, K, W, rank, local_rank, world, dist, dev, N_override=0, detail=True, alu=None):
+    """Device-resident and end-to-end timing of `K` full cycles of workload `c` after `W` warm-up cycles, plus the
+    roofline of its dominant kernel.  Returns the fields of the JSON line that depend on the workload."""
+    import torch
+    from paper_2606_26164_b200 import binding as B, inputs, replicas
     full = inputs.config(c)
-    N = args.N or full.hp.N
+    N = N_override or full.hp.N
     n_osc = max(full.hp.n_osc, 2 * K + W + 1)               # timed cycles are all full cycles (phases 1-6)
     wl = replicas.replica_workload(c, rank, N=N, n_osc=n_osc)
     hp = wl.hp
+    dd = dist if world > 1 else None
 
-    # ---- device-resident timing: W warm-up cycles, then exactly K cycles between CUDA events -------------
+    # ---- device-resident timing: W warm-up cycles, then exactly K cycles between CUDA events.  No per-launch event
+    # bracketing here: chisao_step submits every cycle as ONE CUDA graph launch (the product's default path)
     g = B.Chisao(wl, device=dev)
     for _ in range(W):
         g.step(stats=False)
     st0 = g.stats()
-    # only the two roofline kernels are bracketed with events inside the timed region (two event records per launch
-    # are measurable on the launch-bound configurations); the full per-phase table comes from a second pass below
-    g.timing_enable(("eval_fd", "lbfgs_direction")); g.timing_reset()
-    l0 = g.launch_count()
+    l0, gl0 = g.launch_count(), g.graph_launches()
     sampler = ClockSampler(local_rank); sampler.start()
     time.sleep(0.25)
     ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -177,16 +180,21 @@ def run_ours(args, rank, local_rank, world):
     ms = ev_a.elapsed_time(ev_b)
     clocks = sampler.stop()
     launches = g.launch_count() - l0
+    graphs = g.graph_launches() - gl0
     st1 = g.stats()
-    phase_ms = g.timing()
-    g.timing_enable(True); g.timing_reset()                 # second pass: K more cycles with every kernel class bracketed
+    evals = np.array(st1.evals[:], np.int64) - np.array(st0.evals[:], np.int64)
+    # ---- per-kernel-class times: K more cycles submitted directly, every launch bracketed with CUDA events on the
+    # launching stream (the same kernels, the same state trajectory one cycle later; the brackets cost two event records
+    # per launch, which is why they are not inside the timed region above)
+    g.timing_enable(True); g.timing_reset()
+    st2 = g.stats()
     for _ in range(K):
         g.step(stats=False)
     phase_all = g.timing()
     g.timing_enable(False)
-    evals = np.array(st1.evals[:], np.int64) - np.array(st0.evals[:], np.int64)
-    ms_max = replicas.max_over_ranks(ms, dist if world > 1 else None, dev)
-    total_evals = replicas.sum_over_ranks(float(evals[[0, 1, 2, 5, 6]].sum()), dist if world > 1 else None, dev)
+    evals2 = np.array(g.stats().evals[:], np.int64) - np.array(st2.evals[:], np.int64)
+    ms_max = replicas.max_over_ranks(ms, dd, dev)
+    total_evals = replicas.sum_over_ranks(float(evals[[0, 1, 2, 5, 6]].sum()), dd, dev)
 
     # ---- end to end through the host-buffer C-ABI call (H2D + cycle + D2H inside the timed region) -------
     g2 = B.Chisao(wl, device=dev)
@@ -205,30 +213,33 @@ def run_ours(args, rank, local_rank, world):
         g2.step_host(x_host, x_out, f_out, s_out)           # synchronises before returning
         x_host.copy_(x_out)
     e2e_s = time.perf_counter() - t0
-    e2e_s = replicas.max_over_ranks(e2e_s, dist if world > 1 else None, dev)
+    e2e_s = replicas.max_over_ranks(e2e_s, dd, dev)
     g2.close()
 
-    # ---- roofline of the dominant kernel (k_eval_fd: objective evaluation + FD stencil) -------------------
+    # ---- roofline of the dominant kernel (k_eval_fd: objective evaluation + FD stencil), from the bracketed pass ------
     peaks, peaks_src = measured_peaks()
     fpe = flop_per_eval(wl.obj)
-    fd_evals = float(evals[0] - K * hp.N + evals[2] + evals[6])     # counter 0 also holds the N centre values
-    fd_ms, fd_n = phase_ms["eval_fd"]
-    alu_peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12   # TFLOP/s, FP32 FMA lanes x clock
+    fd_evals = float(evals2[0] - K * hp.N + evals2[2] + evals2[6])  # counter 0 also holds the N centre values
+    fd_ms, fd_n = phase_all["eval_fd"]
+    step_ms2 = sum(v[0] for v in phase_all.values())               # sum of the bracketed kernel times of that pass
+    alu_peak = alu["fp32_fma_tflops"] if alu else 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+    alu_src = alu["source"] if alu else f"nominal: 148 SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json clocks)"
     achieved = fd_evals * fpe / (fd_ms * 1e-3) / 1e12 if fd_ms > 0 else 0.0
-    on_tensor = g.evaluator() != 0                          # dense objectives at d > 32 and RFF at d <= 32 run on tcgen05 (chisao_tc.cuh)
-    if on_tensor:
+    ev_mode = g.evaluator()
+    traffic = TRAFFIC_BYTES_PER_LAUNCH.get(c)
+    if ev_mode != 0:                                        # dense objectives at d > 32 and RFF at d <= 32 run on tcgen05 (chisao_tc.cuh)
         # kind::tf32 peak = measured bf16 cuBLAS throughput (sustained: the kernel is timed inside a long step) x the
         # guide's nominal tf32 : bf16 ratio 1.1 : 2.25.  The 3xTF32 split executes three tensor flops per
         # algorithmic flop of the contraction, so frac <= 1/3 by construction; executed_frac says how busy the pipe is.
-        ev_mode = g.evaluator()                                # 1, 2: kind::tf32;  3: kind::f16 (fp16 hi / lo operands)
-        f16 = ev_mode in (3, 4)                                # 4: random-Fourier phases, six products of 10-bit fp16 pieces
+        f16 = ev_mode in (3, 4)                                # 3: fp16 hi / lo operands; 4: random-Fourier phases, six products of 10-bit fp16 pieces
         peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * (1.0 if f16 else 1.1 / 2.25)
         pipe_rate = 8192 if f16 else 4096                      # flop / clk / SM: one 128x128x16 f16 (x8 tf32) MMA per 64 clocks
         contraction = wl.obj.K * 2.0 * hp.d * (1 if ev_mode == 4 else hp.d)
         nprod = 6.0 if ev_mode == 4 else 3.0                   # tensor flops executed per algorithmic flop of the contraction
         executed = nprod * fd_evals * contraction / (fd_ms * 1e-3) / 1e12 if fd_ms > 0 else 0.0
         roofline = {"bound": "tensor", "kernel": "k_eval_fd_tc", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                    "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(c),
+                    "frac": achieved / peak, "traffic": traffic["bytes"] if traffic else None,
+                    "traffic_source": traffic["source"] if traffic else None,
                     "evaluator": B.EVALUATOR_NAMES[ev_mode],
                     "peak_source": f"bf16_tflops_sustained ({peaks_src} MEASURED_PEAKS.json)" + ("" if f16 else " x 1.1/2.25 (tf32:bf16 nominal)")
                                    + f"; the operand split executes {nprod:.0f} tensor flops per algorithmic flop of the contraction",
@@ -238,17 +249,51 @@ def run_ours(args, rank, local_rank, world):
                     # the kernel runs into the 1000 W power cap, so that clock is well below sm_max_mhz
                     "tensor_peak_at_sampled_clock": (pipe_rate * 148 * clocks["sm_mhz"] * 1e6 / 1e12) if clocks.get("sm_mhz") else None,
                     "executed_frac_at_sampled_clock": (executed / (pipe_rate * 148 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
-                    "fp32_alu_peak_tflops": alu_peak, "vs_fp32_alu_peak": achieved / alu_peak}
+                    "fp32_alu_peak_tflops": alu_peak, "alu_peak_source": alu_src, "vs_fp32_alu_peak": achieved / alu_peak}
     else:
         roofline = {"bound": "alu", "kernel": "k_eval_fd", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
-                    "frac": achieved / alu_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(c),
-                    "peak_source": f"148 SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json clocks)"}
+                    "frac": achieved / alu_peak, "traffic": traffic["bytes"] if traffic else None,
+                    "traffic_source": traffic["source"] if traffic else None,
+                    "peak_source": alu_src, "alu_peak_source": "measured" if alu else "nominal"}
     roofline.update({"launches": fd_n, "ms_per_launch": fd_ms / max(fd_n, 1), "flop_per_eval": fpe,
-                     "share_of_step": fd_ms / ms if ms > 0 else None})
-    # HBM-bound history kernel (two-loop recursion over the spilled (s, y) pairs)
-    dir_ms, dir_n = phase_ms["lbfgs_direction"]
-    hist_bytes = float(evals[7])                            # counted on the device: rows actually read / written
-    hbm = {"bound": "hbm", "kernel": "k_lbfgs_direction", "achieved": hist_bytes / (dir_ms * 1e-3) / 1e9 if dir_ms > 0 else 0.0,
+                     "share_of_step": fd_ms / step_ms2 if step_ms2 > 0 else None,
+                     "timing": "per-launch CUDA events on the launching stream over K cycles submitted directly, right after the "
+                               "timed region (which is one graph launch per cycle); share_of_step = this kernel's time / all bracketed kernel time"})
+    out = {
+        "value": world * hp.N * K / (ms_max * 1e-3), "ms_per_step": ms_max / K,
+        "config": {"workload": WORKLOAD_TEXT[c], "N_per_gpu": hp.N, "d": hp.d, "n_conv": hp.n_conv, "lbfgs_m": hp.lbfgs_m,
+                   "hlc_M": hp.hlc_M, "n_cloud": hp.n_cloud, "n_anti": hp.n_anti, "fd_h": hp.fd_h,
+                   "parallelism": "replicas" if world > 1 else "single",
+                   "submission": f"{graphs} of {K} timed cycles submitted as one CUDA graph launch each",
+                   "line_search": "tile-local rounds (one launch per iteration)" if g.ls_tile_local() else "one launch per trial on compacted worklists",
+                   "l2": f"state per cycle {g.workspace_bytes / 2**20:.0f} MiB vs 126 MB L2: "
+                         + ("inputs larger than L2" if g.workspace_bytes > 126e6 else "fits L2 (latency-bound config)")},
+        "f_evals_per_sec": total_evals / (ms_max * 1e-3),
+        "evals_per_step": float(evals[[0, 1, 2, 5, 6]].sum()) / K,
+        "clocks": clocks,
+        "e2e": {"value": world * hp.N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": hp.N * hp.d * 4,
+                "d2h_bytes_per_step": hp.N * hp.d * 4 + hp.N * 4 + hp.N},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "phase_ms_per_step": {k: round(v[0] / K, 4) for k, v in phase_all.items()},
+    }
+    per_rank = None
+    if world > 1:
+        t = torch.zeros(world, dtype=torch.float64, device=dev); t[rank] = ms
+        dist.all_reduce(t)
+        per_rank = [float(v) / K for v in t.tolist()]
+        out["per_rank_ms_per_step"] = per_rank
+    if not detail:
+        g.close()
+        return out, wl, None
+
+    # HBM-bound history kernel (two-loop recursion over the spilled (s, y) pairs; inside a cycle it also carries the
+    # update of the previous iteration: k_lbfgs_step)
+    dir_ms, dir_n = phase_all["lbfgs_direction"]
+    hist_bytes = float(evals2[7])                           # counted on the device: rows actually read / written
+    upd_ms = phase_all["lbfgs_update"][0]
+    hbm = {"bound": "hbm", "kernel": "k_lbfgs_step + k_lbfgs_update (inside the cycle)",
+           "achieved": hist_bytes / ((dir_ms + upd_ms) * 1e-3) / 1e9 if dir_ms > 0 else 0.0,
            "peak": peaks["hbm_gbs"], "unit": "GB/s", "bytes_per_launch": hist_bytes / max(dir_n, 1),
            "ms_per_launch": dir_ms / max(dir_n, 1)}
     hbm["frac"] = hbm["achieved"] / hbm["peak"]
@@ -270,16 +315,47 @@ def run_ours(args, rank, local_rank, world):
         g3.phase(B.PH_LBFGS_DIRECTION)
     full_ms, full_n = g3.timing()["lbfgs_direction"]
     full_bytes = float(g3.stats().evals[7] - e0)
-    hbm_full = {"bound": "hbm", "kernel": "k_lbfgs_direction (all samples active, len = m)", "achieved": full_bytes / (full_ms * 1e-3) / 1e9,
+    hbm_full = {"bound": "hbm", "kernel": "k_lbfgs_step (direction only; all samples active, len = m)", "achieved": full_bytes / (full_ms * 1e-3) / 1e9,
                 "peak": peaks["hbm_gbs"], "unit": "GB/s", "bytes_per_launch": full_bytes / max(full_n, 1),
                 "ms_per_launch": full_ms / max(full_n, 1)}
     hbm_full["frac"] = hbm_full["achieved"] / hbm_full["peak"]
     g3.close()
+    out["hbm_kernel"], out["hbm_kernel_full_history"] = hbm, hbm_full
+    g.close()
+    return out, wl, evals
+
+
+def run_ours(args, rank, local_rank, world):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_26164_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    K, W, c = args.steps, args.warmup, args.config
+    alu = measured_alu_peaks(dev)
+    res, wl, _ = measure_config(c, K, W, rank, local_rank, world, dist, dev, N_override=args.N, detail=True, alu=alu)
+    hp = wl.hp
+
+    # ---- the other four BASELINE.json configs, short (3 warm-up + 5 cycles each): north_star asks for all five ----------
+    others = None
+    if c == 5 and not args.N and not args.no_other_configs:
+        others = {}
+        for cc in (1, 2, 3, 4):
+            r, _, _ = measure_config(cc, 5, 3, rank, local_rank, world, dist, dev, detail=False, alu=alu)
+            others[f"C{cc}"] = {k: r[k] for k in ("value", "ms_per_step", "f_evals_per_sec", "gpu_launches", "clocks", "e2e",
+                                                  "roofline", "phase_ms_per_step", "config")}
+            others[f"C{cc}"]["steps"], others[f"C{cc}"]["warmup"], others[f"C{cc}"]["unit"] = 5, 3, UNIT
 
     # ---- NEXT-5, reported SEPARATELY (never mixed into `value`): the same cycles with the opt-in stencil-aware FD
     # evaluator of the dense objectives (chisao_set_option; not a black-box evaluation of f)
     stencil = None
     if wl.obj.id in (2, 4) and not args.no_stencil_pass:
+        from paper_2606_26164_b200 import replicas
         g4 = B.Chisao(wl, device=dev)
         g4.set_option(B.OPT_STENCIL_AWARE, 1)
         for _ in range(W):
@@ -302,42 +378,48 @@ def run_ours(args, rank, local_rank, world):
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            cpu, _ = oracle_throughput(c, 1, 0)
-            cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "f_evals_per_sec")}
-        value = world * hp.N * K / (ms_max * 1e-3)
-        bi = hp.N * hp.d * 4
-        bo = hp.N * hp.d * 4 + hp.N * 4 + hp.N
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOAD_TEXT[c], "N_per_gpu": hp.N, "d": hp.d, "n_conv": hp.n_conv, "lbfgs_m": hp.lbfgs_m,
-                       "hlc_M": hp.hlc_M, "n_cloud": hp.n_cloud, "n_anti": hp.n_anti, "fd_h": hp.fd_h,
-                       "parallelism": "replicas" if world > 1 else "single",
-                       "l2": f"state per cycle {g.workspace_bytes / 2**20:.0f} MiB vs 126 MB L2: "
-                             + ("inputs larger than L2" if g.workspace_bytes > 126e6 else "fits L2 (latency-bound config)")},
-            "f_evals_per_sec": total_evals / (ms_max * 1e-3),
-            "evals_per_step": float(evals[[0, 1, 2, 5, 6]].sum()) / K,
-            "clocks": clocks,
-            "e2e": {"value": world * hp.N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo},
-            "gpu_launches": int(launches),
-            "roofline": roofline, "hbm_kernel": hbm, "hbm_kernel_full_history": hbm_full,
-            "phase_ms_per_step": {k: round(v[0] / K, 4) for k, v in phase_all.items()},
-            "phase_ms_note": "second pass of K cycles with every kernel class bracketed by events (not the timed region)",
-            "cpu_baseline": cpu,
-            "stencil_aware_separately": stencil,
-        }
+            # same policy as --impl reference: one warm-up cycle, three timed cycles; all cores, then one core
+            cpu_all, _ = oracle_throughput(c, 3, 1)
+            cpu_one, _ = oracle_throughput(c, 3, 1, threads=1)
+            cpu = {k: cpu_all[k] for k in ("value", "unit", "cores", "kind", "sample", "f_evals_per_sec")}
+            cpu["one_core"] = {k: cpu_one[k] for k in ("value", "unit", "cores", "sample", "f_evals_per_sec")}
+        line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic"}
+        for k in ("config", "f_evals_per_sec", "evals_per_step", "clocks", "e2e", "gpu_launches", "roofline", "hbm_kernel",
+                  "hbm_kernel_full_history", "phase_ms_per_step", "per_rank_ms_per_step"):
+            if k in res:
+                line[k] = res[k]
+        line["phase_ms_note"] = "K cycles submitted directly right after the timed region, every kernel class bracketed by events"
+        line["alu_peaks"] = alu
+        line["cpu_baseline"] = cpu
+        line["stencil_aware_separately"] = stencil
+        line["configs"] = others
         print(json.dumps(line), flush=True)
-    g.close()
     if world > 1:
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per k_eval_fd launch from the committed `ncu --set full`
-# capture (profiles/); None until a capture of that workload exists.
-TRAFFIC_BYTES_PER_LAUNCH = {5: 1.84e7,   # profiles/r1_evalfd_c5_f16.md (full-size launch: 18.35 MB read, 0.07 MB written)
-                            3: 2.26e6,   # profiles/r1_evalfd_c3_rfftc.md (2.26 MB read, 0 written: the gradient stays in L2)
-                            4: 4.33e6}   # profiles/r1_evalfd_c4_quad.md (4.33 MB read, 0 written)
+# dram__bytes_read.sum + dram__bytes_write.sum per k_eval_fd launch, read off the committed `ncu --set full` capture named
+# beside it (profiles/); not measured in this run -- a run under ncu is never a bench value
+TRAFFIC_BYTES_PER_LAUNCH = {
+    5: {"bytes": 1.84e7, "source": "profiles/r1_evalfd_c5_f16.md (full-size launch: 18.35 MB read, 0.07 MB written)"},
+    3: {"bytes": 2.26e6, "source": "profiles/r1_evalfd_c3_rfftc.md (2.26 MB read, 0 written: the gradient stays in L2)"},
+    4: {"bytes": 4.33e6, "source": "profiles/r1_evalfd_c4_quad.md (4.33 MB read, 0 written)"}}
+
+
+def self_launch(args):
+    """`python bench.py --gpus N` without a launcher: start N ranks of this script with torch.distributed.run (one process
+    per GPU, rendezvous on 127.0.0.1) and pass their output through; rank 0 prints the JSON line."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    env.setdefault("NCCL_DEBUG", "INFO"); env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")   # the communicator log names the rank count
+    raise SystemExit(subprocess.call(cmd, env=env))
 
 
 def main():
@@ -350,7 +432,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stencil-pass", action="store_true", help="skip the separately reported NEXT-5 pass")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short C1..C4 sub-records of the default run")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        self_launch(args)
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -230,6 +230,15 @@ CHISAO_API int chisao_timing_enable(chisao_ctx *ctx, int32_t on);
 CHISAO_API int chisao_timing_reset(chisao_ctx *ctx);
 CHISAO_API int chisao_timing_get(chisao_ctx *ctx, int32_t which, double *ms, uint64_t *launches);
 
+/* Pipe-rate probes for the roofline denominators (FP32 FMA and special-function rates are to be
+ * measured in the same run, because the clocks under load differ from the nominal ones).  Runs a hand-written
+ * micro-benchmark kernel (8 CTAs of 256 threads per SM, 8 independent dependency chains per thread) on `stream`, timed with
+ * CUDA events, best of 5 after one warm-up; *value = TFLOP/s (CHISAO_PEAK_FP32_FMA: 2 flop per FFMA) or T operations/s
+ * (CHISAO_PEAK_SFU: MUFU.EX2).  scratch_dev: >= 4 bytes of device memory.  Synchronises.  Not part of the CHISAO path. */
+#define CHISAO_PEAK_FP32_FMA 0
+#define CHISAO_PEAK_SFU 1
+CHISAO_API int chisao_measure_peak(int32_t which, float *scratch_dev, void *stream, double *value);
+
 CHISAO_API const char *chisao_last_error(const chisao_ctx *ctx_or_null);
 CHISAO_API void chisao_destroy(chisao_ctx *ctx);
 

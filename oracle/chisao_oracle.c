@@ -37,6 +37,7 @@ struct orc_ctx {
   /* diagnostics */
   double *p, *ls_margin, *asc_margin, *curv_margin, *ghat, *hlc_f, *hlc_u, *rs_margin;
   int32_t *ls_b, *rs_src, *rs_cand;
+  double *rs_score;                  /* [N][16] diagnostic: the score (min squared distance to the modes) of every candidate */
 };
 
 /* ------------------------------------------------------------------------------------------------
@@ -491,6 +492,7 @@ static void rm_slot(orc_ctx *s, int r, const int *A, int nA, const int *P, int n
       for (int j = 0; j < d; ++j) { double t = cand[j] - xp[j]; d2 += t * t; }
       if (d2 < mind) mind = d2;
     }
+    if (c < 16) s->rs_score[(size_t)r * 16 + c] = mind;
     if (mind > best) { second = best; best = mind; bestc = c; memcpy(out, cand, sizeof(double) * d); }
     else if (mind > second) second = mind;
   }
@@ -779,6 +781,7 @@ orc_ctx *orc_create(const orc_config *cfg, const orc_objective *obj, const float
   s->ls_b = (int32_t *)calloc(N ? N : 1, sizeof(int32_t));
   s->rs_src = (int32_t *)calloc(N ? N : 1, sizeof(int32_t));
   s->rs_cand = (int32_t *)calloc(N ? N : 1, sizeof(int32_t));
+  s->rs_score = DALLOC(N * 16);
   s->gr_enabled = 1; s->f_max = -INFINITY;
   return s;
 }
@@ -789,7 +792,7 @@ void orc_destroy(orc_ctx *s) {
   free(s->x); free(s->f); free(s->g); free(s->v); free(s->S); free(s->Y); free(s->len);
   free(s->stuck); free(s->removed); free(s->stalled); free(s->p); free(s->ls_margin); free(s->asc_margin);
   free(s->curv_margin); free(s->ghat); free(s->hlc_f); free(s->hlc_u); free(s->rs_margin);
-  free(s->ls_b); free(s->rs_src); free(s->rs_cand);
+  free(s->ls_b); free(s->rs_src); free(s->rs_cand); free(s->rs_score);
   free(s);
 }
 
@@ -850,6 +853,7 @@ static int xfer_field(orc_ctx *s, int field, void *u, uint64_t bytes, int to_use
   case ORC_RS_SRC: return xfer(s->rs_src, 4 * N, u, bytes, to_user);
   case ORC_RS_CAND: return xfer(s->rs_cand, 4 * N, u, bytes, to_user);
   case ORC_RS_MARGIN: return xfer(s->rs_margin, 8 * N, u, bytes, to_user);
+  case ORC_RS_SCORE: return xfer(s->rs_score, 8 * N * 16, u, bytes, to_user);
   case ORC_SIGMA: return to_user ? xfer(&s->sigma_eff, 8, u, bytes, 1) : -1;
   }
   return -1;

@@ -60,7 +60,8 @@ enum {
   ORC_P = 20, ORC_LS_B = 21 /*i32: accepted trial, -1 none accepted, -2 skipped*/, ORC_LS_MARGIN = 22,
   ORC_ASC_MARGIN = 23, ORC_CURV_MARGIN = 24, ORC_GHAT = 25, ORC_HLC_F = 26 /*[N][M]*/,
   ORC_RS_SRC = 27 /*i32*/, ORC_RS_CAND = 28 /*i32*/, ORC_RS_MARGIN = 29, ORC_HLC_U = 30 /*[N][M][d]*/,
-  ORC_SIGMA = 33 /*double[1]: smoothing scale used by the last HLC step*/
+  ORC_SIGMA = 33 /*double[1]: smoothing scale used by the last HLC step*/,
+  ORC_RS_SCORE = 34 /*[N][16]: Repulse Monkey, score (min squared L2 distance to the frozen modes) of candidate c of a slot*/
 };
 
 /* units for orc_phase */

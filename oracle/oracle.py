@@ -18,6 +18,7 @@ import build as _build  # noqa: E402  (oracle/build.py)
 X, F, G, V, STUCK, REMOVED, HIST_S, HIST_Y, HIST_LEN, STALLED, CTRL = range(11)
 P, LS_B, LS_MARGIN, ASC_MARGIN, CURV_MARGIN, GHAT, HLC_F, RS_SRC, RS_CAND, RS_MARGIN, HLC_U = range(20, 31)
 SIGMA = 33
+RS_SCORE = 34
 PH_RELEASE_EVAL, PH_STICK, PH_DEDUP, PH_RESEED, PH_HLC_STEP, PH_ANTI_STEP, PH_LBFGS_ITER = 1, 2, 3, 4, 5, 6, 11
 
 _fp = C.POINTER(C.c_float)
@@ -112,7 +113,7 @@ class Oracle:
     def _shape(self, field):
         N, d, m, M = self.N, self.d, self.m, self.M
         return {X: (N, d), G: (N, d), V: (N, d), P: (N, d), GHAT: (N, d), HIST_S: (m, N, d), HIST_Y: (m, N, d),
-                HLC_F: (N, M), HLC_U: (N, M, d), CTRL: (8,), SIGMA: (1,)}.get(field, (N,))
+                HLC_F: (N, M), HLC_U: (N, M, d), CTRL: (8,), SIGMA: (1,), RS_SCORE: (N, 16)}.get(field, (N,))
 
     def get(self, field):
         a = np.empty(self._shape(field), _FIELD_DTYPE.get(field, np.float64))

@@ -33,7 +33,7 @@ TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_upd
 EXPORTS = ("chisao_workspace_bytes", "chisao_init", "chisao_seed_population", "chisao_step", "chisao_step_host",
            "chisao_modes", "chisao_get_state", "chisao_set_state", "chisao_phase", "chisao_get_stats",
            "chisao_set_option", "chisao_get_info", "chisao_launch_count", "chisao_timing_enable", "chisao_timing_reset", "chisao_timing_get",
-           "chisao_last_error", "chisao_destroy")
+           "chisao_measure_peak", "chisao_last_error", "chisao_destroy")
 
 _fp = C.POINTER(C.c_float)
 
@@ -99,6 +99,7 @@ def load_library(path: Optional[str] = None):
     L.chisao_timing_enable.argtypes = [vp, C.c_int32]
     L.chisao_timing_reset.argtypes = [vp]
     L.chisao_timing_get.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+    L.chisao_measure_peak.argtypes = [C.c_int32, vp, vp, C.POINTER(C.c_double)]
     L.chisao_last_error.argtypes = [vp]
     L.chisao_last_error.restype = C.c_char_p
     L.chisao_destroy.argtypes = [vp]
@@ -132,6 +133,24 @@ def workspace_bytes(wl) -> int:
     if rc:
         raise ChisaoError(rc, load_library().chisao_last_error(None).decode())
     return n.value
+
+
+PEAK_FP32_FMA, PEAK_SFU = 0, 1
+
+
+def measure_peak(which: int, device="cuda:0") -> float:
+    """chisao_measure_peak: FP32 FMA rate (TFLOP/s) or MUFU rate (T op/s) of `device`, by the library's own probe kernels"""
+    import torch
+    L = load_library()
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        scratch = torch.zeros(64, dtype=torch.float32, device=dev)
+        v = C.c_double(0.0)
+        rc = L.chisao_measure_peak(int(which), C.c_void_p(scratch.data_ptr()),
+                                   C.c_void_p(torch.cuda.current_stream(dev).cuda_stream), C.byref(v))
+    if rc:
+        raise ChisaoError(rc, "chisao_measure_peak failed")
+    return float(v.value)
 
 
 _FIELD_DTYPE = {STUCK: np.uint8, REMOVED: np.uint8, STALLED: np.uint8, HIST_LEN: np.int32, CTRL: np.int32,

@@ -20,7 +20,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
-UNITS = [("chisao_api.cu", []), ("chisao_lbfgs.cu", []), ("chisao_select.cu", []), ("chisao_tc_kernels.cu", []), ("chisao_stencil.cu", [])] + \
+UNITS = [("chisao_api.cu", []), ("chisao_lbfgs.cu", []), ("chisao_select.cu", []), ("chisao_tc_kernels.cu", []), ("chisao_stencil.cu", []), ("chisao_probe.cu", [])] + \
         [("chisao_eval_obj.cu", [f"-DCHISAO_OBJ_INST={i}"]) for i in range(6)]
 
 

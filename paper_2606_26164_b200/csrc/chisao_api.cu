@@ -366,13 +366,14 @@ struct Scope {   // optional CUDA-event bracket around a launch group
 };
 
 cudaError_t eval_fd(chisao_ctx *c, const float *X, const int32_t *list, const int32_t *count, int mode, float *g_out,
-                    int phase, int iter, int counter, int slot_off = 0) {
+                    int phase, int iter, int counter, int slot_off = 0, int32_t *zero_cnt = nullptr) {
   const State &s = c->st;
   if (s.N == 0) return cudaSuccess;
   FdArgs a{};
   a.X = X; a.list = list; a.count = count; a.max_count = s.N; a.mode = mode; a.d = s.d; a.cycle = c->cycle;
   a.phase = phase; a.iter = iter; a.counter = counter; a.slot_off = slot_off; a.g_out = g_out; a.x = s.x; a.v = s.v; a.lo = s.lo; a.hi = s.hi;
   a.h = c->hp.fd_h; a.mu = c->hp.mu; a.alpha = c->hp.alpha_anti; a.seed = c->hp.seed; a.evals = s.ctrl->evals;
+  a.zero_cnt = zero_cnt;
   const int spt = NT / s.d;
   const int grid = (s.N + spt - 1) / spt;
   Scope sc(c, 0);
@@ -456,38 +457,52 @@ cudaError_t hlc_step(chisao_ctx *c, int iter) {
 
 // ---- units of Algorithm 1 --------------------------------------------------------------------------------
 int run_release_eval(chisao_ctx *ctx) {   // Phase 1 start: release all + f, g at x
-  { Scope sc(ctx, 4); CK(launch_release(ctx->st, ctx->stream)); ctx->launches += 1; }
+  // inside a cycle the first L-BFGS iteration's kernel releases (k_lbfgs_step, STEP_FIRST)
+  if (!(ctx->in_cycle && ctx->hp.n_conv > 0)) { Scope sc(ctx, 4); CK(launch_release(ctx->st, ctx->stream)); ctx->launches += 1; }
   CK(eval_points(ctx, PT_CENTRE, 0, 0));
   CK(eval_fd(ctx, ctx->st.x, nullptr, nullptr, FD_GRAD, ctx->st.g, 1, 0, EV_INIT));
   return CHISAO_OK;
 }
-int run_lbfgs_iter(chisao_ctx *ctx, int it) {   // one L-BFGS iteration (R-4)
+// one L-BFGS iteration (R-4).  As a unit of its own: direction, line search, FD gradient at the accepted
+// points, update.  Inside a cycle the update of iteration it - 1 rides in the direction kernel of iteration it (one pass
+// over x and g per iteration), and the update of the last iteration (run_lbfgs_finish) also writes Phase 2's partials.
+int run_lbfgs_iter(chisao_ctx *ctx, int it) {
   const State &s = ctx->st;
-  CK(cudaMemsetAsync(s.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
-  { Scope sc(ctx, 3); CK(launch_lbfgs_direction(s, ctx->hp, ctx->stream)); ctx->launches += 1; }
+  const int mode = !ctx->in_cycle ? 0 : (it == 1 ? 1 : 2);
+  if (!ctx->in_cycle) CK(cudaMemsetAsync(s.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
+  { Scope sc(ctx, 3); CK(launch_lbfgs_step(s, ctx->hp, mode, ctx->stream)); ctx->launches += 1; }
   if (ctx->ls_tile_local) CK(eval_points(ctx, PT_LS_ALL, 0, it));
   else for (int b = 0; b <= ctx->hp.ls_max; ++b) CK(eval_points(ctx, PT_LS, b, it));
-  CK(eval_fd(ctx, s.xt, s.fd_list, &s.ctrl->fd_cnt, FD_GRAD, s.gn, 1, it, EV_LBFGS_FD));
-  { Scope sc(ctx, 4); CK(launch_lbfgs_update(s, ctx->hp, ctx->stream)); ctx->launches += 1; }
+  // the FD kernel also zeroes worklist 0's counter for the next iteration's direction kernel
+  CK(eval_fd(ctx, s.xt, s.fd_list, &s.ctrl->fd_cnt, FD_GRAD, s.gn, 1, it, EV_LBFGS_FD, 0, &s.ctrl->ls_cnt[0]));
+  if (!ctx->in_cycle) { Scope sc(ctx, 4); CK(launch_lbfgs_update(s, ctx->hp, false, ctx->stream)); ctx->launches += 1; }
+  return CHISAO_OK;
+}
+int run_lbfgs_finish(chisao_ctx *ctx) {   // in a cycle: update of the last iteration + ||g||_inf, f_max partials of Phase 2
+  Scope sc(ctx, 4);
+  CK(launch_lbfgs_update(ctx->st, ctx->hp, true, ctx->stream));
+  ctx->launches += 1;
   return CHISAO_OK;
 }
 int run_stick(chisao_ctx *ctx) {
   Scope sc(ctx, 5);
-  CK(launch_stick(ctx->st, ctx->hp, ctx->stream));
-  ctx->launches += 5;
+  // after run_lbfgs_finish the per-sample gradient norms and f_max are already there
+  const bool have_partials = ctx->in_cycle && ctx->hp.n_conv > 0;
+  CK(launch_stick(ctx->st, ctx->hp, have_partials, ctx->stream));
+  ctx->launches += have_partials ? 3 : 4;
   return CHISAO_OK;
 }
 int run_dedup(chisao_ctx *ctx) {
   Scope sc(ctx, 5);
   const bool dedup_on = (ctx->hp.phase_mask & (1u << 3)) != 0;
   CK(launch_dedup(ctx->st, ctx->hp, !ctx->in_cycle, ctx->stream));
-  ctx->launches += (ctx->in_cycle ? 0 : 3) + (dedup_on ? 2 : 0) + 3;
+  ctx->launches += (ctx->in_cycle ? 0 : 3) + (dedup_on ? 1 : 0) + 3;
   return CHISAO_OK;
 }
 int run_reseed(chisao_ctx *ctx) {
   Scope sc(ctx, 6);
-  CK(launch_reseed(ctx->st, ctx->hp, ctx->cycle, ctx->stream));
-  ctx->launches += 3;
+  CK(launch_reseed(ctx->st, ctx->hp, ctx->cycle, !ctx->in_cycle, ctx->stream));
+  ctx->launches += ctx->in_cycle ? 2 : 3;
   return CHISAO_OK;
 }
 int run_explore_list(chisao_ctx *ctx) {
@@ -672,9 +687,9 @@ static int enqueue_cycle_units(chisao_ctx *ctx) {
   if ((rc = run_release_eval(ctx))) return rc;        // Phase 1: release all, then converge
   for (int it = 1; it <= ctx->hp.n_conv; ++it)
     if ((rc = run_lbfgs_iter(ctx, it))) return rc;
+  if (ctx->hp.n_conv > 0 && (rc = run_lbfgs_finish(ctx))) return rc;
   if ((rc = run_stick(ctx))) return rc;               // Phase 2
-  if ((rc = run_dedup(ctx))) return rc;               // Phase 3
-  CK(cudaMemsetAsync(&ctx->st.ctrl->strategy, 0, 4, ctx->stream));
+  if ((rc = run_dedup(ctx))) return rc;               // Phase 3 (its list kernel also clears ctrl->strategy)
   if (ctx->cycle < ctx->hp.n_osc) {                   // "if k < n_osc"
     if ((rc = run_reseed(ctx))) return rc;            // Phase 4
     if ((rc = run_explore_list(ctx))) return rc;
@@ -776,7 +791,7 @@ int chisao_phase(chisao_ctx *ctx, int32_t phase_id, int32_t iter) {
     case CHISAO_PH_LBFGS_DIRECTION: {
       CK(cudaMemsetAsync(ctx->st.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
       Scope sc(ctx, 3);
-      CK(launch_lbfgs_direction(ctx->st, ctx->hp, ctx->stream));
+      CK(launch_lbfgs_step(ctx->st, ctx->hp, 0, ctx->stream));
       ctx->launches += 1;
       return CHISAO_OK;
     }

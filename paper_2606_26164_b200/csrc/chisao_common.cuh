@@ -90,7 +90,7 @@ struct Hyper {                        // by-value copy of the cycle hyper-parame
 enum { FD_GRAD = 0, FD_ANTI = 1 };
 enum { PT_CENTRE = 0, PT_LS = 1, PT_LS_ALL = 2 };
 // modes of the list-building scan
-enum { SCAN_STICK = 0, SCAN_FINAL = 1, SCAN_EXPLORE = 2 };
+enum { SCAN_STICK = 0, SCAN_FINAL = 1, SCAN_EXPLORE = 2, SCAN_STICK_FLAGS = 3 };
 
 // launchers implemented in the .cu files (all enqueue on `st`, return the cudaError of the launch)
 cudaError_t launch_eval_fd(const DevObj &o, const State &s, const Hyper &h, int cycle, const float *X,
@@ -101,12 +101,14 @@ cudaError_t launch_eval_points(const DevObj &o, const State &s, const Hyper &h, 
 cudaError_t launch_hlc(const DevObj &o, const State &s, const Hyper &h, int cycle, int iter, cudaStream_t st);
 cudaError_t eval_kernels_configure();   // opt-in dynamic shared memory for every instantiation
 
-cudaError_t launch_lbfgs_direction(const State &s, const Hyper &h, cudaStream_t st);
-cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, cudaStream_t st);
+// mode: 0 direction only (stand-alone unit), 1 first iteration of a cycle (release folded in), 2 update of the previous
+// iteration + direction (chisao_lbfgs.cu)
+cudaError_t launch_lbfgs_step(const State &s, const Hyper &h, int mode, cudaStream_t st);
+cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, bool stick_partials, cudaStream_t st);
 cudaError_t launch_release(const State &s, cudaStream_t st);
-cudaError_t launch_stick(const State &s, const Hyper &h, cudaStream_t st);          // ginf, f_max, flags, P0
+cudaError_t launch_stick(const State &s, const Hyper &h, bool have_partials, cudaStream_t st);   // ginf, f_max, flags, P0
 cudaError_t launch_dedup(const State &s, const Hyper &h, bool rebuild_p0, cudaStream_t st);   // removed + lists + GR state
-cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_t st);
+cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, bool standalone, cudaStream_t st);
 cudaError_t launch_explore_list(const State &s, cudaStream_t st);
 // paper-form HLC (Eq. 5) helpers: stage 0 perturb (xt = x + sigma z_k), 1 accumulate (ghat += gn / M), 2 apply
 cudaError_t launch_hlc_sigma(const State &s, const Hyper &h, cudaStream_t st);   // ctrl->sigma_eff (R-18)

@@ -28,6 +28,7 @@ struct FdArgs {
   float h, mu, alpha;
   uint64_t seed;
   unsigned long long *evals;
+  int32_t *zero_cnt;         // counter reset by the kernel (the consumed line-search worklist), or NULL
 };
 
 // stencil-aware FD evaluator for the dense objectives (chisao_stencil.cu; opt-in)
@@ -45,6 +46,7 @@ __global__ void __launch_bounds__(NT, 2) k_eval_fd(const DevObj o, const FdArgs 
   const int spt = NT / d;                          // samples per tile
   const int cnt = a.count ? *a.count : a.max_count;
   const int first = blockIdx.x * spt;
+  if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
   if (first >= cnt) return;
   if (t == 0) { mbar_init(&sm.bar[0], 1); mbar_init(&sm.bar[1], 1); mbar_fence_init(); }
   const int s = t / d, j = t - s * d;

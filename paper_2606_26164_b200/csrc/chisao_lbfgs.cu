@@ -11,7 +11,6 @@
 
 namespace chisao {
 
-constexpr int WARPS_PER_BLOCK = 8;
 
 struct Row2 { float a, b; };
 __device__ __forceinline__ Row2 ld_row2(const float *row, int lane, int d, bool even) {
@@ -86,15 +85,70 @@ __device__ __forceinline__ void axpy4(Row4 &r, float c, Row4 v) {
   r.a = fmaf(c, v.a, r.a); r.b = fmaf(c, v.b, r.b); r.c = fmaf(c, v.c, r.c); r.e = fmaf(c, v.e, r.e);
 }
 
+// ---- history / state update after the FD gradient gn at the accepted trial point (R-4 (v), (vi)) ------------------
+// Curvature pair s = x_t - x, y = gamma+ - gamma = g - gn, stored iff s.y > 1e-10 |s||y| (ring buffer, oldest dropped
+// beyond m); x, f, g <- x_t, f(x_t), gn.  No trial accepted: stalled if the history was already empty, else the
+// history is cleared.  Half-warp per sample; every lane of the warp calls (the dots are shuffles), `in` = the sample
+// exists.  Returns the sample's state AFTER the update in registers, so that the two-loop recursion of the next
+// iteration can follow in the same kernel (k_lbfgs_step).
+struct SampleState { Row4 g, x; int len, head, stalled; bool have_x; unsigned bytes; };
+template <bool VEC>
+__device__ __forceinline__ SampleState lbfgs_update_half(const State &s, int i, bool in, int hl) {
+  constexpr bool vec = VEC;
+  const int d = s.d, m = s.m, N = s.N;
+  const size_t ro = (size_t)(in ? i : 0) * d;
+  SampleState o;
+  const int b = in ? s.ls_b[i] : -2;
+  o.len = in ? s.hist_len[i] : 0; o.head = in ? s.hist_head[i] : 0; o.stalled = in ? (int)s.stalled[i] : 0;
+  o.g = ld_row4h(s.g + ro, hl, d, vec);
+  if (!in) { o.g.a = o.g.b = o.g.c = o.g.e = 0.f; }
+  o.x.a = o.x.b = o.x.c = o.x.e = 0.f; o.have_x = false; o.bytes = 0u;
+  const bool acc = b >= 0;
+  Row4 x = o.x, xt = o.x, gn = o.x;
+  if (acc) { x = ld_row4h(s.x + ro, hl, d, vec); xt = ld_row4h(s.xt + ro, hl, d, vec); gn = ld_row4h(s.gn + ro, hl, d, vec); }
+  Row4 sv, yv;
+  sv.a = xt.a - x.a; sv.b = xt.b - x.b; sv.c = xt.c - x.c; sv.e = xt.e - x.e;
+  yv.a = o.g.a - gn.a; yv.b = o.g.b - gn.b; yv.c = o.g.c - gn.c; yv.e = o.g.e - gn.e;
+  const float sy = dot4(sv, yv), ss = dot4(sv, sv), yy = dot4(yv, yv);   // executed by all 32 lanes
+  if (acc) {
+    const float thr = 1e-10f * sqrtf(ss) * sqrtf(yy);
+    o.bytes = 5u * d * 4u;                                 // x_t, gn, x read; x, g written
+    if (sy > thr) {
+      int ph;
+      if (o.len == m) { ph = o.head; o.head = (o.head + 1 == m) ? 0 : o.head + 1; }
+      else { ph = o.head + o.len; if (ph >= m) ph -= m; o.len += 1; }
+      const size_t off = ((size_t)ph * N + i) * d;
+      st_row4h(s.S + off, hl, d, vec, sv);
+      st_row4h(s.Y + off, hl, d, vec, yv);
+      if (hl == 0) { s.hist_len[i] = o.len; s.hist_head[i] = o.head; }
+      o.bytes += 2u * d * 4u;
+    }
+    st_row4h(s.x + ro, hl, d, vec, xt);
+    st_row4h(s.g + ro, hl, d, vec, gn);
+    if (hl == 0) s.f[i] = s.ft[i];
+    o.g = gn; o.x = xt; o.have_x = true;
+  } else if (b == -1) {
+    if (o.len == 0) { o.stalled = 1; if (hl == 0) s.stalled[i] = 1; }
+    else { o.len = 0; o.head = 0; if (hl == 0) { s.hist_len[i] = 0; s.hist_head[i] = 0; } }
+  }
+  return o;
+}
+
 // One L-BFGS iteration, part 1: skip test, direction by the two-loop recursion (Nocedal & Wright Alg. 7.4;
 // refs [19,20] of PAPER.md:77) with H0 = (s.y / y.y) I of the newest pair, steepest restart when the
 // direction is not an ascent direction for f, first trial step and trial point (R-4).
 // A half-warp owns one sample (two samples per warp, float4 per lane: one 512-byte contiguous request per warp
 // and history plane); MM = compile-time bound on the history length, so the pair loops unroll over registers.
 // Every shuffle is executed by all 32 lanes: inactive samples run with len = 0 and predicated stores.
+// MODE: STEP_ALONE   the unit chisao_phase runs (state as stored);
+//       STEP_FIRST   first iteration of a cycle: "stuck <- False^N" (Alg. 1) and the history reset of
+//                    every Phase 1 (R-5) happen here instead of in a launch of their own;
+//       STEP_UPDATE  iteration it >= 2 of a cycle: the update of iteration it - 1 (lbfgs_update_half) runs first, in the
+//                    same kernel: one launch and one pass over x, g per iteration instead of two.
+enum { STEP_ALONE = 0, STEP_FIRST = 1, STEP_UPDATE = 2 };
 constexpr int DIR_WARPS = 4;   // measured at C5, full history: 4 warps x 4 CTAs per SM 4023 GB/s, 2 x 8 4025, 8 x 2 3884 (finer CTA turnover: less lockstep between load and recursion phases)
-template <int MM, bool VEC>
-__global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_direction(State s, Hyper h) {
+template <int MM, bool VEC, int MODE>
+__global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_step(State s, Hyper h) {
   __shared__ int sh_cnt, sh_base;
   __shared__ unsigned int sh_bytes;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, hl = lane & 15, half = lane >> 4;
@@ -102,15 +156,33 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_direction(State s, 
   const int d = s.d, m = s.m, N = s.N;
   constexpr bool vec = VEC;
   if (threadIdx.x == 0) { sh_cnt = 0; sh_bytes = 0u; }
-  if (blockIdx.x == 0 && threadIdx.x == 0) { s.ctrl->ls_cnt[1] = 0; s.ctrl->ls_cnt[2] = 0; s.ctrl->fd_cnt = 0; }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    s.ctrl->ls_cnt[1] = 0; s.ctrl->ls_cnt[2] = 0; s.ctrl->fd_cnt = 0;
+    if (MODE != STEP_ALONE) s.ctrl->fmax_enc = 0u;       // the cycle's f_max is accumulated by the last update of the pass
+  }
   __syncthreads();
   const bool in = i < N;
   const size_t ro = (size_t)(in ? i : 0) * d;
-  // one round trip for everything the activity test needs (the flags are read whether or not the sample turns out
-  // to be active: three dependent round trips -> two)
-  Row4 g = ld_row4h(s.g + ro, hl, d, vec);
-  const int stalled_i = s.stalled[in ? i : 0], len_i = s.hist_len[in ? i : 0], head_i = s.hist_head[in ? i : 0];
-  if (!in) { g.a = g.b = g.c = g.e = 0.f; }
+  Row4 g, x;
+  x.a = x.b = x.c = x.e = 0.f;
+  int stalled_i, len_i, head_i;
+  bool have_x = false;
+  unsigned upd_bytes = 0u;
+  if constexpr (MODE == STEP_UPDATE) {
+    const SampleState u = lbfgs_update_half<VEC>(s, i, in, hl);
+    g = u.g; x = u.x; have_x = u.have_x; stalled_i = u.stalled; len_i = u.len; head_i = u.head; upd_bytes = u.bytes;
+  } else {
+    // one round trip for everything the activity test needs (the flags are read whether or not the sample turns out
+    // to be active: three dependent round trips -> two)
+    g = ld_row4h(s.g + ro, hl, d, vec);
+    if constexpr (MODE == STEP_FIRST) {
+      stalled_i = 0; len_i = 0; head_i = 0;
+      if (in && hl == 0) { s.stuck[i] = 0; s.removed[i] = 0; s.stalled[i] = 0; s.hist_len[i] = 0; s.hist_head[i] = 0; }
+    } else {
+      stalled_i = s.stalled[in ? i : 0]; len_i = s.hist_len[in ? i : 0]; head_i = s.hist_head[in ? i : 0];
+    }
+    if (!in) { g.a = g.b = g.c = g.e = 0.f; }
+  }
   const float ginf = half_max(fmaxf(fmaxf(fabsf(g.a), fabsf(g.b)), fmaxf(fabsf(g.c), fabsf(g.e))));
   // (i) stationary (Eq. 3's gradient test) or stalled: no work, no evaluations (R-6)
   const bool act = in && !(stalled_i || !(ginf >= h.eps_grad));
@@ -129,17 +201,16 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_direction(State s, 
       Sr[l].a = Sr[l].b = Sr[l].c = Sr[l].e = 0.f; Yr[l] = Sr[l];
     }
   }
-  Row4 x; x.a = x.b = x.c = x.e = 0.f;
-  if (act) x = ld_row4h(s.x + ro, hl, d, vec);
+  if (act && !have_x) x = ld_row4h(s.x + ro, hl, d, vec);
   // block-aggregated append of the searching samples to line-search worklist 0, and the byte counter: the one
   // returning global atomic per CTA is issued here, under the history loads, not at the end of the CTA's life
   int my_slot = 0;
   if (act && hl == 0) my_slot = atomicAdd(&sh_cnt, 1);
-  if (in && hl == 0) atomicAdd(&sh_bytes, (2u * d + (act ? 2u * (unsigned)len_read * d + 2u * d : 0u)) * 4u);
+  if (in && hl == 0) atomicAdd(&sh_bytes, upd_bytes + (2u * d + (act ? 2u * (unsigned)len_read * d + 2u * d : 0u)) * 4u);
   __syncthreads();
   if (threadIdx.x == 0) {
     if (sh_cnt > 0) sh_base = atomicAdd(&s.ctrl->ls_cnt[0], sh_cnt);
-    if (sh_bytes) atomicAdd(&s.ctrl->evals[7], (unsigned long long)sh_bytes);   // g read, p written (+ pairs, x, x_t)
+    if (sh_bytes) atomicAdd(&s.ctrl->evals[7], (unsigned long long)sh_bytes);   // g read, p written (+ pairs, x, x_t; + the update's rows)
   }
   Row4 gam; gam.a = -g.a; gam.b = -g.b; gam.c = -g.c; gam.e = -g.e;
   // a warp none of whose two samples is active skips the recursion altogether (late in phase 2 most are stationary)
@@ -202,46 +273,41 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_direction(State s, 
   if (act && hl == 0) s.ls_list[0][sh_base + my_slot] = i;
 }
 
-// One L-BFGS iteration, part 3 (after the FD gradient gn at the accepted trial point): curvature pair
-// s = x_t - x, y = gamma+ - gamma = g - gn, stored iff s.y > 1e-10 |s||y| (ring buffer, oldest dropped
-// beyond m); x, f, g <- x_t, f(x_t), gn.  No trial accepted: stalled if the history was already empty,
-// else the history is cleared (R-4 (v), (vi)).
-__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_lbfgs_update(State s, Hyper h) {
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  const int i = blockIdx.x * WARPS_PER_BLOCK + wib;
+// One L-BFGS iteration, part 3 as a launch of its own (the unit chisao_phase runs, and the last iteration of a pass):
+// lbfgs_update_half for every sample.  STICK: also Phase 2's per-sample ||grad f||_inf and the f_max partials (what
+// k_ginf_fmax computes, chisao_select.cu), from the gradient and value this kernel has just written -- at the end of
+// a pass the stick test follows at once.
+template <bool VEC, bool STICK>
+__global__ void __launch_bounds__(DIR_WARPS * 32) k_lbfgs_update(State s, Hyper h) {
+  __shared__ float sh_max[DIR_WARPS];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, hl = lane & 15, half = lane >> 4;
+  const int i = (blockIdx.x * DIR_WARPS + wib) * 2 + half;
   if (blockIdx.x == 0 && threadIdx.x == 0) s.ctrl->ls_cnt[0] = 0;
-  if (i >= s.N) return;
-  const int d = s.d, m = s.m, N = s.N;
-  const bool even = (d & 1) == 0;
-  const int b = s.ls_b[i];
-  if (b == -2) return;
-  int len = s.hist_len[i], head = s.hist_head[i];
-  if (b < 0) {
-    if (lane == 0) {
-      if (len == 0) s.stalled[i] = 1; else { s.hist_len[i] = 0; s.hist_head[i] = 0; }
+  const bool in = i < s.N;
+  const SampleState u = lbfgs_update_half<VEC>(s, i, in, hl);
+  if constexpr (STICK) {
+    const float a0 = fabsf(u.g.a), a1 = fabsf(u.g.b), a2 = fabsf(u.g.c), a3 = fabsf(u.g.e);
+    const bool nan = !(a0 == a0) || !(a1 == a1) || !(a2 == a2) || !(a3 == a3);
+    const float gi = half_max(fmaxf(fmaxf(a0, a1), fmaxf(a2, a3)));
+    const unsigned nanmask = __ballot_sync(0xffffffffu, nan);
+    const bool any_nan = (nanmask >> (16 * half)) & 0xFFFFu;
+    float fm = -INFINITY;
+    if (in && hl == 0) {
+      s.ginf[i] = any_nan ? NAN : gi;                    // a NaN gradient can never pass "< eps_grad"
+      const float f = s.f[i];                            // written above by this lane if the trial was accepted
+      if (fabsf(f) <= 3.0e38f) fm = f;                   // finite values only (R-13)
     }
-    return;
+    fm = warp_max(fm);
+    if (lane == 0) sh_max[wib] = fm;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      float mx = sh_max[0];
+#pragma unroll
+      for (int w = 1; w < DIR_WARPS; ++w) mx = fmaxf(mx, sh_max[w]);
+      if (mx > -INFINITY) atomicMax(&s.ctrl->fmax_enc, enc_ordered(mx));
+    }
   }
-  const size_t ro = (size_t)i * d;
-  const Row2 x = ld_row2(s.x + ro, lane, d, even), xt = ld_row2(s.xt + ro, lane, d, even);
-  const Row2 g = ld_row2(s.g + ro, lane, d, even), gn = ld_row2(s.gn + ro, lane, d, even);
-  Row2 sv, yv;
-  sv.a = xt.a - x.a; sv.b = xt.b - x.b;
-  yv.a = g.a - gn.a; yv.b = g.b - gn.b;
-  const float sy = dot2(sv, yv), ss = dot2(sv, sv), yy = dot2(yv, yv);
-  const float thr = 1e-10f * sqrtf(ss) * sqrtf(yy);
-  if (sy > thr) {
-    int ph;
-    if (len == m) { ph = head; head = (head + 1 == m) ? 0 : head + 1; }
-    else { ph = head + len; if (ph >= m) ph -= m; len += 1; }
-    const size_t off = ((size_t)ph * N + i) * d;
-    st_row2(s.S + off, lane, d, even, sv);
-    st_row2(s.Y + off, lane, d, even, yv);
-    if (lane == 0) { s.hist_len[i] = len; s.hist_head[i] = head; }
-  }
-  st_row2(s.x + ro, lane, d, even, xt);
-  st_row2(s.g + ro, lane, d, even, gn);
-  if (lane == 0) s.f[i] = s.ft[i];
+  if (in && hl == 0 && u.bytes) atomicAdd(&s.ctrl->evals[7], (unsigned long long)u.bytes);
 }
 
 cudaError_t launch_release(const State &s, cudaStream_t st) {
@@ -249,25 +315,36 @@ cudaError_t launch_release(const State &s, cudaStream_t st) {
   k_release<<<(s.N + 255) / 256, 256, 0, st>>>(s);
   return cudaGetLastError();
 }
-cudaError_t launch_lbfgs_direction(const State &s, const Hyper &h, cudaStream_t st) {
+cudaError_t launch_lbfgs_step(const State &s, const Hyper &h, int mode, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
   const int per_block = DIR_WARPS * 2, grid = (s.N + per_block - 1) / per_block;
   const bool vec = (s.d & 3) == 0;
-#define CHISAO_DIR(MM)                                                                         \
+#define CHISAO_DIR2(MM, V)                                                                      \
   do {                                                                                         \
-    if (vec) k_lbfgs_direction<MM, true><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);               \
-    else k_lbfgs_direction<MM, false><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);                  \
+    if (mode == STEP_FIRST) k_lbfgs_step<MM, V, STEP_FIRST><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);        \
+    else if (mode == STEP_UPDATE) k_lbfgs_step<MM, V, STEP_UPDATE><<<grid, DIR_WARPS * 32, 0, st>>>(s, h); \
+    else k_lbfgs_step<MM, V, STEP_ALONE><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);                           \
   } while (0)
+#define CHISAO_DIR(MM) do { if (vec) CHISAO_DIR2(MM, true); else CHISAO_DIR2(MM, false); } while (0)
   if (s.m <= 4) CHISAO_DIR(4);
   else if (s.m <= 8) CHISAO_DIR(8);
   else if (s.m <= 10) CHISAO_DIR(10);
   else CHISAO_DIR(16);
 #undef CHISAO_DIR
+#undef CHISAO_DIR2
   return cudaGetLastError();
 }
-cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, cudaStream_t st) {
+cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, bool stick_partials, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
-  k_lbfgs_update<<<(s.N + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK, WARPS_PER_BLOCK * 32, 0, st>>>(s, h);
+  const int per_block = DIR_WARPS * 2, grid = (s.N + per_block - 1) / per_block;
+  const bool vec = (s.d & 3) == 0;
+  if (vec) {
+    if (stick_partials) k_lbfgs_update<true, true><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+    else k_lbfgs_update<true, false><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+  } else {
+    if (stick_partials) k_lbfgs_update<false, true><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+    else k_lbfgs_update<false, false><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);
+  }
   return cudaGetLastError();
 }
 

@@ -37,32 +37,35 @@ __global__ void __launch_bounds__(256) k_ginf_fmax(State s) {
 }
 
 // stuck_i = (||grad f(x_i)||_inf < eps_grad) and (f(x_i) >= f_max + log delta)   (Eq. 3)
-__global__ void k_stick_flags(State s, Hyper h) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= s.N) return;
+__device__ __forceinline__ bool stick_test(const State &s, const Hyper &h, int i) {
   const float fmax = dec_ordered(s.ctrl->fmax_enc);
   const float f = s.f[i];
-  const bool st = (s.ginf[i] < h.eps_grad) && (fabsf(f) <= 3.0e38f) && (f >= fmax + h.log_delta);
-  s.stuck[i] = st ? 1 : 0;
-  s.removed[i] = 0;
+  return (s.ginf[i] < h.eps_grad) && (fabsf(f) <= 3.0e38f) && (f >= fmax + h.log_delta);
 }
 
 // ---- ordered compaction: ascending index lists by class ------------------------------------------------
 // SCAN_STICK  : class 1 = stuck                         -> listP0
-// SCAN_FINAL  : class 0 = unfrozen (not stuck, not removed) -> listA, 1 = stuck -> listP, 2 = removed -> listR
+// SCAN_STICK_FLAGS: the same, and the counting kernel first WRITES the flags of Eq. 3 (stuck, removed <- 0)
+// SCAN_FINAL  : class 0 = unfrozen (not stuck, not removed) -> listA, 1 = stuck -> listP, 2 = removed -> listR; the
+//               counting kernel clears the stuck flag of removed samples ("removed" in Eq. 4 means it no longer is a mode),
+//               the scatter kernel resets the reseed diagnostics
 // SCAN_EXPLORE: class 1 = not stuck and not removed     -> listE
 __device__ __forceinline__ int scan_class(const State &s, int mode, int i) {
   const bool st = s.stuck[i] != 0, rm = s.removed[i] != 0;
-  if (mode == SCAN_STICK) return st ? 1 : -1;
+  if (mode == SCAN_STICK || mode == SCAN_STICK_FLAGS) return st ? 1 : -1;
   if (mode == SCAN_EXPLORE) return (!st && !rm) ? 1 : -1;
   return rm ? 2 : (st ? 1 : 0);
 }
 
-__global__ void __launch_bounds__(SCAN_BLOCK) k_scan_count(State s, int mode, int nb) {
+__global__ void __launch_bounds__(SCAN_BLOCK) k_scan_count(State s, Hyper h, int mode, int nb) {
   __shared__ int cnt[3];
   if (threadIdx.x < 3) cnt[threadIdx.x] = 0;
   __syncthreads();
   const int i = blockIdx.x * SCAN_BLOCK + threadIdx.x;
+  if (i < s.N) {
+    if (mode == SCAN_STICK_FLAGS) { s.stuck[i] = stick_test(s, h, i) ? 1 : 0; s.removed[i] = 0; }
+    else if (mode == SCAN_FINAL && s.removed[i]) s.stuck[i] = 0;
+  }
   const int c = (i < s.N) ? scan_class(s, mode, i) : -1;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
@@ -93,11 +96,12 @@ __global__ void __launch_bounds__(256) k_scan_offsets(State s, int mode, int nb)
   __syncthreads();
   if (threadIdx.x == 0) {
     Ctrl *c = s.ctrl;
-    if (mode == SCAN_STICK) {
+    if (mode == SCAN_STICK || mode == SCAN_STICK_FLAGS) {
       c->nP0 = tot[1]; c->n_stuck = tot[1]; c->k_lost = 0; c->n_active = s.N - tot[1];
     } else if (mode == SCAN_FINAL) {
       c->nA = tot[0]; c->nP = tot[1]; c->nR = tot[2];
       c->k_lost = tot[2]; c->n_stuck = tot[1]; c->n_active = tot[0];
+      c->strategy = 0;                                     // no reseeding yet in this cycle (and none on the last one)
       // Golden Rooster self-disable (R-9): two consecutive GR cycles without new peaks
       if (c->gr_used_last) {
         if (tot[1] > c->gr_prev_modes) c->gr_unproductive = 0; else c->gr_unproductive += 1;
@@ -105,6 +109,7 @@ __global__ void __launch_bounds__(256) k_scan_offsets(State s, int mode, int nb)
       }
     } else {
       c->nE = tot[1];
+      c->n_active = tot[1];                                // who takes part in phases 5-6 (= N - n_stuck after reseeding)
     }
   }
 }
@@ -114,6 +119,7 @@ __global__ void __launch_bounds__(SCAN_BLOCK) k_scan_scatter(State s, int mode, 
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int i = blockIdx.x * SCAN_BLOCK + threadIdx.x;
   const int c = (i < s.N) ? scan_class(s, mode, i) : -1;
+  if (mode == SCAN_FINAL && i < s.N) { s.rs_src[i] = -1; s.rs_cand[i] = -1; }
   int rank = 0;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
@@ -125,19 +131,19 @@ __global__ void __launch_bounds__(SCAN_BLOCK) k_scan_scatter(State s, int mode, 
   if (c >= 0) {
     int off = s.blk_cnt[c * nb + blockIdx.x] + rank;
     for (int ww = 0; ww < w; ++ww) off += wcnt[c][ww];
-    int32_t *dst = (mode == SCAN_STICK) ? s.listP0 : (mode == SCAN_EXPLORE) ? s.listE
+    int32_t *dst = (mode == SCAN_STICK || mode == SCAN_STICK_FLAGS) ? s.listP0 : (mode == SCAN_EXPLORE) ? s.listE
                    : (c == 0 ? s.listA : (c == 1 ? s.listP : s.listR));
     dst[off] = i;
   }
 }
 
-static cudaError_t run_scan(const State &s, int mode, cudaStream_t st) {
+static cudaError_t run_scan(const State &s, const Hyper &h, int mode, cudaStream_t st) {
   const int nb = (s.N + SCAN_BLOCK - 1) / SCAN_BLOCK;
   if (nb == 0) {  // empty population: only the bookkeeping kernel runs
     k_scan_offsets<<<1, 256, 0, st>>>(s, mode, 0);
     return cudaGetLastError();
   }
-  k_scan_count<<<nb, SCAN_BLOCK, 0, st>>>(s, mode, nb);
+  k_scan_count<<<nb, SCAN_BLOCK, 0, st>>>(s, h, mode, nb);
   k_scan_offsets<<<1, 256, 0, st>>>(s, mode, nb);
   k_scan_scatter<<<nb, SCAN_BLOCK, 0, st>>>(s, mode, nb);
   return cudaGetLastError();
@@ -192,39 +198,34 @@ __global__ void __launch_bounds__(128) k_dedup(State s, Hyper h) {
   if (act) s.removed[i] = rem ? 1 : 0;
 }
 
-__global__ void k_apply_removed(State s) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= s.N) return;
-  if (s.removed[i]) s.stuck[i] = 0;
-}
-
-cudaError_t launch_stick(const State &s, const Hyper &h, cudaStream_t st) {
-  cudaError_t e = cudaMemsetAsync(&s.ctrl->fmax_enc, 0, sizeof(uint32_t), st);
-  if (e != cudaSuccess) return e;
-  if (s.N > 0) {
-    k_ginf_fmax<<<(s.N + 7) / 8, 256, 0, st>>>(s);
-    k_stick_flags<<<(s.N + 255) / 256, 256, 0, st>>>(s, h);
+// have_partials: ||grad f||_inf per sample and f_max were written by the last L-BFGS update of the pass
+// (k_lbfgs_update<STICK>, chisao_lbfgs.cu); otherwise (stand-alone unit, n_conv = 0) k_ginf_fmax computes them here
+cudaError_t launch_stick(const State &s, const Hyper &h, bool have_partials, cudaStream_t st) {
+  if (!have_partials) {
+    cudaError_t e = cudaMemsetAsync(&s.ctrl->fmax_enc, 0, sizeof(uint32_t), st);
+    if (e != cudaSuccess) return e;
+    if (s.N > 0) k_ginf_fmax<<<(s.N + 7) / 8, 256, 0, st>>>(s);
   }
-  return run_scan(s, SCAN_STICK, st);
+  return run_scan(s, h, SCAN_STICK_FLAGS, st);
 }
 
 cudaError_t launch_dedup(const State &s, const Hyper &h, bool rebuild_p0, cudaStream_t st) {
   if (s.N > 0) {
     // as a stand-alone unit (chisao_phase) the caller may have edited the flags: rebuild the pre-removal stuck list
     // first; inside a cycle launch_stick has just written it
-    cudaError_t e = rebuild_p0 ? run_scan(s, SCAN_STICK, st) : cudaSuccess;
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(s.removed, 0, s.N, st);
-    if (e != cudaSuccess) return e;
-    if (h.phase_mask & (1u << 3)) {
-      k_dedup<<<(s.N + 127) / 128, 128, 0, st>>>(s, h);
-      k_apply_removed<<<(s.N + 255) / 256, 256, 0, st>>>(s);
+    cudaError_t e = cudaSuccess;
+    if (rebuild_p0) {
+      e = run_scan(s, h, SCAN_STICK, st);
+      if (e != cudaSuccess) return e;
+      e = cudaMemsetAsync(s.removed, 0, s.N, st);          // (inside a cycle the stick test has just cleared the mask)
+      if (e != cudaSuccess) return e;
     }
+    if (h.phase_mask & (1u << 3)) k_dedup<<<(s.N + 127) / 128, 128, 0, st>>>(s, h);
   }
-  return run_scan(s, SCAN_FINAL, st);
+  return run_scan(s, h, SCAN_FINAL, st);                   // its counting kernel clears the stuck flag of removed samples
 }
 
-cudaError_t launch_explore_list(const State &s, cudaStream_t st) { return run_scan(s, SCAN_EXPLORE, st); }
+cudaError_t launch_explore_list(const State &s, cudaStream_t st) { Hyper h{}; return run_scan(s, h, SCAN_EXPLORE, st); }
 
 // ---- Phase 4: reseeding ---------------------------------------------------------------
 // strategy decision + Golden-Rooster basis: QR of a Gaussian d x d matrix by modified Gram-Schmidt with one
@@ -380,15 +381,19 @@ __global__ void k_reseed_finish(State s) {
   if (c->strategy != 0) c->n_active = s.N - c->n_stuck;
 }
 
-cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, cudaStream_t st) {
+// standalone (chisao_phase): reset the diagnostics and fix n_active here; inside a cycle the list kernels before and
+// after this phase do both (k_scan_scatter SCAN_FINAL, k_scan_offsets SCAN_EXPLORE)
+cudaError_t launch_reseed(const State &s, const Hyper &h, int cycle, bool standalone, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
-  cudaError_t e = cudaMemsetAsync(s.rs_src, 0xFF, sizeof(int32_t) * s.N, st);
-  if (e != cudaSuccess) return e;
-  e = cudaMemsetAsync(s.rs_cand, 0xFF, sizeof(int32_t) * s.N, st);
-  if (e != cudaSuccess) return e;
+  if (standalone) {
+    cudaError_t e = cudaMemsetAsync(s.rs_src, 0xFF, sizeof(int32_t) * s.N, st);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(s.rs_cand, 0xFF, sizeof(int32_t) * s.N, st);
+    if (e != cudaSuccess) return e;
+  }
   k_reseed_prepare<<<1, 256, 0, st>>>(s, h, cycle);
   k_reseed<<<(s.N + RS_WARPS - 1) / RS_WARPS, RS_WARPS * 32, 0, st>>>(s, h, cycle);
-  k_reseed_finish<<<1, 1, 0, st>>>(s);
+  if (standalone) k_reseed_finish<<<1, 1, 0, st>>>(s);
   return cudaGetLastError();
 }
 

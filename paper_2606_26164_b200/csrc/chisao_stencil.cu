@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(ST_NT, 1) k_fd_stencil(const DevObj o, const F
   const int t = threadIdx.x, d = a.d;
   const int cnt = a.count ? *a.count : a.max_count;
   const int first = blockIdx.x * ST_NT;
+  if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
   if (first >= cnt) return;
   if (t == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_fence_init(); }
   const bool valid = first + t < cnt;

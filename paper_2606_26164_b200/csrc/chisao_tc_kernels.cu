@@ -31,6 +31,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
   const int spg = TC_GROUP / (2 * d), spt = 2 * spg;
   const int cnt = a.count ? *a.count : a.max_count;
   const int ntiles = (cnt + spt - 1) / spt;
+  if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
   if ((int)blockIdx.x >= ntiles) return;
   tc_begin<OBJ>(sm, t);
   const int tl = t & (TC_GROUP - 1), sg = tl / (2 * d), slot = tl - sg * 2 * d, j = slot >> 1;

@@ -152,3 +152,24 @@ def mode_set_report(xg, fg, xo, fo, tol):
             f"gpu-only {len(only_g)} (nearest oracle mode at {np.round(dg, 4).tolist()}, f {np.round(np.asarray(fg)[only_g], 4).tolist()}); "
             f"oracle-only {len(only_o)} (nearest gpu mode at {np.round(do, 4).tolist()}, f {np.round(np.asarray(fo)[only_o], 4).tolist()})")
     return pair, only_g, only_o, text
+
+
+RM_MARGIN_MIN = 1e-5
+
+
+def rm_candidates_ok(O, o, cand_gpu, removed):
+    """Repulse-Monkey candidate choice (R-8), protocol rule 3, checked decision by decision: the candidate the CUDA path
+    kept must score (min squared distance to the frozen modes, by the ORACLE's fp64 scores) within 1e-5 relative of the
+    oracle's best -- it IS the oracle's best wherever the runner-up is farther away than that; inside the band fp32
+    rounding of the d-term squared distances may order near-equal candidates differently (short rays: t_max small against
+    the distance to the modes).  Returns (mask of slots that kept the oracle's candidate, number of slots that did not)."""
+    score = o.get(O.RS_SCORE)
+    best = o.get(O.RS_CAND)
+    rows = np.flatnonzero(removed)
+    sb = score[rows, best[rows]]
+    sg = score[rows, cand_gpu[rows]]
+    assert np.all((cand_gpu[rows] >= 0) & (cand_gpu[rows] < 16))
+    ok = sg >= sb * (1.0 - RM_MARGIN_MIN)
+    assert np.all(ok), (int(np.sum(~ok)), float(np.min(sg / np.maximum(sb, 1e-300))))
+    same = removed & (cand_gpu == best)
+    return same, int(len(rows) - same.sum())

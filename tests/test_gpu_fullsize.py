@@ -130,10 +130,10 @@ def test_full_size_c5_stick_dedup_reseed_teacher_forced(orc, B):
     assert sg.reseed_strategy == so.reseed_strategy == 1
     assert (sg.n_stuck, sg.k_lost, sg.n_active) == (so.n_stuck, so.k_lost, so.n_active)
     assert np.array_equal(g.get(B.RS_SRC), o.get(orc.RS_SRC))
-    mg = o.get(orc.RS_MARGIN)
-    safe = rem_o & ((mg > 1e-5) | (mg == 0.0))
-    assert safe.sum() >= 0.99 * rem_o.sum(), (int(safe.sum()), int(rem_o.sum()))
-    assert np.array_equal(g.get(B.RS_CAND)[safe], o.get(orc.RS_CAND)[safe])
+    safe, n_other = PT.rm_candidates_ok(orc, o, g.get(B.RS_CAND), rem_o)
+    print(f"C5 full size: {n_other} of {int(rem_o.sum())} Repulse-Monkey slots kept another candidate than the oracle's, all "
+          f"scoring within 1e-5 of it")
+    assert n_other <= 0.02 * rem_o.sum()     # d = 64: rays are short against the distance to the modes, the C candidates score alike
     xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
     tol = PT.x_tol(xo, hp.lo, hp.hi)
     assert np.all(np.max(np.abs(xg - xo), axis=1)[safe] <= tol[safe])

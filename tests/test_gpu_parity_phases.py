@@ -207,13 +207,12 @@ def test_a5_reseed_via_dedup(orc, B, strategy):
     src_o, src_g = o.get(orc.RS_SRC), g.get(B.RS_SRC)
     assert np.array_equal(src_g, src_o)
     if strategy == 1:
-        mg = o.get(orc.RS_MARGIN)
-        safe = removed & ((mg > 1e-5) | (mg == 0.0))     # margin 0: degenerate ray (t_max = 0), both pick candidate 0
-        print(f"RM strategy {strategy}: {int(safe.sum())} of {int(removed.sum())} slots with a safe candidate margin")
-        assert safe.sum() >= 0.99 * removed.sum()            # protocol rule 3 (short rays, t_max ~ 0, give near-identical candidates)
+        safe, n_other = PT.rm_candidates_ok(orc, o, g.get(B.RS_CAND), removed)
+        print(f"RM: {n_other} of {int(removed.sum())} slots kept another candidate than the oracle's (all within 1e-5 of its score)")
+        assert n_other <= max(2, 0.01 * removed.sum())       # protocol rule 3 (d = 8)
     else:
         safe = removed
-    assert np.array_equal(g.get(B.RS_CAND)[safe], o.get(orc.RS_CAND)[safe])
+        assert np.array_equal(g.get(B.RS_CAND)[safe], o.get(orc.RS_CAND)[safe])
     xo, xg = o.get(orc.X), g.get(B.X).astype(np.float64)
     tol = PT.x_tol(xo, hp.lo, hp.hi)
     assert np.all(np.max(np.abs(xg - xo), axis=1)[safe] <= tol[safe])
@@ -425,13 +424,14 @@ def test_line_search_forms_are_bit_identical(B, case):
     for g in (a, b):
         g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
         g.phase(B.PH_RELEASE_EVAL)
+    retried = False
     for it in range(1, 7):
         a.phase(B.PH_LBFGS_ITER, it); b.phase(B.PH_LBFGS_ITER, it)
         for fld in (B.X, B.F, B.G, B.LS_B, B.HIST_LEN, B.HIST_S, B.HIST_Y, B.STALLED, B.XT):
             assert np.array_equal(a.get(fld), b.get(fld), equal_nan=True), (it, fld)
         assert list(a.stats().evals)[:7] == list(b.stats().evals)[:7]
-    lsb = a.get(B.LS_B)
-    assert (lsb > 0).any()                                 # some samples needed more than one trial
+        retried |= bool((a.get(B.LS_B) > 0).any())
+    assert retried                                         # some samples needed more than one trial
     # whole cycles through chisao_step (graph submission) agree as well
     wl.hp.n_osc = 3
     a, b = B.Chisao(wl), B.Chisao(wl)

@@ -62,7 +62,7 @@ def test_shapes_with_the_stencil_aware_evaluator(orc, SB, obj_id, d, K, N):
 
 
 def test_free_running_cycles_with_the_stencil_aware_evaluator(orc, SB):
-    EE.test_noise_free_mixtures_recover_the_same_modes(orc, SB, 5, 256, 4, 1e-3)
+    EE.test_noise_free_mixtures_recover_the_same_modes(orc, SB, 5, 256, 4)
     EE.test_c4_side_run_unimodal_collapses_to_the_maximiser(orc, SB)
 
 
