@@ -19,6 +19,8 @@ LIB = os.path.join(HERE, "libchisao.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+if os.environ.get("CHISAO_EXPERIMENTS"):      # ablation switches of the tensor-core kernels (profiles/; selected by CHISAO_EXP at run time)
+    FLAGS.append("-DCHISAO_EXPERIMENTS")
 
 UNITS = [("chisao_api.cu", []), ("chisao_lbfgs.cu", []), ("chisao_select.cu", []), ("chisao_tc_kernels.cu", []), ("chisao_stencil.cu", []), ("chisao_probe.cu", [])] + \
         [("chisao_eval_obj.cu", [f"-DCHISAO_OBJ_INST={i}"]) for i in range(6)]

@@ -40,7 +40,13 @@ constexpr int TCX_REC = TCX_W_FLOATS + TCX_CA_FLOATS;    // floats per pair reco
 constexpr int TCX16_W_BYTES = TCX_W_BYTES / 2 + 4096;    // fp16 form: W_hi 16 KB | W_lo 16 KB | one K = 16 step holding -c (4 KB)
 constexpr int TCX_RING = 4;                              // c / a ring slots (outlive the W stage by one epilogue)
 constexpr int TCX_PART_BYTES = 2 * 2 * 2 * TC_GROUP * 8;   // [tile parity][half][group][128] float2
-constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES + TCX_PART_BYTES;   // >= the 2 x TC_REC form
+constexpr int TC_FVS_BYTES = 1024 + 8192;                 // Hands Like Clouds: the tile's 256 values | k_hlc_tcx: the centre rows of the next tile's <= 32 samples
+constexpr int TC_SMEM_BYTES = 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES + TCX_PART_BYTES + TC_FVS_BYTES;   // >= the 2 x TC_REC form
+// Hands Like Clouds with generator warps (k_hlc_tcx): the normals of two tiles (256 points x 64 coordinates, fp32) take the
+// place of the kernel scratch and of the first W stage; two fp16 W stages follow
+constexpr int HLCX_U_BYTES = TC_PTS * TC_D * 4;           // 65 536 per tile
+constexpr int HLCX_W_OFF = 2 * HLCX_U_BYTES;              // W stage ring of k_hlc_tcx starts here (relative to the scratch)
+static_assert(HLCX_W_OFF + 2 * TCX16_W_BYTES <= TC_SCRATCH_BYTES + 2 * TCX_W_BYTES, "k_hlc_tcx carve");
 static_assert(2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES >= 2 * TC_REC_BYTES, "shared-memory carve");
 static_assert(3 * TCX16_W_BYTES <= 2 * TCX_W_BYTES, "three fp16 stages fit the two tf32 stages");
 // RFF form: three fixed-point fp16 images of the frequencies [3][4 K-chunks][256 rows][8], then the per-feature constants
@@ -52,6 +58,12 @@ constexpr int RFF_X_BYTES = 4 * TC_GROUP * RFF_TC_D * 2;   // four point images 
 static_assert(RFF_REC_BYTES + 2 * RFF_X_BYTES <= 2 * TCX_W_BYTES, "RFF carve fits the W stage region");
 constexpr uint32_t TC_TMEM_COLS = 512;                   // per group (256 columns): D0 64 | D_hi 64 | D_lo 64 | D1 64
 
+// experiment switches (ablations for profiles/): compiled in only with -DCHISAO_EXPERIMENTS, selected by CHISAO_EXP
+#ifdef CHISAO_EXPERIMENTS
+#define TC_EXP(o, bit) (((o).exp & (bit)) != 0)
+#else
+#define TC_EXP(o, bit) false
+#endif
 struct TcObj {
   int32_t K, d;
   float sigma_noise;
@@ -64,6 +76,7 @@ struct TcObj {
   float rff_s0;           // coefficient of -||x||^2
   float rff_cA, rff_Phi, rff_cL;   // uA / 2 pi;  P_hi = rint(2 pi / uA);  -(2 pi / uA - P_hi) uA   (range reduction, tc_rff_tile)
   int32_t nchunk;         // ceil(K / 64) feature chunks
+  int32_t exp;            // experiment switches (CHISAO_EXP in the environment, read by tc_configure; 0 in production)
 };
 
 // shared-memory carve (all offsets are arithmetic so that nothing is indexed dynamically through a pointer table):
@@ -85,8 +98,15 @@ struct TcSmem {
   }
   // x-stationary form: a ring of W pair stages (2 x 64 KB with tf32 operands, 3 x 36 KB with fp16 operands) with its own
   // "landed" / "free" barriers, then the c / a ring
-  __device__ __forceinline__ float *Bx(int st, int stage_bytes) const {
-    return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + st * stage_bytes);
+  __device__ __forceinline__ float *Bx(int st, int stage_bytes, int woff = TC_SCRATCH_BYTES) const {
+    return reinterpret_cast<float *>(base + 1024 + woff + st * stage_bytes);
+  }
+  __device__ __forceinline__ uint64_t *xfree(int g) const { return reinterpret_cast<uint64_t *>(base) + 28 + g; }  // k_hlc_tcx: X image of group g may be overwritten (8 warps)
+  __device__ __forceinline__ uint64_t *ufree(int b) const { return reinterpret_cast<uint64_t *>(base) + 30 + b; }  // k_hlc_tcx: normals buffer b read out (8 warps)
+  __device__ __forceinline__ uint64_t *ufull(int b) const { return reinterpret_cast<uint64_t *>(base) + 32 + b; }  // k_hlc_tcx: normals buffer b written (4 warps)
+  __device__ __forceinline__ float *xrows() const { return fvs() + 256; }   // k_hlc_tcx: [32][64] centre rows
+  __device__ __forceinline__ float *fvs() const {
+    return reinterpret_cast<float *>(base + 1024 + TC_SCRATCH_BYTES + 2 * TCX_W_BYTES + TCX_RING * TCX_CA_BYTES + TCX_PART_BYTES);
   }
   __device__ __forceinline__ uint64_t *bbarx(int st) const { return reinterpret_cast<uint64_t *>(base) + 18 + st; }
   __device__ __forceinline__ uint64_t *fbarx(int st) const { return reinterpret_cast<uint64_t *>(base) + 21 + st; }
@@ -217,10 +237,11 @@ __device__ __forceinline__ void tc_setup(const TcSmem &sm, int t, int fbar_count
   if (t == 32) {
     mbar_init(sm.bbar(0), 1); mbar_init(sm.bbar(1), 1); mbar_init(sm.mbar(0), 1); mbar_init(sm.mbar(1), 1);
     mbar_init(sm.fbar(0), fbar_count); mbar_init(sm.fbar(1), fbar_count);
-    mbar_init(sm.dbar(0), 8); mbar_init(sm.dbar(1), 8); mbar_init(sm.xbar(0), 4); mbar_init(sm.xbar(1), 4);
+    mbar_init(sm.dbar(0), 4); mbar_init(sm.dbar(1), 4); mbar_init(sm.xbar(0), 4); mbar_init(sm.xbar(1), 4);
     mbar_init(sm.cbar(0), 1); mbar_init(sm.cbar(1), 1); mbar_init(sm.cbar(2), 1); mbar_init(sm.cbar(3), 1);
     for (int st = 0; st < 3; ++st) { mbar_init(sm.bbarx(st), 1); mbar_init(sm.fbarx(st), 1); }
     for (int gs = 0; gs < 4; ++gs) mbar_init(sm.rdbar(gs), 4);
+    for (int q = 0; q < 2; ++q) { mbar_init(sm.xfree(q), 4); mbar_init(sm.ufree(q), 8); mbar_init(sm.ufull(q), 4); }
     mbar_fence_init();
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
@@ -259,16 +280,19 @@ __device__ __forceinline__ int tcx_tiles_of_cta(int ntiles) {
   return ((int)blockIdx.x < ntiles) ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 }
 
-__device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int ntc) {
+__device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int ntc, int nst_force = 0, int woff = TC_SCRATCH_BYTES) {
   const int total = ntc * o.npair;
-  const int nst = o.f16 ? 3 : 2;
+  const int nst = nst_force ? nst_force : (o.f16 ? 3 : 2);
   const uint32_t wbytes = o.f16 ? TCX16_W_BYTES : TCX_W_BYTES;       // fp16 images: hi | lo | -c (same record stride)
   for (int G = 0, p = 0, st = 0, lap = 0; G < total; ++G) {
     const int rs = G & (TCX_RING - 1);
     if (lap > 0) mbar_wait(sm.fbarx(st), (lap - 1) & 1);      // the MMAs of pair G - nst have retired in both groups
     const float *r = o.recs + (size_t)p * TCX_REC;
+    if (TC_EXP(o, 32) && G >= nst) mbar_arrive(sm.bbarx(st));      // experiment: no W traffic after the first stages
+    else {
     mbar_expect_tx(sm.bbarx(st), wbytes);
-    bulk_g2s(sm.Bx(st, (int)wbytes), r, wbytes, sm.bbarx(st));
+    bulk_g2s(sm.Bx(st, (int)wbytes, woff), r, wbytes, sm.bbarx(st));
+    }
     // ring slot rs was last read by the drains of pair G - 4; they precede the MMAs of pair G - 3, whose retirement
     // the wait above (pair G - 2 or G - 3) implies
     mbar_expect_tx(sm.cbar(rs), TCX_CA_BYTES);
@@ -279,14 +303,14 @@ __device__ __forceinline__ void tcx_loader(const TcObj &o, const TcSmem &sm, int
 }
 
 // all 32 lanes of warp 9 run the loop (warp-uniform control flow); one elected lane issues
-__device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int ntc) {
+__device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int ntc, int nst_force = 0, int woff = TC_SCRATCH_BYTES) {
   const uint32_t tm = *sm.tmem();
-  const int nst = o.f16 ? 3 : 2, stage_bytes = o.f16 ? TCX16_W_BYTES : TCX_W_BYTES;
+  const int nst = nst_force ? nst_force : (o.f16 ? 3 : 2), stage_bytes = o.f16 ? TCX16_W_BYTES : TCX_W_BYTES;
   int G = 0, st = 0, lap = 0;
   for (int it = 0; it < ntc; ++it)
     for (int p = 0; p < o.npair; ++p, ++G) {
       mbar_wait(sm.bbarx(st), lap & 1);
-      const uint64_t dBh = tc_desc(smem_u32(sm.Bx(st, stage_bytes)), 2048, 128), dBl = dBh + (uint64_t)((TCX_W_BYTES / 2) >> 4);
+      const uint64_t dBh = tc_desc(smem_u32(sm.Bx(st, stage_bytes, woff)), 2048, 128), dBl = dBh + (uint64_t)((TCX_W_BYTES / 2) >> 4);
 #pragma unroll 1
       for (int g = 0; g < 2; ++g) {
         if (p == 0) mbar_wait(sm.xbar(g), it & 1);              // this tile's X image is in TMEM
@@ -329,12 +353,15 @@ __device__ __forceinline__ void tcx_issuer(const TcObj &o, const TcSmem &sm, int
 // Compute threads (t < TC_PTS).  load(tile, x) fills the thread's point of that tile (thread t = point t & 127 of
 // group t >> 7; coordinates >= d zero) and returns a small per-tile context; finish(tile, f, ctx) consumes the value.
 // Both are called by all 256 compute threads, in tile order; load(tile + 1) runs before finish(tile).
-template <class Load, class Finish>
+// EXT (k_hlc_tcx): the X images are written by other warps (hlcx_generator); the compute threads only drain.  `load` is
+// not called, finish is finish(tile, f, it), and after the wait for a group's last MMAs of a tile every warp arrives on
+// xfree(g): the image may be overwritten.
+template <bool EXT = false, class Load, class Finish>
 __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, int t, int ntc, Load load, Finish finish) {
   const uint32_t tm = *sm.tmem();
-  const int npair = o.npair, w = t >> 5, lane = t & 31, wq = w & 3, hf = w >> 2, own = t >> 7;
+  const int npair = o.npair, w = t >> 5, lane = t & 31, wq = w & 3, own = t >> 7;
   const uint32_t lanes = tm + ((uint32_t)(wq * 32) << 16);
-  const uint32_t xaddr = lanes + (uint32_t)(own * 256), rd = lanes + (uint32_t)(128 + 64 * hf);
+  const uint32_t xaddr = lanes + (uint32_t)(own * 256), rd = xaddr + 128u;   // the thread's point = TMEM lane t & 127 of group t >> 7
   auto write_x = [&](const float (&xv)[TC_D]) {        // hi / lo images of the thread's point -> its TMEM lane
     if (o.f16) {   // two fp16 per 32-bit column (element 2c in the low half): hi in columns [0, 32), lo in [32, 64)
 #pragma unroll
@@ -366,44 +393,52 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
     __syncwarp();
     if (lane == 0) mbar_arrive(sm.xbar(own));
   };
-  if (o.f16) {   // the constant operand row (1, 1, 1, 0, ...) of the -c step: columns [64, 80) of the thread's own lane, once
+  if (!EXT && o.f16) {   // the constant operand row (1, 1, 1, 0, ...) of the -c step: columns [64, 80) of the thread's own lane, once
     uint32_t one[16];
 #pragma unroll
     for (int c = 0; c < 16; ++c) one[c] = 0u;
     one[0] = 0x3C003C00u; one[1] = 0x00003C00u;
     tc_st16u(xaddr + 64, one);
   }
-  float xn[TC_D];
-  auto cn = load((int)blockIdx.x, xn);
-  write_x(xn);
+  float xn[EXT ? 1 : TC_D];
+  decltype(load(0, xn)) cn{};
+  if constexpr (!EXT) { cn = load((int)blockIdx.x, xn); write_x(xn); }
   int G = 0;
   for (int it = 0; it < ntc; ++it) {
     const int tile = (int)blockIdx.x + it * (int)gridDim.x;
     const bool more = it + 1 < ntc;
     const auto cc = cn;
-    float m0 = -INFINITY, s0 = 0.0f, m1 = -INFINITY, s1 = 0.0f;
+    float m = -INFINITY, s = 0.0f;                    // online log-sum-exp of the thread's point over all components
     for (int p = 0; p < npair; ++p, ++G) {
-      const bool swap = more && (p == npair - 1);
-      if (swap) cn = load(tile + (int)gridDim.x, xn);  // global loads in flight under the waits below
+      const bool swap = !EXT && more && (p == npair - 1);
+      if constexpr (!EXT) { if (swap) cn = load(tile + (int)gridDim.x, xn); }  // global loads in flight under the waits below
       const int rs = G & (TCX_RING - 1);
       mbar_wait(sm.cbar(rs), (G >> 2) & 1);           // c, a of this pair have landed
       const float *ca = sm.CA(rs);
-      const float4 *c4 = reinterpret_cast<const float4 *>(ca + 64 * hf);
-      const float a_k = ca[128 + hf];                 // a = -inf pads an odd K
+      mbar_wait(sm.mbar(own), G & 1);                 // the group's MMAs of this pair have retired
+      if (EXT && p == npair - 1) { __syncwarp(); if (lane == 0) mbar_arrive(sm.xfree(own)); }   // ... the last of the tile: the X image is free
+      asm volatile("tcgen05.fence::after_thread_sync;");
 #pragma unroll
-      for (int g = 0; g < 2; ++g) {
-        mbar_wait(sm.mbar(g), G & 1);
-        asm volatile("tcgen05.fence::after_thread_sync;");
+      for (int hf = 0; hf < 2; ++hf) {                // the two components of the pair: accumulator columns [64 hf, 64 hf + 64)
         uint32_t r[64];
-        const uint32_t taddr = rd + (uint32_t)(g * 256);
-        tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        asm volatile("tcgen05.fence::before_thread_sync;");
-        __syncwarp();
-        if (lane == 0) mbar_arrive(sm.dbar(g));       // accumulators are in registers: the next MMAs may overwrite them
-        if (swap && g == own) write_x(xn);            // this group's last MMAs of the tile have retired
+        const uint32_t taddr = rd + (uint32_t)(64 * hf);
+        if (!TC_EXP(o, 16)) {
+          tc_ld16(taddr, r, 0); tc_ld16(taddr, r, 1); tc_ld16(taddr, r, 2); tc_ld16(taddr, r, 3);
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        } else {
+#pragma unroll
+          for (int n = 0; n < 64; ++n) r[n] = 0x3f800000u;
+        }
+        if (hf == 1) {                                // both components are in registers: the next MMAs may overwrite the accumulators
+          asm volatile("tcgen05.fence::before_thread_sync;");
+          __syncwarp();
+          if (lane == 0) mbar_arrive(sm.dbar(own));
+          if constexpr (!EXT) { if (swap) write_x(xn); }   // this group's last MMAs of the tile have retired
+        }
+        const float a_k = ca[128 + hf];               // a = -inf pads an odd K
         float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
-        if (o.f16) {                                  // -c went through the tensor pipe
+        if (TC_EXP(o, 8)) { q0 = __uint_as_float(r[0]) + __uint_as_float(r[63]); }
+        else if (o.f16) {                             // -c went through the tensor pipe
 #pragma unroll
           for (int n = 0; n < 64; n += 4) {
             const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
@@ -411,6 +446,7 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
             q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
           }
         } else {
+          const float4 *c4 = reinterpret_cast<const float4 *>(ca + 64 * hf);
 #pragma unroll
           for (int n = 0; n < 64; n += 4) {
             const float4 c = c4[n >> 2];
@@ -420,26 +456,12 @@ __device__ __forceinline__ void tcx_compute(const TcObj &o, const TcSmem &sm, in
           }
         }
         const float v = fmaf(-0.5f, (q0 + q1) + (q2 + q3), a_k);
-        if (g == 0) {
-          const float mn = fmaxf(m0, v);
-          if (mn > -INFINITY) { s0 = s0 * __expf(m0 - mn) + __expf(v - mn); m0 = mn; }
-        } else {
-          const float mn = fmaxf(m1, v);
-          if (mn > -INFINITY) { s1 = s1 * __expf(m1 - mn) + __expf(v - mn); m1 = mn; }
-        }
+        const float mn = fmaxf(m, v);
+        if (mn > -INFINITY) { s = s * __expf(m - mn) + __expf(v - mn); m = mn; }
       }
     }
-    // the two component halves of every point meet: part[tile parity][hf][g][point] = (m, s); the barrier of the
-    // next tile separates this tile's reads from the writes of the tile after it
-    float2 *part = sm.part() + (it & 1) * (4 * TC_GROUP);
-    part[(hf * 2 + 0) * TC_GROUP + wq * 32 + lane] = make_float2(m0, s0);
-    part[(hf * 2 + 1) * TC_GROUP + wq * 32 + lane] = make_float2(m1, s1);
-    asm volatile("bar.sync 3, %0;" ::"n"(TC_PTS) : "memory");
-    const float2 pa = part[(0 * 2 + own) * TC_GROUP + (t & (TC_GROUP - 1))];
-    const float2 pb = part[(1 * 2 + own) * TC_GROUP + (t & (TC_GROUP - 1))];
-    const float mm = fmaxf(pa.x, pb.x);
-    const float f = (mm > -INFINITY) ? mm + logf(pa.y * __expf(pa.x - mm) + pb.y * __expf(pb.x - mm)) : -INFINITY;
-    finish(tile, f, cc);
+    const float f = (m > -INFINITY) ? m + logf(s) : -INFINITY;
+    if constexpr (EXT) finish(tile, f, it); else finish(tile, f, cc);
   }
 }
 
@@ -813,9 +835,10 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
   if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) {
     const int ntc = tcx_tiles_of_cta(ntiles);
     const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+    const int nst = TC_EXP(o, 1) ? 2 : 0;                   // experiment: two W stages instead of three
     if (warp < TC_PTS / 32) tcx_compute(o, sm, t, ntc, load, finish);
-    else if (warp == TC_PTS / 32) { if (t == TC_PTS) tcx_loader(o, sm, ntc); }
-    else tcx_issuer(o, sm, ntc);
+    else if (warp == TC_PTS / 32) { if (t == TC_PTS) tcx_loader(o, sm, ntc, nst); }
+    else tcx_issuer(o, sm, ntc, nst);
   } else if constexpr (OBJ == CHISAO_OBJ_RFF) {
     // persistent over tiles; the frequencies' images and the per-feature constants land once (53 248 bytes)
     const int ntc = tcx_tiles_of_cta(ntiles);

@@ -305,8 +305,180 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   tc_teardown(sm, t);
 }
 
+// ---- Hands Like Clouds, GMM_FULL with fp16 operands: normals generated ONCE, by warps of their own ---------------------
+// k_hlc_tc above generates the d normals of a draw twice (for the evaluation point and again for the reduction), on
+// the warps that drain the accumulators, while the tensor pipe waits: at C5 the kernel ran at 0.45 of the FD kernel's
+// evaluation rate.  Here four more warps (10..13; warp w owns TMEM lanes 32 (w & 3) .. + 31 of both groups) generate
+// the normals of the NEXT tile under the current tile's MMAs: they keep u in shared memory for the reduction
+// (two tiles of 256 x 64 fp32, XOR-swizzled 16-byte chunks), form x + sigma u, split it into fp16 hi / lo and write
+// the X image of their 32 points straight into TMEM.  The compute warps only drain (tcx_compute<EXT>), add the noise and
+// reduce.  Barriers: xfree(g) "the group's last MMAs of the tile retired" (compute -> generators), xbar(g) "X image
+// written" (generators -> issuer), ufull(b) / ufree(b) for the two normals buffers.
+constexpr int HLCX_THREADS = TC_THREADS + 128;
+__device__ __forceinline__ float *hlcx_u_chunk(const TcSmem &sm, int buf, int pt, int c4) {   // 16-byte chunk c4 of point pt
+  return reinterpret_cast<float *>(sm.scratch() + (size_t)buf * HLCX_U_BYTES + (size_t)pt * (TC_D * 4) + (size_t)((c4 ^ (pt & 15)) * 16));
+}
+// Software pipeline of a generator warp over the CTA's tiles:  A(0);  for it: B(it); A(it + 1)
+//   A(it): the normals of tile `it` -> normals buffer it & 1 (after the reduction of tile it - 2 has read it), and the
+//          centre rows of the tile's samples -> shared memory;  this is the expensive part (Philox + Box-Muller, ~70
+//          instructions per normal) and runs under the MMAs of tile it - 1
+//   B(it): after the group's last MMAs of tile it - 1 have retired: x + sigma u from shared memory, fp16 hi / lo split,
+//          tcgen05.st into the X image, "image written" -- a few hundred instructions on the tensor pipe's critical path
+__device__ __forceinline__ void gen_sync() { asm volatile("bar.sync 5, 128;" ::: "memory"); }   // the four generator warps
+__device__ __forceinline__ void hlcx_generator(const TcObj &o, const TcSmem &sm, const HlcArgs &a, int t, int ntc, int cnt, int spt, float sigma) {
+  const uint32_t tm = *sm.tmem();
+  const int lane = t & 31, q = (t >> 5) & 3, d = a.d, M = a.M;
+  const int gt = q * 32 + lane;                                    // index among the 128 generator threads
+  const uint32_t lanes = tm + ((uint32_t)(q * 32) << 16);
+  {   // the constant operand row (1, 1, 1, 0, ...) of the -c step: columns [64, 80) of both groups, once
+    uint32_t one[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) one[c] = 0u;
+    one[0] = 0x3C003C00u; one[1] = 0x00003C00u;
+    tc_st16u(lanes + 64, one);
+    tc_st16u(lanes + 256 + 64, one);
+  }
+  const uint32_t tg = rng_tag(5, a.iter, PUR_HLC_U);
+  float4 *xr4 = reinterpret_cast<float4 *>(sm.xrows());
+  auto phase_a = [&](int it) {
+    const int tile = (int)blockIdx.x + it * (int)gridDim.x, first = tile * spt, buf = it & 1;
+    if (it >= 2) mbar_wait(sm.ufree(buf), ((it >> 1) - 1) & 1);    // the reduction of tile it - 2 has read this buffer
+    // centre rows of the tile's samples (zero beyond the list and beyond d): [spt][16] float4
+    for (int e = gt; e < spt * (TC_D / 4); e += 128) {
+      const int sr = e >> 4, c4 = e & 15;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (first + sr < cnt && 4 * c4 < d) v = *reinterpret_cast<const float4 *>(a.x + (size_t)a.list[first + sr] * d + 4 * c4);
+      xr4[e] = v;
+    }
+#pragma unroll 1
+    for (int g = 0; g < 2; ++g) {
+      const int pt = g * TC_GROUP + q * 32 + lane;
+      const int s = pt / M, k = pt - s * M;
+      const bool valid = (s < spt) && (first + s < cnt);
+      const int i = valid ? a.list[first + s] : 0;
+      const uint32_t b0 = ((uint32_t)k * (uint32_t)d) >> 2;        // first Philox block of the draw (d is a multiple of 4)
+#pragma unroll 4
+      for (int c4 = 0; c4 < TC_D / 4; ++c4) {
+        float4 u = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (valid && 4 * c4 < d && !TC_EXP(o, 2)) {
+          const uint4 w = philox_block(a.seed, b0 + (uint32_t)c4, (uint32_t)i, (uint32_t)a.cycle, tg);
+          box_muller(w.x, w.y, u.x, u.y);
+          box_muller(w.z, w.w, u.z, u.w);
+        }
+        *reinterpret_cast<float4 *>(hlcx_u_chunk(sm, buf, pt, c4)) = u;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(sm.ufull(buf));                     // (mbarrier.arrive has release semantics: the stores above are visible to the waiters)
+    gen_sync();                                                    // the centre rows are complete
+  };
+  auto phase_b = [&](int it) {
+    const int buf = it & 1;
+#pragma unroll 1
+    for (int g = 0; g < 2; ++g) {
+      const int pt = g * TC_GROUP + q * 32 + lane;
+      const int s = min(pt / M, HLC_MAX_SPT - 1);                  // (rows of idle points are zero like their normals)
+      const uint32_t xaddr = lanes + (uint32_t)(g * 256);
+      if (it >= 1) mbar_wait(sm.xfree(g), (it - 1) & 1);            // the group's MMAs of the previous tile are done with the image
+      asm volatile("tcgen05.fence::after_thread_sync;");
+#pragma unroll
+      for (int hq = 0; hq < 2; ++hq) {                             // coordinates 32 hq .. 32 hq + 31
+        uint32_t h[16], l[16];
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+          const int c4 = 8 * hq + b;
+          const float4 u = *reinterpret_cast<const float4 *>(hlcx_u_chunk(sm, buf, pt, c4));
+          const float4 xv = (pt / M < spt) ? xr4[s * (TC_D / 4) + c4] : make_float4(0.f, 0.f, 0.f, 0.f);
+          const float x0 = fmaf(sigma, u.x, xv.x), x1 = fmaf(sigma, u.y, xv.y), x2 = fmaf(sigma, u.z, xv.z), x3 = fmaf(sigma, u.w, xv.w);
+          const __half h0 = __float2half_rn(x0), h1 = __float2half_rn(x1), h2 = __float2half_rn(x2), h3 = __float2half_rn(x3);
+          const __half l0 = __float2half_rn(x0 - __half2float(h0)), l1 = __float2half_rn(x1 - __half2float(h1));
+          const __half l2 = __float2half_rn(x2 - __half2float(h2)), l3 = __float2half_rn(x3 - __half2float(h3));
+          h[2 * b] = (uint32_t)__half_as_ushort(h0) | ((uint32_t)__half_as_ushort(h1) << 16);
+          h[2 * b + 1] = (uint32_t)__half_as_ushort(h2) | ((uint32_t)__half_as_ushort(h3) << 16);
+          l[2 * b] = (uint32_t)__half_as_ushort(l0) | ((uint32_t)__half_as_ushort(l1) << 16);
+          l[2 * b + 1] = (uint32_t)__half_as_ushort(l2) | ((uint32_t)__half_as_ushort(l3) << 16);
+        }
+        tc_st16u(xaddr + 16 * hq, h);
+        tc_st16u(xaddr + 32 + 16 * hq, l);
+      }
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      asm volatile("tcgen05.fence::before_thread_sync;");
+      __syncwarp();
+      if (lane == 0) mbar_arrive(sm.xbar(g));
+    }
+    gen_sync();                                                    // every warp is done with the centre rows: A(it + 1) may overwrite them
+  };
+  phase_a(0);
+  for (int it = 0; it < ntc; ++it) {
+    phase_b(it);
+    if (it + 1 < ntc) phase_a(it + 1);
+  }
+}
+
+__global__ void __launch_bounds__(HLCX_THREADS, 1) k_hlc_tcx(const TcObj o, const HlcArgs a) {
+  extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
+  const TcSmem sm = tc_carve(tc_smem_raw);
+  const int t = threadIdx.x, d = a.d, M = a.M;
+  const float sigma = *a.sigma_dev;
+  if (sigma == 0.0f) return;                       // no spread among the unfrozen samples: nobody moves (R-18)
+  const int spt = min(TC_PTS / M, HLC_MAX_SPT);
+  const int cnt = a.count ? *a.count : a.max_count;
+  const int ntiles = (cnt + spt - 1) / spt;
+  if ((int)blockIdx.x >= ntiles) return;
+  tc_setup(sm, t, 1);
+  const int ntc = tcx_tiles_of_cta(ntiles);
+  const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+  if (warp < TC_PTS / 32) {
+    const int s = t / M, k = t - s * M;
+    float *fvs = sm.fvs();
+    auto noload = [](int, float (&)[1]) -> int { return 0; };
+    // Positions are only written by the tile that owns the sample; the generators read the NEXT tile's (other) samples.
+    auto finish = [&](int tile, float val, int it) {
+      const int first = tile * spt, buf = it & 1;
+      const bool valid = (s < spt) && (first + s < cnt);
+      const int i = valid ? a.list[first + s] : 0;
+      compute_sync();                        // the previous tile's reduction has read fvs
+      if (valid) {
+        val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
+        a.hlc_f[(size_t)i * M + k] = val;
+      } else {
+        val = 0.f;
+      }
+      fvs[t] = val;
+      mbar_wait(sm.ufull(buf), (it >> 1) & 1);   // the tile's normals are in shared memory
+      compute_sync();
+      const int nval = TC_EXP(o, 4) ? 0 : min(spt, cnt - first);
+      for (int item = t; item < nval * d; item += TC_PTS) {
+        const int ss = item / d, j = item - ss * d;
+        const int ii = a.list[first + ss];
+        float b = 0.0f;
+        if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
+        float acc = 0.0f;
+        for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, hlcx_u_chunk(sm, buf, ss * M + kk, j >> 2)[j & 3], acc);
+        const float gh = acc / ((float)M * sigma);
+        a.ghat[(size_t)ii * d + j] = gh;
+        const float xo = a.x[(size_t)ii * d + j];
+        a.x[(size_t)ii * d + j] = clipf(fmaf(a.eta, gh, xo), a.lo[j], a.hi[j]);
+      }
+      __syncwarp();
+      if ((t & 31) == 0) mbar_arrive(sm.ufree(buf));
+      if (t == 0) atomicAdd(&a.evals[EV_HLC], (unsigned long long)nval * (unsigned long long)M);
+    };
+    tcx_compute<true>(o, sm, t, ntc, noload, finish);
+  } else if (warp == TC_PTS / 32) {
+    if (t == TC_PTS) tcx_loader(o, sm, ntc, 2, HLCX_W_OFF);
+  } else if (warp == TC_PTS / 32 + 1) {
+    tcx_issuer(o, sm, ntc, 2, HLCX_W_OFF);
+  } else {
+    hlcx_generator(o, sm, a, t, ntc, cnt, spt, sigma);
+  }
+  tc_teardown(sm, t);
+}
+
 // ---- launchers ------------------------------------------------------------------------------------------------
 static int g_tc_sms = 148;
+static int g_exp = 0;
+static bool g_hlc_plain = false;   // CHISAO_HLC_PLAIN in the environment: keep k_hlc_tc for GMM_FULL (A/B measurements)
 static inline int tc_grid(int obj_id, int ntiles) {   // persistent CTAs, one per SM
   (void)obj_id;
   return ntiles > g_tc_sms ? g_tc_sms : ntiles;
@@ -316,15 +488,19 @@ cudaError_t tc_configure() {
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
     g_tc_sms = sms;
+  g_hlc_plain = getenv("CHISAO_HLC_PLAIN") != nullptr;
+  g_exp = getenv("CHISAO_EXP") ? atoi(getenv("CHISAO_EXP")) : 0;
 #define CFG(K) if ((e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES)) != cudaSuccess) return e;
   CFG(k_eval_fd_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_fd_tc<CHISAO_OBJ_QUAD>)
   CFG(k_eval_points_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_eval_points_tc<CHISAO_OBJ_QUAD>)
   CFG(k_hlc_tc<CHISAO_OBJ_GMM_FULL>) CFG(k_hlc_tc<CHISAO_OBJ_QUAD>)
   CFG(k_eval_fd_tc<CHISAO_OBJ_RFF>) CFG(k_eval_points_tc<CHISAO_OBJ_RFF>) CFG(k_hlc_tc<CHISAO_OBJ_RFF>)
+  CFG(k_hlc_tcx)
 #undef CFG
   return cudaSuccess;
 }
-cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samples, cudaStream_t st) {
+cudaError_t launch_fd_tc(int obj_id, const TcObj &o_in, const FdArgs &a, int n_samples, cudaStream_t st) {
+  TcObj o = o_in; o.exp = g_exp;
   const int spt = fd_tc_samples_per_tile(a.d);
   const int grid = tc_grid(obj_id, (n_samples + spt - 1) / spt);
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_fd_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
@@ -332,7 +508,8 @@ cudaError_t launch_fd_tc(int obj_id, const TcObj &o, const FdArgs &a, int n_samp
   else k_eval_fd_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
-cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samples, cudaStream_t st) {
+cudaError_t launch_pt_tc(int obj_id, const TcObj &o_in, const PtArgs &a, int n_samples, cudaStream_t st) {
+  TcObj o = o_in; o.exp = g_exp;
   const int ntiles = (n_samples + TC_PTS - 1) / TC_PTS;
   const int grid = (a.mode == PT_LS_ALL) ? ntiles : tc_grid(obj_id, ntiles);   // tile-local rounds: one tile per CTA
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
@@ -340,11 +517,13 @@ cudaError_t launch_pt_tc(int obj_id, const TcObj &o, const PtArgs &a, int n_samp
   else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
-cudaError_t launch_hlc_tc(int obj_id, const TcObj &o, const HlcArgs &a, int n_samples, cudaStream_t st) {
+cudaError_t launch_hlc_tc(int obj_id, const TcObj &o_in, const HlcArgs &a, int n_samples, cudaStream_t st) {
+  TcObj o = o_in; o.exp = g_exp;
   const int spt = TC_PTS / a.M < HLC_MAX_SPT ? TC_PTS / a.M : HLC_MAX_SPT;
   const int grid = tc_grid(obj_id, (n_samples + spt - 1) / spt);
   if (obj_id == CHISAO_OBJ_QUAD) k_hlc_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else if (obj_id == CHISAO_OBJ_RFF) k_hlc_tc<CHISAO_OBJ_RFF><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
+  else if (o.f16 && (a.d & 3) == 0 && !g_hlc_plain) k_hlc_tcx<<<grid, HLCX_THREADS, TC_SMEM_BYTES, st>>>(o, a);   // normals generated once, by warps of their own
   else k_hlc_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
