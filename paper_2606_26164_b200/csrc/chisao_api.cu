@@ -408,6 +408,8 @@ cudaError_t eval_points(chisao_ctx *c, int mode, int b, int iter) {
     a.X = s.x; a.list = nullptr; a.count = nullptr;
   } else if (mode == PT_LS_ALL) {
     a.X = s.xt; a.list = s.ls_list[0]; a.count = &s.ctrl->ls_cnt[0];
+    // FP32-FMA evaluators at d <= 32: the rows x, p, g of a tile stay in shared memory over the rounds (<= 96 KB more)
+    a.rows_in_smem = (!c->use_tc && c->obj.DP <= 32 && eval_smem_bytes(c->obj, ls_rows_bytes(c->obj.DP)) <= 200 * 1024) ? 1 : 0;
   } else {
     a.X = s.xt; a.list = s.ls_list[b % 3]; a.count = &s.ctrl->ls_cnt[b % 3];
     a.next_list = s.ls_list[(b + 1) % 3]; a.next_cnt = &s.ctrl->ls_cnt[(b + 1) % 3];

@@ -310,6 +310,10 @@ __device__ __forceinline__ void eval_tile(const DevObj &o, const EvalSmem &sm, i
   for (int pp = 0; pp < PPT; ++pp) { m[pp] = -INFINITY; s[pp] = 0.0f; }
   const int nchunks = (o.K + o.kc - 1) / o.kc;
   const uint32_t chunk_floats = (uint32_t)o.kc * o.rec;
+  if (nchunks == 1 && use != 0) {
+    // the whole objective fits one chunk and an earlier call of this CTA has landed it in buffer 0: it is still there
+    accum_records<OBJ, DP>(sm.chunk[0], o.K, o.rec, sm.pts, t, o.s0, m, s);
+  } else {
   if (t == 0) {  // first chunk
     const int n0 = min(o.kc, o.K);
     mbar_expect_tx(&sm.bar[use & 1], (uint32_t)n0 * o.rec * 4);
@@ -331,6 +335,7 @@ __device__ __forceinline__ void eval_tile(const DevObj &o, const EvalSmem &sm, i
     accum_records<OBJ, DP>(sm.chunk[u & 1], nrec, o.rec, sm.pts, t, o.s0, m, s);
   }
   use += nchunks;
+  }
 #pragma unroll
   for (int pp = 0; pp < PPT; ++pp) {
     if constexpr (OBJ == CHISAO_OBJ_RFF) {

@@ -102,6 +102,7 @@ struct PtArgs {
   float *xt;                 // [N][d] trial points (rewritten on reject)
   const float *x, *p, *g, *lo, *hi;
   int32_t *ls_b, *next_list, *next_cnt, *fd_list, *fd_cnt, *zero_cnt;
+  int32_t rows_in_smem;      // PT_LS_ALL: the launch carries 3 x [DP/4][PTILE] float4 of extra shared memory for the rows x, p, g
   float c1, shrink;
   uint64_t seed;
   unsigned long long *evals;
@@ -170,21 +171,40 @@ __global__ void __launch_bounds__(NT, 2) k_eval_points(const DevObj o, const PtA
   if (t == 0) { mbar_init(&sm.bar[0], 1); mbar_init(&sm.bar[1], 1); mbar_fence_init(); }
   const bool vec = (d & 3) == 0;
   int idx[PPT]; bool valid[PPT];
+  // PT_LS_ALL with rows_in_smem: the rows x, p, g of the thread's samples stay in shared memory for all rounds
+  // (thread-private float4 columns like the staged points), f, the Armijo term and the step in registers: a round
+  // touches global memory only for the bounds and, when a sample leaves the loop, for its results
+  float4 *XS = reinterpret_cast<float4 *>(sm.extra), *PS = XS + (DP / 4) * PTILE, *GS = PS + (DP / 4) * PTILE;
+  const bool rows = a.mode == PT_LS_ALL && a.rows_in_smem;
+  float f_i[PPT], dec_i[PPT], t_i[PPT];
 #pragma unroll
   for (int pp = 0; pp < PPT; ++pp) {
     const int e = first + pp * NT + t;
     valid[pp] = e < cnt;
     idx[pp] = valid[pp] ? (a.list ? a.list[e] : e) : 0;
+    f_i[pp] = 0.f; dec_i[pp] = 0.f; t_i[pp] = 0.f;
+    if (rows && valid[pp]) {
+      const int i = idx[pp];
+      f_i[pp] = a.f[i]; dec_i[pp] = a.dec[i]; t_i[pp] = a.tcur[i];
+#pragma unroll
+      for (int c4 = 0; c4 < DP / 4; ++c4) {
+        XS[c4 * PTILE + pp * NT + t] = ld_row4(a.x + (size_t)i * d, c4, d, vec);
+        PS[c4 * PTILE + pp * NT + t] = ld_row4(a.p + (size_t)i * d, c4, d, vec);
+        GS[c4 * PTILE + pp * NT + t] = ld_row4(a.g + (size_t)i * d, c4, d, vec);
+      }
+    }
   }
   uint32_t use = 0;
   unsigned int nev = 0;                                   // evaluations done by this thread (PT_LS_ALL)
   for (int b = a.b;; ++b) {
+    if (!(rows && b > a.b)) {                             // (with the rows in shared memory, a retry has written its next point already)
 #pragma unroll
-    for (int pp = 0; pp < PPT; ++pp) {
-      const float *row = a.X + (size_t)idx[pp] * d;
+      for (int pp = 0; pp < PPT; ++pp) {
+        const float *row = a.X + (size_t)idx[pp] * d;
 #pragma unroll
-      for (int c4 = 0; c4 < DP / 4; ++c4)
-        sm.pts[c4 * PTILE + pp * NT + t] = valid[pp] ? ld_row4(row, c4, d, vec) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int c4 = 0; c4 < DP / 4; ++c4)
+          sm.pts[c4 * PTILE + pp * NT + t] = valid[pp] ? ld_row4(row, c4, d, vec) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
     }
     __syncthreads();
     float fv[PPT];
@@ -200,7 +220,7 @@ __global__ void __launch_bounds__(NT, 2) k_eval_points(const DevObj o, const PtA
           a.f[i] = fv[pp] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, 0, 0);
         } else {
           val = fv[pp] + eval_noise(o.sigma_noise, a.seed, a.cycle, i, 1, a.iter, 2 * d + 1 + b);
-          accept = ls_accept(val, a.f[i], a.dec[i], a.c1);
+          accept = ls_accept(val, rows ? f_i[pp] : a.f[i], rows ? dec_i[pp] : a.dec[i], a.c1);
           retry = !accept && (b < a.ls_max);
           nev += 1u;
         }
@@ -212,7 +232,41 @@ __global__ void __launch_bounds__(NT, 2) k_eval_points(const DevObj o, const PtA
           const int sr = warp_append(a.next_cnt, retry);
           if (retry) a.next_list[sr] = i;
         }
-        if (retry) {
+        if (rows) {
+          const int col = pp * NT + t;
+          if (valid[pp] && !retry && b > a.b) {           // the sample leaves the loop: its last trial point and step go back to the state
+            a.tcur[i] = t_i[pp]; a.dec[i] = dec_i[pp];
+            for (int c4 = 0; 4 * c4 < d; ++c4) {
+              const float4 v = sm.pts[c4 * PTILE + col];
+              float *dst = a.xt + (size_t)i * d + 4 * c4;
+              if (vec) *reinterpret_cast<float4 *>(dst) = v;
+              else {
+                dst[0] = v.x;
+                if (4 * c4 + 1 < d) dst[1] = v.y;
+                if (4 * c4 + 2 < d) dst[2] = v.z;
+                if (4 * c4 + 3 < d) dst[3] = v.w;
+              }
+            }
+          }
+          if (retry) {   // same arithmetic, in the same coordinate order, as ls_retry_row
+            const float tn = t_i[pp] * a.shrink;
+            t_i[pp] = tn;
+            float dsum = 0.0f;
+#pragma unroll
+            for (int c4 = 0; c4 < DP / 4; ++c4) {
+              if (4 * c4 < d) {
+                const float4 xo = XS[c4 * PTILE + col], pv = PS[c4 * PTILE + col], gv = GS[c4 * PTILE + col];
+                float4 xn = make_float4(0.f, 0.f, 0.f, 0.f);
+                { xn.x = clipf(fmaf(tn, pv.x, xo.x), a.lo[4 * c4], a.hi[4 * c4]); dsum = fmaf(-gv.x, xn.x - xo.x, dsum); }
+                if (4 * c4 + 1 < d) { xn.y = clipf(fmaf(tn, pv.y, xo.y), a.lo[4 * c4 + 1], a.hi[4 * c4 + 1]); dsum = fmaf(-gv.y, xn.y - xo.y, dsum); }
+                if (4 * c4 + 2 < d) { xn.z = clipf(fmaf(tn, pv.z, xo.z), a.lo[4 * c4 + 2], a.hi[4 * c4 + 2]); dsum = fmaf(-gv.z, xn.z - xo.z, dsum); }
+                if (4 * c4 + 3 < d) { xn.w = clipf(fmaf(tn, pv.w, xo.w), a.lo[4 * c4 + 3], a.hi[4 * c4 + 3]); dsum = fmaf(-gv.w, xn.w - xo.w, dsum); }
+                sm.pts[c4 * PTILE + col] = xn;            // own column: read only by this thread in eval_tile
+              }
+            }
+            dec_i[pp] = dsum;
+          }
+        } else if (retry) {
           const float tn = a.tcur[i] * a.shrink;
           a.tcur[i] = tn;
           a.dec[i] = ls_retry_row(a, i, d, tn);          // rewrites x_t of sample i (read back by this thread only)
@@ -374,9 +428,10 @@ cudaError_t launch_fd_obj(const DevObj &o, const FdArgs &a, int grid, cudaStream
   }
   return cudaGetLastError();
 }
+inline size_t ls_rows_bytes(int DP) { return (size_t)3 * (DP / 4) * PTILE * 16; }
 template <int OBJ>
 cudaError_t launch_pt_obj(const DevObj &o, const PtArgs &a, int grid, cudaStream_t st) {
-  const size_t sh = eval_smem_bytes(o, 0);
+  const size_t sh = eval_smem_bytes(o, a.rows_in_smem ? ls_rows_bytes(o.DP) : 0);
   switch (o.DP) {
     case 8: k_eval_points<OBJ, 8><<<grid, NT, sh, st>>>(o, a); break;
     case 32: k_eval_points<OBJ, 32><<<grid, NT, sh, st>>>(o, a); break;

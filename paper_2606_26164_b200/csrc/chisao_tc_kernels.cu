@@ -235,7 +235,11 @@ __device__ __forceinline__ void hlc_normals(uint64_t seed, int i, int cycle, int
   }
 }
 
-// Hands Like Clouds on the tensor-core evaluator: point t of the tile = (sample t / M, draw t % M), M <= 128
+// Hands Like Clouds on the tensor-core evaluator: point t of the tile = (sample t / M, draw t % M), M <= 128.
+// QUAD and RFF forms: a draw's normals are generated once, in load, and kept in shared memory for the reduction (row t
+// of one of two buffers, by tile parity: the QUAD form fetches a tile's point two tiles ahead of its finish).  The
+// x-stationary GMM_FULL form has no shared memory left for them (its W stages fill it): it regenerates them in finish --
+// with fp16 operands k_hlc_tcx below takes its place.
 struct HlcCtx { int i; bool valid; };
 template <int OBJ>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const HlcArgs a) {
@@ -250,6 +254,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   if ((int)blockIdx.x >= ntiles) return;
   tc_begin<OBJ>(sm, t);
   const int s = t / M, k = t - s * M;
+  constexpr bool KEEP_U = OBJ != CHISAO_OBJ_GMM_FULL;
+  constexpr int US = (OBJ == CHISAO_OBJ_RFF) ? RFF_TC_D + 1 : TC_D + 1;      // row stride of the normals (conflict-free)
+  // buffer 0 in the kernel scratch; buffer 1 behind it (RFF: 2 x 33 KB fit the scratch) or behind the resident QUAD record
+  float *Us0 = reinterpret_cast<float *>(sm.scratch());
+  float *Us1 = (OBJ == CHISAO_OBJ_RFF) ? Us0 + TC_PTS * US
+                                       : reinterpret_cast<float *>(sm.scratch() + TC_SCRATCH_BYTES + ((TC_REC_BYTES + 255) & ~255));
+  static_assert(2 * TC_PTS * (RFF_TC_D + 1) * 4 <= TC_SCRATCH_BYTES, "RFF: two normals buffers in the scratch");
+  static_assert(TC_PTS * (TC_D + 1) * 4 <= TC_SCRATCH_BYTES && ((TC_REC_BYTES + 255) & ~255) + TC_PTS * (TC_D + 1) * 4 <= 2 * TCX_W_BYTES, "QUAD: normals buffers");
+  auto ubuf = [&](int tile) { return ((((tile - (int)blockIdx.x) / (int)gridDim.x) & 1) && KEEP_U) ? Us1 : Us0; };
   auto load = [&](int tile, float (&x)[TC_D]) -> HlcCtx {
     HlcCtx c;
     const int first = tile * spt;
@@ -258,6 +271,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
     if (c.valid) {
       float u[TC_D];
       hlc_normals(a.seed, c.i, a.cycle, a.iter, k, d, u);
+      if constexpr (KEEP_U) {
+        float *row = ubuf(tile) + t * US;
+#pragma unroll
+        for (int q = 0; q < US - 1; ++q) row[q] = u[q];
+      }
       tc_load_row(a.x + (size_t)c.i * d, d, (d & 3) == 0, x);
 #pragma unroll
       for (int q = 0; q < TC_D; ++q) x[q] = fmaf(sigma, u[q], x[q]);   // evaluation points are not clipped (R-12)
@@ -271,16 +289,18 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   // (load of the tile precedes its finish); tiles own disjoint samples.
   auto finish = [&](int tile, float val, const HlcCtx &c) {
     const int first = tile * spt, i = c.i;
-    compute_sync();                        // the previous tile's estimate has been read out of the scratch
-    float *Us = reinterpret_cast<float *>(sm.scratch());        // [256][65] normals (scratch is 72 KB)
-    float *fvs = Us + TC_PTS * 65;                              // [256] values
+    float *Us = ubuf(tile);
+    float *fvs = sm.fvs();                                      // [256] values
+    if constexpr (!KEEP_U) compute_sync();                      // the previous tile's estimate has been read out of the scratch
     if (c.valid) {
       val += eval_noise(o.sigma_noise, a.seed, a.cycle, i, 5, a.iter, k);
       a.hlc_f[(size_t)i * M + k] = val;
-      float u[TC_D];
-      hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
+      if constexpr (!KEEP_U) {
+        float u[TC_D];
+        hlc_normals(a.seed, i, a.cycle, a.iter, k, d, u);
 #pragma unroll
-      for (int q = 0; q < TC_D; ++q) Us[t * 65 + q] = u[q];
+        for (int q = 0; q < TC_D; ++q) Us[t * US + q] = u[q];
+      }
     } else {
       val = 0.f;
     }
@@ -293,12 +313,13 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
       float b = 0.0f;
       if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
       float acc = 0.0f;
-      for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, Us[(ss * M + kk) * 65 + j], acc);
+      for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, Us[(ss * M + kk) * US + j], acc);
       const float gh = acc / ((float)M * sigma);
       a.ghat[(size_t)ii * d + j] = gh;
       const float xo = a.x[(size_t)ii * d + j];
       a.x[(size_t)ii * d + j] = clipf(fmaf(a.eta, gh, xo), a.lo[j], a.hi[j]);
     }
+    if constexpr (KEEP_U) compute_sync();                       // everybody has read fvs and this buffer: the next loads may overwrite them
     if (t == 0) atomicAdd(&a.evals[EV_HLC], (unsigned long long)nval * (unsigned long long)M);
   };
   tc_run<OBJ>(o, sm, t, ntiles, load, finish);
