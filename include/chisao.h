@@ -203,6 +203,14 @@ CHISAO_API int chisao_get_stats(chisao_ctx *ctx, chisao_stats *stats);
  * of the small objectives and for QUAD / RFF on the tensor cores, 0 for the x-stationary GMM_FULL evaluator (a tile
  * streams the whole mixture: retries must stay dense), for which 1 returns CHISAO_E_INVALID. */
 #define CHISAO_OPT_LS_TILE_LOCAL 3
+/* CHISAO_OPT_LBFGS_RESIDENT (default: on where it exists): Phase 1 in its history-RESIDENT form -- one launch runs all
+ * n_conv L-BFGS iterations (and, inside chisao_step, the release + first evaluation before them and Phase 2's partials after
+ * them) for the samples a CTA keeps for the whole pass, with the (s, y) history in registers and never in HBM
+ * (BASELINE.json north_star).  It exists for the FP32-FMA evaluators when d is 1, 2, 4, 8, 16 or 32, the
+ * objective's parameters fit one shared-memory chunk and lbfgs_m <= 16 (C1, C2), else 1 returns CHISAO_E_INVALID; 0
+ * selects the spill form (history in HBM, one group of launches per iteration), the only one at larger d or with the
+ * tensor-core evaluators.  Both are checked against the oracle by the same teacher-forced tests. */
+#define CHISAO_OPT_LBFGS_RESIDENT 4
 CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value);
 
 /* Which evaluator the context runs (decided at chisao_init from the objective, d and the value ranges):
@@ -215,6 +223,7 @@ CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value)
 #define CHISAO_INFO_EVALUATOR 1
 #define CHISAO_INFO_GRAPH_LAUNCHES 2   /* cycles submitted as a CUDA graph so far */
 #define CHISAO_INFO_LS_TILE_LOCAL 3    /* 1 if the line search runs every trial of a tile in one launch */
+#define CHISAO_INFO_LBFGS_RESIDENT 4   /* 1 if Phase 1 runs in its history-resident form */
 CHISAO_API int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value);
 
 /* Number of kernel launches this context has enqueued so far (host counter). */

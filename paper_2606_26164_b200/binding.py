@@ -23,9 +23,11 @@ PH_LBFGS_DIRECTION = 12
 OPT_STENCIL_AWARE = 1
 OPT_CUDA_GRAPH = 2
 OPT_LS_TILE_LOCAL = 3
+OPT_LBFGS_RESIDENT = 4
 INFO_EVALUATOR = 1
 INFO_GRAPH_LAUNCHES = 2
 INFO_LS_TILE_LOCAL = 3
+INFO_LBFGS_RESIDENT = 4
 EVALUATOR_NAMES = ("fp32-fma", "tcgen05 3xTF32 (x - c)", "tcgen05 x-stationary tf32 hi/lo", "tcgen05 x-stationary fp16 hi/lo",
                    "tcgen05 exact fixed-point fp16 pieces (random-Fourier phases)")
 TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_update", "select", "reseed")
@@ -238,6 +240,12 @@ class Chisao:
         """chisao_get_info(INFO_LS_TILE_LOCAL): the line search runs every trial of a tile in one launch"""
         v = C.c_int32(0)
         self._ck(self._L.chisao_get_info(self._h, INFO_LS_TILE_LOCAL, C.byref(v)))
+        return bool(v.value)
+
+    def lbfgs_resident(self) -> bool:
+        """chisao_get_info(INFO_LBFGS_RESIDENT): Phase 1 runs as one launch with the (s, y) history in registers"""
+        v = C.c_int32(0)
+        self._ck(self._L.chisao_get_info(self._h, INFO_LBFGS_RESIDENT, C.byref(v)))
         return bool(v.value)
 
     def graph_launches(self) -> int:

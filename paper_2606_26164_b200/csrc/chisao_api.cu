@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "chisao_eval_kernels.cuh"
+#include "chisao_resident.cuh"
 #include <cuda_fp16.h>
 #include "chisao_tc.cuh"
 
@@ -62,6 +63,9 @@ struct chisao_ctx {
   // (FP32-FMA evaluators of the small objectives, QUAD and RFF on the tensor cores); one launch per trial on compacted
   // worklists otherwise (GMM_FULL: a tile streams the whole mixture, the retries must stay dense)
   bool ls_tile_local = false;
+  // Phase 1 as ONE launch with the (s, y) history in registers (chisao_resident.cuh): FP32-FMA evaluators, d a power of
+  // two <= 32, parameters in one chunk, m <= 16
+  bool resident = false, resident_ok = false;
   bool in_cycle = false; // enqueue_cycle is running: the launch sequence may rely on what the previous unit left behind
 };
 
@@ -468,8 +472,27 @@ int run_release_eval(chisao_ctx *ctx) {   // Phase 1 start: release all (PAPER.m
 // one L-BFGS iteration (R-4).  As a unit of its own: direction, line search, FD gradient at the accepted
 // points, update.  Inside a cycle the update of iteration it - 1 rides in the direction kernel of iteration it (one pass
 // over x and g per iteration), and the update of the last iteration (run_lbfgs_finish) also writes Phase 2's partials.
+cudaError_t launch_resident(chisao_ctx *c, int it0, int it1, bool diag, bool stick) {
+  ResArgs a{};
+  a.s = c->st; a.h = c->hp; a.cycle = c->cycle; a.it0 = it0; a.it1 = it1; a.write_diag = diag ? 1 : 0; a.stick_partials = stick ? 1 : 0;
+  switch (c->obj.id) {
+    case 0: return launch_resident_obj_0(c->obj, a, c->stream);
+    case 1: return launch_resident_obj_1(c->obj, a, c->stream);
+    case 2: return launch_resident_obj_2(c->obj, a, c->stream);
+    case 3: return launch_resident_obj_3(c->obj, a, c->stream);
+    case 4: return launch_resident_obj_4(c->obj, a, c->stream);
+    default: return launch_resident_obj_5(c->obj, a, c->stream);
+  }
+}
 int run_lbfgs_iter(chisao_ctx *ctx, int it) {
   const State &s = ctx->st;
+  if (ctx->resident) {                       // (stand-alone unit; inside a cycle the whole pass is one launch: run_phase1_resident)
+    if (s.N == 0) return CHISAO_OK;
+    Scope sc(ctx, 0);
+    CK(launch_resident(ctx, it, it, true, false));
+    ctx->launches += 1;
+    return CHISAO_OK;
+  }
   const int mode = !ctx->in_cycle ? 0 : (it == 1 ? 1 : 2);
   if (!ctx->in_cycle) CK(cudaMemsetAsync(s.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
   { Scope sc(ctx, 3); CK(launch_lbfgs_step(s, ctx->hp, mode, ctx->stream)); ctx->launches += 1; }
@@ -478,6 +501,16 @@ int run_lbfgs_iter(chisao_ctx *ctx, int it) {
   // the FD kernel also zeroes worklist 0's counter for the next iteration's direction kernel
   CK(eval_fd(ctx, s.xt, s.fd_list, &s.ctrl->fd_cnt, FD_GRAD, s.gn, 1, it, EV_LBFGS_FD, 0, &s.ctrl->ls_cnt[0]));
   if (!ctx->in_cycle) { Scope sc(ctx, 4); CK(launch_lbfgs_update(s, ctx->hp, false, ctx->stream)); ctx->launches += 1; }
+  return CHISAO_OK;
+}
+// Phase 1 of a cycle in the history-resident form: release + f, g at the start positions, n_conv iterations and Phase 2's
+// partials in one launch
+int run_phase1_resident(chisao_ctx *ctx) {
+  if (ctx->st.N == 0) return CHISAO_OK;
+  CK(cudaMemsetAsync(&ctx->st.ctrl->fmax_enc, 0, sizeof(uint32_t), ctx->stream));
+  Scope sc(ctx, 0);
+  CK(launch_resident(ctx, 0, ctx->hp.n_conv, false, true));
+  ctx->launches += 1;
   return CHISAO_OK;
 }
 int run_lbfgs_finish(chisao_ctx *ctx) {   // in a cycle: update of the last iteration + ||g||_inf, f_max partials of Phase 2
@@ -489,7 +522,7 @@ int run_lbfgs_finish(chisao_ctx *ctx) {   // in a cycle: update of the last iter
 int run_stick(chisao_ctx *ctx) {
   Scope sc(ctx, 5);
   // after run_lbfgs_finish the per-sample gradient norms and f_max are already there
-  const bool have_partials = ctx->in_cycle && ctx->hp.n_conv > 0;
+  const bool have_partials = ctx->in_cycle && (ctx->hp.n_conv > 0 || ctx->resident);
   CK(launch_stick(ctx->st, ctx->hp, have_partials, ctx->stream));
   ctx->launches += have_partials ? 3 : 4;
   return CHISAO_OK;
@@ -650,6 +683,20 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
     }
     ctx->ls_tile_local = ctx->use_tc ? (obj->id != CHISAO_OBJ_GMM_FULL) : (cost <= 32768.0);
     if (getenv("CHISAO_LS_PER_TRIAL")) ctx->ls_tile_local = false;
+    const int dd_ = obj->d;
+    ctx->resident_ok = !ctx->use_tc && dd_ <= 32 && (dd_ & (dd_ - 1)) == 0 && o.kc >= o.K && cfg->lbfgs_m <= 16 &&
+                       eval_smem_bytes(o, resident_extra_bytes()) <= 200 * 1024;
+    ctx->resident = ctx->resident_ok && !getenv("CHISAO_LBFGS_SPILL");
+    if (ctx->resident_ok) {
+      switch (o.id) {
+        case 0: CKI(configure_resident_obj_0()); break;
+        case 1: CKI(configure_resident_obj_1()); break;
+        case 2: CKI(configure_resident_obj_2()); break;
+        case 3: CKI(configure_resident_obj_3()); break;
+        case 4: CKI(configure_resident_obj_4()); break;
+        default: CKI(configure_resident_obj_5()); break;
+      }
+    }
   }
   // zero everything except the parameter records, then upload parameters and bounds
   CKI(cudaMemsetAsync(workspace_dev, 0, need, ctx->stream));
@@ -686,10 +733,14 @@ static int enqueue_cycle(chisao_ctx *ctx) {
 }
 static int enqueue_cycle_units(chisao_ctx *ctx) {
   int rc;
-  if ((rc = run_release_eval(ctx))) return rc;        // Phase 1: release all, then converge
-  for (int it = 1; it <= ctx->hp.n_conv; ++it)
-    if ((rc = run_lbfgs_iter(ctx, it))) return rc;
-  if (ctx->hp.n_conv > 0 && (rc = run_lbfgs_finish(ctx))) return rc;
+  if (ctx->resident) {
+    if ((rc = run_phase1_resident(ctx))) return rc;   // Phase 1 in one launch, history in registers
+  } else {
+    if ((rc = run_release_eval(ctx))) return rc;      // Phase 1: release all, then converge
+    for (int it = 1; it <= ctx->hp.n_conv; ++it)
+      if ((rc = run_lbfgs_iter(ctx, it))) return rc;
+    if (ctx->hp.n_conv > 0 && (rc = run_lbfgs_finish(ctx))) return rc;
+  }
   if ((rc = run_stick(ctx))) return rc;               // Phase 2
   if ((rc = run_dedup(ctx))) return rc;               // Phase 3 (its list kernel also clears ctrl->strategy)
   if (ctx->cycle < ctx->hp.n_osc) {                   // "if k < n_osc"
@@ -950,6 +1001,13 @@ int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value) {
     return CHISAO_OK;
   }
   if (option == CHISAO_OPT_CUDA_GRAPH) { ctx->graph_on = value != 0; return CHISAO_OK; }
+  if (option == CHISAO_OPT_LBFGS_RESIDENT) {
+    if (value && !ctx->resident_ok)
+      return fail(ctx, CHISAO_E_INVALID, "the history-resident L-BFGS pass needs an FP32-FMA evaluator, d in {1,2,4,8,16,32}, parameters in one chunk, m <= 16");
+    ctx->resident = value != 0;
+    for (auto &ge : ctx->gexec) if (ge) { cudaGraphExecDestroy(ge); ge = nullptr; }   // another topology
+    return CHISAO_OK;
+  }
   if (option == CHISAO_OPT_LS_TILE_LOCAL) {
     if (value && ctx->use_tc && ctx->obj.id == CHISAO_OBJ_GMM_FULL)
       return fail(ctx, CHISAO_E_INVALID, "the tile-local line search does not exist for the x-stationary GMM_FULL evaluator");
@@ -963,6 +1021,7 @@ int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value) {
 int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value) {
   if (ctx && value && which == CHISAO_INFO_GRAPH_LAUNCHES) { *value = (int32_t)ctx->graph_launches; return CHISAO_OK; }
   if (ctx && value && which == CHISAO_INFO_LS_TILE_LOCAL) { *value = ctx->ls_tile_local ? 1 : 0; return CHISAO_OK; }
+  if (ctx && value && which == CHISAO_INFO_LBFGS_RESIDENT) { *value = ctx->resident ? 1 : 0; return CHISAO_OK; }
   if (!ctx || !value || which != CHISAO_INFO_EVALUATOR) return CHISAO_E_INVALID;
   *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_RFF ? 4 : (ctx->obj.id == CHISAO_OBJ_QUAD ? 1 : (ctx->tc.f16 ? 3 : 2)));
   return CHISAO_OK;

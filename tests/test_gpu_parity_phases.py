@@ -41,11 +41,15 @@ def test_a1_eval_and_fd_gradient(orc, B, c, N):
 
 
 @pytest.mark.parametrize("c,N", CASES)
-def test_a2_lbfgs_iterations_teacher_forced(orc, B, c, N):
-    """a2: direction, accepted trial, updated position, curvature pair, history bookkeeping, per iteration."""
+def test_a2_lbfgs_iterations_teacher_forced(orc, B, c, N, resident=None):
+    """a2: direction, accepted trial, updated position, curvature pair, history bookkeeping, per iteration.  C1 and C2 run
+    Phase 1 in its history-resident form (one launch, (s, y) in registers) by default; `resident` forces a form."""
     wl = inputs.config(c, N=N)
     hp = wl.hp
     o, g = _pair(orc, B, wl)
+    if resident is not None:
+        g.set_option(B.OPT_LBFGS_RESIDENT, int(resident))
+    assert g.lbfgs_resident() == ((c in (1, 2)) if resident is None else resident)
     o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
     o.phase(orc.PH_RELEASE_EVAL)
     n_dec = n_excl = 0
@@ -420,6 +424,9 @@ def test_line_search_forms_are_bit_identical(B, case):
           "rastrigin5": lambda: inputs.appendix_d("rastrigin", 5, 400, fd_h=1e-3, eps_grad=1e-3)}[case]()
     a, b = B.Chisao(wl), B.Chisao(wl)
     a.set_option(B.OPT_LS_TILE_LOCAL, 1); b.set_option(B.OPT_LS_TILE_LOCAL, 0)
+    for g in (a, b):
+        if g.lbfgs_resident():
+            g.set_option(B.OPT_LBFGS_RESIDENT, 0)          # the two line-search forms belong to the spill form of Phase 1
     assert a.ls_tile_local() and not b.ls_tile_local()
     for g in (a, b):
         g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
@@ -436,6 +443,9 @@ def test_line_search_forms_are_bit_identical(B, case):
     wl.hp.n_osc = 3
     a, b = B.Chisao(wl), B.Chisao(wl)
     a.set_option(B.OPT_LS_TILE_LOCAL, 1); b.set_option(B.OPT_LS_TILE_LOCAL, 0)
+    for g in (a, b):
+        if g.lbfgs_resident():
+            g.set_option(B.OPT_LBFGS_RESIDENT, 0)
     for k in range(3):
         sa, sb = a.step(), b.step()
         for fld in (B.X, B.F, B.G, B.STUCK):
@@ -482,3 +492,55 @@ def test_anti_step_in_place_update_on_multi_tile_persistent_ctas(orc, B, kind, d
         xt = PT.x_tol(xo, wl.hp.lo, wl.hp.hi) + vtol
         assert np.all(ex <= xt), (t, int(np.sum(ex > xt)), float(np.max(ex / xt)))
     assert g.stats().evals[6] == 3 * N * 2 * d
+
+
+@pytest.mark.parametrize("c,N", [(1, 256), (2, 777)])
+def test_a2_spill_form_at_small_d(orc, B, c, N):
+    """the spill form of Phase 1 (history in HBM, launches per iteration) on the configurations whose default is the
+    resident form: same teacher-forced check"""
+    test_a2_lbfgs_iterations_teacher_forced(orc, B, c, N, resident=False)
+
+
+def test_resident_form_selection(B):
+    for c, want in ((1, True), (2, True), (3, False), (4, False), (5, False)):
+        assert B.Chisao(inputs.config(c, N=64)).lbfgs_resident() == want
+    g = B.Chisao(inputs.config(4, N=64))
+    with pytest.raises(B.ChisaoError) as ei:
+        g.set_option(B.OPT_LBFGS_RESIDENT, 1)
+    assert ei.value.code == B.E_INVALID
+    # d = 3 is not a power of two: spill form; d = 16 with a small diagonal mixture: resident
+    assert not B.Chisao(inputs.custom(inputs.gmm_diag(3, 3, 2.0, 43), 3.0, 64)).lbfgs_resident()
+    assert B.Chisao(inputs.custom(inputs.gmm_diag(16, 3, 2.0, 43), 3.0, 64)).lbfgs_resident()
+
+
+@pytest.mark.parametrize("case", ["c1", "c2", "diag16", "iso1", "rastrigin4"])
+def test_resident_pass_whole_cycles_against_the_oracle(orc, B, case):
+    """chisao_step with Phase 1 as ONE launch (release + f, g + n_conv iterations + Phase 2's partials): per cycle the
+    evaluation counters of the start evaluation are exact, the stuck counts follow the oracle's (free-running fp32 / fp64
+    trajectories: small differences allowed where samples sit at the thresholds), and the two forms of Phase 1 agree
+    with each other to the same degree."""
+    wl = {"c1": lambda: inputs.config(1, n_osc=4), "c2": lambda: inputs.config(2, N=1500, n_osc=4, noise=0.0),
+          "diag16": lambda: inputs.custom(inputs.gmm_diag(16, 5, 3.0, 9), 4.0, 300, fd_h=1e-2, eps_grad=1e-3, n_conv=25, lbfgs_m=12, n_osc=3, hlc_baseline=1),
+          "iso1": lambda: inputs.custom(inputs.gmm_iso(1, 3, 0.4, 2.0, 5), 3.0, 200, fd_h=1e-3, eps_grad=1e-3, n_conv=15, lbfgs_m=3, n_osc=3, hlc_baseline=1),
+          "rastrigin4": lambda: inputs.appendix_d("rastrigin", 4, 400, fd_h=1e-3, eps_grad=1e-3, n_osc=3, hlc_baseline=1)}[case]()
+    hp = wl.hp
+    a, b, o = B.Chisao(wl), B.Chisao(wl), orc.Oracle(wl, threads=8)
+    b.set_option(B.OPT_LBFGS_RESIDENT, 0)
+    assert a.lbfgs_resident() and not b.lbfgs_resident()
+    prev = [0, 0]
+    for k in range(hp.n_osc):
+        sa, sb, so = a.step(), b.step(), o.step()
+        for q, st in enumerate((sa, sb)):
+            assert st.evals[0] - prev[q] == hp.N * (2 * hp.d + 1)           # release + f, g at the start positions
+            prev[q] = st.evals[0]
+            assert st.evals[2] % (2 * hp.d) == 0 and st.evals[1] >= st.evals[2] // (2 * hp.d)
+            assert abs(st.n_stuck - so.n_stuck) <= max(2, 0.03 * hp.N), (k, q, st.n_stuck, so.n_stuck)
+            assert abs(st.f_max - so.f_max) <= 1e-4 * max(abs(so.f_max), 1.0) + (0 if wl.obj.sigma_noise == 0 else 1.0)
+        xa = a.get(B.X)
+        assert np.isfinite(xa).all() and np.all(xa >= hp.lo[None, :]) and np.all(xa <= hp.hi[None, :])
+    assert a.launch_count() < 0.5 * b.launch_count()
+    xo, fo, _ = o.modes()
+    for g_ in (a, b):
+        xg, fg, _, n = g_.modes()
+        pair, only_g, only_o, text = PT.mode_set_report(xg, fg, xo, fo, 2e-3 if case != "rastrigin4" else 5e-3)
+        assert len(only_g) <= max(1, 0.1 * len(fo)) and len(only_o) <= max(1, 0.1 * len(fo)), text
