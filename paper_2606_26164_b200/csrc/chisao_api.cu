@@ -159,7 +159,8 @@ size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *b
   const size_t o_lo = F(d), o_hi = F(d);
   const size_t o_f = F(N), o_ft = F(N), o_dec = F(N), o_tcur = F(N), o_ginf = F(N);
   const size_t o_g = F(N * d), o_v = F(N * d), o_xt = F(N * d), o_gn = F(N * d), o_p = F(N * d), o_gh = F(N * d);
-  const size_t o_S = F(m * N * d), o_Y = F(m * N * d);
+  const size_t hp_ = history_plane_floats(N, d);
+  const size_t o_S = F(m * hp_), o_Y = F(m * hp_);
   const size_t o_hl = F(N), o_hh = F(N), o_lsb = F(N), o_rss = F(N), o_rsc = F(N);
   const size_t o_st = L.take(N), o_rm = L.take(N), o_sl = L.take(N);
   size_t o_lists[9];
@@ -176,7 +177,7 @@ size_t carve(const chisao_config &c, const chisao_objective &o, unsigned char *b
     st->lo = P(o_lo); st->hi = P(o_hi);
     st->f = P(o_f); st->ft = P(o_ft); st->dec = P(o_dec); st->tcur = P(o_tcur); st->ginf = P(o_ginf);
     st->g = P(o_g); st->v = P(o_v); st->xt = P(o_xt); st->gn = P(o_gn); st->p = P(o_p); st->ghat = P(o_gh);
-    st->S = P(o_S); st->Y = P(o_Y);
+    st->S = P(o_S); st->Y = P(o_Y); st->hplane = hp_;
     st->hist_len = I(o_hl); st->hist_head = I(o_hh); st->ls_b = I(o_lsb); st->rs_src = I(o_rss); st->rs_cand = I(o_rsc);
     st->stuck = base + o_st; st->removed = base + o_rm; st->stalled = base + o_sl;
     st->listA = I(o_lists[0]); st->listP = I(o_lists[1]); st->listR = I(o_lists[2]); st->listE = I(o_lists[3]);
@@ -495,7 +496,7 @@ int run_lbfgs_iter(chisao_ctx *ctx, int it) {
   }
   const int mode = !ctx->in_cycle ? 0 : (it == 1 ? 1 : 2);
   if (!ctx->in_cycle) CK(cudaMemsetAsync(s.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
-  { Scope sc(ctx, 3); CK(launch_lbfgs_step(s, ctx->hp, mode, ctx->stream)); ctx->launches += 1; }
+  { Scope sc(ctx, 3); CK(launch_lbfgs_step(s, ctx->hp, mode, ctx->in_cycle ? it : 0, ctx->stream)); ctx->launches += 1; }
   if (ctx->ls_tile_local) CK(eval_points(ctx, PT_LS_ALL, 0, it));
   else for (int b = 0; b <= ctx->hp.ls_max; ++b) CK(eval_points(ctx, PT_LS, b, it));
   // the FD kernel also zeroes worklist 0's counter for the next iteration's direction kernel
@@ -844,7 +845,7 @@ int chisao_phase(chisao_ctx *ctx, int32_t phase_id, int32_t iter) {
     case CHISAO_PH_LBFGS_DIRECTION: {
       CK(cudaMemsetAsync(ctx->st.ctrl->ls_cnt, 0, sizeof(int32_t) * 4, ctx->stream));
       Scope sc(ctx, 3);
-      CK(launch_lbfgs_step(ctx->st, ctx->hp, 0, ctx->stream));
+      CK(launch_lbfgs_step(ctx->st, ctx->hp, 0, 0, ctx->stream));
       ctx->launches += 1;
       return CHISAO_OK;
     }
@@ -938,7 +939,7 @@ int chisao_get_state(chisao_ctx *ctx, int32_t field, void *dst, size_t bytes) {
     std::vector<float> phys(m * N * d);
     std::vector<int32_t> head(N), len(N);
     if (N) {
-      CK(cudaMemcpyAsync(phys.data(), field == CHISAO_HIST_S ? s.S : s.Y, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+      CK(cudaMemcpy2DAsync(phys.data(), N * d * 4, field == CHISAO_HIST_S ? s.S : s.Y, s.hplane * 4, N * d * 4, m, cudaMemcpyDeviceToHost, ctx->stream));
       CK(cudaMemcpyAsync(head.data(), s.hist_head, N * 4, cudaMemcpyDeviceToHost, ctx->stream));
       CK(cudaMemcpyAsync(len.data(), s.hist_len, N * 4, cudaMemcpyDeviceToHost, ctx->stream));
     }
@@ -977,7 +978,7 @@ int chisao_set_state(chisao_ctx *ctx, int32_t field, const void *src, size_t byt
     // logical order in, physical = logical: ring heads are reset (set HIST_S, HIST_Y and HIST_LEN together)
     if (bytes != m * N * d * 4) return fail(ctx, CHISAO_E_INVALID, "wrong size for history field");
     if (bytes) {
-      CK(cudaMemcpyAsync(field == CHISAO_HIST_S ? s.S : s.Y, src, bytes, cudaMemcpyHostToDevice, ctx->stream));
+      CK(cudaMemcpy2DAsync(field == CHISAO_HIST_S ? s.S : s.Y, s.hplane * 4, src, N * d * 4, N * d * 4, m, cudaMemcpyHostToDevice, ctx->stream));
       CK(cudaMemsetAsync(s.hist_head, 0, N * 4, ctx->stream));
     }
     CK(cudaStreamSynchronize(ctx->stream));

@@ -54,6 +54,7 @@ struct DevObj {
 };
 
 inline int padded_dim(int d) { return d <= 8 ? 8 : (d <= 32 ? 32 : 64); }
+inline size_t history_plane_floats(size_t N, size_t d) { return N * d + 2112; }   // + 8448 bytes = 33 x 256: rows stay 256-byte aligned at d = 64
 inline int record_floats(int id, int DP) {
   switch (id) {
     case CHISAO_OBJ_GMM_ISO: return DP + 4;
@@ -69,7 +70,10 @@ inline int record_floats(int id, int DP) {
 struct State {
   int32_t N, d, m, M;
   float *x, *f, *g, *v, *xt, *ft, *gn, *p, *dec, *tcur, *ginf;
-  float *S, *Y;                       // [m][N][d] ring buffers (physical slots)
+  float *S, *Y;                       // [m] planes of [N][d] (physical ring slots), `hplane` floats apart
+  size_t hplane;                      // plane stride in floats: N d plus a pad that keeps the planes of one sample from
+                                      // sitting a power of two apart (at C5 N d 4 = 2^24 bytes: every one of a sample's 2 m
+                                      // history rows would map to the same DRAM channel / bank group)
   int32_t *hist_len, *hist_head, *ls_b;
   uint8_t *stuck, *removed, *stalled;
   int32_t *listA, *listP, *listR, *listE, *listP0, *ls_list[3], *fd_list;
@@ -103,7 +107,7 @@ cudaError_t eval_kernels_configure();   // opt-in dynamic shared memory for ever
 
 // mode: 0 direction only (stand-alone unit), 1 first iteration of a cycle (release folded in), 2 update of the previous
 // iteration + direction (chisao_lbfgs.cu)
-cudaError_t launch_lbfgs_step(const State &s, const Hyper &h, int mode, cudaStream_t st);
+cudaError_t launch_lbfgs_step(const State &s, const Hyper &h, int mode, int it, cudaStream_t st);
 cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, bool stick_partials, cudaStream_t st);
 cudaError_t launch_release(const State &s, cudaStream_t st);
 cudaError_t launch_stick(const State &s, const Hyper &h, bool have_partials, cudaStream_t st);   // ginf, f_max, flags, P0

@@ -117,7 +117,7 @@ __device__ __forceinline__ SampleState lbfgs_update_half(const State &s, int i, 
       int ph;
       if (o.len == m) { ph = o.head; o.head = (o.head + 1 == m) ? 0 : o.head + 1; }
       else { ph = o.head + o.len; if (ph >= m) ph -= m; o.len += 1; }
-      const size_t off = ((size_t)ph * N + i) * d;
+      const size_t off = ((size_t)ph * s.hplane + (size_t)i * d);
       st_row4h(s.S + off, hl, d, vec, sv);
       st_row4h(s.Y + off, hl, d, vec, yv);
       if (hl == 0) { s.hist_len[i] = o.len; s.hist_head[i] = o.head; }
@@ -147,8 +147,22 @@ __device__ __forceinline__ SampleState lbfgs_update_half(const State &s, int i, 
 //                    same kernel: one launch and one pass over x, g per iteration instead of two.
 enum { STEP_ALONE = 0, STEP_FIRST = 1, STEP_UPDATE = 2 };
 constexpr int DIR_WARPS = 4;   // measured at C5, full history: 4 warps x 4 CTAs per SM 4023 GB/s, 2 x 8 4025, 8 x 2 3884 (finer CTA turnover: less lockstep between load and recursion phases)
-template <int MM, bool VEC, int MODE>
-__global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_step(State s, Hyper h) {
+// SH: the 2 len history rows of a sample are staged in SHARED memory by cp.async (16 bytes per lane and row, no
+// register staging) instead of being held in registers: 61 registers instead of 128 and five CTAs per SM instead of
+// four.  Each lane reads back exactly the 16-byte chunks it copied, so no barrier is needed.  Needs d % 4 == 0 (VEC).
+// Measured (B200, round 2): with short histories and many stationary samples -- the iterations of a cycle before the
+// ring is full -- it is the faster form (C5 cycle: 0.62 against 0.78 ms for the 18 launches); with every sample active and
+// a full ring the register form streams better (0.59 against 0.55 of the HBM copy bandwidth: the staged rows cost a
+// shared-memory read in front of every shuffle-reduced dot, and the recursion's ~8 k cycles of dependent shuffles per
+// sample, not the bytes in flight, bound both).  launch_lbfgs_step therefore stages through shared memory while the
+// history cannot be full yet (iteration it <= m of a cycle) and keeps the rows in registers otherwise; a per-row
+// bulk-copy (TMA) staging was measured too: 0.53.
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+template <int MM, bool VEC, int MODE, bool SH>
+__global__ void __launch_bounds__(DIR_WARPS * 32, SH ? 5 : 4) k_lbfgs_step(State s, Hyper h) {
+  extern __shared__ float4 hist_smem[];
   __shared__ int sh_cnt, sh_base;
   __shared__ unsigned int sh_bytes;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, hl = lane & 15, half = lane >> 4;
@@ -189,18 +203,40 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_step(State s, Hyper
   int len = act ? len_i : 0;
   const int len_read = len;
   const int head = act ? head_i : 0;
-  Row4 Sr[MM], Yr[MM];
+  Row4 Sr[SH ? 1 : MM], Yr[SH ? 1 : MM];
+  float4 *hS = hist_smem + (size_t)((wib * 2 + half) * 2 * MM) * 16 + hl, *hY = hS + MM * 16;   // row l at [l * 16]
+  // rows up to the longer history of the warp's two samples take part in the (warp-uniform) loops; the shorter
+  // sample's missing rows are zero
+  const int lw = SH ? max(len, __shfl_xor_sync(0xffffffffu, len, 16)) : MM;
+  if constexpr (SH) {
+    static_assert(!SH || VEC, "the shared-memory form needs float4 rows");
+#pragma unroll
+    for (int l = 0; l < MM; ++l) {
+      if (l < len && 4 * hl < d) {
+        int ph = head + l; if (ph >= m) ph -= m;
+        const size_t off = ((size_t)ph * s.hplane + (size_t)i * d) + 4 * hl;
+        cp_async16(hS + l * 16, s.S + off);
+        cp_async16(hY + l * 16, s.Y + off);
+      } else if (l < lw) {
+        hS[l * 16] = make_float4(0.f, 0.f, 0.f, 0.f); hY[l * 16] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  } else {
 #pragma unroll
   for (int l = 0; l < MM; ++l) {
     if (l < len) {
       int ph = head + l; if (ph >= m) ph -= m;
-      const size_t off = ((size_t)ph * N + i) * d;
+      const size_t off = ((size_t)ph * s.hplane + (size_t)i * d);
       Sr[l] = ld_row4h(s.S + off, hl, d, vec);
       Yr[l] = ld_row4h(s.Y + off, hl, d, vec);
     } else {
       Sr[l].a = Sr[l].b = Sr[l].c = Sr[l].e = 0.f; Yr[l] = Sr[l];
     }
   }
+  }
+  auto rowS = [&](int l) -> Row4 { if constexpr (SH) { const float4 v = hS[l * 16]; Row4 r; r.a = v.x; r.b = v.y; r.c = v.z; r.e = v.w; return r; } else return Sr[l]; };
+  auto rowY = [&](int l) -> Row4 { if constexpr (SH) { const float4 v = hY[l * 16]; Row4 r; r.a = v.x; r.b = v.y; r.c = v.z; r.e = v.w; return r; } else return Yr[l]; };
   if (act && !have_x) x = ld_row4h(s.x + ro, hl, d, vec);
   // block-aggregated append of the searching samples to line-search worklist 0, and the byte counter: the one
   // returning global atomic per CTA is issued here, under the history loads, not at the end of the CTA's life
@@ -218,30 +254,49 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, 4) k_lbfgs_step(State s, Hyper
   p.a = p.b = p.c = p.e = 0.f; xt = p;
   bool restart = false;
   float t0 = 0.f, dec = 0.f;
+  if constexpr (SH) asm volatile("cp.async.wait_all;" ::: "memory");
   if (__any_sync(0xffffffffu, act)) {
   const float gn2 = dot4(g, g);
   // straight-line code over all MM slots: rows beyond len are zero and rho = 0 there, so they contribute nothing,
   // and no shuffle sits under a branch (the compiler would otherwise wrap each one in a convergence region)
   float rho[MM], al[MM];
 #pragma unroll
-  for (int l = 0; l < MM; ++l) { const float sy = dot4(Sr[l], Yr[l]); rho[l] = (l < len) ? 1.0f / sy : 0.0f; }
+  for (int l = 0; l < MM; ++l) {
+    rho[l] = 0.0f; al[l] = 0.0f;
+    if (l < lw) { const float sy = dot4(rowS(l), rowY(l)); rho[l] = (l < len) ? 1.0f / sy : 0.0f; }
+  }
   Row4 r = gam;
+  // (shared-memory form: the rows of step l - 1 are fetched before the shuffle chain of step l starts)
+  Row4 Sn = rowS(SH ? max(lw - 1, 0) : MM - 1), Ynx = rowY(SH ? max(lw - 1, 0) : MM - 1);
 #pragma unroll
-  for (int l = MM - 1; l >= 0; --l) { al[l] = rho[l] * dot4(Sr[l], r); axpy4(r, -al[l], Yr[l]); }
+  for (int l = MM - 1; l >= 0; --l) if (l < lw) {
+    const Row4 Sc = SH ? Sn : rowS(l), Yc = SH ? Ynx : rowY(l);
+    if (SH && l > 0) { Sn = rowS(l - 1); Ynx = rowY(l - 1); }
+    al[l] = rho[l] * dot4(Sc, r); axpy4(r, -al[l], Yc);
+  }
   // newest pair (logical len - 1): its y row is re-read (an L1/L2 hit) rather than selected out of the register
   // array, which would turn the array into local memory; s.y of that pair = 1 / rho
   Row4 Yn; Yn.a = Yn.b = Yn.c = Yn.e = 0.f;
   float rho_n = 1.0f;
   if (len > 0) {
-    int ph = head + len - 1; if (ph >= m) ph -= m;
-    Yn = ld_row4h(s.Y + ((size_t)ph * N + i) * d, hl, d, vec);
+    if constexpr (SH) Yn = rowY(len - 1);                // (shared memory can be indexed dynamically)
+    else {
+      int ph = head + len - 1; if (ph >= m) ph -= m;
+      Yn = ld_row4h(s.Y + ((size_t)ph * s.hplane + (size_t)i * d), hl, d, vec);
+    }
   }
 #pragma unroll
   for (int l = 0; l < MM; ++l) rho_n = (l == len - 1) ? rho[l] : rho_n;
   if (len > 0) { const float h0 = 1.0f / (rho_n * dot4(Yn, Yn)); r.a *= h0; r.b *= h0; r.c *= h0; r.e *= h0; }
   else { (void)dot4(Yn, Yn); }
 #pragma unroll
-  for (int l = 0; l < MM; ++l) { const float beta = rho[l] * dot4(Yr[l], r); axpy4(r, al[l] - beta, Sr[l]); }
+  Sn = rowS(0); Ynx = rowY(0);
+#pragma unroll
+  for (int l = 0; l < MM; ++l) if (l < lw) {
+    const Row4 Sc = SH ? Sn : rowS(l), Yc = SH ? Ynx : rowY(l);
+    if (SH && l + 1 < lw) { Sn = rowS(l + 1); Ynx = rowY(l + 1); }
+    const float beta = rho[l] * dot4(Yc, r); axpy4(r, al[l] - beta, Sc);
+  }
   p.a = -r.a; p.b = -r.b; p.c = -r.c; p.e = -r.e;
   const float gp = dot4(gam, p);
   restart = false;
@@ -315,24 +370,45 @@ cudaError_t launch_release(const State &s, cudaStream_t st) {
   k_release<<<(s.N + 255) / 256, 256, 0, st>>>(s);
   return cudaGetLastError();
 }
-cudaError_t launch_lbfgs_step(const State &s, const Hyper &h, int mode, cudaStream_t st) {
-  if (s.N == 0) return cudaSuccess;
-  const int per_block = DIR_WARPS * 2, grid = (s.N + per_block - 1) / per_block;
-  const bool vec = (s.d & 3) == 0;
-#define CHISAO_DIR2(MM, V)                                                                      \
-  do {                                                                                         \
-    if (mode == STEP_FIRST) k_lbfgs_step<MM, V, STEP_FIRST><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);        \
-    else if (mode == STEP_UPDATE) k_lbfgs_step<MM, V, STEP_UPDATE><<<grid, DIR_WARPS * 32, 0, st>>>(s, h); \
-    else k_lbfgs_step<MM, V, STEP_ALONE><<<grid, DIR_WARPS * 32, 0, st>>>(s, h);                           \
-  } while (0)
-#define CHISAO_DIR(MM) do { if (vec) CHISAO_DIR2(MM, true); else CHISAO_DIR2(MM, false); } while (0)
-  if (s.m <= 4) CHISAO_DIR(4);
-  else if (s.m <= 8) CHISAO_DIR(8);
-  else if (s.m <= 10) CHISAO_DIR(10);
-  else CHISAO_DIR(16);
-#undef CHISAO_DIR
-#undef CHISAO_DIR2
+static bool g_step_regs = false;   // CHISAO_STEP_REGS in the environment: keep the register form of the history (A/B measurements)
+template <int MM, bool VEC, int MODE, bool SH>
+static cudaError_t launch_step_one(const State &s, const Hyper &h, int grid, cudaStream_t st) {
+  const size_t sh = SH ? (size_t)DIR_WARPS * 2 * 2 * MM * 16 * sizeof(float4) : 0;
+  if (SH) {
+    static bool configured = false;
+    if (!configured) {
+      cudaError_t e = cudaFuncSetAttribute(k_lbfgs_step<MM, VEC, MODE, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
+      if (e != cudaSuccess) return e;
+      configured = true;
+    }
+  }
+  k_lbfgs_step<MM, VEC, MODE, SH><<<grid, DIR_WARPS * 32, sh, st>>>(s, h);
   return cudaGetLastError();
+}
+template <int MM, bool VEC, bool SH>
+static cudaError_t launch_step_mode(const State &s, const Hyper &h, int mode, int grid, cudaStream_t st) {
+  if (mode == STEP_FIRST) return launch_step_one<MM, VEC, STEP_FIRST, false>(s, h, grid, st);   // (empty history: nothing to stage)
+  if (mode == STEP_UPDATE) return launch_step_one<MM, VEC, STEP_UPDATE, SH>(s, h, grid, st);
+  return launch_step_one<MM, VEC, STEP_ALONE, SH>(s, h, grid, st);
+}
+template <int MM>
+static cudaError_t launch_step_mm(const State &s, const Hyper &h, int mode, bool staged, int grid, cudaStream_t st) {
+  const bool vec = (s.d & 3) == 0;
+  if (!vec) return launch_step_mode<MM, false, false>(s, h, mode, grid, st);
+  if (!staged) return launch_step_mode<MM, true, false>(s, h, mode, grid, st);
+  return launch_step_mode<MM, true, true>(s, h, mode, grid, st);
+}
+// `it`: iteration of the cycle (0 for the stand-alone unit): after it - 1 updates a history holds at most it - 1 pairs
+cudaError_t launch_lbfgs_step(const State &s, const Hyper &h, int mode, int it, cudaStream_t st) {
+  if (s.N == 0) return cudaSuccess;
+  static bool env_read = false;
+  if (!env_read) { g_step_regs = getenv("CHISAO_STEP_REGS") != nullptr; env_read = true; }
+  const int per_block = DIR_WARPS * 2, grid = (s.N + per_block - 1) / per_block;
+  const bool staged = !g_step_regs && mode == STEP_UPDATE && it - 1 < s.m;   // the ring cannot be full yet
+  if (s.m <= 4) return launch_step_mm<4>(s, h, mode, staged, grid, st);
+  if (s.m <= 8) return launch_step_mm<8>(s, h, mode, staged, grid, st);
+  if (s.m <= 10) return launch_step_mm<10>(s, h, mode, staged, grid, st);
+  return launch_step_mm<16>(s, h, mode, staged, grid, st);
 }
 cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, bool stick_partials, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;

@@ -121,8 +121,8 @@ __global__ void __launch_bounds__(NT, 2) k_lbfgs_resident(const DevObj o, const 
     for (int l = 0; l < MM; ++l)
       if (l < len) {
         int ph = head + l; if (ph >= m) ph -= m;
-        Sr[l] = s.S[((size_t)ph * N + i) * d + j];
-        Yr[l] = s.Y[((size_t)ph * N + i) * d + j];
+        Sr[l] = s.S[((size_t)ph * s.hplane + (size_t)i * d + j)];
+        Yr[l] = s.Y[((size_t)ph * s.hplane + (size_t)i * d + j)];
       }
   }
   if (!in) { g = 0.f; x = 0.f; }
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(NT, 2) k_lbfgs_resident(const DevObj o, const 
     s.x[e] = x; s.g[e] = g;
 #pragma unroll
     for (int l = 0; l < MM; ++l)
-      if (l < len) { s.S[((size_t)l * N + i) * d + j] = Sr[l]; s.Y[((size_t)l * N + i) * d + j] = Yr[l]; }
+      if (l < len) { s.S[((size_t)l * s.hplane + (size_t)i * d + j)] = Sr[l]; s.Y[((size_t)l * s.hplane + (size_t)i * d + j)] = Yr[l]; }
     if (j == 0) { s.f[i] = f; s.hist_len[i] = len; s.hist_head[i] = 0; s.stalled[i] = (uint8_t)stalled; }
   }
   if (a.stick_partials) {                                  // Phase 2's partials (what k_ginf_fmax computes)

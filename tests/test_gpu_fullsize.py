@@ -83,7 +83,7 @@ def test_full_size_c5_cycle_with_noise_invariants(B):
 
 def test_full_size_c5_stick_dedup_reseed_teacher_forced(orc, B):
     """a3, a4, a5 at BASELINE.json's full C5 size (N = 65536, d = 64), teacher-forced from a seeded synthetic
-    post-convergence state (inputs.synthetic_converged_state: ~31 000 samples in 300 tight clusters, exact f ties,
+    post-convergence state (inputs.synthetic_converged_state: ~34 000 samples in 300 tight clusters, exact f ties,
     gradient norms straddling eps_grad, non-finite entries): the ordered scan runs 64 blocks through the single-CTA
     offset kernel, k_dedup tiles ~30 000 stuck rows, k_reseed scores ~30 000 slots x 4 candidates against the modes.
     Flags, lists (through the counts and the removed mask), K_lost, reseed sources and candidates are compared
@@ -91,7 +91,7 @@ def test_full_size_c5_stick_dedup_reseed_teacher_forced(orc, B):
     wl = inputs.config(5)
     hp = wl.hp
     N = hp.N
-    x, f, gr = inputs.synthetic_converged_state(wl)
+    x, f, gr = inputs.synthetic_converged_state(wl, frac_clustered=0.65)     # > 50 % of the population stuck in 300 clusters
     o, g = orc.Oracle(wl, threads=16), B.Chisao(wl)
     ctrl = [3, 1, 0, 0, 0, 0, 0, 0]
     for fo_, fg_, val in ((orc.X, B.X, x), (orc.F, B.F, f), (orc.G, B.G, gr), (orc.CTRL, B.CTRL, ctrl)):
@@ -102,7 +102,7 @@ def test_full_size_c5_stick_dedup_reseed_teacher_forced(orc, B):
     assert sg.f_max == np.float32(so.f_max)
     assert np.array_equal(g.get(B.STUCK), o.get(orc.STUCK))
     assert (sg.n_stuck, sg.k_lost, sg.n_active) == (so.n_stuck, so.k_lost, so.n_active)
-    assert 20000 < sg.n_stuck < 40000 and not g.get(B.STUCK)[[5, 17, 33, 41]].any()
+    assert 0.5 * N < sg.n_stuck < 40000 and not g.get(B.STUCK)[[5, 17, 33, 41]].any()
     # a4: Eq. 4, every pair decided by fp32 differences of fp32 coordinates on both sides; pairs whose L-inf distance is
     # within rounding of eps_dup are excluded (protocol rule 3)
     o.phase(orc.PH_DEDUP); g.phase(B.PH_DEDUP)
