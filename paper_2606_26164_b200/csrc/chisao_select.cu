@@ -151,51 +151,76 @@ static cudaError_t run_scan(const State &s, const Hyper &h, int mode, cudaStream
 
 // ---- Phase 3 (Eq. 4; R-7): removed_i = stuck_i and exists j != i stuck within eps_dup in
 // L-infinity with f_j > f_i or (f_j = f_i and j < i); every test against the pre-removal stuck set. ------
+// Thread = one stuck sample i (its row in registers); a CTA of 128 samples walks ONE of DEDUP_SPLIT slices of the stuck list
+// in 64-row shared-memory tiles (rows as float4, read by all threads at once: broadcast).  Per pair: the f / index rule
+// first (it discards half of the pairs), then coordinate 0 (it discards almost every pair of different clusters), then
+// the remaining coordinates eight at a time with an early exit.  The slices of a sample's comparison run in different CTAs
+// (grid.y), so that a few hundred blocks of stuck samples still fill 148 SMs; a slice that finds a dominating
+// duplicate sets removed[i] (the mask is zero before the launch).  Worst case measured at C5 -- 52 % of N = 65536 stuck in
+// 300 clusters, 1.2e9 pairs -- in profiles/r2_worstcase_select_c5.md.
 constexpr int DEDUP_TILE = 64;
+constexpr int DEDUP_SPLIT = 8;
 __global__ void __launch_bounds__(128) k_dedup(State s, Hyper h) {
-  __shared__ float tx[DEDUP_TILE][CHISAO_MAX_D + 1];
+  __shared__ float4 tx[DEDUP_TILE][CHISAO_MAX_D / 4];
   __shared__ float tf[DEDUP_TILE];
   __shared__ int ti[DEDUP_TILE];
   const int n = s.ctrl->nP0, d = s.d;
   const int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (blockIdx.x * blockDim.x >= n) return;
+  const int per = (((n + DEDUP_SPLIT - 1) / DEDUP_SPLIT) + DEDUP_TILE - 1) / DEDUP_TILE * DEDUP_TILE;   // slice length, whole tiles
+  const int jbeg = blockIdx.y * per, jend = min(n, jbeg + per);
+  if (jbeg >= n) return;
   const bool act = q < n;
   const int i = act ? s.listP0[q] : -1;
   float xi[CHISAO_MAX_D];
 #pragma unroll
   for (int c = 0; c < CHISAO_MAX_D; ++c) xi[c] = (act && c < d) ? s.x[(size_t)i * d + c] : 0.0f;
   const float fi = act ? s.f[i] : 0.0f;
+  const float eps = h.eps_dup;
+  const int d4 = (d + 3) / 4;
   bool rem = false;
-  for (int j0 = 0; j0 < n; j0 += DEDUP_TILE) {
+  for (int j0 = jbeg; j0 < jend; j0 += DEDUP_TILE) {
     __syncthreads();
-    for (int e = threadIdx.x; e < DEDUP_TILE * d; e += blockDim.x) {
-      const int r = e / d, c = e - r * d;
-      tx[r][c] = (j0 + r < n) ? s.x[(size_t)s.listP0[j0 + r] * d + c] : 0.0f;
+    for (int e = threadIdx.x; e < DEDUP_TILE * d4; e += blockDim.x) {
+      const int r = e / d4, c4 = e - r * d4;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (j0 + r < jend) {
+        const float *row = s.x + (size_t)s.listP0[j0 + r] * d;
+        v.x = row[4 * c4];
+        if (4 * c4 + 1 < d) v.y = row[4 * c4 + 1];
+        if (4 * c4 + 2 < d) v.z = row[4 * c4 + 2];
+        if (4 * c4 + 3 < d) v.w = row[4 * c4 + 3];
+      }
+      tx[r][c4] = v;
     }
     if (threadIdx.x < DEDUP_TILE) {
       const int jj = j0 + threadIdx.x;
-      ti[threadIdx.x] = (jj < n) ? s.listP0[jj] : -1;
-      tf[threadIdx.x] = (jj < n) ? s.f[s.listP0[jj]] : 0.0f;
+      ti[threadIdx.x] = (jj < jend) ? s.listP0[jj] : -1;
+      tf[threadIdx.x] = (jj < jend) ? s.f[s.listP0[jj]] : 0.0f;
     }
     __syncthreads();
     if (act && !rem) {
-      const int lim = min(DEDUP_TILE, n - j0);
+      const int lim = min(DEDUP_TILE, jend - j0);
       for (int r = 0; r < lim && !rem; ++r) {
         const int j = ti[r];
-        if (j == i) continue;
         const float fj = tf[r];
-        if (!(fj > fi || (fj == fi && j < i))) continue;
+        if (j == i || !(fj > fi || (fj == fi && j < i))) continue;   // Eq. 4 (R-7): only a better (or equal and earlier) sample removes i
+        if (!(fabsf(xi[0] - tx[r][0].x) < eps)) continue;
         bool close = true;
 #pragma unroll
-        for (int c = 0; c < CHISAO_MAX_D; ++c) {
-          if (c < d) close = close && (fabsf(xi[c] - tx[r][c]) < h.eps_dup);
-          if ((c & 7) == 7 && !close) break;
+        for (int c4 = 0; c4 < CHISAO_MAX_D / 4; ++c4) {
+          if (4 * c4 < d) {
+            const float4 v = tx[r][c4];                      // (coordinates beyond d are zero on both sides)
+            close = close && (fabsf(xi[4 * c4] - v.x) < eps) && (fabsf(xi[4 * c4 + 1] - v.y) < eps) &&
+                    (fabsf(xi[4 * c4 + 2] - v.z) < eps) && (fabsf(xi[4 * c4 + 3] - v.w) < eps);
+          }
+          if ((c4 & 1) == 1 && !close) break;
         }
         rem = close;
       }
     }
   }
-  if (act) s.removed[i] = rem ? 1 : 0;
+  if (act && rem) s.removed[i] = 1;
 }
 
 // have_partials: ||grad f||_inf per sample and f_max were written by the last L-BFGS update of the pass
@@ -220,7 +245,7 @@ cudaError_t launch_dedup(const State &s, const Hyper &h, bool rebuild_p0, cudaSt
       e = cudaMemsetAsync(s.removed, 0, s.N, st);          // (inside a cycle the stick test has just cleared the mask)
       if (e != cudaSuccess) return e;
     }
-    if (h.phase_mask & (1u << 3)) k_dedup<<<(s.N + 127) / 128, 128, 0, st>>>(s, h);
+    if (h.phase_mask & (1u << 3)) k_dedup<<<dim3((s.N + 127) / 128, DEDUP_SPLIT), 128, 0, st>>>(s, h);
   }
   return run_scan(s, h, SCAN_FINAL, st);                   // its counting kernel clears the stuck flag of removed samples
 }
