@@ -122,3 +122,20 @@ def test_replica_reductions_over_gloo_world_size_2(tmp_path):
     res = subprocess.run(cmd, capture_output=True, text=True, env=env, timeout=240)
     assert res.returncode == 0, res.stderr[-2000:]
     assert res.stdout.count("ok") == 2
+
+
+def test_bench_gpus_2_self_launches_two_ranks_and_rank_0_prints_one_line():
+    """`python bench.py --gpus 2` with no launcher around it starts two ranks itself (bench.py: self_launch); the
+    reference arm needs no GPU, so the launch path is checked here: rank 0 prints the one JSON line with n_gpus = 2,
+    rank 1 exits 0 without output."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_PORT")}
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "1",
+           "--steps", "3", "--warmup", "1"]
+    res = subprocess.run(cmd, capture_output=True, text=True, env=env, timeout=300, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, res.stdout[-2000:]
+    rec = json.loads(lines[0])
+    assert rec["n_gpus"] == 2 and rec["impl"] == "reference" and rec["scaling"] == "weak"
+    assert rec["value"] > 0 and rec["e2e"]["h2d_bytes_per_step"] == 0
