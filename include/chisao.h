@@ -248,6 +248,30 @@ CHISAO_API int chisao_timing_get(chisao_ctx *ctx, int32_t which, double *ms, uin
 #define CHISAO_PEAK_SFU 1
 CHISAO_API int chisao_measure_peak(int32_t which, float *scratch_dev, void *stream, double *value);
 
+/* Phase 2 of a cycle -- the stick test, Eq. 3 (Alg. 1 "f_max <- max_i f(x_i)", R-13) -- on the CALLER'S
+ * arrays, for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): no context, no workspace, and the call makes NO cudaMalloc / cudaFree or other allocating call.
+ *   stuck_i = (max_j |g_ij| < eps_grad) and f_i finite and (f_i >= f_max + log_delta),  f_max = max over the finite f_i
+ * -- the same arithmetic, in the same precision, as CHISAO_PH_STICK of a context (a NaN in row i of g gives stuck_i = 0).
+ * Arguments, all DEVICE pointers owned by the caller, on the current device:
+ *   g_dev [N][d] fp32 row-major, f_dev [N] fp32 (read);  stuck_dev [N] u8 (written: 0 / 1);
+ *   n_stuck_dev (may be NULL) int32: the number of stuck samples;  f_max_dev (may be NULL) fp32: f_max, -inf if no f_i is
+ *   finite or N = 0.  0 <= N <= CHISAO_STATIC_MAX_N, 1 <= d <= CHISAO_MAX_D.
+ * Asynchronous on `stream` (a cudaStream_t; NULL = the default stream); returns CHISAO_E_INVALID for N beyond
+ * CHISAO_STATIC_MAX_N (or bad N, d, null pointers) and CHISAO_E_CUDA for runtime errors, with the text in
+ * chisao_last_error(NULL).
+ * Scratch: the per-sample ||grad f||_inf and the running f_max live in a file-scope device array of
+ * CHISAO_STATIC_SCRATCH_BYTES (1 MiB + 256 bytes), which every GPU that loads the library holds until the process exits;
+ * its device address is looked up on the first call on a device (cudaGetSymbolAddress -- make that first call outside a
+ * stream capture).  Every call on a device shares the array and finds the previous call's contents in it: the call clears what
+ * must start at zero on `stream` first.  Calls that OVERLAP on the GPU (different streams without a dependency between them)
+ * race on it; calls on one stream, or ordered by events, are safe. */
+#define CHISAO_STATIC_MAX_N 262144
+#define CHISAO_STATIC_SCRATCH_BYTES (256 + 4 * CHISAO_STATIC_MAX_N)
+CHISAO_API int chisao_stick_test_static(const float *g_dev, const float *f_dev, int32_t N, int32_t d, float eps_grad,
+                                        float log_delta, uint8_t *stuck_dev, int32_t *n_stuck_dev, float *f_max_dev,
+                                        void *stream);
+
 CHISAO_API const char *chisao_last_error(const chisao_ctx *ctx_or_null);
 CHISAO_API void chisao_destroy(chisao_ctx *ctx);
 

@@ -35,7 +35,9 @@ TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_upd
 EXPORTS = ("chisao_workspace_bytes", "chisao_init", "chisao_seed_population", "chisao_step", "chisao_step_host",
            "chisao_modes", "chisao_get_state", "chisao_set_state", "chisao_phase", "chisao_get_stats",
            "chisao_set_option", "chisao_get_info", "chisao_launch_count", "chisao_timing_enable", "chisao_timing_reset", "chisao_timing_get",
-           "chisao_measure_peak", "chisao_last_error", "chisao_destroy")
+           "chisao_measure_peak", "chisao_stick_test_static", "chisao_last_error", "chisao_destroy")
+STATIC_MAX_N = 262144                       # CHISAO_STATIC_MAX_N
+STATIC_SCRATCH_BYTES = 256 + 4 * STATIC_MAX_N
 
 _fp = C.POINTER(C.c_float)
 
@@ -102,6 +104,7 @@ def load_library(path: Optional[str] = None):
     L.chisao_timing_reset.argtypes = [vp]
     L.chisao_timing_get.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
     L.chisao_measure_peak.argtypes = [C.c_int32, vp, vp, C.POINTER(C.c_double)]
+    L.chisao_stick_test_static.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_float, C.c_float, vp, vp, vp, vp]
     L.chisao_last_error.argtypes = [vp]
     L.chisao_last_error.restype = C.c_char_p
     L.chisao_destroy.argtypes = [vp]
@@ -153,6 +156,31 @@ def measure_peak(which: int, device="cuda:0") -> float:
     if rc:
         raise ChisaoError(rc, "chisao_measure_peak failed")
     return float(v.value)
+
+
+def stick_test_static(g, f, eps_grad: float, log_delta: float, stuck, n_stuck=None, f_max=None, stream=None) -> None:
+    """chisao_stick_test_static: Eq. 3 on the caller's DEVICE tensors with no device allocation (the scratch is a static
+    array inside the library, STATIC_SCRATCH_BYTES per GPU; N <= STATIC_MAX_N).  g [N][d] fp32, f [N] fp32 are read;
+    stuck [N] uint8 and, if given, n_stuck [1] int32 and f_max [1] fp32 are written.  Asynchronous on `stream` (default:
+    torch's current stream of g's device).  Calls that overlap on the GPU race on the shared scratch."""
+    import torch
+    L = load_library()
+    N, d = (int(g.shape[0]), int(g.shape[1]))
+    for t, dt, n in ((g, torch.float32, N * d), (f, torch.float32, N), (stuck, torch.uint8, N)):
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() == n and t.device == g.device):
+            raise ValueError("stick_test_static: g [N][d] f32, f [N] f32, stuck [N] u8: contiguous CUDA tensors on one device")
+    for t, dt in ((n_stuck, torch.int32), (f_max, torch.float32)):
+        if t is not None and not (t.is_cuda and t.dtype == dt and t.numel() >= 1 and t.device == g.device):
+            raise ValueError("stick_test_static: n_stuck int32 [1] / f_max f32 [1] on g's device")
+    with torch.cuda.device(g.device):
+        st = stream if stream is not None else torch.cuda.current_stream(g.device)
+        rc = L.chisao_stick_test_static(C.c_void_p(g.data_ptr()), C.c_void_p(f.data_ptr()), N, d, float(eps_grad),
+                                        float(log_delta), C.c_void_p(stuck.data_ptr()),
+                                        C.c_void_p(n_stuck.data_ptr() if n_stuck is not None else None),
+                                        C.c_void_p(f_max.data_ptr() if f_max is not None else None),
+                                        C.c_void_p(st.cuda_stream))
+    if rc:
+        raise ChisaoError(rc, (L.chisao_last_error(None) or b"").decode())
 
 
 _FIELD_DTYPE = {STUCK: np.uint8, REMOVED: np.uint8, STALLED: np.uint8, HIST_LEN: np.int32, CTRL: np.int32,

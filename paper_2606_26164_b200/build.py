@@ -22,7 +22,7 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
 if os.environ.get("CHISAO_EXPERIMENTS"):      # ablation switches of the tensor-core kernels (profiles/; selected by CHISAO_EXP at run time)
     FLAGS.append("-DCHISAO_EXPERIMENTS")
 
-UNITS = [("chisao_api.cu", []), ("chisao_lbfgs.cu", []), ("chisao_select.cu", []), ("chisao_tc_kernels.cu", []), ("chisao_stencil.cu", []), ("chisao_probe.cu", [])] + \
+UNITS = [("chisao_api.cu", []), ("chisao_lbfgs.cu", []), ("chisao_select.cu", []), ("chisao_tc_kernels.cu", []), ("chisao_stencil.cu", []), ("chisao_probe.cu", []), ("chisao_static.cu", [])] + \
         [("chisao_eval_obj.cu", [f"-DCHISAO_OBJ_INST={i}"]) for i in range(6)]
 
 

@@ -34,6 +34,9 @@ struct TimedRec { int cls; cudaEvent_t a, b; };
 
 }  // namespace
 
+// for the entry points that live in other translation units (chisao_static.cu): the text chisao_last_error(NULL) returns
+namespace chisao { void set_global_error(const char *msg) { g_last_error = msg ? msg : ""; } }
+
 struct chisao_ctx {
   chisao_config cfg;
   Hyper hp;
