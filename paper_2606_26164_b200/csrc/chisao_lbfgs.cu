@@ -479,7 +479,7 @@ __device__ __forceinline__ SampleStateQ lbfgs_update_quad(const State &s, int i,
 __host__ __device__ inline size_t quad_smem_bytes(int m, int d) { return (size_t)2 * ((size_t)m * QS * d + 64) * 4 + 16; }
 
 template <int MM, int MODE, bool FULL>
-__global__ void __launch_bounds__(32) k_lbfgs_step_quad(State s, Hyper h) {
+__global__ void __launch_bounds__(32, 5) k_lbfgs_step_quad(State s, Hyper h) {
   extern __shared__ __align__(128) unsigned char quad_smem[];
   const int lane = threadIdx.x, sidx = lane >> 2, q = lane & 3;
   const int d = FULL ? 64 : s.d, m = s.m, N = s.N;

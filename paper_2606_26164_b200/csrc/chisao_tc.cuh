@@ -677,8 +677,10 @@ __device__ __forceinline__ void quad_issuer(const TcSmem &sm, int ntc) {
   for (int it = 0; it < ntc; ++it) quad_issue_tile(sm, tm, dBh, dBl, it);
 }
 
-template <class Load, class Finish>
-__device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish) {
+// patch(ctx, x): what the caller still has to do to the point load() requested (the FD kernel replaces one coordinate);
+// it runs where x is first consumed, a tile after load() -- arithmetic inside load() would wait for the row right there.
+template <class Load, class Finish, class Patch>
+__device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish, Patch patch) {
   const uint32_t tm = *sm.tmem();
   const int g = t >> 7, lane = t & 31;
   const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
@@ -687,7 +689,8 @@ __device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, in
   mbar_wait(sm.bbar(0), 0);                                      // c has landed
   const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(0) + 2 * TC_D * TC_D);
   float x[TC_D];
-  auto write_a = [&]() {                                         // A = x - c as tf32 hi / lo -> the thread's TMEM lane
+  auto write_a = [&](auto &ctx) {                                // A = x - c as tf32 hi / lo -> the thread's TMEM lane
+    patch(ctx, x);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       float h[16], l[16];
@@ -709,14 +712,14 @@ __device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, in
     if (lane == 0) mbar_arrive(sm.xbar(g));
   };
   auto c0 = load((int)blockIdx.x, x);                            // context of the tile being finished
-  write_a();
+  write_a(c0);
   auto c1 = c0;                                                  // context of the tile whose operand is written next
   if (ntc > 1) c1 = load((int)blockIdx.x + stride, x);
   for (int it = 0; it < ntc; ++it) {
     const int tile = (int)blockIdx.x + it * stride, st = it & 1;
     mbar_wait(sm.cbar(2 * g + st), (it >> 1) & 1);               // MMAs of tile `it` retired: the operand image is free
     asm volatile("tcgen05.fence::after_thread_sync;");
-    if (it + 1 < ntc) write_a();                                 // tile it + 1 (x was fetched one iteration ago)
+    if (it + 1 < ntc) write_a(c1);                               // tile it + 1 (x was fetched one iteration ago)
     uint32_t r[64];
     const uint32_t ta = lane_base + 128 + (uint32_t)(64 * st);
     tc_ld16s64(ta, r, 0); tc_ld16s64(ta + 16, r, 1); tc_ld16s64(ta + 32, r, 2); tc_ld16s64(ta + 48, r, 3);
@@ -830,8 +833,8 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
 
 // Run the evaluator over `ntiles` tiles of 256 points; called by every thread of the CTA after tc_begin.
 //   GMM_FULL: persistent x-stationary form, any grid <= ntiles;  QUAD: one tile per CTA (grid = ntiles).
-template <int OBJ, class Load, class Finish>
-__device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish) {
+template <int OBJ, class Load, class Finish, class Patch>
+__device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish, Patch patch) {
   if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) {
     const int ntc = tcx_tiles_of_cta(ntiles);
     const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
@@ -855,7 +858,8 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
     for (int it = 0; it < ntc; ++it) {
       const int tile = (int)blockIdx.x + it * (int)gridDim.x;
       float x[TC_D];
-      const auto c = load(tile, x);
+      auto c = load(tile, x);
+      patch(c, x);
       const float f = tc_rff_tile(o, sm, x, t, it);
       finish(tile, f, c);
     }
@@ -869,8 +873,12 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
       return;
     }
     if (warp > TC_PTS / 32) { quad_issuer(sm, tcx_tiles_of_cta(ntiles)); return; }
-    tc_quad_run(o, sm, t, ntiles, load, finish);
+    tc_quad_run(o, sm, t, ntiles, load, finish, patch);
   }
+}
+template <int OBJ, class Load, class Finish>
+__device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish) {
+  tc_run<OBJ>(o, sm, t, ntiles, load, finish, [](auto &, float (&)[TC_D]) {});
 }
 template <int OBJ>
 __device__ __forceinline__ void tc_begin(const TcSmem &sm, int t) { tc_setup(sm, t, OBJ == CHISAO_OBJ_GMM_FULL ? 1 : 2); }

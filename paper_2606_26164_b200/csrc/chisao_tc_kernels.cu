@@ -52,14 +52,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
       const float *row = a.X + (size_t)c.i * d;
       tc_load_row(row, d, (d & 3) == 0, x);
       c.xj = row[j];
-      c.xp = (slot & 1) ? c.xj - a.h : c.xj + a.h;
-      // replace coordinate j by compare-and-select over the whole row: every lane runs the same straight-line code (a
-      // dynamically indexed register array would be lowered to a branch tree over j, and the warp-collective tcgen05
-      // instructions of the evaluator need every lane on the same path), and nothing waits for the row here -- the
-      // global loads stay in flight until the evaluator first touches x
+      if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) c.xp = (slot & 1) ? c.xj - a.h : c.xj + a.h;
+      // QUAD / RFF: nothing here may touch the loaded values -- the row is requested a tile ahead and patched (below)
+      // where the evaluator first consumes it; arithmetic on it here would wait for the loads on the spot
       if constexpr (OBJ != CHISAO_OBJ_GMM_FULL) {
-#pragma unroll
-        for (int q = 0; q < TC_D; ++q) x[q] = (q == j) ? c.xp : x[q];
       } else {
         // GMM_FULL (the row is consumed within the same pair iteration anyway; 64 selects cost registers there): the
         // thread's own row goes through shared memory and comes back with coordinate j patched
@@ -98,7 +94,19 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
     }
     if (t == 0) atomicAdd(&a.evals[a.counter], (unsigned long long)min(spt, cnt - tile * spt) * 2ull * d);
   };
-  tc_run<OBJ>(o, sm, t, ntiles, load, finish);
+  // replace coordinate j by compare-and-select over the whole row: every lane runs the same straight-line code (a
+  // dynamically indexed register array would be lowered to a branch tree over j, and the warp-collective tcgen05
+  // instructions of the evaluator need every lane on the same path)
+  auto patch = [&](FdCtx &c, float (&x)[TC_D]) {
+    if constexpr (OBJ != CHISAO_OBJ_GMM_FULL) {
+      c.xp = (slot & 1) ? c.xj - a.h : c.xj + a.h;
+      if (c.valid) {
+#pragma unroll
+        for (int q = 0; q < TC_D; ++q) x[q] = (q == j) ? c.xp : x[q];
+      } else c.xp = 0.f;
+    }
+  };
+  tc_run<OBJ>(o, sm, t, ntiles, load, finish, patch);
   tc_teardown(sm, t);
 }
 
