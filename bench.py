@@ -235,7 +235,7 @@ def measure_config(c, K, W, rank, local_rank, world, dist, dev, N_override=0, de
         # kind::tf32 peak = measured bf16 cuBLAS throughput (sustained: the kernel is timed inside a long step) x the
         # guide's nominal tf32 : bf16 ratio 1.1 : 2.25.  The 3xTF32 split executes three tensor flops per
         # algorithmic flop of the contraction, so frac <= 1/3 by construction; executed_frac says how busy the pipe is.
-        f16 = ev_mode in (3, 4)                                # 3: fp16 hi / lo operands; 4: random-Fourier phases, six products of 10-bit fp16 pieces
+        f16 = ev_mode in (3, 4, 5)                                # 3, 5: fp16 hi / lo operands; 4: random-Fourier phases, six products of 10-bit fp16 pieces
         peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * (1.0 if f16 else 1.1 / 2.25)
         pipe_rate = 8192 if f16 else 4096                      # flop / clk / SM: one 128x128x16 f16 (x8 tf32) MMA per 64 clocks
         contraction = wl.obj.K * 2.0 * hp.d * (1 if ev_mode == 4 else hp.d)

@@ -219,7 +219,8 @@ CHISAO_API int chisao_set_option(chisao_ctx *ctx, int32_t option, int32_t value)
  * for GMM_FULL at d > 32 when max |W| and the box radius lie in [2^-3, 2^13]); 4 tensor cores,
  * random-Fourier phases w_j . x as an exact contraction of 10-bit fixed-point fp16 pieces (RFF at d <= 32, K <= 256
  * with max |w| and the box radius + 8 sigma_s + h in [2^-7, 2^10]; CHISAO_RFF_FP64 in the environment keeps the
- * FP32-FMA evaluator with fp64 phases). */
+ * FP32-FMA evaluator with fp64 phases); 5 tensor cores, QUAD at d > 32 with A = 2^k (x - c) per point and 2^ws W as fp16
+ * hi / lo operands (kind::f16; the default for QUAD, CHISAO_TC_TF32 in the environment keeps form 1). */
 #define CHISAO_INFO_EVALUATOR 1
 #define CHISAO_INFO_GRAPH_LAUNCHES 2   /* cycles submitted as a CUDA graph so far */
 #define CHISAO_INFO_LS_TILE_LOCAL 3    /* 1 if the line search runs every trial of a tile in one launch */

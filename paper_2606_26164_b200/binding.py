@@ -29,7 +29,7 @@ INFO_GRAPH_LAUNCHES = 2
 INFO_LS_TILE_LOCAL = 3
 INFO_LBFGS_RESIDENT = 4
 EVALUATOR_NAMES = ("fp32-fma", "tcgen05 3xTF32 (x - c)", "tcgen05 x-stationary tf32 hi/lo", "tcgen05 x-stationary fp16 hi/lo",
-                   "tcgen05 exact fixed-point fp16 pieces (random-Fourier phases)")
+                   "tcgen05 exact fixed-point fp16 pieces (random-Fourier phases)", "tcgen05 scaled fp16 hi/lo (x - c)")
 TIMING_CLASSES = ("eval_fd", "eval_points", "hlc", "lbfgs_direction", "lbfgs_update", "select", "reseed")
 
 EXPORTS = ("chisao_workspace_bytes", "chisao_init", "chisao_seed_population", "chisao_step", "chisao_step_host",

@@ -258,6 +258,32 @@ void pack_tc_records(const chisao_objective &o, std::vector<float> &out) {
   }
 }
 
+// QUAD record for kind::f16 (chisao_tc.cuh, tc_quad_run16): fp16 hi / lo images of 2^ws W -- element (n, c) at 16-bit index
+// (c/8)*512 + n*8 + (c%8), hi image at byte 0, lo image at byte 8192 -- then c where the tf32 record has it
+void pack_quad16_record(const chisao_objective &o, int ws, std::vector<float> &out) {
+  const int d = o.d;
+  out.assign((size_t)TC_REC, 0.0f);
+  uint16_t *img = reinterpret_cast<uint16_t *>(out.data());
+  for (int n = 0; n < d; ++n)
+    for (int c = 0; c < d; ++c) {
+      const float w = std::ldexp(o.mats[(size_t)n * d + c], ws);
+      const __half h = __float2half_rn(w), l = __float2half_rn(w - __half2float(h));
+      const size_t idx = (size_t)(c / 8) * 512 + (size_t)n * 8 + (c % 8);
+      img[idx] = __half_as_ushort(h); img[4096 + idx] = __half_as_ushort(l);
+    }
+  for (int j = 0; j < d; ++j) out[2 * TC_D * TC_D + j] = o.means[j];
+}
+// scale of the QUAD fp16 images: max |2^ws W| in [4096, 8192); false if W is zero or not finite, or the tf32 form is forced
+bool quad16_scale(const chisao_objective &o, int *ws) {
+  float wmax = 0.f;
+  for (size_t e = 0; e < (size_t)o.d * o.d; ++e) wmax = std::max(wmax, std::fabs(o.mats[e]));
+  if (!(wmax > 0.f) || !std::isfinite(wmax) || getenv("CHISAO_TC_TF32")) return false;
+  int e2 = 0;
+  std::frexp(wmax, &e2);                      // wmax = m 2^e2, m in [0.5, 1)
+  *ws = 13 - e2;                              // 2^ws wmax in [4096, 8192)
+  return *ws >= -40 && *ws <= 40;
+}
+
 // x-stationary pair records of GMM_FULL (chisao_tc.cuh): B image of the pair [W_2p ; W_2p+1] (128 rows, hi then lo),
 // c = W mu (fp64 product, rounded once), a; an odd K is padded with a zero component of weight a = -inf
 void pack_tcx_records(const chisao_objective &o, std::vector<float> &out) {
@@ -659,6 +685,8 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
   ctx->use_tc = wants_tc(*obj, *cfg);
   if (ctx->use_tc) {
     ctx->tc.f16 = (obj->id == CHISAO_OBJ_GMM_FULL && fp16_split_ok(*obj, *cfg)) ? 1 : 0;
+    ctx->tc.quad_ws = 0;
+    if (obj->id == CHISAO_OBJ_QUAD) { int ws = 0; if (quad16_scale(*obj, &ws)) { ctx->tc.f16 = 1; ctx->tc.quad_ws = ws; } }
     if (obj->id == CHISAO_OBJ_RFF) {
       int ex = 0, ew = 0;
       rff_tc_scales(*obj, *cfg, &ex, &ew);
@@ -667,7 +695,8 @@ int chisao_init(chisao_ctx **out, const chisao_config *cfg, const chisao_objecti
       ctx->tc.rff_s0 = obj->scalar0; ctx->tc.nchunk = (obj->K + 63) / 64;
       const double uA = std::ldexp(1.0, ex + ew - 18), P = 6.283185307179586476925 / uA, Phi = std::nearbyint(P);
       ctx->tc.rff_cA = (float)(uA / 6.283185307179586476925); ctx->tc.rff_Phi = (float)Phi; ctx->tc.rff_cL = (float)(-(P - Phi) * uA);
-    } else if (ctx->tc.f16) pack_tcx16_records(*obj, ctx->tc_host);
+    } else if (ctx->tc.f16 && obj->id == CHISAO_OBJ_QUAD) pack_quad16_record(*obj, ctx->tc.quad_ws, ctx->tc_host);
+    else if (ctx->tc.f16) pack_tcx16_records(*obj, ctx->tc_host);
     else if (obj->id == CHISAO_OBJ_GMM_FULL) pack_tcx_records(*obj, ctx->tc_host);
     else pack_tc_records(*obj, ctx->tc_host);
     ctx->tc.npair = (obj->K + 1) / 2;
@@ -1027,7 +1056,7 @@ int chisao_get_info(const chisao_ctx *ctx, int32_t which, int32_t *value) {
   if (ctx && value && which == CHISAO_INFO_LS_TILE_LOCAL) { *value = ctx->ls_tile_local ? 1 : 0; return CHISAO_OK; }
   if (ctx && value && which == CHISAO_INFO_LBFGS_RESIDENT) { *value = ctx->resident ? 1 : 0; return CHISAO_OK; }
   if (!ctx || !value || which != CHISAO_INFO_EVALUATOR) return CHISAO_E_INVALID;
-  *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_RFF ? 4 : (ctx->obj.id == CHISAO_OBJ_QUAD ? 1 : (ctx->tc.f16 ? 3 : 2)));
+  *value = !ctx->use_tc ? 0 : (ctx->obj.id == CHISAO_OBJ_RFF ? 4 : (ctx->obj.id == CHISAO_OBJ_QUAD ? (ctx->tc.f16 ? 5 : 1) : (ctx->tc.f16 ? 3 : 2)));
   return CHISAO_OK;
 }
 

@@ -69,7 +69,8 @@ struct TcObj {
   float sigma_noise;
   const float *recs;      // device [K][TC_REC] (QUAD) or [npair][TCX_REC] (GMM_FULL, x-stationary form)
   int32_t npair;          // ceil(K / 2)
-  int32_t f16;            // x-stationary form: operands split into fp16 hi / lo (kind::f16) instead of tf32 hi / lo
+  int32_t f16;            // operands split into fp16 hi / lo (kind::f16) instead of tf32 hi / lo (GMM_FULL x-stationary form, QUAD)
+  int32_t quad_ws;        // QUAD fp16 form: the W images hold 2^quad_ws W
   // RFF form (tc_rff_tile): fixed-point scales of the operand pieces and the -s0 ||x||^2 coefficient
   float rff_S0;           // 2^(9 - ex): x * S0 rounds to the first 10-bit piece (|x| < 2^ex)
   float rff_uA;           // 2^(ex + ew - 18): value of one unit of the exact accumulator (|w| < 2^ew)
@@ -740,6 +741,138 @@ __device__ __forceinline__ void tc_quad_run(const TcObj &o, const TcSmem &sm, in
   }
 }
 
+// ---- QUAD on kind::f16 (TcObj::f16): scaled fp16 hi / lo operands, operand image double-buffered --------------------------
+// f(x) = -1/2 |W (x - c)|^2 with f -> 0 at the optimum, so the operand must keep its RELATIVE precision however small
+// x - c is: the thread scales its point's difference by a power of two, v = 2^k (x - c) with max_c |v_c| in [8, 16), before
+// the fp16 hi / lo split (hi + lo carries 22 bits as long as lo stays above fp16's subnormal spacing: |v_c| >= 2^-13 max),
+// the W images hold 2^ws W (max |2^ws W| in [4096, 8192): entries down to 2^-15 max |W| keep 22 bits), and the sum of squares
+// is multiplied by 2^(-2 (k + ws)) -- all scalings exact.  The three products hi hi + lo hi + hi lo are 12 MMAs of
+// M128 N64 K16 per tile and group (kind::tf32: 24 of K8 at half the rate).  An operand image is 64 TMEM columns instead
+// of 128, so a group holds TWO of them (columns [0, 64) and [64, 128); accumulators [128, 192), [192, 256)): the image of
+// tile n + 2 is written as soon as the MMAs of tile n have retired, while those of tile n + 1 run -- in the tf32 form the
+// single image serialises "write A" and "multiply".  Barriers: image b of group g written -> xbar(g) (b = 0) / dbar(g)
+// (b = 1); accumulator stage read out -> rdbar; MMAs retired -> cbar, as in the tf32 form.
+__device__ __forceinline__ float quad_write_a16(uint32_t acol, float (&x)[TC_D], const float4 *mu4, int ws) {
+  float vmax = 0.f;
+#pragma unroll
+  for (int c4 = 0; c4 < TC_D / 4; ++c4) {
+    const float4 mu = mu4[c4];
+    x[4 * c4] -= mu.x; x[4 * c4 + 1] -= mu.y; x[4 * c4 + 2] -= mu.z; x[4 * c4 + 3] -= mu.w;
+    vmax = fmaxf(fmaxf(vmax, fmaxf(fabsf(x[4 * c4]), fabsf(x[4 * c4 + 1]))), fmaxf(fabsf(x[4 * c4 + 2]), fabsf(x[4 * c4 + 3])));
+  }
+  int k = 3 - ((int)((__float_as_uint(vmax) >> 23) & 0xffu) - 127);
+  k = min(max(k, -30), 40);
+  const float sc = __uint_as_float((uint32_t)(k + 127) << 23);
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    uint32_t h[16], l[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+      const float v0 = x[32 * q + 2 * c] * sc, v1 = x[32 * q + 2 * c + 1] * sc;
+      const __half2 hh = __floats2half2_rn(v0, v1);
+      const float2 hf = __half22float2(hh);
+      const __half2 ll = __floats2half2_rn(v0 - hf.x, v1 - hf.y);
+      h[c] = *reinterpret_cast<const uint32_t *>(&hh);
+      l[c] = *reinterpret_cast<const uint32_t *>(&ll);
+    }
+    tc_st16u(acol + 16 * q, h);
+    tc_st16u(acol + 32 + 16 * q, l);
+  }
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  return __uint_as_float((uint32_t)(127 - 2 * (k + ws)) << 23);
+}
+// MMAs of tile `it`: dbl = images alternate between the two buffers (persistent form), else always buffer 0 (rounds)
+__device__ __forceinline__ void quad_issue_tile16(const TcSmem &sm, uint32_t tm, uint64_t dBh, int it, bool dbl) {
+  const int st = it & 1, n = it >> 1;
+  const uint64_t dBl = dBh + (uint64_t)((TC_D * TC_D * 2) >> 4);
+#pragma unroll 1
+  for (int g = 0; g < 2; ++g) {
+    const int buf = dbl ? st : 0;
+    mbar_wait(buf ? sm.dbar(g) : sm.xbar(g), (dbl ? n : it) & 1);   // operand image of tile `it` written by the group's 4 warps
+    if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);       // accumulators of tile it - 2 are in registers
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (elect_one()) {
+      const uint32_t gcol = tm + (uint32_t)(g * 256), acc = gcol + 128 + (uint32_t)(64 * st), ah = gcol + (uint32_t)(64 * buf);
+#pragma unroll
+      for (int pr = 0; pr < 3; ++pr) {
+        const uint32_t a0 = (pr == 1) ? ah + 32 : ah;
+        const uint64_t b0 = (pr == 2) ? dBl : dBh;
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+          tc_mma_ts_f16(acc, a0 + (uint32_t)(ks * 8), b0 + (uint64_t)(ks * (2048 >> 4)), TC_IDESC_F16_N64, (pr | ks) ? 1u : 0u);
+      }
+      tc_commit(sm.cbar(2 * g + st));
+    }
+    __syncwarp();
+  }
+}
+__device__ __forceinline__ void quad_issuer16(const TcSmem &sm, int ntc) {
+  mbar_wait(sm.bbar(0), 0);
+  const uint32_t tm = *sm.tmem();
+  const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128);
+  for (int it = 0; it < ntc; ++it) quad_issue_tile16(sm, tm, dBh, it, true);
+}
+// DEEP: load(tile n + 3) is called before finish(tile n + 1) -- the FD and point kernels, whose load / finish keep nothing
+// per tile outside their contexts.  Otherwise the call order of the tf32 form is kept (load(n + 2) after finish(n);
+// k_hlc_tc keeps the normals of a tile in one of two buffers chosen by the tile's parity): the image of tile n + 1 is
+// written after the MMAs of tile n have retired, into the other buffer.
+template <bool DEEP, class Load, class Finish, class Patch>
+__device__ __forceinline__ void tc_quad_run16(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish, Patch patch) {
+  const uint32_t tm = *sm.tmem();
+  const int g = t >> 7, lane = t & 31;
+  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
+  const int ntc = tcx_tiles_of_cta(ntiles);
+  const int stride = (int)gridDim.x;
+  mbar_wait(sm.bbar(0), 0);                                      // c has landed
+  const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(0) + 2 * TC_D * TC_D);
+  float x[TC_D];
+  auto write_a = [&](auto &ctx, int buf) -> float {              // image of the point in x -> buffer buf; "written" to the issuer
+    patch(ctx, x);
+    const float u = quad_write_a16(lane_base + (uint32_t)(64 * buf), x, mu4, o.quad_ws);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(buf ? sm.dbar(g) : sm.xbar(g));
+    return u;
+  };
+  // contexts and unscale factors of the tile being finished (0), the next (1) and the one after (2)
+  auto c0 = load((int)blockIdx.x, x);
+  float u0 = write_a(c0, 0), u1 = 0.f, u2 = 0.f;
+  auto c1 = c0, c2 = c0;
+  if (ntc > 1) { c1 = load((int)blockIdx.x + stride, x); if (DEEP) u1 = write_a(c1, 1); }
+  if (DEEP && ntc > 2) c2 = load((int)blockIdx.x + 2 * stride, x);
+  for (int it = 0; it < ntc; ++it) {
+    const int tile = (int)blockIdx.x + it * stride, st = it & 1;
+    mbar_wait(sm.cbar(2 * g + st), (it >> 1) & 1);               // MMAs of tile `it` retired: image st and accumulator stage st are ours
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    if (!DEEP && it + 1 < ntc) u1 = write_a(c1, st ^ 1);         // tile it + 1 (its point was requested one iteration ago)
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+    {
+      uint32_t r[64];
+      const uint32_t ta = lane_base + 128 + (uint32_t)(64 * st);
+      tc_ld16s64(ta, r, 0); tc_ld16s64(ta + 16, r, 1); tc_ld16s64(ta + 32, r, 2); tc_ld16s64(ta + 48, r, 3);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      asm volatile("tcgen05.fence::before_thread_sync;");
+      __syncwarp();
+      if (lane == 0) mbar_arrive(sm.rdbar(2 * g + st));          // the stage may be overwritten (tile it + 2)
+#pragma unroll
+      for (int n = 0; n < 64; n += 4) {
+        const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
+                    z3 = __uint_as_float(r[n + 3]);
+        q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+      }
+    }
+    if (DEEP && it + 2 < ntc) u2 = write_a(c2, st);              // tile it + 2 (its point was requested two iterations ago)
+    finish(tile, -0.5f * u0 * ((q0 + q1) + (q2 + q3)), c0);
+    if (DEEP) {
+      c0 = c1; u0 = u1; c1 = c2; u1 = u2;
+      if (it + 3 < ntc) c2 = load(tile + 3 * stride, x);
+    } else {
+      c0 = c1; u0 = u1;
+      if (it + 2 < ntc) c1 = load(tile + 2 * stride, x);
+    }
+  }
+}
+
 // ---- tile-local rounds (QUAD and RFF forms): ONE tile per CTA, evaluated again and again until no thread asks for
 // another round (the line search: evaluate -> Armijo -> shrink; chisao_tc_kernels.cu, PT_LS_ALL).  The 256 compute
 // threads and the MMA-issuer warp vote at a named barrier after every round (bar.red.or); the loader warp has
@@ -775,7 +908,8 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
       for (int r = 0;; ++r) { rff_issue_tile(o, sm, tm, wa, xa, r); if (!round_vote(false)) break; }
     } else {
       const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
-      for (int r = 0;; ++r) { quad_issue_tile(sm, tm, dBh, dBl, r); if (!round_vote(false)) break; }
+      if (o.f16) { for (int r = 0;; ++r) { quad_issue_tile16(sm, tm, dBh, r, false); if (!round_vote(false)) break; } }
+      else { for (int r = 0;; ++r) { quad_issue_tile(sm, tm, dBh, dBl, r); if (!round_vote(false)) break; } }
     }
     return;
   }
@@ -790,6 +924,9 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
     } else {
       const float4 *mu4 = reinterpret_cast<const float4 *>(sm.B(0) + 2 * TC_D * TC_D);
       const int st = r & 1;
+      float unscale = 1.0f;
+      if (o.f16) unscale = quad_write_a16(lane_base, x, mu4, o.quad_ws);   // (warp-uniform branch)
+      else {
 #pragma unroll
       for (int q = 0; q < 4; ++q) {                        // A = x - c as tf32 hi / lo -> the thread's TMEM lane (as tc_quad_run)
         float h[16], l[16];
@@ -806,6 +943,7 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
       }
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       asm volatile("tcgen05.fence::before_thread_sync;");
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(sm.xbar(g));
       mbar_wait(sm.cbar(2 * g + st), (r >> 1) & 1);         // MMAs of round r retired
@@ -824,7 +962,7 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
                     z3 = __uint_as_float(rr[n + 3]);
         q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
       }
-      f = -0.5f * ((q0 + q1) + (q2 + q3));
+      f = -0.5f * unscale * ((q0 + q1) + (q2 + q3));
     }
     const bool again = finish(r, f);
     if (!round_vote(again)) break;
@@ -833,7 +971,7 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
 
 // Run the evaluator over `ntiles` tiles of 256 points; called by every thread of the CTA after tc_begin.
 //   GMM_FULL: persistent x-stationary form, any grid <= ntiles;  QUAD: one tile per CTA (grid = ntiles).
-template <int OBJ, class Load, class Finish, class Patch>
+template <int OBJ, bool DEEP = false, class Load, class Finish, class Patch>
 __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, int ntiles, Load load, Finish finish, Patch patch) {
   if constexpr (OBJ == CHISAO_OBJ_GMM_FULL) {
     const int ntc = tcx_tiles_of_cta(ntiles);
@@ -870,6 +1008,11 @@ __device__ __forceinline__ void tc_run(const TcObj &o, const TcSmem &sm, int t, 
         mbar_expect_tx(sm.bbar(0), TC_REC_BYTES);
         bulk_g2s(sm.B(0), o.recs, TC_REC_BYTES, sm.bbar(0));
       }
+      return;
+    }
+    if (o.f16) {                                               // (warp-uniform)
+      if (warp > TC_PTS / 32) { quad_issuer16(sm, tcx_tiles_of_cta(ntiles)); return; }
+      tc_quad_run16<DEEP>(o, sm, t, ntiles, load, finish, patch);
       return;
     }
     if (warp > TC_PTS / 32) { quad_issuer(sm, tcx_tiles_of_cta(ntiles)); return; }

@@ -23,6 +23,149 @@ __device__ __forceinline__ void tc_load_row(const float *row, int d, bool vec, f
 // in place from the finish of the group that owns it -- a row shared by both groups could be read half-updated.
 __host__ __device__ inline int fd_tc_samples_per_tile(int d) { return 2 * (TC_GROUP / (2 * d)); }
 struct FdCtx { int i; float xj, xp; bool valid; };
+
+// ---- FD stencil on the QUAD fp16 form: the operand image of a tile is built ONCE per warp ------------------------------------
+// At 32 < d <= 64 the 128 points of a group are the 2d stencil points of ONE sample: every thread's operand row is the
+// sample's 2^k (x - c) with one coordinate moved by +-h.  Instead of 128 threads each subtracting, scaling and splitting
+// the same 64 numbers (quad_write_a16: ~450 instructions per thread and tile, which bound the kernel), lane l of every warp
+// does coordinates l and l + 32, the warp's 64 hi and 64 lo halves meet in 256 bytes of shared memory, every lane reads
+// the packed row back (16 broadcast LDS.128), patches the word that holds its own coordinate and stores the row to its TMEM
+// lane.  The scale 2^k is taken from max_c |x_c - c_c| + h, a bound on every point of the stencil.  Same pipeline as
+// tc_quad_run16<DEEP>: rows are requested three tiles ahead, the image of tile n + 2 is built while the MMAs of tile
+// n + 1 run.
+struct Fd16Pre { float xa, xb; int i; bool valid; };
+template <class Finish>
+__device__ __forceinline__ void tc_quad_fd16(const TcObj &o, const TcSmem &sm, int t, int ntiles, const FdArgs &a, int cnt, Finish finish) {
+  const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+  if (warp == TC_PTS / 32) {
+    if (t == TC_PTS) {
+      mbar_expect_tx(sm.bbar(0), TC_REC_BYTES);
+      bulk_g2s(sm.B(0), o.recs, TC_REC_BYTES, sm.bbar(0));
+    }
+    return;
+  }
+  if (warp > TC_PTS / 32) { quad_issuer16(sm, tcx_tiles_of_cta(ntiles)); return; }
+  const uint32_t tm = *sm.tmem();
+  const int g = t >> 7, lane = t & 31, w4 = (t >> 5) & 3, tl = t & 127, d = a.d;
+  const int slot = tl, j = slot >> 1;
+  const bool lane_pt = tl < 2 * d;                          // the thread has a stencil point (d < 64: the last lanes idle)
+  const uint32_t lane_base = tm + ((uint32_t)(w4 * 32) << 16) + (uint32_t)(g * 256);
+  const int ntc = tcx_tiles_of_cta(ntiles), stride = (int)gridDim.x;
+  mbar_wait(sm.bbar(0), 0);                                 // W images and c have landed
+  const float *mu = sm.B(0) + 2 * TC_D * TC_D;              // (zero beyond d)
+  const float mua = mu[lane], mub = mu[lane + 32], muj = mu[j];
+  uint16_t *stage = reinterpret_cast<uint16_t *>(sm.scratch()) + (t >> 5) * 128;   // the warp's 64 hi + 64 lo halves
+  auto pre = [&](int tile) -> Fd16Pre {                     // the sample of this group in `tile`: two coordinates per lane
+    Fd16Pre p;
+    const int e = tile * 2 + g;
+    p.valid = e < cnt;
+    p.i = p.valid ? (a.list ? a.list[e] : e) : 0;
+    const float *row = a.X + (size_t)p.i * d;
+    p.xa = (p.valid && lane < d) ? row[lane] : 0.f;
+    p.xb = (p.valid && lane + 32 < d) ? row[lane + 32] : 0.f;
+    return p;
+  };
+  auto halves = [](float v, uint32_t &hi, uint32_t &lo) {
+    const __half hh = __float2half_rn(v);
+    hi = (uint32_t)__half_as_ushort(hh);
+    lo = (uint32_t)__half_as_ushort(__float2half_rn(v - __half2float(hh)));
+  };
+  auto build = [&](const Fd16Pre &p, int buf, FdCtx &c) -> float {
+    const float va = p.xa - mua, vb = p.xb - mub;
+    const float vmax = warp_max(fmaxf(fabsf(va), fabsf(vb))) + a.h;
+    int k = 3 - ((int)((__float_as_uint(vmax) >> 23) & 0xffu) - 127);
+    k = min(max(k, -30), 40);
+    const float sc = __uint_as_float((uint32_t)(k + 127) << 23);
+    uint32_t ha, la, hb, lb;
+    halves(va * sc, ha, la); halves(vb * sc, hb, lb);
+    __syncwarp();                                           // the previous image has been read back by every lane
+    stage[lane] = (uint16_t)ha; stage[lane + 32] = (uint16_t)hb; stage[64 + lane] = (uint16_t)la; stage[96 + lane] = (uint16_t)lb;
+    __syncwarp();
+    uint32_t h[32], l[32];
+    const uint4 *sv = reinterpret_cast<const uint4 *>(stage);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const uint4 u = sv[q], v = sv[8 + q];
+      h[4 * q] = u.x; h[4 * q + 1] = u.y; h[4 * q + 2] = u.z; h[4 * q + 3] = u.w;
+      l[4 * q] = v.x; l[4 * q + 1] = v.y; l[4 * q + 2] = v.z; l[4 * q + 3] = v.w;
+    }
+    // the thread's own coordinate j = 16 w4 + lane / 2 sits in lane j mod 32 (first or second coordinate of that lane)
+    const float xj = __shfl_sync(0xffffffffu, (w4 < 2) ? p.xa : p.xb, j & 31);
+    c.i = p.i; c.valid = p.valid && lane_pt;
+    c.xj = c.valid ? xj : 0.f;
+    c.xp = c.valid ? ((slot & 1) ? xj - a.h : xj + a.h) : 0.f;
+    uint32_t hj, lj;
+    halves((c.xp - muj) * sc, hj, lj);
+    // its halves go into word j / 2 = 8 w4 + lane / 4 of the hi and of the lo image, half j & 1 (static register indices:
+    // one warp-uniform branch per warp of the group, eight candidate words each)
+    if (c.valid) {
+      const int tw = lane >> 2;
+      const uint32_t keep = (j & 1) ? 0x0000FFFFu : 0xFFFF0000u, sh = (j & 1) ? 16u : 0u;
+#pragma unroll
+      for (int wq = 0; wq < 4; ++wq)
+        if (w4 == wq) {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const bool me = tw == q;
+            h[8 * wq + q] = me ? ((h[8 * wq + q] & keep) | (hj << sh)) : h[8 * wq + q];
+            l[8 * wq + q] = me ? ((l[8 * wq + q] & keep) | (lj << sh)) : l[8 * wq + q];
+          }
+        }
+    }
+    const uint32_t acol = lane_base + (uint32_t)(64 * buf);
+    {
+      uint32_t v16[16];
+#pragma unroll
+      for (int q = 0; q < 16; ++q) v16[q] = h[q];
+      tc_st16u(acol, v16);
+#pragma unroll
+      for (int q = 0; q < 16; ++q) v16[q] = h[16 + q];
+      tc_st16u(acol + 16, v16);
+#pragma unroll
+      for (int q = 0; q < 16; ++q) v16[q] = l[q];
+      tc_st16u(acol + 32, v16);
+#pragma unroll
+      for (int q = 0; q < 16; ++q) v16[q] = l[16 + q];
+      tc_st16u(acol + 48, v16);
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(buf ? sm.dbar(g) : sm.xbar(g));
+    return __uint_as_float((uint32_t)(127 - 2 * (k + o.quad_ws)) << 23);
+  };
+  FdCtx c0{}, c1{}, c2{};
+  Fd16Pre P = pre((int)blockIdx.x);
+  float u0 = build(P, 0, c0), u1 = 0.f, u2 = 0.f;
+  if (ntc > 1) { P = pre((int)blockIdx.x + stride); u1 = build(P, 1, c1); }
+  if (ntc > 2) P = pre((int)blockIdx.x + 2 * stride);
+  for (int it = 0; it < ntc; ++it) {
+    const int tile = (int)blockIdx.x + it * stride, st = it & 1;
+    mbar_wait(sm.cbar(2 * g + st), (it >> 1) & 1);          // MMAs of tile `it` retired: image st and accumulator stage st are ours
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+    {
+      uint32_t r[64];
+      const uint32_t ta = lane_base + 128 + (uint32_t)(64 * st);
+      tc_ld16s64(ta, r, 0); tc_ld16s64(ta + 16, r, 1); tc_ld16s64(ta + 32, r, 2); tc_ld16s64(ta + 48, r, 3);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      asm volatile("tcgen05.fence::before_thread_sync;");
+      __syncwarp();
+      if (lane == 0) mbar_arrive(sm.rdbar(2 * g + st));
+#pragma unroll
+      for (int n = 0; n < 64; n += 4) {
+        const float z0 = __uint_as_float(r[n]), z1 = __uint_as_float(r[n + 1]), z2 = __uint_as_float(r[n + 2]),
+                    z3 = __uint_as_float(r[n + 3]);
+        q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
+      }
+    }
+    if (it + 2 < ntc) u2 = build(P, st, c2);
+    finish(tile, -0.5f * u0 * ((q0 + q1) + (q2 + q3)), c0);
+    c0 = c1; u0 = u1; c1 = c2; u1 = u2;
+    if (it + 3 < ntc) P = pre(tile + 3 * stride);
+  }
+}
+
 template <int OBJ>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, const FdArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
@@ -106,7 +249,14 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
       } else c.xp = 0.f;
     }
   };
-  tc_run<OBJ>(o, sm, t, ntiles, load, finish, patch);
+  if constexpr (OBJ == CHISAO_OBJ_QUAD) {
+    if (o.f16 && spg == 1) {                               // (d > 32: a group's 128 points are one sample's stencil)
+      tc_quad_fd16(o, sm, t, ntiles, a, cnt, finish);
+      tc_teardown(sm, t);
+      return;
+    }
+  }
+  tc_run<OBJ, true>(o, sm, t, ntiles, load, finish, patch);
   tc_teardown(sm, t);
 }
 

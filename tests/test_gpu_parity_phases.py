@@ -379,7 +379,7 @@ def test_ablation_switches_phase_mask(orc, B):
 def test_tensor_evaluator_selection_and_tf32_fallback(orc, B, monkeypatch):
     """chisao_get_info: which evaluator chisao_init chose; the tf32 hi/lo form (forced by CHISAO_TC_TF32, or chosen
     when the box radius leaves fp16's range) passes the same a1 parity as the fp16 hi/lo form"""
-    for c, want in ((5, 3), (4, 1), (3, 4), (1, 0)):
+    for c, want in ((5, 3), (4, 5), (3, 4), (1, 0)):
         g = B.Chisao(inputs.config(c, N=64))
         assert g.evaluator() == want, (c, g.evaluator())
         g.close()
@@ -400,6 +400,11 @@ def test_tensor_evaluator_selection_and_tf32_fallback(orc, B, monkeypatch):
     assert g.evaluator() == 2
     g.close()
     test_a1_eval_and_fd_gradient(orc, B, 5, 200)
+    g = B.Chisao(inputs.config(4, N=64))
+    assert g.evaluator() == 1                                # QUAD: 3xTF32 with A = x - c
+    g.close()
+    test_a1_eval_and_fd_gradient(orc, B, 4, 200)
+    test_quad_values_near_the_optimum(orc, B, "tf32", monkeypatch)
     monkeypatch.delenv("CHISAO_TC_TF32")
     # a box of radius 9000 > 2^13: fp16 would overflow -> tf32 operands, same tolerances
     wl = inputs.custom(inputs.gmm_full(40, 3, 3.0, 77), 9000.0, 300, seed=5, fd_h=4.0)
@@ -410,6 +415,40 @@ def test_tensor_evaluator_selection_and_tf32_fallback(orc, B, monkeypatch):
     fo, fg = o.get(orc.F), g.get(B.F).astype(np.float64)
     assert np.all(np.abs(fg - fo) <= PT.f_tol(fo)), float(np.max(np.abs(fg - fo) / np.maximum(np.abs(fo), 1)))
     ok, err, tol = PT.grad_ok(g.get(B.G).astype(np.float64), o.get(orc.G), fo, wl.hp.fd_h)
+    assert np.all(ok), float(np.max(err / tol))
+
+
+@pytest.mark.parametrize("form", ["f16", "tf32"])
+def test_quad_values_near_the_optimum(orc, B, form, monkeypatch):
+    """QUAD (C4): f = -1/2 |W (x - c)|^2 -> 0 at the optimum, where the 1e-5 max(|f|, 1) bar is an ABSOLUTE 1e-5 on values
+    that span twelve orders of magnitude.  Samples sit at distances 1e-6 .. 6 from c (along random directions, along the
+    stiffest and along the softest direction of W).  Both operand forms (scaled fp16 hi / lo on kind::f16, the default;
+    tf32 hi / lo) must meet the bar; both keep the RELATIVE accuracy of the product, which is asserted as well, and the
+    FD gradient follows rule 2."""
+    if form == "tf32":
+        monkeypatch.setenv("CHISAO_TC_TF32", "1")
+    wl = inputs.config(4, N=768)
+    hp = wl.hp
+    rng = np.random.default_rng(31)
+    c = np.asarray(wl.obj.means, np.float64).reshape(-1)[:hp.d]
+    W = np.asarray(wl.obj.mats, np.float64).reshape(hp.d, hp.d)
+    _, _, vt = np.linalg.svd(W)
+    dirs = rng.standard_normal((hp.N, hp.d))
+    dirs[0::3] = vt[0] * np.sign(rng.standard_normal((len(dirs[0::3]), 1)))      # stiffest direction of W
+    dirs[1::3] = vt[-1] * np.sign(rng.standard_normal((len(dirs[1::3]), 1)))     # softest
+    dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    radius = 10.0 ** rng.uniform(-6.0, np.log10(6.0), hp.N)
+    wl.x0 = np.clip(c + dirs * radius[:, None], hp.lo, hp.hi).astype(np.float32)
+    o, g = _pair(orc, B, wl)
+    assert g.evaluator() == (5 if form == "f16" else 1)
+    o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0]); g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    o.phase(orc.PH_RELEASE_EVAL); g.phase(B.PH_RELEASE_EVAL)
+    fo, fg = o.get(orc.F), g.get(B.F).astype(np.float64)
+    assert fo.min() < -1e3 and fo.max() > -1e-9                 # the values do span the range
+    assert np.all(np.abs(fg - fo) <= PT.f_tol(fo)), float(np.max(np.abs(fg - fo) / np.maximum(np.abs(fo), 1)))
+    # relative: 22-bit operands in a 64-term product of condition <= kappa; far looser than what is measured (~1e-6)
+    assert np.all(np.abs(fg - fo) <= 2e-5 * np.abs(fo) + 1e-30), float(np.max(np.abs(fg - fo) / np.abs(fo)))
+    ok, err, tol = PT.grad_ok(g.get(B.G).astype(np.float64), o.get(orc.G), fo, hp.fd_h)
     assert np.all(ok), float(np.max(err / tol))
 
 
@@ -473,7 +512,7 @@ def test_anti_step_in_place_update_on_multi_tile_persistent_ctas(orc, B, kind, d
     obj = inputs.quad(d, 71 + d, lam_max=50.0) if kind == "quad" else inputs.rff(d, 64, 72 + d)
     wl = inputs.custom(obj, 4.0, N, seed=321 + d, fd_h=5e-2, eps_grad=1e-3, alpha_anti=2e-2 if kind == "rff" else 2e-3, mu=0.9)
     o, g = orc.Oracle(wl, threads=8), B.Chisao(wl)
-    assert g.evaluator() in (1, 4)
+    assert g.evaluator() in (5, 4)
     o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, N]); g.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, N])
     for t in (1, 2, 3):
         PT.sync_oracle_to_gpu(o, g, orc, B, with_history=False)
