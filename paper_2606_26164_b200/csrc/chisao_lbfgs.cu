@@ -622,15 +622,16 @@ __global__ void __launch_bounds__(32, 5) k_lbfgs_step_quad(State s, Hyper h) {
       axpyq(r, -al[l], ld_rowq_sh<FULL>(aY + roff[l], mp));
       axpyq(r, -al[l - 1], ld_rowq_sh<FULL>(aY + roff[l - 1], mp));
     }
-    float rho_n = 1.0f;
-    int roff_n = 4 * zoff;
-#pragma unroll
-    for (int l = 0; l < MM; ++l) if (l == len_read - 1) { rho_n = rho[l]; roff_n = roff[l]; }
     {
-      const RowQ Yn = ld_rowq_sh<FULL>(aY + roff_n, mp);
-      const float yy = dotq(Yn, Yn);
+      // H0 = (s.y / y.y) I of the newest pair: its row offset is arithmetic (a select over rho[] and roff[] by len would
+      // put both arrays in local memory), and s.y is taken again rather than looked up
+      int phn = head + len_read - 1; if (phn >= m) phn -= m;
+      const int roff_n = 4 * ((len_read > 0) ? phn * plane_floats + sidx * d : zoff);
+      const RowQ Yn = ld_rowq_sh<FULL>(aY + roff_n, mp), Sn = ld_rowq_sh<FULL>(aS + roff_n, mp);
+      float yy = pdotq(Yn, Yn), syn = pdotq(Sn, Yn);
+      quad_sum2(yy, syn);
       if (len_read > 0) {
-        const float h0 = 1.0f / (rho_n * yy);
+        const float h0 = syn / yy;
 #pragma unroll
         for (int k = 0; k < 4; ++k) { r.v[k].x *= h0; r.v[k].y *= h0; r.v[k].z *= h0; r.v[k].w *= h0; }
       }
