@@ -315,15 +315,27 @@ def measure_config(c, K, W, rank, local_rank, world, dist, dev, N_override=0, de
     g3.set(B.HIST_LEN, np.full(hp.N, hp.lbfgs_m, np.int32))
     for _ in range(3):
         g3.phase(B.PH_LBFGS_DIRECTION)
-    e0 = g3.stats().evals[7]
+    # (a) per launch: every launch bracketed by its own pair of events (the library's class timers)
     g3.timing_enable(True); g3.timing_reset()
     for _ in range(20):
         g3.phase(B.PH_LBFGS_DIRECTION)
-    full_ms, full_n = g3.timing()["lbfgs_direction"]
+    br_ms, br_n = g3.timing()["lbfgs_direction"]
+    g3.timing_enable(False)
+    # (b) the figure reported: one pair of events on the launching stream around 20 launches back to back (launch gaps
+    # included), i.e. the average launch duration over the timed region
+    e0 = g3.stats().evals[7]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(g3.stream)
+    for _ in range(20):
+        g3.phase(B.PH_LBFGS_DIRECTION)
+    ev1.record(g3.stream)
+    ev1.synchronize()
+    full_ms, full_n = float(ev0.elapsed_time(ev1)), 20
     full_bytes = float(g3.stats().evals[7] - e0)
-    hbm_full = {"bound": "hbm", "kernel": "k_lbfgs_step (direction only; all samples active, len = m)", "achieved": full_bytes / (full_ms * 1e-3) / 1e9,
+    hbm_full = {"bound": "hbm", "kernel": "k_lbfgs_step_quad at 32 < d <= 64, else k_lbfgs_step (direction only; all samples active, len = m)", "achieved": full_bytes / (full_ms * 1e-3) / 1e9,
                 "peak": peaks["hbm_gbs"], "unit": "GB/s", "bytes_per_launch": full_bytes / max(full_n, 1),
-                "ms_per_launch": full_ms / max(full_n, 1)}
+                "ms_per_launch": full_ms / max(full_n, 1), "ms_per_launch_bracketed_singly": br_ms / max(br_n, 1),
+                "timing": "one CUDA-event pair on the launching stream around 20 launches back to back"}
     hbm_full["frac"] = hbm_full["achieved"] / hbm_full["peak"]
     g3.close()
     out["hbm_kernel"], out["hbm_kernel_full_history"] = hbm, hbm_full
@@ -409,9 +421,9 @@ def run_ours(args, rank, local_rank, world):
 # dram__bytes_read.sum + dram__bytes_write.sum per k_eval_fd launch, read off the committed `ncu --set full` capture named
 # beside it (profiles/); not measured in this run -- a run under ncu is never a bench value
 TRAFFIC_BYTES_PER_LAUNCH = {
-    5: {"bytes": 1.84e7, "source": "profiles/r1_evalfd_c5_f16.md (full-size launch: 18.35 MB read, 0.07 MB written)"},
-    3: {"bytes": 2.26e6, "source": "profiles/r1_evalfd_c3_rfftc.md (2.26 MB read, 0 written: the gradient stays in L2)"},
-    4: {"bytes": 4.33e6, "source": "profiles/r1_evalfd_c4_quad.md (4.33 MB read, 0 written)"}}
+    5: {"bytes": 1.86e7, "source": "profiles/r2_evalfd_c5.md (full-size launch: 18.5 MB read, 0.08 MB written)"},
+    3: {"bytes": 2.26e6, "source": "profiles/r1_evalfd_c3_rfftc.md (2.26 MB read, 0 written: the gradient stays in L2; kernel unchanged since)"},
+    4: {"bytes": 4.36e6, "source": "profiles/r2_c2_c3_c4.md, r2_evalfd_c4.csv (4.36 MB read, 0 written)"}}
 
 
 def self_launch(args):
