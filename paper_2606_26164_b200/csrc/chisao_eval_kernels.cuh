@@ -103,6 +103,7 @@ struct PtArgs {
   const float *x, *p, *g, *lo, *hi;
   int32_t *ls_b, *next_list, *next_cnt, *fd_list, *fd_cnt, *zero_cnt;
   int32_t rows_in_smem;      // PT_LS_ALL: the launch carries 3 x [DP/4][PTILE] float4 of extra shared memory for the rows x, p, g
+  int32_t tc_pts;            // PT_LS_ALL on the tensor-core evaluators: worklist entries per CTA, 256 or 128 (set by launch_pt_tc)
   float c1, shrink;
   uint64_t seed;
   unsigned long long *evals;

@@ -516,14 +516,14 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
 // MMA issuer of the RFF form (warp 9, warp-uniform control flow, one elected lane issues): chunk c of group g goes to
 // accumulator stage c & 1 as soon as the group's point images are written (xbar) and that stage has been read out
 // (rdbar); tcgen05.commit signals cbar(2 g + stage).
-__device__ __forceinline__ void rff_issue_tile(const TcObj &o, const TcSmem &sm, uint32_t tm, uint32_t wa, uint32_t xa, int it) {
+__device__ __forceinline__ void rff_issue_tile(const TcObj &o, const TcSmem &sm, uint32_t tm, uint32_t wa, uint32_t xa, int it, int ng = 2) {
   const int nch = o.nchunk;
   for (int c = 0; c < nch; ++c) {
     const int st = c & 1;
     const int n = it * (st ? nch / 2 : (nch + 1) / 2) + (c >> 1);   // earlier issues into this stage
     const uint64_t dW = tc_desc(wa + (uint32_t)(c * 1024), 4096, 128);
 #pragma unroll 1
-    for (int g = 0; g < 2; ++g) {
+    for (int g = 0; g < ng; ++g) {
       if (c == 0) mbar_wait(sm.xbar(g), it & 1);
       if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);
       asm volatile("tcgen05.fence::after_thread_sync;");
@@ -649,10 +649,10 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
 // its operand image is written (xbar) and its stage has been read out (rdbar), i.e. while the compute warps still
 // square, sum and finish tile n.  The compute warps never meet at a barrier; the point of tile n + 2 is fetched from
 // global memory right after tile n is finished and consumed after the wait for the MMAs of tile n + 1.  TMEM per group (256 g): A_hi 64 | A_lo 64 | accumulators 2 x 64.
-__device__ __forceinline__ void quad_issue_tile(const TcSmem &sm, uint32_t tm, uint64_t dBh, uint64_t dBl, int it) {
+__device__ __forceinline__ void quad_issue_tile(const TcSmem &sm, uint32_t tm, uint64_t dBh, uint64_t dBl, int it, int ng = 2) {
   const int st = it & 1, n = it >> 1;                            // n earlier issues into this stage
 #pragma unroll 1
-  for (int g = 0; g < 2; ++g) {
+  for (int g = 0; g < ng; ++g) {
     mbar_wait(sm.xbar(g), it & 1);                               // operand image of tile `it` written by the group's 4 warps
     if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);     // accumulators of tile it - 2 are in registers
     asm volatile("tcgen05.fence::after_thread_sync;");
@@ -783,11 +783,11 @@ __device__ __forceinline__ float quad_write_a16(uint32_t acol, float (&x)[TC_D],
   return __uint_as_float((uint32_t)(127 - 2 * (k + ws)) << 23);
 }
 // MMAs of tile `it`: dbl = images alternate between the two buffers (persistent form), else always buffer 0 (rounds)
-__device__ __forceinline__ void quad_issue_tile16(const TcSmem &sm, uint32_t tm, uint64_t dBh, int it, bool dbl) {
+__device__ __forceinline__ void quad_issue_tile16(const TcSmem &sm, uint32_t tm, uint64_t dBh, int it, bool dbl, int ng = 2) {
   const int st = it & 1, n = it >> 1;
   const uint64_t dBl = dBh + (uint64_t)((TC_D * TC_D * 2) >> 4);
 #pragma unroll 1
-  for (int g = 0; g < 2; ++g) {
+  for (int g = 0; g < ng; ++g) {
     const int buf = dbl ? st : 0;
     mbar_wait(buf ? sm.dbar(g) : sm.xbar(g), (dbl ? n : it) & 1);   // operand image of tile `it` written by the group's 4 warps
     if (n > 0) mbar_wait(sm.rdbar(2 * g + st), (n - 1) & 1);       // accumulators of tile it - 2 are in registers
@@ -878,16 +878,18 @@ __device__ __forceinline__ void tc_quad_run16(const TcObj &o, const TcSmem &sm, 
 // threads and the MMA-issuer warp vote at a named barrier after every round (bar.red.or); the loader warp has
 // nothing to do after the record has landed.  Round r uses accumulator stage r & 1 and the barrier phases of tile
 // iteration r of the persistent forms above.
-__device__ __forceinline__ bool round_vote(bool again) {       // 256 compute threads + the issuer warp
+__device__ __forceinline__ bool round_vote(bool again, int ng) {   // 128 ng compute threads + the issuer warp
   uint32_t res;
   asm volatile(
-      "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 q, %1, 0;\n\tbar.red.or.pred p, 4, 288, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(res) : "r"((uint32_t)again) : "memory");
+      "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 q, %1, 0;\n\tbar.red.or.pred p, 4, %2, q;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(res) : "r"((uint32_t)again), "r"(128 * ng + 32) : "memory");
   return res != 0u;
 }
 // load(r, x): the thread's point of round r;  finish(r, f) -> true if the thread wants another round
+// ng = 1: only group 0 (threads 0 .. 127) holds points -- the launcher halves the tile when the worklist would otherwise
+// fill fewer CTAs than there are SMs; the second group's warps leave at once and the issuer skips it.
 template <int OBJ, class Load, class Finish>
-__device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int t, Load load, Finish finish) {
+__device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int t, int ng, Load load, Finish finish) {
   static_assert(OBJ == CHISAO_OBJ_QUAD || OBJ == CHISAO_OBJ_RFF, "tile-local rounds exist for the QUAD and RFF forms");
   const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
   const uint32_t rec_bytes = (OBJ == CHISAO_OBJ_RFF) ? (uint32_t)RFF_REC_BYTES : (uint32_t)TC_REC_BYTES;
@@ -905,15 +907,16 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
     if constexpr (OBJ == CHISAO_OBJ_RFF) {
       unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
       const uint32_t wa = smem_u32(wbase), xa = wa + RFF_REC_BYTES;
-      for (int r = 0;; ++r) { rff_issue_tile(o, sm, tm, wa, xa, r); if (!round_vote(false)) break; }
+      for (int r = 0;; ++r) { rff_issue_tile(o, sm, tm, wa, xa, r, ng); if (!round_vote(false, ng)) break; }
     } else {
       const uint64_t dBh = tc_desc(smem_u32(sm.B(0)), 1024, 128), dBl = dBh + (uint64_t)((TC_D * TC_D * 4) >> 4);
-      if (o.f16) { for (int r = 0;; ++r) { quad_issue_tile16(sm, tm, dBh, r, false); if (!round_vote(false)) break; } }
-      else { for (int r = 0;; ++r) { quad_issue_tile(sm, tm, dBh, dBl, r); if (!round_vote(false)) break; } }
+      if (o.f16) { for (int r = 0;; ++r) { quad_issue_tile16(sm, tm, dBh, r, false, ng); if (!round_vote(false, ng)) break; } }
+      else { for (int r = 0;; ++r) { quad_issue_tile(sm, tm, dBh, dBl, r, ng); if (!round_vote(false, ng)) break; } }
     }
     return;
   }
   const int g = t >> 7, lane = t & 31;
+  if (g >= ng) return;                                     // (warp-uniform)
   const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
   for (int r = 0;; ++r) {
     float x[TC_D];
@@ -965,7 +968,7 @@ __device__ __forceinline__ void tc_rounds(const TcObj &o, const TcSmem &sm, int 
       f = -0.5f * unscale * ((q0 + q1) + (q2 + q3));
     }
     const bool again = finish(r, f);
-    if (!round_vote(again)) break;
+    if (!round_vote(again, ng)) break;
   }
 }
 

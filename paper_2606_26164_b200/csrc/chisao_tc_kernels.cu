@@ -267,15 +267,16 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
   const TcSmem sm = tc_carve(tc_smem_raw);
   const int t = threadIdx.x, d = a.d;
   const int cnt = a.count ? *a.count : a.max_count;
-  const int ntiles = (cnt + TC_PTS - 1) / TC_PTS;
+  const int ppc = (OBJ != CHISAO_OBJ_GMM_FULL && a.mode == PT_LS_ALL) ? a.tc_pts : TC_PTS;   // worklist entries per CTA
+  const int ntiles = (cnt + ppc - 1) / ppc;
   if (blockIdx.x == 0 && t == 0 && a.zero_cnt) *a.zero_cnt = 0;
   if ((int)blockIdx.x >= ntiles) return;
   tc_begin<OBJ>(sm, t);
   if constexpr (OBJ != CHISAO_OBJ_GMM_FULL) {
     if (a.mode == PT_LS_ALL) {
-      // every trial b = 0 .. ls_max of the CTA's 256 worklist entries in one launch (tc_rounds): round r = trial b
-      const int e = (int)blockIdx.x * TC_PTS + t;
-      bool active = (t < TC_PTS) && (e < cnt);
+      // every trial b = 0 .. ls_max of the CTA's 256 (or 128) worklist entries in one launch (tc_rounds): round r = trial b
+      const int e = (int)blockIdx.x * ppc + t;
+      bool active = (t < ppc) && (e < cnt);
       const int i = active ? a.list[e] : 0;
       unsigned int nev = 0;
       auto load = [&](int, float (&x)[TC_D]) {
@@ -304,7 +305,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_points_tc(const TcObj o,
         active = retry;
         return retry;
       };
-      tc_rounds<OBJ>(o, sm, t, load, finish);
+      tc_rounds<OBJ>(o, sm, t, ppc / TC_GROUP, load, finish);
       if (t < TC_PTS) {
         nev = warp_sum_u(nev);
         if ((t & 31) == 0 && nev) atomicAdd(&a.evals[EV_LS], (unsigned long long)nev);
@@ -687,10 +688,14 @@ cudaError_t launch_fd_tc(int obj_id, const TcObj &o_in, const FdArgs &a, int n_s
   else k_eval_fd_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   return cudaGetLastError();
 }
-cudaError_t launch_pt_tc(int obj_id, const TcObj &o_in, const PtArgs &a, int n_samples, cudaStream_t st) {
+cudaError_t launch_pt_tc(int obj_id, const TcObj &o_in, const PtArgs &a_in, int n_samples, cudaStream_t st) {
   TcObj o = o_in; o.exp = g_exp;
-  const int ntiles = (n_samples + TC_PTS - 1) / TC_PTS;
-  const int grid = (a.mode == PT_LS_ALL) ? ntiles : tc_grid(obj_id, ntiles);   // tile-local rounds: one tile per CTA
+  PtArgs a = a_in;
+  // tile-local rounds: one tile per CTA; a worklist that would fill fewer CTAs than there are SMs is cut into tiles of
+  // one group (128 entries): every round of a tile costs a full tile evaluation, and half-size tiles on twice the SMs halve it
+  a.tc_pts = (a.mode == PT_LS_ALL && obj_id != CHISAO_OBJ_GMM_FULL && (n_samples + TC_PTS - 1) / TC_PTS < g_tc_sms) ? TC_GROUP : TC_PTS;
+  const int ntiles = (n_samples + a.tc_pts - 1) / a.tc_pts;
+  const int grid = (a.mode == PT_LS_ALL) ? ntiles : tc_grid(obj_id, (n_samples + TC_PTS - 1) / TC_PTS);
   if (obj_id == CHISAO_OBJ_QUAD) k_eval_points_tc<CHISAO_OBJ_QUAD><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else if (obj_id == CHISAO_OBJ_RFF) k_eval_points_tc<CHISAO_OBJ_RFF><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
   else k_eval_points_tc<CHISAO_OBJ_GMM_FULL><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(o, a);
