@@ -561,13 +561,11 @@ __device__ __forceinline__ void rff_issuer(const TcObj &o, const TcSmem &sm, int
 // feature pair (packed fp32):  k = rint(A cA + b / 2 pi);  r = A - k P_hi (exact integers);
 //                              angle = r uA + (k cL + (BC uB + b));  s += a cos(angle)
 // with P_hi = rint(2 pi / uA), cL = -(2 pi / uA - P_hi) uA, cA = uA / 2 pi.
-__device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t, int it) {
-  const uint32_t tm = *sm.tmem();
+// the thread's point -> its row of the four images; "written" to the issuer; returns |x|^2
+__device__ __forceinline__ float rff_write_x(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t) {
   const int g = t >> 7, tl = t & (TC_GROUP - 1), lane = t & 31;
-  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
   unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
   unsigned char *ximg = wbase + RFF_REC_BYTES + g * RFF_X_BYTES;
-  const float4 *prm = reinterpret_cast<const float4 *>(wbase + RFF_W_BYTES);   // per feature pair: (bt0, bt1, b0, b1) (a0, a1, 0, 0)
   const float S0 = o.rff_S0, U0 = 1.0f / S0;
   float nrm = 0.0f;
   // the thread's row of the four point images: n0 | n1 | 2^-10 n1 | 2^-10 n2
@@ -594,6 +592,15 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core's reads
   __syncwarp();
   if (lane == 0) mbar_arrive(sm.xbar(g));
+  return nrm;
+}
+// the chunk loop of tile iteration `it`: sum_j a_j cos(w_j . x + b_j) of the thread's point
+__device__ __forceinline__ float rff_chunks(const TcObj &o, const TcSmem &sm, int t, int it) {
+  const uint32_t tm = *sm.tmem();
+  const int g = t >> 7, lane = t & 31;
+  const uint32_t lane_base = tm + ((uint32_t)(((t >> 5) & 3) * 32) << 16) + (uint32_t)(g * 256);
+  unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
+  const float4 *prm = reinterpret_cast<const float4 *>(wbase + RFF_W_BYTES);   // per feature pair: (bt0, bt1, b0, b1) (a0, a1, 0, 0)
   const uint64_t cA2 = pk2(o.rff_cA, o.rff_cA), nP2 = pk2(-o.rff_Phi, -o.rff_Phi), cL2 = pk2(o.rff_cL, o.rff_cL);
   const uint64_t uA2 = pk2(o.rff_uA, o.rff_uA), uB2 = pk2(o.rff_uA * (1.0f / 1024.0f), o.rff_uA * (1.0f / 1024.0f));
   const uint64_t mg2 = pk2(12582912.0f, 12582912.0f), nmg2 = pk2(-12582912.0f, -12582912.0f);
@@ -639,7 +646,11 @@ __device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, c
   }
   float a0, a1, b0, b1;
   upk2(sA, a0, a1); upk2(sB, b0, b1);
-  return fmaf(-o.rff_s0, nrm, (a0 + a1) + (b0 + b1));
+  return (a0 + a1) + (b0 + b1);
+}
+__device__ __forceinline__ float tc_rff_tile(const TcObj &o, const TcSmem &sm, const float (&x)[TC_D], int t, int it) {
+  const float nrm = rff_write_x(o, sm, x, t);
+  return fmaf(-o.rff_s0, nrm, rff_chunks(o, sm, t, it));
 }
 
 // ---- QUAD (K = 1), persistent form ----------------------------------------------------------------------------------

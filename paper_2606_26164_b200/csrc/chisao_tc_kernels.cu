@@ -166,6 +166,100 @@ __device__ __forceinline__ void tc_quad_fd16(const TcObj &o, const TcSmem &sm, i
   }
 }
 
+// ---- FD stencil on the RFF form at d = 32: the point images of a sample's 64 stencil points are built ONCE per warp --------
+// A warp's 32 points belong to one sample (2d = 64 points per sample, two samples per group): lane l cuts coordinate l of
+// the sample into its fixed-point pieces (rff_split: ~17 instructions per coordinate, 32 coordinates per point in
+// rff_write_x -- a quarter of the kernel's instructions, which bound it), the warp's 4 x 32 halves meet in 256 bytes of
+// shared memory, every lane reads the packed row back (16 broadcast LDS.128), stores it as its row of the four images and
+// stores the pieces of its own coordinate (x_j +- h, cut by the lane itself) over it.  |x|^2 = (sum_c x_c^2 - x_j^2) + (x_j +- h)^2.
+// The next tile's coordinate is requested before the chunk loop of the current one.
+template <class Finish>
+__device__ __forceinline__ void tc_rff_fd32(const TcObj &o, const TcSmem &sm, int t, int ntiles, const FdArgs &a, int cnt, Finish finish) {
+  const int ntc = tcx_tiles_of_cta(ntiles);
+  const int warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // provably warp-uniform role index
+  if (warp == TC_PTS / 32) {
+    if (t == TC_PTS) {
+      mbar_expect_tx(sm.bbar(0), RFF_REC_BYTES);
+      bulk_g2s(sm.Bx(0, 0), o.recs, RFF_REC_BYTES, sm.bbar(0));
+    }
+    return;
+  }
+  if (warp > TC_PTS / 32) { rff_issuer(o, sm, ntc); return; }
+  mbar_wait(sm.bbar(0), 0);
+  const int g = t >> 7, tl = t & 127, lane = t & 31, w4 = (t >> 5) & 3;
+  const int slot = tl & 63, j = slot >> 1;                  // j = 16 (w4 & 1) + lane / 2
+  unsigned char *wbase = reinterpret_cast<unsigned char *>(sm.Bx(0, 0));
+  unsigned char *ximg = wbase + RFF_REC_BYTES + g * RFF_X_BYTES;
+  uint16_t *stage = reinterpret_cast<uint16_t *>(sm.scratch()) + (t >> 5) * 128;   // the warp's 4 x 32 halves
+  const float S0 = o.rff_S0, U0 = 1.0f / S0;
+  const int stride = (int)gridDim.x;
+  auto halves4 = [&](float v, uint32_t (&hv)[4]) {
+    float n0, n1, n2;
+    rff_split(v, S0, U0, n0, n1, n2);
+    hv[0] = (uint32_t)__half_as_ushort(__float2half_rn(n0));
+    hv[1] = (uint32_t)__half_as_ushort(__float2half_rn(n1));
+    hv[2] = (uint32_t)__half_as_ushort(__float2half_rn(n1 * (1.0f / 1024.0f)));
+    hv[3] = (uint32_t)__half_as_ushort(__float2half_rn(n2 * (1.0f / 1024.0f)));
+  };
+  struct Pre { float xc; int i; bool valid; };
+  auto pre = [&](int tile) -> Pre {                         // coordinate `lane` of the warp's sample in `tile`
+    Pre p;
+    const int e = tile * 4 + 2 * g + (w4 >> 1);
+    p.valid = e < cnt;
+    p.i = p.valid ? (a.list ? a.list[e] : e) : 0;
+    p.xc = p.valid ? a.X[(size_t)p.i * 32 + lane] : 0.f;
+    return p;
+  };
+  Pre P = pre((int)blockIdx.x);
+  for (int it = 0; it < ntc; ++it) {
+    const int tile = (int)blockIdx.x + it * stride;
+    const Pre cur = P;
+    uint32_t hv[4];
+    halves4(cur.xc, hv);
+    __syncwarp();                                           // the previous tile's staged row has been read by every lane
+    stage[lane] = (uint16_t)hv[0]; stage[32 + lane] = (uint16_t)hv[1]; stage[64 + lane] = (uint16_t)hv[2]; stage[96 + lane] = (uint16_t)hv[3];
+    __syncwarp();
+    uint32_t img[4][16];                                    // [image][4 chunks x 4 words]: halves of coordinates 8 kc + 2 w, + 1
+    const uint4 *sv = reinterpret_cast<const uint4 *>(stage);
+#pragma unroll
+    for (int pi = 0; pi < 4; ++pi)
+#pragma unroll
+      for (int kc = 0; kc < 4; ++kc) {
+        const uint4 u = sv[4 * pi + kc];
+        img[pi][4 * kc] = u.x; img[pi][4 * kc + 1] = u.y; img[pi][4 * kc + 2] = u.z; img[pi][4 * kc + 3] = u.w;
+      }
+    const float ssq = warp_sum(cur.xc * cur.xc);
+    const float xj = __shfl_sync(0xffffffffu, cur.xc, j);
+    FdCtx c;
+    c.i = cur.i; c.valid = cur.valid;
+    c.xj = c.valid ? xj : 0.f;
+    c.xp = c.valid ? ((slot & 1) ? xj - a.h : xj + a.h) : 0.f;
+    uint32_t pv[4];
+    halves4(c.xp, pv);
+#pragma unroll
+    for (int kc = 0; kc < 4; ++kc) {
+      unsigned char *dst = ximg + kc * 2048 + tl * 16;
+#pragma unroll
+      for (int pi = 0; pi < 4; ++pi)
+        *reinterpret_cast<uint4 *>(dst + 8192 * pi) = make_uint4(img[pi][4 * kc], img[pi][4 * kc + 1], img[pi][4 * kc + 2], img[pi][4 * kc + 3]);
+    }
+    // own coordinate j: its four halves are stored over the row just written (same thread: program order), chunk j / 8,
+    // position j % 8 -- no register of the row is indexed dynamically
+    {
+      unsigned char *own = ximg + (j >> 3) * 2048 + tl * 16 + (j & 7) * 2;
+#pragma unroll
+      for (int pi = 0; pi < 4; ++pi) *reinterpret_cast<uint16_t *>(own + 8192 * pi) = (uint16_t)pv[pi];
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(sm.xbar(g));
+    const float nrm = c.valid ? (ssq - xj * xj) + c.xp * c.xp : 0.f;
+    if (it + 1 < ntc) P = pre(tile + stride);               // in flight during the chunk loop
+    const float f = fmaf(-o.rff_s0, nrm, rff_chunks(o, sm, t, it));
+    finish(tile, f, c);
+  }
+}
+
 template <int OBJ>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, const FdArgs a) {
   extern __shared__ __align__(1024) unsigned char tc_smem_raw[];
@@ -252,6 +346,13 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_eval_fd_tc(const TcObj o, con
   if constexpr (OBJ == CHISAO_OBJ_QUAD) {
     if (o.f16 && spg == 1) {                               // (d > 32: a group's 128 points are one sample's stencil)
       tc_quad_fd16(o, sm, t, ntiles, a, cnt, finish);
+      tc_teardown(sm, t);
+      return;
+    }
+  }
+  if constexpr (OBJ == CHISAO_OBJ_RFF) {
+    if (d == 32) {                                         // (a warp's 32 points are stencil points of one sample)
+      tc_rff_fd32(o, sm, t, ntiles, a, cnt, finish);
       tc_teardown(sm, t);
       return;
     }
