@@ -521,7 +521,8 @@ def test_gmm_full_keeps_the_per_trial_line_search(B):
         assert B.Chisao(inputs.config(c, N=64)).ls_tile_local()
 
 
-@pytest.mark.parametrize("kind,d,N", [("quad", 50, 1000), ("rff", 24, 2000), ("quad", 33, 1400), ("rff", 5, 5000)])
+@pytest.mark.parametrize("kind,d,N", [("quad", 50, 1000), ("rff", 24, 2000), ("quad", 33, 1400), ("rff", 5, 5000), ("rff", 32, 3001),
+                                      ("quad", 64, 1001)])
 def test_anti_step_in_place_update_on_multi_tile_persistent_ctas(orc, B, kind, d, N):
     """Eq. 6 rewrites x and v in place from the FD kernel's epilogue.  On the tensor-core evaluators the two groups of
     128 points of a CTA run unsynchronised, so the 2d stencil points of a sample must never straddle them (a row could
