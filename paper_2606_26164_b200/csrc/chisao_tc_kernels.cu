@@ -55,11 +55,17 @@ __device__ __forceinline__ void tc_quad_fd16(const TcObj &o, const TcSmem &sm, i
   const float *mu = sm.B(0) + 2 * TC_D * TC_D;              // (zero beyond d)
   const float mua = mu[lane], mub = mu[lane + 32], muj = mu[j];
   uint16_t *stage = reinterpret_cast<uint16_t *>(sm.scratch()) + (t >> 5) * 128;   // the warp's 64 hi + 64 lo halves
-  auto pre = [&](int tile) -> Fd16Pre {                     // the sample of this group in `tile`: two coordinates per lane
-    Fd16Pre p;
+  // The worklist entry of a tile is requested one tile before its row (a dependent index -> row chain issued in one go
+  // stalls the warp at the address computation for a whole L2 round trip: in-order issue), the row two tiles before the
+  // operand build that consumes it.
+  auto pre_idx = [&](int tile) -> int {
     const int e = tile * 2 + g;
-    p.valid = e < cnt;
-    p.i = p.valid ? (a.list ? a.list[e] : e) : 0;
+    return (tile < ntiles && e < cnt) ? (a.list ? a.list[e] : e) : -1;
+  };
+  auto pre_row = [&](int idx) -> Fd16Pre {                  // the sample of this group: two coordinates per lane
+    Fd16Pre p;
+    p.valid = idx >= 0;
+    p.i = p.valid ? idx : 0;
     const float *row = a.X + (size_t)p.i * d;
     p.xa = (p.valid && lane < d) ? row[lane] : 0.f;
     p.xb = (p.valid && lane + 32 < d) ? row[lane + 32] : 0.f;
@@ -135,10 +141,12 @@ __device__ __forceinline__ void tc_quad_fd16(const TcObj &o, const TcSmem &sm, i
     return __uint_as_float((uint32_t)(127 - 2 * (k + o.quad_ws)) << 23);
   };
   FdCtx c0{}, c1{}, c2{};
-  Fd16Pre P = pre((int)blockIdx.x);
+  const int b0 = (int)blockIdx.x;
+  Fd16Pre P = pre_row(pre_idx(b0));
   float u0 = build(P, 0, c0), u1 = 0.f, u2 = 0.f;
-  if (ntc > 1) { P = pre((int)blockIdx.x + stride); u1 = build(P, 1, c1); }
-  if (ntc > 2) P = pre((int)blockIdx.x + 2 * stride);
+  if (ntc > 1) { P = pre_row(pre_idx(b0 + stride)); u1 = build(P, 1, c1); }
+  Fd16Pre Pa = pre_row(pre_idx(b0 + 2 * stride)), Pb = pre_row(pre_idx(b0 + 3 * stride));   // rows of tiles it + 2, it + 3
+  int idx_n = pre_idx(b0 + 4 * stride);                                                       // entry of tile it + 4
   for (int it = 0; it < ntc; ++it) {
     const int tile = (int)blockIdx.x + it * stride, st = it & 1;
     mbar_wait(sm.cbar(2 * g + st), (it >> 1) & 1);          // MMAs of tile `it` retired: image st and accumulator stage st are ours
@@ -159,10 +167,12 @@ __device__ __forceinline__ void tc_quad_fd16(const TcObj &o, const TcSmem &sm, i
         q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
       }
     }
-    if (it + 2 < ntc) u2 = build(P, st, c2);
+    if (it + 2 < ntc) u2 = build(Pa, st, c2);
     finish(tile, -0.5f * u0 * ((q0 + q1) + (q2 + q3)), c0);
     c0 = c1; u0 = u1; c1 = c2; u1 = u2;
-    if (it + 3 < ntc) P = pre(tile + 3 * stride);
+    Pa = Pb;
+    Pb = pre_row(idx_n);                                     // tile it + 4: consumed two iterations from now
+    idx_n = pre_idx(tile + 5 * stride);
   }
 }
 
@@ -202,15 +212,21 @@ __device__ __forceinline__ void tc_rff_fd32(const TcObj &o, const TcSmem &sm, in
     hv[3] = (uint32_t)__half_as_ushort(__float2half_rn(n2 * (1.0f / 1024.0f)));
   };
   struct Pre { float xc; int i; bool valid; };
-  auto pre = [&](int tile) -> Pre {                         // coordinate `lane` of the warp's sample in `tile`
-    Pre p;
+  // (the worklist entry is requested one tile before the row: a dependent index -> row chain issued in one go stalls
+  // the warp at the address computation, in-order issue)
+  auto pre_idx = [&](int tile) -> int {
     const int e = tile * 4 + 2 * g + (w4 >> 1);
-    p.valid = e < cnt;
-    p.i = p.valid ? (a.list ? a.list[e] : e) : 0;
+    return (tile < ntiles && e < cnt) ? (a.list ? a.list[e] : e) : -1;
+  };
+  auto pre_row = [&](int idx) -> Pre {                      // coordinate `lane` of the warp's sample
+    Pre p;
+    p.valid = idx >= 0;
+    p.i = p.valid ? idx : 0;
     p.xc = p.valid ? a.X[(size_t)p.i * 32 + lane] : 0.f;
     return p;
   };
-  Pre P = pre((int)blockIdx.x);
+  Pre P = pre_row(pre_idx((int)blockIdx.x));
+  int idx_n = pre_idx((int)blockIdx.x + stride);
   for (int it = 0; it < ntc; ++it) {
     const int tile = (int)blockIdx.x + it * stride;
     const Pre cur = P;
@@ -254,7 +270,8 @@ __device__ __forceinline__ void tc_rff_fd32(const TcObj &o, const TcSmem &sm, in
     __syncwarp();
     if (lane == 0) mbar_arrive(sm.xbar(g));
     const float nrm = c.valid ? (ssq - xj * xj) + c.xp * c.xp : 0.f;
-    if (it + 1 < ntc) P = pre(tile + stride);               // in flight during the chunk loop
+    P = pre_row(idx_n);                                     // tile it + 1: in flight during the chunk loop
+    idx_n = pre_idx(tile + 2 * stride);
     const float f = fmaf(-o.rff_s0, nrm, rff_chunks(o, sm, t, it));
     finish(tile, f, c);
   }
