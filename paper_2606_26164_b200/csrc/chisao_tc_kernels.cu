@@ -147,7 +147,10 @@ __device__ __forceinline__ void tc_quad_fd16(const TcObj &o, const TcSmem &sm, i
   if (ntc > 1) { P = pre_row(pre_idx(b0 + stride)); u1 = build(P, 1, c1); }
   Fd16Pre Pa = pre_row(pre_idx(b0 + 2 * stride)), Pb = pre_row(pre_idx(b0 + 3 * stride));   // rows of tiles it + 2, it + 3
   int idx_n = pre_idx(b0 + 4 * stride);                                                       // entry of tile it + 4
-  for (int it = 0; it < ntc; ++it) {
+  // one tile; Px holds the row of tile it + 2 on entry and the (requested) row of tile it + 4 on exit.  The loop below
+  // alternates between two such registers sets instead of rotating them: a register move of a value whose load is
+  // still in flight waits for the load (21 % of the kernel's stall samples sat on that move).
+  auto step = [&](int it, Fd16Pre &Px) {
     const int tile = (int)blockIdx.x + it * stride, st = it & 1;
     mbar_wait(sm.cbar(2 * g + st), (it >> 1) & 1);          // MMAs of tile `it` retired: image st and accumulator stage st are ours
     asm volatile("tcgen05.fence::after_thread_sync;");
@@ -167,22 +170,18 @@ __device__ __forceinline__ void tc_quad_fd16(const TcObj &o, const TcSmem &sm, i
         q0 = fmaf(z0, z0, q0); q1 = fmaf(z1, z1, q1); q2 = fmaf(z2, z2, q2); q3 = fmaf(z3, z3, q3);
       }
     }
-    if (it + 2 < ntc) u2 = build(Pa, st, c2);
+    if (it + 2 < ntc) u2 = build(Px, st, c2);
     finish(tile, -0.5f * u0 * ((q0 + q1) + (q2 + q3)), c0);
     c0 = c1; u0 = u1; c1 = c2; u1 = u2;
-    Pa = Pb;
-    Pb = pre_row(idx_n);                                     // tile it + 4: consumed two iterations from now
+    Px = pre_row(idx_n);                                     // tile it + 4: consumed two iterations from now, from this same set
     idx_n = pre_idx(tile + 5 * stride);
+  };
+  for (int it = 0; it < ntc; it += 2) {
+    step(it, Pa);
+    if (it + 1 < ntc) step(it + 1, Pb);
   }
 }
 
-// ---- FD stencil on the RFF form at d = 32: the point images of a sample's 64 stencil points are built ONCE per warp --------
-// A warp's 32 points belong to one sample (2d = 64 points per sample, two samples per group): lane l cuts coordinate l of
-// the sample into its fixed-point pieces (rff_split: ~17 instructions per coordinate, 32 coordinates per point in
-// rff_write_x -- a quarter of the kernel's instructions, which bound it), the warp's 4 x 32 halves meet in 256 bytes of
-// shared memory, every lane reads the packed row back (16 broadcast LDS.128), stores it as its row of the four images and
-// stores the pieces of its own coordinate (x_j +- h, cut by the lane itself) over it.  |x|^2 = (sum_c x_c^2 - x_j^2) + (x_j +- h)^2.
-// The next tile's coordinate is requested before the chunk loop of the current one.
 template <class Finish>
 __device__ __forceinline__ void tc_rff_fd32(const TcObj &o, const TcSmem &sm, int t, int ntiles, const FdArgs &a, int cnt, Finish finish) {
   const int ntc = tcx_tiles_of_cta(ntiles);
