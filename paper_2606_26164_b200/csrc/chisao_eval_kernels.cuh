@@ -383,8 +383,10 @@ __global__ void __launch_bounds__(NT, 2) k_hlc(const DevObj o, const HlcArgs a) 
     const int s = item / d, j = item - s * d;
     const int i = a.list[first + s];
     float b = 0.0f;
-    if (a.baseline) {
-      for (int k = 0; k < M; ++k) b += fvs[s * M + k] / (float)M;
+    if (a.baseline) {   // (f / M = f * (1 / M) exactly when M is a power of two: M multiplications instead of M divisions per item)
+      const bool m_pow2 = (M & (M - 1)) == 0;
+      const float inv_m = 1.0f / (float)M;
+      for (int k = 0; k < M; ++k) b += m_pow2 ? fvs[s * M + k] * inv_m : fvs[s * M + k] / (float)M;
     }
     float acc = 0.0f;
     for (int k = 0; k < M; ++k) acc = fmaf(fvs[s * M + k] - b, get4(U[(j >> 2) * PTILE + s * M + k], j & 3), acc);

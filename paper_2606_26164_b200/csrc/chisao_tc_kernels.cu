@@ -525,6 +525,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
   const float sigma = *a.sigma_dev;
   if (sigma == 0.0f) return;                       // no spread among the unfrozen samples: nobody moves (R-18)
   const int spt = min(TC_PTS / M, HLC_MAX_SPT);
+  const bool m_pow2 = (M & (M - 1)) == 0;              // f / M = f * (1 / M) exactly: the baseline's M divisions per item become multiplications
+  const float inv_m = 1.0f / (float)M;
   const int cnt = a.count ? *a.count : a.max_count;
   const int ntiles = (cnt + spt - 1) / spt;
   if ((int)blockIdx.x >= ntiles) return;
@@ -587,7 +589,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
       const int ss = item / d, j = item - ss * d;
       const int ii = a.list[first + ss];
       float b = 0.0f;
-      if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
+      if (a.baseline) for (int kk = 0; kk < M; ++kk) b += m_pow2 ? fvs[ss * M + kk] * inv_m : fvs[ss * M + kk] / (float)M;
       float acc = 0.0f;
       for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, Us[(ss * M + kk) * US + j], acc);
       const float gh = acc / ((float)M * sigma);
@@ -719,6 +721,8 @@ __global__ void __launch_bounds__(HLCX_THREADS, 1) k_hlc_tcx(const TcObj o, cons
   const float sigma = *a.sigma_dev;
   if (sigma == 0.0f) return;                       // no spread among the unfrozen samples: nobody moves (R-18)
   const int spt = min(TC_PTS / M, HLC_MAX_SPT);
+  const bool m_pow2 = (M & (M - 1)) == 0;              // f / M = f * (1 / M) exactly: the baseline's M divisions per item become multiplications
+  const float inv_m = 1.0f / (float)M;
   const int cnt = a.count ? *a.count : a.max_count;
   const int ntiles = (cnt + spt - 1) / spt;
   if ((int)blockIdx.x >= ntiles) return;
@@ -749,7 +753,7 @@ __global__ void __launch_bounds__(HLCX_THREADS, 1) k_hlc_tcx(const TcObj o, cons
         const int ss = item / d, j = item - ss * d;
         const int ii = a.list[first + ss];
         float b = 0.0f;
-        if (a.baseline) for (int kk = 0; kk < M; ++kk) b += fvs[ss * M + kk] / (float)M;
+        if (a.baseline) for (int kk = 0; kk < M; ++kk) b += m_pow2 ? fvs[ss * M + kk] * inv_m : fvs[ss * M + kk] / (float)M;
         float acc = 0.0f;
         for (int kk = 0; kk < M; ++kk) acc = fmaf(fvs[ss * M + kk] - b, hlcx_u_chunk(sm, buf, ss * M + kk, j >> 2)[j & 3], acc);
         const float gh = acc / ((float)M * sigma);
