@@ -422,7 +422,7 @@ def run_ours(args, rank, local_rank, world):
 # beside it (profiles/); not measured in this run -- a run under ncu is never a bench value
 TRAFFIC_BYTES_PER_LAUNCH = {
     5: {"bytes": 1.86e7, "source": "profiles/r2_evalfd_c5.md (full-size launch: 18.5 MB read, 0.08 MB written)"},
-    3: {"bytes": 2.26e6, "source": "profiles/r1_evalfd_c3_rfftc.md (2.26 MB read, 0 written: the gradient stays in L2; kernel unchanged since)"},
+    3: {"bytes": 4.38e6, "source": "profiles/r2_c2_c3_c4.md, r2_evalfd_c3.csv (4.38 MB read, 0 written: the gradient stays in L2)"},
     4: {"bytes": 4.36e6, "source": "profiles/r2_c2_c3_c4.md, r2_evalfd_c4.csv (4.36 MB read, 0 written)"}}
 
 
