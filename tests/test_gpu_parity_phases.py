@@ -126,6 +126,43 @@ def test_a2_wrapped_rings_on_the_quad_step_kernel(orc, B, kind, d, N, m):
     test_a2_lbfgs_iterations_teacher_forced(orc, B, 0, N, wl=wl, n_it=14 if m < 14 else 8)
 
 
+@pytest.mark.parametrize("kind,d,N,m", [("gmm_full", 40, 400, 4), ("quad", 64, 300, 4), ("gmm_full", 64, 250, 6)])
+def test_fused_quad_step_kernel_inside_a_cycle_follows_the_unit_sequence(B, kind, d, N, m):
+    """Inside chisao_step the iterations it > m of a pass run the quad step kernel with the update of iteration it - 1 fused
+    in front (the pair it stores goes to HBM and, from registers, into the shared-memory copy of the history); iterations
+    2 .. m run the half-warp form with the history staged through shared memory.  The unit sequence chisao_phase runs
+    (RELEASE_EVAL, n_conv x LBFGS_ITER, STICK) uses the stand-alone forms (direction kernel, separate update kernel), which
+    the a2 tests compare with the oracle step by step.  Same evaluator, same line search, fp32 on both sides: the two
+    Phase-1 passes differ by the summation order of a few dots, so after n_conv = 14 iterations (m = 4 / 6: wrapped rings)
+    positions, values and flags agree closely -- a wrong row, plane or pair in the fused kernel would not."""
+    if kind == "quad":
+        wl = inputs.custom(inputs.quad(d, 600 + d, lam_max=30.0), 4.0, N, seed=50 + d, fd_h=1e-2, eps_grad=0.05, n_conv=14,
+                           lbfgs_m=m, n_osc=3, phase_mask=0)
+    else:
+        wl = inputs.custom(inputs.gmm_full(d, 3, 3.0, 88 + d), 4.0, N, seed=50 + d, fd_h=1e-2, eps_grad=1e-2, n_conv=14,
+                           lbfgs_m=m, n_osc=3, phase_mask=0)
+    hp = wl.hp
+    a, b = B.Chisao(wl), B.Chisao(wl)
+    sa = a.step()                                            # phases 1-2 of cycle 1 (phases 3-6 masked off)
+    b.set(B.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
+    b.phase(B.PH_RELEASE_EVAL)
+    for it in range(1, hp.n_conv + 1):
+        b.phase(B.PH_LBFGS_ITER, it)
+    b.phase(B.PH_STICK)
+    sb = b.stats()
+    xa, xb = a.get(B.X).astype(np.float64), b.get(B.X).astype(np.float64)
+    fa, fb = a.get(B.F).astype(np.float64), b.get(B.F).astype(np.float64)
+    dx = np.max(np.abs(xa - xb), axis=1)
+    close = dx <= 1e-3 * 4.0
+    assert close.mean() >= 0.95, (float(close.mean()), float(np.max(dx)))   # (a differing Armijo decision sends a sample elsewhere for a while)
+    assert np.all(np.abs(fa - fb)[close] <= 1e-3 * np.maximum(np.abs(fb[close]), 1.0))
+    assert np.array_equal(a.get(B.HIST_LEN)[close] > 0, b.get(B.HIST_LEN)[close] > 0)
+    assert int(a.get(B.HIST_LEN).max()) == m                 # the rings did fill
+    assert abs(sa.n_stuck - sb.n_stuck) <= max(2, 0.02 * N), (sa.n_stuck, sb.n_stuck)
+    assert abs(sa.f_max - sb.f_max) <= 1e-4 * max(abs(sb.f_max), 1.0)
+    assert list(sa.evals)[0] == list(sb.evals)[0]
+
+
 def _converged_pair(orc, B, wl, n_conv=None):
     o, g = _pair(orc, B, wl)
     o.set(orc.CTRL, [1, 1, 0, 0, 0, 0, 0, 0])
