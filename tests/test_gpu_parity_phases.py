@@ -155,7 +155,7 @@ def test_fused_quad_step_kernel_inside_a_cycle_follows_the_unit_sequence(B, kind
     dx = np.max(np.abs(xa - xb), axis=1)
     close = dx <= 1e-3 * 4.0
     assert close.mean() >= 0.95, (float(close.mean()), float(np.max(dx)))   # (a differing Armijo decision sends a sample elsewhere for a while)
-    assert np.all(np.abs(fa - fb)[close] <= 1e-3 * np.maximum(np.abs(fb[close]), 1.0))
+    assert np.all(np.abs(fa - fb)[close] <= 5e-3 * np.maximum(np.abs(fb[close]), 1.0))   # (|grad f| up to ~1 at these points, dx up to 4e-3)
     assert np.array_equal(a.get(B.HIST_LEN)[close] > 0, b.get(B.HIST_LEN)[close] > 0)
     assert int(a.get(B.HIST_LEN).max()) == m                 # the rings did fill
     assert abs(sa.n_stuck - sb.n_stuck) <= max(2, 0.02 * N), (sa.n_stuck, sb.n_stuck)
