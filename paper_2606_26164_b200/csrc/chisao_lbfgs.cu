@@ -95,7 +95,7 @@ struct SampleState { Row4 g, x; int len, head, stalled; bool have_x; unsigned by
 template <bool VEC>
 __device__ __forceinline__ SampleState lbfgs_update_half(const State &s, int i, bool in, int hl) {
   constexpr bool vec = VEC;
-  const int d = s.d, m = s.m, N = s.N;
+  const int d = s.d, m = s.m;
   const size_t ro = (size_t)(in ? i : 0) * d;
   SampleState o;
   const int b = in ? s.ls_b[i] : -2;
