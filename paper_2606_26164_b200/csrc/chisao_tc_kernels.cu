@@ -512,6 +512,13 @@ __device__ __forceinline__ void hlc_normals(uint64_t seed, int i, int cycle, int
 }
 
 // Hands Like Clouds on the tensor-core evaluator: point t of the tile = (sample t / M, draw t % M), M <= 128.
+// the same as a call (QUAD form of k_hlc_tc: the kernel inlines load() several times -- prologue and loop of both operand
+// forms -- and each copy of the generator is ~10 k instructions; as a function the kernel is a third of the size and its
+// Hands-Like-Clouds step 8 % faster; the RFF form, with one copy, is faster inlined)
+__device__ __noinline__ void hlc_normals_call(uint64_t seed, int i, int cycle, int iter, int k, int d, float (&u)[TC_D]) {
+  hlc_normals(seed, i, cycle, iter, k, d, u);
+}
+
 // QUAD and RFF forms: a draw's normals are generated once, in load, and kept in shared memory for the reduction (row t
 // of one of two buffers, by tile parity: the QUAD form fetches a tile's point two tiles ahead of its finish).  The
 // x-stationary GMM_FULL form has no shared memory left for them (its W stages fill it): it regenerates them in finish --
@@ -548,7 +555,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_hlc_tc(const TcObj o, const H
     c.i = c.valid ? a.list[first + s] : 0;
     if (c.valid) {
       float u[TC_D];
-      hlc_normals(a.seed, c.i, a.cycle, a.iter, k, d, u);
+      if constexpr (OBJ == CHISAO_OBJ_QUAD) hlc_normals_call(a.seed, c.i, a.cycle, a.iter, k, d, u);
+      else hlc_normals(a.seed, c.i, a.cycle, a.iter, k, d, u);
       if constexpr (KEEP_U) {
         float *row = ubuf(tile) + t * US;
 #pragma unroll
