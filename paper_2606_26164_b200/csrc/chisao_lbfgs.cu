@@ -161,7 +161,7 @@ __device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
 }
 template <int MM, bool VEC, int MODE, bool SH>
-__global__ void __launch_bounds__(DIR_WARPS * 32, SH ? 5 : 4) k_lbfgs_step(State s, Hyper h) {
+__global__ void __launch_bounds__(DIR_WARPS * 32, SH ? 5 : 4) k_lbfgs_step(State s, Hyper h, int hrows) {
   extern __shared__ float4 hist_smem[];
   __shared__ int sh_cnt, sh_base;
   __shared__ unsigned int sh_bytes;
@@ -204,7 +204,9 @@ __global__ void __launch_bounds__(DIR_WARPS * 32, SH ? 5 : 4) k_lbfgs_step(State
   const int len_read = len;
   const int head = act ? head_i : 0;
   Row4 Sr[SH ? 1 : MM], Yr[SH ? 1 : MM];
-  float4 *hS = hist_smem + (size_t)((wib * 2 + half) * 2 * MM) * 16 + hl, *hY = hS + MM * 16;   // row l at [l * 16]
+  // (hrows <= MM rows per sample and array are staged: inside a cycle a history holds at most it - 1 pairs, and the fewer
+  // rows a CTA reserves the more CTAs an SM holds)
+  float4 *hS = hist_smem + (size_t)((wib * 2 + half) * 2 * hrows) * 16 + hl, *hY = hS + hrows * 16;   // row l at [l * 16]
   // rows up to the longer history of the warp's two samples take part in the (warp-uniform) loops; the shorter
   // sample's missing rows are zero
   const int lw = SH ? max(len, __shfl_xor_sync(0xffffffffu, len, 16)) : MM;
@@ -724,31 +726,35 @@ cudaError_t launch_release(const State &s, cudaStream_t st) {
 }
 static bool g_step_regs = false;   // CHISAO_STEP_REGS in the environment: keep the register form of the history (A/B measurements)
 template <int MM, bool VEC, int MODE, bool SH>
-static cudaError_t launch_step_one(const State &s, const Hyper &h, int grid, cudaStream_t st) {
-  const size_t sh = SH ? (size_t)DIR_WARPS * 2 * 2 * MM * 16 * sizeof(float4) : 0;
+static cudaError_t launch_step_one(const State &s, const Hyper &h, int grid, int hrows, cudaStream_t st) {
+  hrows = SH ? std::max(1, std::min(hrows, MM)) : MM;
+  const size_t sh = SH ? (size_t)DIR_WARPS * 2 * 2 * hrows * 16 * sizeof(float4) : 0;
   if (SH) {
     static bool configured = false;
     if (!configured) {
-      cudaError_t e = cudaFuncSetAttribute(k_lbfgs_step<MM, VEC, MODE, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
+      const size_t shmax = (size_t)DIR_WARPS * 2 * 2 * MM * 16 * sizeof(float4);
+      cudaError_t e = cudaFuncSetAttribute(k_lbfgs_step<MM, VEC, MODE, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmax);
+      if (e != cudaSuccess) return e;
+      e = cudaFuncSetAttribute(k_lbfgs_step<MM, VEC, MODE, SH>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
       if (e != cudaSuccess) return e;
       configured = true;
     }
   }
-  k_lbfgs_step<MM, VEC, MODE, SH><<<grid, DIR_WARPS * 32, sh, st>>>(s, h);
+  k_lbfgs_step<MM, VEC, MODE, SH><<<grid, DIR_WARPS * 32, sh, st>>>(s, h, hrows);
   return cudaGetLastError();
 }
 template <int MM, bool VEC, bool SH>
-static cudaError_t launch_step_mode(const State &s, const Hyper &h, int mode, int grid, cudaStream_t st) {
-  if (mode == STEP_FIRST) return launch_step_one<MM, VEC, STEP_FIRST, false>(s, h, grid, st);   // (empty history: nothing to stage)
-  if (mode == STEP_UPDATE) return launch_step_one<MM, VEC, STEP_UPDATE, SH>(s, h, grid, st);
-  return launch_step_one<MM, VEC, STEP_ALONE, SH>(s, h, grid, st);
+static cudaError_t launch_step_mode(const State &s, const Hyper &h, int mode, int grid, int hrows, cudaStream_t st) {
+  if (mode == STEP_FIRST) return launch_step_one<MM, VEC, STEP_FIRST, false>(s, h, grid, hrows, st);   // (empty history: nothing to stage)
+  if (mode == STEP_UPDATE) return launch_step_one<MM, VEC, STEP_UPDATE, SH>(s, h, grid, hrows, st);
+  return launch_step_one<MM, VEC, STEP_ALONE, SH>(s, h, grid, hrows, st);
 }
 template <int MM>
-static cudaError_t launch_step_mm(const State &s, const Hyper &h, int mode, bool staged, int grid, cudaStream_t st) {
+static cudaError_t launch_step_mm(const State &s, const Hyper &h, int mode, bool staged, int grid, int hrows, cudaStream_t st) {
   const bool vec = (s.d & 3) == 0;
-  if (!vec) return launch_step_mode<MM, false, false>(s, h, mode, grid, st);
-  if (!staged) return launch_step_mode<MM, true, false>(s, h, mode, grid, st);
-  return launch_step_mode<MM, true, true>(s, h, mode, grid, st);
+  if (!vec) return launch_step_mode<MM, false, false>(s, h, mode, grid, hrows, st);
+  if (!staged) return launch_step_mode<MM, true, false>(s, h, mode, grid, hrows, st);
+  return launch_step_mode<MM, true, true>(s, h, mode, grid, hrows, st);
 }
 static int g_step_quad = 1;        // CHISAO_STEP_QUAD in the environment: 0 never, 1 where the register form would run (default), 2 also for it <= m
 template <int MM, int MODE, bool FULL>
@@ -788,10 +794,11 @@ cudaError_t launch_lbfgs_step(const State &s, const Hyper &h, int mode, int it, 
     if (s.m <= 10) return launch_quad_mm<10>(s, h, mode, st);
     return launch_quad_mm<16>(s, h, mode, st);
   }
-  if (s.m <= 4) return launch_step_mm<4>(s, h, mode, staged, grid, st);
-  if (s.m <= 8) return launch_step_mm<8>(s, h, mode, staged, grid, st);
-  if (s.m <= 10) return launch_step_mm<10>(s, h, mode, staged, grid, st);
-  return launch_step_mm<16>(s, h, mode, staged, grid, st);
+  const int hrows = staged ? it - 1 : s.m;                  // pairs a history can hold in this launch
+  if (s.m <= 4) return launch_step_mm<4>(s, h, mode, staged, grid, hrows, st);
+  if (s.m <= 8) return launch_step_mm<8>(s, h, mode, staged, grid, hrows, st);
+  if (s.m <= 10) return launch_step_mm<10>(s, h, mode, staged, grid, hrows, st);
+  return launch_step_mm<16>(s, h, mode, staged, grid, hrows, st);
 }
 cudaError_t launch_lbfgs_update(const State &s, const Hyper &h, bool stick_partials, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
