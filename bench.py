@@ -202,16 +202,17 @@ def measure_config(c, K, W, rank, local_rank, world, dist, dev, N_override=0, de
     x_out = torch.empty_like(x_host).pin_memory()
     f_out = torch.empty(hp.N, dtype=torch.float32).pin_memory()
     s_out = torch.empty(hp.N, dtype=torch.uint8).pin_memory()
+    # (the population a step returns is the next step's input: the two pinned buffers swap roles, no host-side copy)
     for _ in range(W):
         g2.step_host(x_host, x_out, f_out, s_out)
-        x_host.copy_(x_out)
+        x_host, x_out = x_out, x_host
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for _ in range(K):
-        g2.step_host(x_host, x_out, f_out, s_out)           # synchronises before returning
-        x_host.copy_(x_out)
+        g2.step_host(x_host, x_out, f_out, s_out)           # H2D of x, one cycle, D2H of x, f, stuck; synchronises before returning
+        x_host, x_out = x_out, x_host
     e2e_s = time.perf_counter() - t0
     e2e_s = replicas.max_over_ranks(e2e_s, dd, dev)
     g2.close()
