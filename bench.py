@@ -104,19 +104,27 @@ def oracle_throughput(c: int, steps: int, warmup: int, threads: int = 0):
     # ~1.5 s of one core per sample-cycle at C5: 8 samples per thread keep one step in the 10-20 s range
     per_thread = {1: 256, 2: 256, 3: 24, 4: 32, 5: 8}[c]
     Ns = min(full.hp.N, max(8, per_thread * threads))
-    wl = inputs.config(c, N=Ns, n_osc=max(full.hp.n_osc, steps + warmup + 1))
+    wl = inputs.config(c, N=Ns, n_osc=max(full.hp.n_osc, 2 * steps + warmup + 1))
     o = O.Oracle(wl, threads=threads)
     for _ in range(warmup):
         o.step()
-    ev0 = sum(o.stats().evals)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        o.step()
-    dt = time.perf_counter() - t0
-    ev = sum(o.stats().evals) - ev0
+    # two timed passes of `steps` cycles, the faster one reported: the first seconds of a fresh process on an idle box run
+    # at anything between 0.55 and 1.0 of the settled rate (measured on the GPU boxes: host clocks ramping up), which made
+    # the two arms that time this same function disagree by up to 40 %
+    best = None
+    for _ in range(2):
+        ev0 = sum(o.stats().evals)
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            o.step()
+        dt = time.perf_counter() - t0
+        ev = sum(o.stats().evals) - ev0
+        if best is None or dt < best[0]:
+            best = (dt, ev)
+    dt, ev = best
     o.close()
     return {"value": Ns * steps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"{Ns} of {full.hp.N} samples x {steps} full cycle(s) after {warmup} warm-up cycle(s), fp64, "
+            "sample": f"{Ns} of {full.hp.N} samples x {steps} full cycle(s) (the faster of two passes) after {warmup} warm-up cycle(s), fp64, "
                       f"OpenMP over samples on {threads} of {cores} host cores; per-sample cost is N-independent except deduplication",
             "f_evals_per_sec": ev / dt, "seconds": dt}, wl
 
