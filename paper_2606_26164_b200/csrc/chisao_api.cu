@@ -554,14 +554,14 @@ int run_stick(chisao_ctx *ctx) {
   // after run_lbfgs_finish the per-sample gradient norms and f_max are already there
   const bool have_partials = ctx->in_cycle && (ctx->hp.n_conv > 0 || ctx->resident);
   CK(launch_stick(ctx->st, ctx->hp, have_partials, ctx->stream));
-  ctx->launches += have_partials ? 3 : 4;
+  ctx->launches += (have_partials ? 0 : 1) + scan_launches(ctx->st.N);
   return CHISAO_OK;
 }
 int run_dedup(chisao_ctx *ctx) {
   Scope sc(ctx, 5);
   const bool dedup_on = (ctx->hp.phase_mask & (1u << 3)) != 0;
   CK(launch_dedup(ctx->st, ctx->hp, !ctx->in_cycle, ctx->stream));
-  ctx->launches += (ctx->in_cycle ? 0 : 3) + (dedup_on ? 1 : 0) + 3;
+  ctx->launches += (ctx->in_cycle ? 0 : scan_launches(ctx->st.N)) + (dedup_on ? 1 : 0) + scan_launches(ctx->st.N);
   return CHISAO_OK;
 }
 int run_reseed(chisao_ctx *ctx) {
@@ -573,7 +573,7 @@ int run_reseed(chisao_ctx *ctx) {
 int run_explore_list(chisao_ctx *ctx) {
   Scope sc(ctx, 5);
   CK(launch_explore_list(ctx->st, ctx->stream));
-  ctx->launches += 3;
+  ctx->launches += scan_launches(ctx->st.N);
   return CHISAO_OK;
 }
 int run_hlc(chisao_ctx *ctx, int t) {

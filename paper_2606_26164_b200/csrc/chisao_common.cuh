@@ -21,6 +21,10 @@ enum { PUR_INIT = 0, PUR_NOISE = 1, PUR_HLC_U = 2, PUR_RS_SRC = 3, PUR_RS_T = 4,
 enum { EV_INIT = 0, EV_LS = 1, EV_LBFGS_FD = 2, EV_HLC = 5, EV_ANTI = 6 };
 
 // ---- device control block (one per context, lives in the workspace) ----------------------------
+// populations up to this size run an ordered scan as ONE launch (k_scan_small), larger ones as three (chisao_select.cu)
+constexpr int SCAN_SMALL_MAX = 4096;
+__host__ __device__ inline int scan_launches(int N) { return (N == 0 || N <= SCAN_SMALL_MAX) ? 1 : 3; }
+
 struct Ctrl {
   int32_t cycle, gr_enabled, gr_unproductive, gr_prev_modes, gr_used_last, k_lost, n_stuck, n_active;
   int32_t strategy;        // reseed strategy of the current cycle

@@ -137,10 +137,72 @@ __global__ void __launch_bounds__(SCAN_BLOCK) k_scan_scatter(State s, int mode, 
   }
 }
 
+// The whole ordered scan in ONE launch for small populations (N <= SCAN_SMALL_MAX: C1, C2 -- launch-bound configurations,
+// where the three kernels above cost three launch latencies for a few microseconds of work): one CTA walks the chunks of
+// 1024 samples in order, keeps a running offset per class, and scatters at once; same flags, lists (ascending) and
+// bookkeeping as k_scan_count + k_scan_offsets + k_scan_scatter.
+static_assert(SCAN_SMALL_MAX % SCAN_BLOCK == 0, "whole chunks");
+__global__ void __launch_bounds__(SCAN_BLOCK) k_scan_small(State s, Hyper h, int mode, int nb) {
+  __shared__ int wcnt[3][SCAN_BLOCK / 32];
+  __shared__ int run[3];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (threadIdx.x < 3) run[threadIdx.x] = 0;
+  __syncthreads();
+  for (int b = 0; b < nb; ++b) {
+    const int i = b * SCAN_BLOCK + threadIdx.x;
+    if (i < s.N) {
+      if (mode == SCAN_STICK_FLAGS) { s.stuck[i] = stick_test(s, h, i) ? 1 : 0; s.removed[i] = 0; }
+      else if (mode == SCAN_FINAL && s.removed[i]) s.stuck[i] = 0;
+      if (mode == SCAN_FINAL) { s.rs_src[i] = -1; s.rs_cand[i] = -1; }
+    }
+    const int c = (i < s.N) ? scan_class(s, mode, i) : -1;
+    int rank = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const unsigned mk = __ballot_sync(0xffffffffu, c == k);
+      if (lane == 0) wcnt[k][w] = __popc(mk);
+      if (c == k) rank = __popc(mk & ((1u << lane) - 1u));
+    }
+    __syncthreads();
+    if (c >= 0) {
+      int off = run[c] + rank;
+      for (int ww = 0; ww < w; ++ww) off += wcnt[c][ww];
+      int32_t *dst = (mode == SCAN_STICK || mode == SCAN_STICK_FLAGS) ? s.listP0 : (mode == SCAN_EXPLORE) ? s.listE
+                     : (c == 0 ? s.listA : (c == 1 ? s.listP : s.listR));
+      dst[off] = i;
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) { int t = 0; for (int ww = 0; ww < SCAN_BLOCK / 32; ++ww) t += wcnt[threadIdx.x][ww]; run[threadIdx.x] += t; }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    Ctrl *c = s.ctrl;
+    const int tot[3] = {run[0], run[1], run[2]};
+    if (mode == SCAN_STICK || mode == SCAN_STICK_FLAGS) {
+      c->nP0 = tot[1]; c->n_stuck = tot[1]; c->k_lost = 0; c->n_active = s.N - tot[1];
+    } else if (mode == SCAN_FINAL) {
+      c->nA = tot[0]; c->nP = tot[1]; c->nR = tot[2];
+      c->k_lost = tot[2]; c->n_stuck = tot[1]; c->n_active = tot[0];
+      c->strategy = 0;
+      if (c->gr_used_last) {                                  // Golden Rooster self-disable (R-9)
+        if (tot[1] > c->gr_prev_modes) c->gr_unproductive = 0; else c->gr_unproductive += 1;
+        if (c->gr_unproductive >= 2) c->gr_enabled = 0;
+      }
+    } else {
+      c->nE = tot[1];
+      c->n_active = tot[1];
+    }
+  }
+}
+
 static cudaError_t run_scan(const State &s, const Hyper &h, int mode, cudaStream_t st) {
   const int nb = (s.N + SCAN_BLOCK - 1) / SCAN_BLOCK;
   if (nb == 0) {  // empty population: only the bookkeeping kernel runs
     k_scan_offsets<<<1, 256, 0, st>>>(s, mode, 0);
+    return cudaGetLastError();
+  }
+  if (s.N <= SCAN_SMALL_MAX) {
+    k_scan_small<<<1, SCAN_BLOCK, 0, st>>>(s, h, mode, nb);
     return cudaGetLastError();
   }
   k_scan_count<<<nb, SCAN_BLOCK, 0, st>>>(s, h, mode, nb);
